@@ -1,0 +1,148 @@
+/* smolgp.h -- C ABI of the B200-native (sm_100a) integrated-GP state-space library.
+ *
+ * What it computes: exact Gaussian-process inference for exposure-integrated, possibly
+ * overlapping measurements (arXiv:2601.02527) through the augmented linear-Gaussian state-space
+ * model of the paper: one integral state z_i per instrument (Eq. 3.17), reset at each
+ * exposure start (Eq. 3.11/3.18) and observed as z_i/delta_n at each exposure end
+ * (Eq. 3.12).  Inference is the parallel-in-time (associative-scan) Kalman filter and
+ * smoother of section 3.4 with the log marginal likelihood of Eq. 2.26.
+ * "P:<n>" = line n of the paper text; DESIGN.md lists the readings taken where the
+ * text is silent or garbled.
+ *
+ * Conventions
+ *  - Every function returns SMOLGP_OK (0) or a negative smolgp_status; nothing throws, exits or
+ *    prints.  smolgp_last_error(ctx) gives a ctx-owned NUL-terminated message for the last failure.
+ *  - Array arguments are DEVICE pointers (8-byte aligned, caller-owned, not retained after the
+ *    call returns unless stated) in the entry points without suffix, and HOST pointers in the
+ *    *_host entry points, which copy in and out on the ctx stream and synchronise before
+ *    returning.  Kernel descriptions (smolgp_kernel) are always small HOST structs.
+ *  - All times are in one unit (seconds in the shipped workloads); all arithmetic is fp64.
+ *  - Outputs are in the caller's exposure order (the order of t_start/t_end), per series.
+ *  - Work is enqueued on the ctx stream; the device entry points return after the work is
+ *    enqueued except where a status needs a read-back (smolgp_build_events; the numeric flag of
+ *    smolgp_loglik/smolgp_condition, which is read after a stream synchronise).
+ *  - There is no CPU fallback: without a CUDA device smolgp_create fails with SMOLGP_ECUDA.
+ */
+#ifndef SMOLGP_H
+#define SMOLGP_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SMOLGP_OK = 0,
+  SMOLGP_EINVAL = -1,       /* bad argument: N<=0, non-finite time, t_end<=t_start, instrument out of range, sigma<=0 */
+  SMOLGP_EOVERLAP = -2,     /* an instrument overlaps itself (t_n^e > t_{n+1}^s) */
+  SMOLGP_EUNSUPPORTED = -3, /* augmented dimension above SMOLGP_MAX_DIM, unknown family, too many instruments */
+  SMOLGP_ENOMEM = -4,
+  SMOLGP_ECUDA = -5,
+  SMOLGP_ENUMERIC = -6      /* a non-finite value or a non-positive innovation variance was met */
+} smolgp_status;
+
+#define SMOLGP_MAX_DIM 32  /* max augmented state dimension n = d + N_inst */
+#define SMOLGP_MAX_INST 16 /* max number of instruments */
+
+/* kernel families (state-space forms: DESIGN.md "Models"; SHO: App. B) */
+enum {
+  SMOLGP_MATERN32 = 0,           /* p0 = ell                                   d = 2 */
+  SMOLGP_MATERN52 = 1,           /* p0 = ell                                   d = 3 */
+  SMOLGP_SHO = 2,                /* p0 = omega0 [rad/time], p1 = Q             d = 2 */
+  SMOLGP_MATERN32_X_PERIODIC = 3 /* p0 = ell, p1 = period, p2 = ell_periodic, order = J:
+                                    Matern-3/2 times the order-J cosine series of the periodic
+                                    kernel (products of kernels: App. C.2)  d = 2 + 4J */
+};
+
+/* one additive component of the kernel (sums of kernels: App. C.1) */
+typedef struct {
+  int32_t family;
+  int32_t order;      /* J for MATERN32_X_PERIODIC, else ignored */
+  uint32_t inst_mask; /* bit i set <=> the component enters instrument i's integrand H_i (Eq. 3.2) */
+  double sigma;       /* amplitude: k(0) = sigma^2 (times the series' sum for the periodic product) */
+  double p0, p1, p2;
+} smolgp_component;
+
+typedef struct {
+  int32_t n_comp;
+  const smolgp_component* comp; /* host memory */
+} smolgp_kernel;
+
+typedef struct smolgp_ctx smolgp_ctx;       /* device id, stream, workspace arena */
+typedef struct smolgp_events smolgp_events; /* immutable device-resident event stream */
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (NULL = the legacy
+ * default stream); the caller keeps ownership of the stream. */
+int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream);
+void smolgp_destroy(smolgp_ctx* ctx);
+const char* smolgp_last_error(const smolgp_ctx* ctx);
+
+/* Tuning knobs (all optional).  name = "chunk": events per scan chunk at the leaf level
+ * (0 = automatic; >= the series length selects the sequential one-group-per-series filter of
+ * SURVEY 8(a) row a8); "group": dense-combine fan-in of the upper scan levels (default 8);
+ * "lanes": threads cooperating on one chunk (0 = automatic; 8, 16 or 32). */
+int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);
+
+/* Step a1.  Turns N exposures [t_start[n], t_end[n]] of instrument
+ * instrument[n] in [0, n_inst) into the time-sorted stream of K = 2N events (one reset event per
+ * start, one observe event per end; at equal times ends come before starts so that back-to-back
+ * exposures of one instrument, the Fig. 2 case P:543, are legal).  Device radix sort on the
+ * order-preserving 64-bit image of the times; the reset/observe flags, the per-event set of idle
+ * instruments and the validation that no instrument overlaps itself come from an
+ * exclusive XOR scan of the instrument bits.  The three inputs are DEVICE pointers; the result
+ * is owned by the caller (smolgp_free_events) and can be reused across kernels and data.
+ * Errors: EINVAL, EOVERLAP, EUNSUPPORTED (n_inst > SMOLGP_MAX_INST), ENOMEM, ECUDA. */
+int smolgp_build_events(smolgp_ctx* ctx, int64_t N, const double* t_start, const double* t_end,
+                        const int32_t* instrument, int32_t n_inst, smolgp_events** out);
+int smolgp_build_events_host(smolgp_ctx* ctx, int64_t N, const double* t_start, const double* t_end,
+                             const int32_t* instrument, int32_t n_inst, smolgp_events** out);
+void smolgp_free_events(smolgp_events* ev);
+
+/* Read back the event stream (HOST output arrays of length 2N, any may be NULL): event time,
+ * kind (1 = start/reset, 0 = end/observe), instrument, exposure index.  For tests. */
+int smolgp_events_export(smolgp_ctx* ctx, const smolgp_events* ev, double* t, int32_t* kind,
+                         int32_t* instrument, int32_t* exposure);
+
+/* Steps a2 + a3 + a5 (Eq. 2.17-2.19, 3.7-3.10; Eq. 3.20-3.21 + forward scan; Eq. 2.26).
+ * y: [batch][N] data; noise_sigma: [N] per-exposure white-noise standard deviation (> 0);
+ * amp: [batch] per-series kernel amplitude scale (k_p = amp_p^2 k) or NULL (= 1);
+ * loglik: [batch] output, Eq. 2.26 including the N log(2 pi)/2 constant. */
+int smolgp_loglik(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                  int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                  double* loglik);
+int smolgp_loglik_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                       int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                       double* loglik);
+
+/* Steps a2-a6 (+ a7 when M > 0).  As smolgp_loglik, plus the posterior of the noise-free exposure
+ * average at every observation (mean_obs, var_obs: [batch][N]; H~ m^, H~ P^ H~^T of P:460) and,
+ * when M > 0, the posterior of the instantaneous latent of instrument query_instrument at the
+ * M query times (Algorithm 1; mean_query, var_query: [batch][M]).  loglik may be NULL. */
+int smolgp_condition(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                     int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                     int64_t M, const double* t_query, int32_t query_instrument,
+                     double* mean_obs, double* var_obs, double* mean_query, double* var_query,
+                     double* loglik);
+int smolgp_condition_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                          int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                          int64_t M, const double* t_query, int32_t query_instrument,
+                          double* mean_obs, double* var_obs, double* mean_query, double* var_query,
+                          double* loglik);
+
+/* Step a2 alone, for tests: the augmented transition A~ = [Phi 0; Phi-bar I] and process noise
+ * Q~ (Eq. 3.7-3.10; Eq. 3.17-3.19 for several instruments) of one step of length dt,
+ * in raw (unscaled) state units, row-major n x n, HOST outputs.  n_out receives n = d + n_inst. */
+int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kernel, int32_t n_inst, double dt,
+                           double* A, double* Q, int32_t* n_out);
+
+/* Launch accounting for bench.py: number of kernels this ctx has launched so far. */
+int64_t smolgp_launch_count(const smolgp_ctx* ctx);
+
+/* FP64 FMA throughput probe (roofline denominator): runs a register-only
+ * DFMA kernel on the ctx stream and returns the achieved TFLOP/s in *tflops. */
+int smolgp_probe_fp64(smolgp_ctx* ctx, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SMOLGP_H */

@@ -1,0 +1,120 @@
+// Internal declarations shared by the translation units of libsmolgp_b200.so (CUDA product path).
+// Nothing here is used by, or shared with, oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/smolgp.h"
+
+#define SG_NMAX SMOLGP_MAX_DIM
+#define SG_MAXINST SMOLGP_MAX_INST
+#define SG_MAXBLK 16 /* max number of block-diagonal blocks of F (App. C.1 stacking) */
+#define SG_MAXBD 4   /* max block dimension */
+#define SG_KT 18     /* Taylor order of the small-step discretisation */
+#define SG_BE (SG_MAXBD + 1)
+
+enum { BLK_M32 = 0, BLK_M52 = 1, BLK_SHO = 2, BLK_M32ROT = 3 };
+
+// One block-diagonal block of the base model in its own non-dimensional units ("block units"):
+// time in units of T_b (1/lambda or 1/omega0), state x''_i = x_i / (sigma_b lambda^i), so that all
+// constants below are O(1).  The block is augmented with its own integral I'' = int H'' x'' dt''
+// (Eq. 3.3-3.6): F~'' = [F'' 0; H'' 0], L~ Qc L~^T = [W'' 0; 0 0].
+struct BlockConst {
+  int family, dim, off; // off = offset of the block inside x
+  int sho_case;         // SHO: 0 underdamped (Q > 1/2), 1 critical, 2 overdamped
+  double inv_T;         // 1 / T_b
+  double rho;           // inf-norm of F~''  (step size control of the Taylor regime)
+  double a, b;          // SHO: a = 1/(2Q), b = sqrt(|1 - a^2|);  M32ROT: b = omega'' = j omega_p T_b
+  double pinf[SG_MAXBD * SG_MAXBD];             // stationary covariance in block units
+  double tayA[SG_KT + 1][SG_BE * SG_BE];        // F~''^k / k!
+  double tayQ[SG_KT + 1][SG_BE * SG_BE];        // Gamma_k / k!, Gamma_1 = W~'', Gamma_{k+1} = F~ Gamma_k + Gamma_k F~^T
+};
+
+// Whole model, device resident (built on the host by model.cu for each call's kernel).
+struct ModelDev {
+  int n, d, n_inst, nblk;
+  int disc_stride;                 // doubles per event in the discretisation array
+  int disc_off[SG_MAXBLK];         // offset of block b inside one event's record
+  int row_lo[SG_NMAX], row_hi[SG_NMAX]; // x-row i of F only touches columns [row_lo, row_hi)
+  double cz[SG_MAXINST][SG_MAXBLK]; // c_qb: coupling of block b's integral into z_q (equilibrated units), 0 if masked out
+  double tau[SG_MAXINST];          // z_q is carried as z_q / tau_q
+  double p0[SG_NMAX * SG_NMAX];    // prior covariance blkdiag(Pinf'', 0) (Eq. 3.19, reading R6)
+  BlockConst blk[SG_MAXBLK];
+};
+
+// per-event record layout inside the discretisation array, block b at disc_off[b]:
+//   Phi (dim*dim, row-major) | phibar (dim) | Qxx (dim*dim) | q12 (dim) | q22 (1)      [block units]
+static inline int disc_block_size(int dim) { return 2 * dim * dim + 2 * dim + 1; }
+
+// event meta word: bit 0 kind (1 = start/reset, 0 = end/observe), bits 1..5 instrument,
+// bits 8..23 zero-mask Z_k (instruments whose z is zeroed after event k: idle ones, and the
+// event's own instrument in both cases: reset at a start, idle after an end).
+#define META_KIND(m) ((m) & 1u)
+#define META_INST(m) (((m) >> 1) & 31u)
+#define META_ZMASK(m) (((m) >> 8) & 0xFFFFu)
+
+struct smolgp_events {
+  int device;
+  int64_t N, K;
+  int n_inst;
+  double* t;       // [K] event time
+  double* dt;      // [K] t_k - t_{k-1}, dt_0 = 0
+  double* delta;   // [K] exposure length of the event's exposure
+  uint32_t* meta;  // [K]
+  int32_t* obs;    // [K] exposure index
+  double tau[SG_MAXINST]; // per-instrument power-of-two scale of z (host copy)
+  double t_first, t_last;
+};
+
+struct smolgp_ctx {
+  int device;
+  cudaStream_t stream;
+  std::string err;
+  int64_t launches;
+  int64_t opt_chunk, opt_group, opt_lanes;
+  // workspace arena (grown on demand, reused across calls)
+  void* arena;
+  size_t arena_bytes;
+  int* d_flags; // device status word(s)
+  int sm_count;
+  size_t smem_optin;
+};
+
+#define SG_CUDA(ctx, call)                                                            \
+  do {                                                                                \
+    cudaError_t e__ = (call);                                                         \
+    if (e__ != cudaSuccess) {                                                         \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);               \
+      return SMOLGP_ECUDA;                                                            \
+    }                                                                                 \
+  } while (0)
+
+// model.cu
+int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const double* tau, ModelDev* out);
+// disc.cu
+int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_model, const double* dt,
+                   int64_t K, double* disc);
+// events.cu
+int sg_sort_pairs(smolgp_ctx* ctx, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
+                  int64_t n, uint32_t* hist);
+// scan.cu
+struct ScanArgs {
+  const ModelDev* d_model;
+  const ModelDev* h_model;
+  const smolgp_events* ev;
+  const double* disc;
+  int64_t batch;
+  const double* y;     // [batch][N]
+  const double* sigma; // [N]
+  const double* amp;   // [batch] or NULL
+  double* loglik;      // [batch] or NULL
+  double* mean;        // [batch][N] or NULL
+  double* var;         // [batch][N] or NULL
+  int want_smooth;
+};
+int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a);
+// arena helper
+int sg_arena(smolgp_ctx* ctx, size_t bytes, void** out);
