@@ -1,0 +1,179 @@
+// disc.cu -- step a2: per-event discretisation of every block of the augmented model.
+//
+// For a step of length Delta the augmented block [x_b; I_b] (I_b = int H_b x_b dt, Eq. 3.3-3.6,
+// P:365-381) needs Phi~ = exp(F~ Delta) = [Phi 0; Phi-bar 1] (Eq. 3.7) and
+// Q~ = int_0^Delta Phi~(s) L~ Qc L~^T Phi~(s)^T ds (Eq. 3.10).  The paper offers the
+// Van Loan block exponential (Eq. 3.9, B13) and warns that it is unstable over long gaps (P:193,
+// P:407) -- and the printed closed forms (B12, B19, B20) cancel catastrophically for short steps.
+// Here, per block and in the block's own O(1) units:
+//   1. h = Delta'' / 2^s with rho h <= 1/4: Phi~(h), Q~(h) by their Taylor series (Horner, the
+//      coefficients F~^k/k!, Gamma_k/k! are host-built constants) -- exact to rounding, no cancellation;
+//   2. s doublings  Q~(2h) = Q~(h) + Phi~(h) Q~(h) Phi~(h)^T,  Phi-bar(2h) = Phi-bar(h) (Phi(h) + I)
+//      (sums of PSD terms; no growing exponential ever appears), where Phi(h) at every level is the
+//      CLOSED FORM of the family (B10, and its Matern analogues) instead of a repeated
+//      square, so the error grows like s eps, not 2^s eps;
+//   3. Phi(Delta) itself from the closed form.
+// One thread per (event, block); output record layout in common.h.
+#include "common.h"
+
+template <int DB>
+__device__ __forceinline__ void phi_closed(const BlockConst& B, double h, double (&P)[DB][DB]);
+
+template <>
+__device__ __forceinline__ void phi_closed<2>(const BlockConst& B, double h, double (&P)[2][2]) {
+  if (B.family == BLK_M32 || (B.family == BLK_SHO && B.sho_case == 1)) {
+    // repeated root -1:  e^{-h} (I + h (F + I)),  F + I = [1 1; -1 -1]   (B10 with Q = 1/2)
+    const double e = exp(-h);
+    P[0][0] = e * (1.0 + h); P[0][1] = e * h; P[1][0] = -e * h; P[1][1] = e * (1.0 - h);
+  } else if (B.sho_case == 0) {
+    // underdamped: e^{-a h} [cos(b h) I + sin(b h)/b (F + a I)],  F + a I = [a 1; -1 -a]   (B10)
+    const double e = exp(-B.a * h);
+    double sn, cs;
+    sincos(B.b * h, &sn, &cs);
+    const double sb = sn / B.b;
+    P[0][0] = e * (cs + B.a * sb); P[0][1] = e * sb; P[1][0] = -e * sb; P[1][1] = e * (cs - B.a * sb);
+  } else {
+    // overdamped: cos -> cosh, sin/b -> sinh/beta, with the decaying exponentials combined
+    const double e1 = exp(-(B.a - B.b) * h), e2 = exp(-(B.a + B.b) * h);
+    const double ch = 0.5 * (e1 + e2), sb = 0.5 * (e1 - e2) / B.b;
+    P[0][0] = ch + B.a * sb; P[0][1] = sb; P[1][0] = -sb; P[1][1] = ch - B.a * sb;
+  }
+}
+template <>
+__device__ __forceinline__ void phi_closed<3>(const BlockConst& B, double h, double (&P)[3][3]) {
+  // triple root -1:  e^{-h} (I + h N + h^2/2 N^2),  N = F + I = [1 1 0; 0 1 1; -1 -3 -2]
+  const double e = exp(-h), h2 = 0.5 * h * h;
+  // N^2 = [1 2 1; -1 -2 -1; 1 2 1]
+  P[0][0] = e * (1.0 + h + h2);  P[0][1] = e * (h + 2.0 * h2);        P[0][2] = e * h2;
+  P[1][0] = e * (-h2);           P[1][1] = e * (1.0 + h - 2.0 * h2);  P[1][2] = e * (h - h2);
+  P[2][0] = e * (-h + h2);       P[2][1] = e * (-3.0 * h + 2.0 * h2); P[2][2] = e * (1.0 - 2.0 * h + h2);
+}
+template <>
+__device__ __forceinline__ void phi_closed<4>(const BlockConst& B, double h, double (&P)[4][4]) {
+  // Phi_M32(h) (x) R(omega h)   (C7: the transition of a product is the Kronecker product)
+  const double e = exp(-h);
+  const double M[2][2] = {{e * (1.0 + h), e * h}, {-e * h, e * (1.0 - h)}};
+  double sn, cs;
+  sincos(B.b * h, &sn, &cs);
+  const double R[2][2] = {{cs, -sn}, {sn, cs}};
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+      for (int a2 = 0; a2 < 2; ++a2)
+#pragma unroll
+        for (int c2 = 0; c2 < 2; ++c2) P[2 * a + c][2 * a2 + c2] = M[a][a2] * R[c][c2];
+}
+
+template <int DB>
+__device__ void disc_block(const BlockConst& B, double dts, double* __restrict__ out) {
+  constexpr int M = DB + 1;
+  double h = dts;
+  int s = 0;
+  {
+    double x = B.rho * dts;
+    while (x > 0.25 && s < 64) { x *= 0.5; h *= 0.5; ++s; }
+  }
+  double A[M][M], Q[M][M];
+#pragma unroll
+  for (int i = 0; i < M; ++i)
+#pragma unroll
+    for (int j = 0; j < M; ++j) { A[i][j] = B.tayA[SG_KT][i * SG_BE + j]; Q[i][j] = B.tayQ[SG_KT][i * SG_BE + j]; }
+  for (int k = SG_KT - 1; k >= 0; --k) {
+#pragma unroll
+    for (int i = 0; i < M; ++i)
+#pragma unroll
+      for (int j = 0; j < M; ++j) {
+        A[i][j] = fma(A[i][j], h, B.tayA[k][i * SG_BE + j]);
+        Q[i][j] = fma(Q[i][j], h, B.tayQ[k][i * SG_BE + j]);
+      }
+  }
+  for (int lev = 0; lev < s; ++lev) {
+    if (lev > 0) {
+      double P[DB][DB];
+      phi_closed<DB>(B, h, P);
+#pragma unroll
+      for (int i = 0; i < DB; ++i)
+#pragma unroll
+        for (int j = 0; j < DB; ++j) A[i][j] = P[i][j];
+    }
+    double T[M][M];
+#pragma unroll
+    for (int i = 0; i < M; ++i)
+#pragma unroll
+      for (int j = 0; j < M; ++j) {
+        double acc = 0.0;
+#pragma unroll
+        for (int l = 0; l < M; ++l) acc = fma(A[i][l], Q[l][j], acc);
+        T[i][j] = acc;
+      }
+#pragma unroll
+    for (int i = 0; i < M; ++i)
+#pragma unroll
+      for (int j = 0; j <= i; ++j) {
+        double acc = Q[i][j];
+#pragma unroll
+        for (int l = 0; l < M; ++l) acc = fma(T[i][l], A[j][l], acc);
+        Q[i][j] = acc;
+      }
+#pragma unroll
+    for (int i = 0; i < M; ++i)
+#pragma unroll
+      for (int j = i + 1; j < M; ++j) Q[i][j] = Q[j][i];
+    double pb[DB];
+#pragma unroll
+    for (int c = 0; c < DB; ++c) {
+      double acc = A[DB][c];
+#pragma unroll
+      for (int l = 0; l < DB; ++l) acc = fma(A[DB][l], A[l][c], acc);
+      pb[c] = acc;
+    }
+#pragma unroll
+    for (int c = 0; c < DB; ++c) A[DB][c] = pb[c];
+    h *= 2.0;
+  }
+  if (s > 0) {
+    double P[DB][DB];
+    phi_closed<DB>(B, dts, P);
+#pragma unroll
+    for (int i = 0; i < DB; ++i)
+#pragma unroll
+      for (int j = 0; j < DB; ++j) A[i][j] = P[i][j];
+  }
+  // record: Phi | phibar | Qxx | q12 | q22
+#pragma unroll
+  for (int i = 0; i < DB; ++i)
+#pragma unroll
+    for (int j = 0; j < DB; ++j) { out[i * DB + j] = A[i][j]; out[DB * DB + DB + i * DB + j] = Q[i][j]; }
+#pragma unroll
+  for (int j = 0; j < DB; ++j) { out[DB * DB + j] = A[DB][j]; out[2 * DB * DB + DB + j] = Q[DB][j]; }
+  out[2 * DB * DB + 2 * DB] = Q[DB][DB];
+}
+
+__global__ void __launch_bounds__(128) k_disc(const ModelDev* __restrict__ Mp, const double* __restrict__ dt, int64_t K,
+                                              double* __restrict__ disc) {
+  const int nblk = Mp->nblk;
+  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= K * nblk) return;
+  const int64_t k = gid / nblk;
+  const int b = (int)(gid - k * nblk);
+  const BlockConst& B = Mp->blk[b];
+  const double dts = dt[k] * B.inv_T;
+  double* out = disc + k * (int64_t)Mp->disc_stride + Mp->disc_off[b];
+  switch (B.dim) {
+    case 2: disc_block<2>(B, dts, out); break;
+    case 3: disc_block<3>(B, dts, out); break;
+    default: disc_block<4>(B, dts, out); break;
+  }
+}
+
+int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_model, const double* dt,
+                   int64_t K, double* disc) {
+  const int64_t total = K * h_model->nblk;
+  const int64_t blocks = (total + 127) / 128;
+  k_disc<<<(unsigned)blocks, 128, 0, ctx->stream>>>(d_model, dt, K, disc);
+  ctx->launches++;
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
+}

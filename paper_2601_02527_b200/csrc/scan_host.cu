@@ -1,0 +1,160 @@
+// scan_host.cu -- host orchestration of the scan kernels (level plan, workspace carving, launches).
+// Included at the end of scan.cu (same translation unit as the kernels it launches).
+
+struct LevelPlan {
+  int T;                // number of dense levels (0 = single chunk per series)
+  int64_t cnt[40];      // cnt[l] = elements per series at level l (l = 1..T)
+};
+
+static int pick_lanes(const smolgp_ctx* ctx, int n) {
+  if (ctx->opt_lanes == 8 || ctx->opt_lanes == 16 || ctx->opt_lanes == 32) return (int)ctx->opt_lanes;
+  return n <= 4 ? 8 : (n <= 8 ? 16 : 32);
+}
+
+template <int G>
+static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, int n, size_t tb, bool fold) {
+  const int gd = fold ? fold0_group_doubles(n) : down0_group_doubles(n);
+  const size_t per_group = (size_t)gd * 8;
+  // groups per CTA: as many as fit in ~100 KB (two CTAs per SM), at most 128 threads
+  int gpc = 128 / G;
+  while (gpc > 1 && tb + per_group * gpc > 100 * 1024) gpc >>= 1;
+  const size_t smem = tb + per_group * gpc;
+  if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+  const int64_t groups = P.batch * P.c1;
+  const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
+  if (fold) {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fold0<G><<<blocks, gpc * G, smem, ctx->stream>>>(P);
+  } else {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_down0<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_down0<G><<<blocks, gpc * G, smem, ctx->stream>>>(P);
+  }
+  ctx->launches++;
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
+}
+
+static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, int n, size_t tb, bool fold, int G) {
+  switch (G) {
+    case 8: return launch_level0<8>(ctx, P, n, tb, fold);
+    case 16: return launch_level0<16>(ctx, P, n, tb, fold);
+    default: return launch_level0<32>(ctx, P, n, tb, fold);
+  }
+}
+
+static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, size_t tb, bool fold) {
+  const int gd = fold ? foldD_group_doubles(n) : downD_group_doubles(n);
+  const size_t per_group = (size_t)gd * 8;
+  int gpc = 2;
+  while (gpc > 1 && tb + per_group * gpc > 110 * 1024) gpc >>= 1;
+  const size_t smem = tb + per_group * gpc;
+  if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+  const int64_t groups = D.batch * D.cout;
+  dim3 grid((unsigned)((groups + gpc - 1) / gpc), fold ? 1 : (D.want_suffix ? 2 : 1));
+  if (fold) {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_foldD<<<grid, gpc * 32, smem, ctx->stream>>>(D);
+  } else {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_downD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_downD<<<grid, gpc * 32, smem, ctx->stream>>>(D);
+  }
+  ctx->launches++;
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
+}
+
+int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
+  const ModelDev* hm = a.h_model;
+  const int n = hm->n;
+  const int64_t K = a.ev->K, N = a.ev->N, batch = a.batch;
+  int nent = 0;
+  for (int b = 0; b < hm->nblk; ++b) nent += hm->blk[b].dim * hm->blk[b].dim;
+  const size_t tb = tables_bytes(n, hm->d, hm->n_inst, hm->nblk, nent);
+  const int G = pick_lanes(ctx, n);
+  const int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 8;
+
+  // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
+  // already fills it runs one chunk per series (the sequential filter)
+  int64_t Lc = ctx->opt_chunk;
+  if (Lc <= 0) {
+    const size_t per_group = (size_t)down0_group_doubles(n) * 8;
+    int64_t resident = (int64_t)ctx->sm_count * (int64_t)((200 * 1024) / (per_group ? per_group : 1));
+    const int64_t cap = (int64_t)ctx->sm_count * 64 * (32 / G);
+    if (resident > cap) resident = cap;
+    if (resident < ctx->sm_count) resident = ctx->sm_count;
+    const int64_t target = 2 * resident;
+    if (batch >= target) Lc = K;
+    else {
+      Lc = (batch * K + target - 1) / target;
+      if (Lc < 16) Lc = 16;
+      if (Lc > 512) Lc = 512;
+    }
+  }
+  if (Lc > K) Lc = K;
+  if (Lc < 2) Lc = 2;
+  LevelPlan pl;
+  pl.T = 0;
+  const int64_t c1 = (K + Lc - 1) / Lc;
+  if (c1 > 1) {
+    pl.T = 1;
+    pl.cnt[1] = c1;
+    while (pl.cnt[pl.T] > g) { pl.cnt[pl.T + 1] = (pl.cnt[pl.T] + g - 1) / g; pl.T++; }
+  }
+  const int es = elem_size(n), ss = state_size(n);
+  // workspace
+  size_t bytes = 256;
+  auto add = [&](size_t b) { size_t o = bytes; bytes += (b + 255) / 256 * 256; return o; };
+  size_t oE[40], oPRE[40], oSUF[40];
+  for (int l = 1; l <= pl.T; ++l) {
+    oE[l] = add((size_t)batch * pl.cnt[l] * es * 8);
+    oPRE[l] = add((size_t)batch * pl.cnt[l] * ss * 8);
+    oSUF[l] = a.want_smooth ? add((size_t)batch * pl.cnt[l] * ss * 8) : 0;
+  }
+  const size_t oX = a.want_smooth ? add((size_t)batch * N * ss * 8) : 0;
+  const size_t oLL = add((size_t)batch * c1 * 8);
+  void* ws;
+  int rc = sg_arena(ctx, bytes, &ws);
+  if (rc) return rc;
+  char* w = (char*)ws;
+
+  ScanDev P;
+  P.M = a.d_model; P.disc = a.disc; P.dt = a.ev->dt; P.delta = a.ev->delta; P.meta = a.ev->meta; P.obs = a.ev->obs;
+  P.y = a.y; P.sigma = a.sigma; P.amp = a.amp; P.K = K; P.N = N; P.batch = batch; P.Lc = (int)Lc; P.c1 = c1;
+  P.E1 = pl.T ? (double*)(w + oE[1]) : nullptr;
+  P.PRE1 = pl.T ? (const double*)(w + oPRE[1]) : nullptr;
+  P.SUF1 = (pl.T && a.want_smooth) ? (const double*)(w + oSUF[1]) : nullptr;
+  P.xbuf = a.want_smooth ? (double*)(w + oX) : nullptr;
+  P.llpart = (double*)(w + oLL);
+  P.mean = a.mean; P.var = a.var; P.flags = ctx->d_flags; P.want_smooth = a.want_smooth;
+
+  if (pl.T) {
+    rc = launch_level0_any(ctx, P, n, tb, true, G);
+    if (rc) return rc;
+    for (int l = 1; l < pl.T; ++l) {
+      DenseArgs D = {};
+      D.M = a.d_model; D.Ein = (const double*)(w + oE[l]); D.Eout = (double*)(w + oE[l + 1]);
+      D.cin = pl.cnt[l]; D.cout = pl.cnt[l + 1]; D.batch = batch; D.g = g;
+      rc = launch_dense(ctx, D, n, tb, true);
+      if (rc) return rc;
+    }
+    for (int l = pl.T; l >= 1; --l) {
+      DenseArgs D = {};
+      D.M = a.d_model; D.Ein = (const double*)(w + oE[l]); D.cin = pl.cnt[l]; D.batch = batch;
+      D.want_suffix = a.want_smooth;
+      if (l == pl.T) { D.cout = 1; D.g = (int)pl.cnt[l]; D.PREup = nullptr; D.SUFup = nullptr; }
+      else { D.cout = pl.cnt[l + 1]; D.g = g; D.PREup = (const double*)(w + oPRE[l + 1]); D.SUFup = a.want_smooth ? (const double*)(w + oSUF[l + 1]) : nullptr; }
+      D.PRE = (double*)(w + oPRE[l]); D.SUF = a.want_smooth ? (double*)(w + oSUF[l]) : nullptr;
+      rc = launch_dense(ctx, D, n, tb, false);
+      if (rc) return rc;
+    }
+  }
+  rc = launch_level0_any(ctx, P, n, tb, false, G);
+  if (rc) return rc;
+  if (a.loglik) {
+    const int wpb = 4;
+    k_ll_reduce<<<(unsigned)((batch + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(P.llpart, c1, batch, N, a.amp, a.loglik);
+    ctx->launches++;
+    SG_CUDA(ctx, cudaGetLastError());
+  }
+  return SMOLGP_OK;
+}
