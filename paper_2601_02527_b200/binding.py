@@ -1,0 +1,229 @@
+"""Thin ctypes binding of libsmolgp_b200.so (include/smolgp.h).  Argument marshalling only: every
+step of the path runs inside the CUDA library.  Device entry points take torch CUDA tensors (torch
+is used for device memory and streams, nothing else); *_host entry points take numpy arrays.
+There is no CPU fallback: loading fails loudly when the library is missing or cannot be built."""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import _build
+
+MATERN32, MATERN52, SHO, MATERN32_X_PERIODIC = 0, 1, 2, 3
+STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM", -5: "ECUDA", -6: "ENUMERIC"}
+EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
+           "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
+           "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
+           "smolgp_launch_count", "smolgp_probe_fp64"]
+
+
+class SmolgpError(RuntimeError):
+    def __init__(self, rc, msg):
+        super().__init__("smolgp: %s (%d): %s" % (STATUS.get(rc, "?"), rc, msg))
+        self.rc = rc
+
+
+class _Comp(C.Structure):
+    _fields_ = [("family", C.c_int32), ("order", C.c_int32), ("inst_mask", C.c_uint32), ("sigma", C.c_double),
+                ("p0", C.c_double), ("p1", C.c_double), ("p2", C.c_double)]
+
+
+class _Kernel(C.Structure):
+    _fields_ = [("n_comp", C.c_int32), ("comp", C.POINTER(_Comp))]
+
+
+_lib = None
+
+
+def lib():
+    """Loads (building if stale) the shared library.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        so = _build.build()
+        L = C.CDLL(so)
+        vp, i64, i32, dp = C.c_void_p, C.c_int64, C.c_int32, C.c_void_p
+        L.smolgp_create.argtypes = [C.POINTER(vp), C.c_int, vp]
+        L.smolgp_destroy.argtypes = [vp]
+        L.smolgp_destroy.restype = None
+        L.smolgp_last_error.argtypes = [vp]
+        L.smolgp_last_error.restype = C.c_char_p
+        L.smolgp_set_option.argtypes = [vp, C.c_char_p, i64]
+        for f in (L.smolgp_build_events, L.smolgp_build_events_host):
+            f.argtypes = [vp, i64, dp, dp, dp, i32, C.POINTER(vp)]
+        L.smolgp_free_events.argtypes = [vp]
+        L.smolgp_free_events.restype = None
+        L.smolgp_events_export.argtypes = [vp, vp, dp, dp, dp, dp]
+        for f in (L.smolgp_loglik, L.smolgp_loglik_host):
+            f.argtypes = [vp, vp, C.POINTER(_Kernel), i64, dp, dp, dp, dp]
+        for f in (L.smolgp_condition, L.smolgp_condition_host):
+            f.argtypes = [vp, vp, C.POINTER(_Kernel), i64, dp, dp, dp, i64, dp, i32, dp, dp, dp, dp, dp]
+        L.smolgp_discretise_host.argtypes = [vp, C.POINTER(_Kernel), i32, C.c_double, dp, dp, C.POINTER(i32)]
+        L.smolgp_launch_count.argtypes = [vp]
+        L.smolgp_launch_count.restype = i64
+        L.smolgp_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
+        _lib = L
+    return _lib
+
+
+def _kernel(kernel):
+    arr = (_Comp * len(kernel))()
+    for i, k in enumerate(kernel):
+        arr[i] = _Comp(int(k["family"]), int(k.get("order", 0)), int(k["inst_mask"]) & 0xFFFFFFFF, float(k["sigma"]),
+                       float(k.get("p0", 0.0)), float(k.get("p1", 0.0)), float(k.get("p2", 0.0)))
+    return _Kernel(len(kernel), arr), arr
+
+
+def _dptr(t):
+    """device pointer of a contiguous torch CUDA tensor (None -> NULL)"""
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "expected a contiguous CUDA tensor"
+    return t.data_ptr()
+
+
+def _hptr(a):
+    return None if a is None else a.ctypes.data
+
+
+class Events:
+    def __init__(self, ctx, handle, N, n_inst):
+        self.ctx, self.handle, self.N, self.n_inst = ctx, handle, N, n_inst
+
+    def export(self):
+        K = 2 * self.N
+        t = np.empty(K)
+        kind, inst, idx = (np.empty(K, dtype=np.int32) for _ in range(3))
+        self.ctx._check(lib().smolgp_events_export(self.ctx.handle, self.handle, _hptr(t), _hptr(kind), _hptr(inst), _hptr(idx)))
+        return t, kind, inst, idx
+
+    def free(self):
+        if self.handle:
+            lib().smolgp_free_events(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Context:
+    """smolgp_ctx.  stream: a torch.cuda.Stream or None (default stream)."""
+
+    def __init__(self, device=0, stream=None):
+        h = C.c_void_p()
+        sp = None if stream is None else C.c_void_p(stream.cuda_stream)
+        rc = lib().smolgp_create(C.byref(h), int(device), sp)
+        if rc != 0:
+            raise SmolgpError(rc, "smolgp_create failed (no CUDA device?)")
+        self.handle = h
+        self.device = device
+
+    def _check(self, rc):
+        if rc != 0:
+            raise SmolgpError(rc, lib().smolgp_last_error(self.handle).decode())
+
+    def set_option(self, name, value):
+        self._check(lib().smolgp_set_option(self.handle, name.encode(), int(value)))
+
+    def launch_count(self):
+        return int(lib().smolgp_launch_count(self.handle))
+
+    def probe_fp64(self):
+        v = C.c_double()
+        self._check(lib().smolgp_probe_fp64(self.handle, C.byref(v)))
+        return v.value
+
+    # ---- a1 ----
+    def smolgp_build_events(self, t_start, t_end, instrument, n_inst):
+        """device tensors: t_start, t_end float64 [N]; instrument int32 [N]"""
+        N = t_start.numel()
+        h = C.c_void_p()
+        self._check(lib().smolgp_build_events(self.handle, N, _dptr(t_start), _dptr(t_end), _dptr(instrument), int(n_inst), C.byref(h)))
+        return Events(self, h, N, n_inst)
+
+    def smolgp_build_events_host(self, t_start, t_end, instrument, n_inst):
+        ts, te = np.ascontiguousarray(t_start, np.float64), np.ascontiguousarray(t_end, np.float64)
+        ins = np.ascontiguousarray(instrument, np.int32)
+        h = C.c_void_p()
+        self._check(lib().smolgp_build_events_host(self.handle, ts.size, _hptr(ts), _hptr(te), _hptr(ins), int(n_inst), C.byref(h)))
+        return Events(self, h, ts.size, n_inst)
+
+    # ---- a2-a5 ----
+    def smolgp_loglik(self, ev, kernel, y, noise_sigma, amp=None, out=None):
+        import torch
+        batch = 1 if y.dim() == 1 else y.shape[0]
+        if out is None:
+            out = torch.empty(batch, dtype=torch.float64, device=y.device)
+        k, keep = _kernel(kernel)
+        self._check(lib().smolgp_loglik(self.handle, ev.handle, C.byref(k), batch, _dptr(y), _dptr(noise_sigma), _dptr(amp), _dptr(out)))
+        return out
+
+    def smolgp_loglik_host(self, ev, kernel, y, noise_sigma, amp=None):
+        y = np.ascontiguousarray(y, np.float64)
+        batch = 1 if y.ndim == 1 else y.shape[0]
+        sg = np.ascontiguousarray(noise_sigma, np.float64)
+        am = None if amp is None else np.ascontiguousarray(amp, np.float64)
+        out = np.empty(batch)
+        k, keep = _kernel(kernel)
+        self._check(lib().smolgp_loglik_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y), _hptr(sg), _hptr(am), _hptr(out)))
+        return out
+
+    # ---- a2-a7 ----
+    def smolgp_condition(self, ev, kernel, y, noise_sigma, amp=None, t_query=None, query_instrument=0, out=None):
+        """returns dict(mean, var, loglik[, mean_query, var_query]) of device tensors"""
+        import torch
+        batch = 1 if y.dim() == 1 else y.shape[0]
+        N = ev.N
+        if out is None:
+            out = dict(mean=torch.empty((batch, N), dtype=torch.float64, device=y.device),
+                       var=torch.empty((batch, N), dtype=torch.float64, device=y.device),
+                       loglik=torch.empty(batch, dtype=torch.float64, device=y.device))
+        M = 0 if t_query is None else t_query.numel()
+        if M and "mean_query" not in out:
+            out["mean_query"] = torch.empty((batch, M), dtype=torch.float64, device=y.device)
+            out["var_query"] = torch.empty((batch, M), dtype=torch.float64, device=y.device)
+        k, keep = _kernel(kernel)
+        self._check(lib().smolgp_condition(self.handle, ev.handle, C.byref(k), batch, _dptr(y), _dptr(noise_sigma), _dptr(amp),
+                                           M, _dptr(t_query), int(query_instrument), _dptr(out["mean"]), _dptr(out["var"]),
+                                           _dptr(out.get("mean_query")), _dptr(out.get("var_query")), _dptr(out["loglik"])))
+        return out
+
+    def smolgp_condition_host(self, ev, kernel, y, noise_sigma, amp=None, t_query=None, query_instrument=0, out=None):
+        y = np.ascontiguousarray(y, np.float64)
+        batch = 1 if y.ndim == 1 else y.shape[0]
+        N = ev.N
+        sg = np.ascontiguousarray(noise_sigma, np.float64)
+        am = None if amp is None else np.ascontiguousarray(amp, np.float64)
+        tq = None if t_query is None else np.ascontiguousarray(t_query, np.float64)
+        M = 0 if tq is None else tq.size
+        if out is None:
+            out = dict(mean=np.empty((batch, N)), var=np.empty((batch, N)), loglik=np.empty(batch))
+            if M:
+                out["mean_query"], out["var_query"] = np.empty((batch, M)), np.empty((batch, M))
+        k, keep = _kernel(kernel)
+        self._check(lib().smolgp_condition_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y), _hptr(sg), _hptr(am), M,
+                                                _hptr(tq), int(query_instrument), _hptr(out["mean"]), _hptr(out["var"]),
+                                                _hptr(out.get("mean_query")), _hptr(out.get("var_query")), _hptr(out["loglik"])))
+        return out
+
+    def smolgp_discretise_host(self, kernel, n_inst, dt):
+        k, keep = _kernel(kernel)
+        n = C.c_int32()
+        A = np.zeros((32, 32))
+        Q = np.zeros((32, 32))
+        self._check(lib().smolgp_discretise_host(self.handle, C.byref(k), int(n_inst), float(dt), _hptr(A), _hptr(Q), C.byref(n)))
+        nn = n.value
+        return A.ravel()[:nn * nn].reshape(nn, nn).copy(), Q.ravel()[:nn * nn].reshape(nn, nn).copy()
+
+    def close(self):
+        if self.handle:
+            lib().smolgp_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,291 @@
+// api.cu -- the C ABI of include/smolgp.h: context, workspace, and the entry points that chain
+// discretisation (disc.cu) and the scans (scan.cu).  No CPU fallback anywhere: every entry point
+// needs a CUDA device and fails with SMOLGP_ECUDA without one.
+#include <math.h>
+#include <string.h>
+
+#include "common.h"
+
+int sg_arena(smolgp_ctx* ctx, size_t bytes, void** out) {
+  if (bytes > ctx->arena_bytes) {
+    if (ctx->arena) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->arena); ctx->arena = nullptr; ctx->arena_bytes = 0; }
+    size_t want = bytes + bytes / 8;
+    if (cudaMalloc(&ctx->arena, want) != cudaSuccess) {
+      cudaGetLastError();
+      want = bytes;
+      if (cudaMalloc(&ctx->arena, want) != cudaSuccess) { cudaGetLastError(); ctx->arena = nullptr; ctx->err = "out of device memory (workspace)"; return SMOLGP_ENOMEM; }
+    }
+    ctx->arena_bytes = want;
+  }
+  *out = ctx->arena;
+  return SMOLGP_OK;
+}
+
+extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
+  if (!out) return SMOLGP_EINVAL;
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return SMOLGP_ECUDA; }
+  if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
+  smolgp_ctx* c = new smolgp_ctx();
+  c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0;
+  c->opt_chunk = 0; c->opt_group = 8; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = new ModelDev();
+  int v = 0;
+  cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device); c->sm_count = v;
+  cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device); c->smem_optin = (size_t)v;
+  if (cudaMalloc(&c->d_flags, 64) != cudaSuccess) { cudaGetLastError(); delete c->hmodel; delete c; return SMOLGP_ENOMEM; }
+  cudaMemset(c->d_flags, 0, 64);
+  *out = c;
+  return SMOLGP_OK;
+}
+
+extern "C" void smolgp_destroy(smolgp_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->device);
+  cudaStreamSynchronize(ctx->stream);
+  cudaFree(ctx->arena);
+  cudaFree(ctx->pers);
+  cudaFree(ctx->d_flags);
+  delete ctx->hmodel;
+  delete ctx;
+}
+
+extern "C" const char* smolgp_last_error(const smolgp_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+extern "C" int64_t smolgp_launch_count(const smolgp_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value) {
+  if (!ctx || !name) return SMOLGP_EINVAL;
+  if (!strcmp(name, "chunk")) ctx->opt_chunk = value;
+  else if (!strcmp(name, "group")) ctx->opt_group = value;
+  else if (!strcmp(name, "lanes")) ctx->opt_lanes = value;
+  else { ctx->err = std::string("unknown option ") + name; return SMOLGP_EINVAL; }
+  return SMOLGP_OK;
+}
+
+// validation of sigma > 0 happens on the device inside the filter (S > 0 check) and here for amp
+static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                    const double* y, const double* sigma, const double* amp, double* mean, double* var,
+                    double* loglik, int want_smooth) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (!ev || !kernel || !y || !sigma || batch <= 0) { ctx->err = "null or empty argument"; return SMOLGP_EINVAL; }
+  if (want_smooth && (!mean || !var)) { ctx->err = "condition: mean_obs and var_obs are required"; return SMOLGP_EINVAL; }
+  if (!want_smooth && !loglik) { ctx->err = "loglik: output pointer is null"; return SMOLGP_EINVAL; }
+  if (ev->device != ctx->device) { ctx->err = "events belong to another device"; return SMOLGP_EINVAL; }
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  ModelDev& hm = *ctx->hmodel;
+  int rc = sg_build_model(ctx, kernel, ev->n_inst, ev->tau, &hm);
+  if (rc) return rc;
+  const size_t model_b = (sizeof(ModelDev) + 255) / 256 * 256;
+  const size_t disc_b = ((size_t)ev->K * hm.disc_stride * 8 + 255) / 256 * 256;
+  if (ctx->pers_bytes < model_b + disc_b) {
+    if (ctx->pers) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->pers); ctx->pers = nullptr; ctx->pers_bytes = 0; }
+    if (cudaMalloc(&ctx->pers, model_b + disc_b) != cudaSuccess) { cudaGetLastError(); ctx->pers = nullptr; ctx->err = "out of device memory (discretisation)"; return SMOLGP_ENOMEM; }
+    ctx->pers_bytes = model_b + disc_b;
+  }
+  void* pers = ctx->pers;
+  ModelDev* dm = (ModelDev*)pers;
+  double* disc = (double*)((char*)pers + model_b);
+  SG_CUDA(ctx, cudaMemcpyAsync(dm, &hm, sizeof(ModelDev), cudaMemcpyHostToDevice, ctx->stream));
+  SG_CUDA(ctx, cudaMemsetAsync(ctx->d_flags, 0, sizeof(int), ctx->stream));
+  rc = sg_launch_disc(ctx, dm, &hm, ev->dt, ev->K, disc);
+  if (rc) return rc;
+  ScanArgs a;
+  a.d_model = dm; a.h_model = &hm; a.ev = ev; a.disc = disc; a.batch = batch; a.y = y; a.sigma = sigma; a.amp = amp;
+  a.loglik = loglik; a.mean = mean; a.var = var; a.want_smooth = want_smooth;
+  rc = sg_run_scan(ctx, a);
+  if (rc) return rc;
+  int flags = 0;
+  SG_CUDA(ctx, cudaMemcpyAsync(&flags, ctx->d_flags, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+  SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  if (flags) { ctx->err = "non-finite value or non-positive innovation variance (check noise_sigma > 0, amp > 0, finite y)"; return SMOLGP_ENUMERIC; }
+  return SMOLGP_OK;
+}
+
+extern "C" int smolgp_loglik(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                             const double* y, const double* noise_sigma, const double* amp, double* loglik) {
+  return run_path(ctx, ev, kernel, batch, y, noise_sigma, amp, nullptr, nullptr, loglik, 0);
+}
+
+extern "C" int smolgp_condition(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                                const double* y, const double* noise_sigma, const double* amp, int64_t M,
+                                const double* t_query, int32_t query_instrument, double* mean_obs, double* var_obs,
+                                double* mean_query, double* var_query, double* loglik) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (M > 0) { ctx->err = "condition: query-time prediction (Algorithm 1) is not built yet"; return SMOLGP_EUNSUPPORTED; }
+  (void)t_query; (void)query_instrument; (void)mean_query; (void)var_query;
+  return run_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1);
+}
+
+// ---- host-pointer variants: copies inside the call, on the ctx stream -------------------------------
+struct HostStage {
+  double *y = nullptr, *sigma = nullptr, *amp = nullptr, *mean = nullptr, *var = nullptr, *ll = nullptr;
+  ~HostStage() { cudaFree(y); cudaFree(sigma); cudaFree(amp); cudaFree(mean); cudaFree(var); cudaFree(ll); }
+};
+
+static int host_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                     const double* y, const double* sigma, const double* amp, double* mean, double* var,
+                     double* loglik, int want_smooth) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (!ev || !y || !sigma || batch <= 0) { ctx->err = "null or empty argument"; return SMOLGP_EINVAL; }
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  const int64_t N = ev->N;
+  HostStage s;
+  const size_t bn = (size_t)batch * N * 8;
+  if (cudaMalloc(&s.y, bn) || cudaMalloc(&s.sigma, N * 8) || (amp && cudaMalloc(&s.amp, batch * 8)) ||
+      (want_smooth && (cudaMalloc(&s.mean, bn) || cudaMalloc(&s.var, bn))) || cudaMalloc(&s.ll, batch * 8)) {
+    cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM;
+  }
+  cudaStream_t st = ctx->stream;
+  SG_CUDA(ctx, cudaMemcpyAsync(s.y, y, bn, cudaMemcpyHostToDevice, st));
+  SG_CUDA(ctx, cudaMemcpyAsync(s.sigma, sigma, N * 8, cudaMemcpyHostToDevice, st));
+  if (amp) SG_CUDA(ctx, cudaMemcpyAsync(s.amp, amp, batch * 8, cudaMemcpyHostToDevice, st));
+  int rc = run_path(ctx, ev, kernel, batch, s.y, s.sigma, amp ? s.amp : nullptr, s.mean, s.var, s.ll, want_smooth);
+  if (rc) return rc;
+  if (want_smooth) {
+    SG_CUDA(ctx, cudaMemcpyAsync(mean, s.mean, bn, cudaMemcpyDeviceToHost, st));
+    SG_CUDA(ctx, cudaMemcpyAsync(var, s.var, bn, cudaMemcpyDeviceToHost, st));
+  }
+  if (loglik) SG_CUDA(ctx, cudaMemcpyAsync(loglik, s.ll, batch * 8, cudaMemcpyDeviceToHost, st));
+  SG_CUDA(ctx, cudaStreamSynchronize(st));
+  return SMOLGP_OK;
+}
+
+extern "C" int smolgp_loglik_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                                  const double* y, const double* noise_sigma, const double* amp, double* loglik) {
+  if (ctx && !loglik) { ctx->err = "loglik: output pointer is null"; return SMOLGP_EINVAL; }
+  return host_path(ctx, ev, kernel, batch, y, noise_sigma, amp, nullptr, nullptr, loglik, 0);
+}
+
+extern "C" int smolgp_condition_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                                     int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                                     int64_t M, const double* t_query, int32_t query_instrument, double* mean_obs,
+                                     double* var_obs, double* mean_query, double* var_query, double* loglik) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (M > 0) { ctx->err = "condition: query-time prediction (Algorithm 1) is not built yet"; return SMOLGP_EUNSUPPORTED; }
+  (void)t_query; (void)query_instrument; (void)mean_query; (void)var_query;
+  if (!mean_obs || !var_obs) { ctx->err = "condition: mean_obs and var_obs are required"; return SMOLGP_EINVAL; }
+  return host_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1);
+}
+
+// ---- step a2 alone (tests): A~ and Q~ of one step in raw state units ---------------------------------
+extern "C" int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kernel, int32_t n_inst, double dt,
+                                      double* A, double* Q, int32_t* n_out) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (!A || !Q || !(dt >= 0) || !isfinite(dt)) { ctx->err = "discretise: bad argument"; return SMOLGP_EINVAL; }
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  ModelDev& hm = *ctx->hmodel;
+  double tau[SG_MAXINST];
+  for (int q = 0; q < SG_MAXINST; ++q) tau[q] = 1.0;
+  int rc = sg_build_model(ctx, kernel, n_inst, tau, &hm);
+  if (rc) return rc;
+  const int n = hm.n, d = hm.d;
+  if (n_out) *n_out = n;
+  void* ws;
+  const size_t model_b = (sizeof(ModelDev) + 255) / 256 * 256;
+  rc = sg_arena(ctx, model_b + 256 + (size_t)hm.disc_stride * 8, &ws);
+  if (rc) return rc;
+  ModelDev* dm = (ModelDev*)ws;
+  double* ddt = (double*)((char*)ws + model_b);
+  double* drec = ddt + 32;
+  SG_CUDA(ctx, cudaMemcpyAsync(dm, &hm, sizeof(ModelDev), cudaMemcpyHostToDevice, ctx->stream));
+  SG_CUDA(ctx, cudaMemcpyAsync(ddt, &dt, 8, cudaMemcpyHostToDevice, ctx->stream));
+  rc = sg_launch_disc(ctx, dm, &hm, ddt, 1, drec);
+  if (rc) return rc;
+  std::vector<double> rec(hm.disc_stride);
+  SG_CUDA(ctx, cudaMemcpyAsync(rec.data(), drec, hm.disc_stride * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  // block units -> raw units: x_i = s_i x''_i with s = sigma_b lambda^(derivative order); z = tau z' (tau = 1).
+  // sigma_b / T-scale come back out of cz: cz[q][b] = sigma_b T_b / tau_q for instruments in the mask, so
+  // recompute the scales from the kernel description instead (mask-independent).
+  std::vector<double> sc(n, 1.0), sigb(hm.nblk, 0.0);
+  {
+    int b = 0;
+    for (int c = 0; c < kernel->n_comp; ++c) {
+      const smolgp_component& k = kernel->comp[c];
+      if (k.family == SMOLGP_MATERN32_X_PERIODIC) {
+        const long double x = 1.0L / ((long double)k.p2 * k.p2);
+        for (int j = 0; j <= k.order; ++j) {
+          long double term = 1.0L;
+          for (int m = 1; m <= j; ++m) term *= (x / 2) / m;
+          long double sum = term;
+          for (int m = 1; m < 80; ++m) { term *= (x / 2) * (x / 2) / ((long double)m * (m + j)); sum += term; }
+          sigb[b++] = (double)(k.sigma * sqrtl((j == 0 ? 1.0L : 2.0L) * sum * expl(-x)));
+        }
+      } else sigb[b++] = k.sigma;
+    }
+  }
+  for (int b = 0; b < hm.nblk; ++b) {
+    const BlockConst& B = hm.blk[b];
+    for (int i = 0; i < B.dim; ++i) {
+      const int order = (B.family == BLK_M32ROT) ? i / 2 : i;
+      sc[B.off + i] = sigb[b] * pow(B.inv_T, order);
+    }
+  }
+  for (int i = 0; i < n * n; ++i) { A[i] = 0; Q[i] = 0; }
+  for (int b = 0; b < hm.nblk; ++b) {
+    const BlockConst& B = hm.blk[b];
+    const int db = B.dim, o = B.off;
+    const double* r = rec.data() + hm.disc_off[b];
+    const double Tb = 1.0 / B.inv_T;
+    for (int i = 0; i < db; ++i)
+      for (int j = 0; j < db; ++j) {
+        A[(o + i) * n + o + j] = sc[o + i] * r[i * db + j] / sc[o + j];
+        Q[(o + i) * n + o + j] = sc[o + i] * r[db * db + db + i * db + j] * sc[o + j];
+      }
+    for (int q = 0; q < n_inst; ++q) {
+      if (hm.cz[q][b] == 0.0) continue;
+      const double c = sigb[b] * Tb; // I = sigma_b T_b I''
+      for (int j = 0; j < db; ++j) {
+        A[(d + q) * n + o + j] = c * r[db * db + j] / sc[o + j];
+        const double v = c * r[2 * db * db + db + j] * sc[o + j];
+        Q[(d + q) * n + o + j] = v;
+        Q[(o + j) * n + d + q] = v;
+      }
+      for (int q2 = 0; q2 < n_inst; ++q2)
+        if (hm.cz[q2][b] != 0.0) Q[(d + q) * n + d + q2] += c * c * r[2 * db * db + 2 * db];
+    }
+  }
+  for (int q = 0; q < n_inst; ++q) A[(d + q) * n + d + q] = 1.0;
+  return SMOLGP_OK;
+}
+
+// ---- FP64 FMA probe --------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_probe_dfma(double* out, int iters) {
+  double a0 = threadIdx.x * 1e-3, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999, c = 1e-9;
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) out[0] = s;
+}
+
+extern "C" int smolgp_probe_fp64(smolgp_ctx* ctx, double* tflops) {
+  if (!ctx || !tflops) return SMOLGP_EINVAL;
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  void* ws;
+  int rc = sg_arena(ctx, 256, &ws);
+  if (rc) return rc;
+  const int iters = 1 << 15, blocks = ctx->sm_count * 8, threads = 256;
+  cudaEvent_t e0, e1;
+  SG_CUDA(ctx, cudaEventCreate(&e0));
+  SG_CUDA(ctx, cudaEventCreate(&e1));
+  k_probe_dfma<<<blocks, threads, 0, ctx->stream>>>((double*)ws, iters / 8);
+  float best = 1e30f;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(e0, ctx->stream);
+    k_probe_dfma<<<blocks, threads, 0, ctx->stream>>>((double*)ws, iters);
+    cudaEventRecord(e1, ctx->stream);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  ctx->launches += 4;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  SG_CUDA(ctx, cudaGetLastError());
+  *tflops = 2.0 * 8.0 * (double)iters * blocks * threads / (best * 1e-3) / 1e12;
+  return SMOLGP_OK;
+}

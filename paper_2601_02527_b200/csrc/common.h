@@ -79,6 +79,9 @@ struct smolgp_ctx {
   void* arena;
   size_t arena_bytes;
   int* d_flags; // device status word(s)
+  void* pers;   // model + discretisation array of the current call (kept across calls)
+  size_t pers_bytes;
+  ModelDev* hmodel; // host copy of the current model
   int sm_count;
   size_t smem_optin;
 };
