@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- events/sec of the whole hot path (event build, discretisation,
+filter scan, smoother, log-likelihood, posterior at the observations) on BASELINE.json's headline
+workload: config 3 (quasiperiodic kernel, n = 21, N = 100 000 exposures, K = 200 000 events, fp64).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3]
+
+One JSON line on stdout (rank 0).  `value` = events/s with inputs resident in HBM; `e2e` = the same
+through the *_host C-ABI calls from pinned host buffers (copies inside the timed region).  Under
+torchrun (N > 1) every rank runs an independent replica of the workload on its own GPU (the path
+does not shard: DESIGN.md "Multi-GPU": replicas only, no collective) and `value` is the aggregate.
+`--impl reference` times the CPU oracle (oracle/, fp64 build) on a bounded sample of the workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2601_02527_b200 import workloads as W  # noqa: E402
+
+FP64_PEAK_TFLOPS = 37.2  # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz
+
+
+def w_useful_flops(n):
+    """dense flop count of the sequential algorithm per event (predict + update +
+    smoother gain/update): 10.3 n^3 + 9 n^2."""
+    return 10.3 * n ** 3 + 9.0 * n ** 2
+
+
+def min_bytes(n):
+    """inputs 24 B/event + outputs 8 B/event + one write and one read of the filtered
+    (m, P) between the passes."""
+    return 32 + 2 * 8 * (n + n * (n + 1) // 2)
+
+
+def model_dim(w):
+    d = 0
+    for c in w["kernel"]:
+        d += {W.MATERN32: 2, W.MATERN52: 3, W.SHO: 2}.get(c["family"], 2 + 4 * c["order"])
+    return d + w["n_inst"]
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline leg and --impl reference): the fp64 build of oracle/smolgp_oracle.c,
+# as it stands, single thread (the recursion is sequential in k), on a bounded sample = the first
+# `n_sample` exposures of the workload.
+# ----------------------------------------------------------------------------------------------
+def oracle_step(w, n_sample):
+    import oracle
+    sl = slice(0, n_sample)
+    y = w["y"][0, sl] if w["y"].ndim == 2 else w["y"][sl]
+    kern = w["kernel"]
+    if w.get("amp") is not None:
+        kern = [dict(k, sigma=k["sigma"] * float(w["amp"][0])) for k in kern]
+    t0 = time.perf_counter()
+    oracle.ssm(kern, w["n_inst"], w["t_start"][sl], w["t_end"][sl], w["instrument"][sl], y, w["sigma"][sl],
+               flags=oracle.FLAG_IDLE_ZERO | oracle.FLAG_TWO_FILTER, prec="f64")
+    return time.perf_counter() - t0
+
+
+def oracle_sample_size(w, target_s):
+    """exposures such that one oracle pass takes about target_s seconds (calibrated on 500)."""
+    N = w["t_start"].size
+    n0 = min(500, N)
+    t = oracle_step(w, n0)
+    return int(max(n0, min(N, n0 * target_s / max(t, 1e-6))))
+
+
+def run_reference(args, w, cfgname):
+    import oracle
+    oracle.build()
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    ns = oracle_sample_size(w, 4.0)
+    for _ in range(args.warmup):
+        oracle_step(w, min(ns, 2000))
+    ts = [oracle_step(w, ns) for _ in range(args.steps)]
+    tot = sum(ts)
+    val = 2.0 * ns * args.steps / tot
+    sample = "first %d of %d exposures (%d events) per step, oracle fp64 build, sequential filter + two-filter smoother, 1 thread" % (ns, w["t_start"].size, 2 * ns)
+    line = {"impl": "reference", "metric": "events/sec, loglik + smoother", "value": val, "unit": "events/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfgname, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "events/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------
+# CUDA arm
+# ----------------------------------------------------------------------------------------------
+def run_cuda(args, w, cfgname):
+    import torch
+    import torch.distributed as dist
+    from paper_2601_02527_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    ctx = B.Context(local)  # NULL stream = the legacy default stream = torch's current stream here
+    N = w["t_start"].size
+    batch = w["batch"] or 1
+    n = model_dim(w)
+    K_events = 2 * N * batch
+    h2d = lambda a: torch.tensor(a, device=dev)
+    ts, te, ins, y, sg = (h2d(w[k]) for k in ("t_start", "t_end", "instrument", "y", "sigma"))
+    amp = None if w["amp"] is None else h2d(w["amp"])
+    out = dict(mean=torch.empty((batch, N), dtype=torch.float64, device=dev),
+               var=torch.empty((batch, N), dtype=torch.float64, device=dev),
+               loglik=torch.empty(batch, dtype=torch.float64, device=dev))
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)  # > the 126 MB L2
+
+    def step():
+        ev = ctx.smolgp_build_events(ts, te, ins, w["n_inst"])                       # a1
+        ctx.smolgp_condition(ev, w["kernel"], y, sg, amp=amp, out=out)               # a2-a6
+        ev.free()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ctx.profile(True)
+    l0 = ctx.launch_count()
+    evs = []
+    barrier()
+    for _ in range(args.steps):
+        flush.fill_(1)  # evict L2 between timed iterations (not timed)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); step(); b.record()
+        evs.append((a, b))
+    barrier()
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    launches = ctx.launch_count() - l0
+    prof = ctx.profile_read()
+    ctx.profile(False)
+
+    # ---- end to end: host buffers (pinned), copies inside the timed region, through the *_host C ABI ----
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hts, hte, hins, hy, hsg = (pin(w[k]) for k in ("t_start", "t_end", "instrument", "y", "sigma"))
+    hamp = None if w["amp"] is None else pin(w["amp"])
+    hout = dict(mean=pin(np.empty((batch, N))), var=pin(np.empty((batch, N))), loglik=pin(np.empty(batch)))
+
+    def step_e2e():
+        ev = ctx.smolgp_build_events_host(hts, hte, hins, w["n_inst"])
+        ctx.smolgp_condition_host(ev, w["kernel"], hy, hsg, amp=hamp, out=hout)
+        ev.free()
+
+    for _ in range(3):
+        step_e2e()
+    barrier()
+    evs2 = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); step_e2e(); b.record()
+        evs2.append((a, b))
+    barrier()
+    ms_e2e = sum(a.elapsed_time(b) for a, b in evs2)
+    clocks = sampler.stop() if rank == 0 else None
+    fp64_probe = ctx.probe_fp64() if rank == 0 else None
+
+    if world > 1:  # max over ranks
+        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_e2e = t.tolist()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    value = world * K_events * args.steps / (ms * 1e-3)
+    e2e_value = world * K_events * args.steps / (ms_e2e * 1e-3)
+    # ---- roofline of the dominant kernel (device time from the ctx's own CUDA events) ----
+    top = max(prof, key=lambda k: prof[k][0])
+    t_top_ms = prof[top][0] / prof[top][1]           # average launch duration
+    launches_per_step = prof[top][1] / args.steps
+    flops_launch = K_events * w_useful_flops(n) / launches_per_step
+    achieved = flops_launch / (t_top_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md); register-only DFMA probe measured %.1f TFLOP/s in this run" % fp64_probe,
+                "work_model": "W_useful = 10.3 n^3 + 9 n^2 flop/event (SURVEY 8(d)), n = %d" % n,
+                "kernel_share_of_step": prof[top][0] / ms,
+                "hbm": {"min_bytes_per_event": min_bytes(n), "achieved_gbs": K_events * min_bytes(n) * args.steps / (ms * 1e-3) / 1e9},
+                "kernels_ms_per_step": {k: v[0] / args.steps for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
+    # ---- CPU baseline: the oracle as it stands, bounded sample ----
+    import oracle
+    oracle.build()
+    ns = oracle_sample_size(w, 12.0)
+    t_cpu = oracle_step(w, ns)
+    cpu = {"value": 2.0 * ns / t_cpu, "unit": "events/s", "cores": 1, "kind": "oracle",
+           "sample": "first %d of %d exposures (%d events), oracle fp64 build, sequential filter + two-filter smoother, 1 thread, %.1f s" % (ns, N, 2 * ns, t_cpu)}
+    line = {"metric": "events/sec, loglik + smoother (posterior at observations)", "value": value, "unit": "events/s",
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfgname, "N": N, "events": 2 * N, "batch": batch, "state_dim": n,
+                       "path": "a1 build_events + a2 discretise + a3 filter scan + a4 smoother + a5 loglik + a6 posterior",
+                       "l2": "flushed (512 MiB write) between timed iterations", "parallelism": "replicas x%d" % world},
+            "e2e": {"value": e2e_value, "unit": "events/s",
+                    "h2d_bytes_per_step": int(hts.nbytes + hte.nbytes + hins.nbytes + hy.nbytes + hsg.nbytes + (0 if hamp is None else hamp.nbytes)),
+                    "d2h_bytes_per_step": int(hout["mean"].nbytes + hout["var"].nbytes + hout["loglik"].nbytes),
+                    "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+            "loglik": float(hout["loglik"][0])}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+CFG_NAMES = {1: "cfg1 Matern-3/2 N=1e3", 2: "cfg2 SHO two instruments N=2e4",
+             3: "cfg3 quasiperiodic Matern-3/2 x periodic(J=4), 3 overlapping instruments, n=21, N=1e5 (K=2e5 events)",
+             4: "cfg4 joint multi-instrument n=17 N=1e6", 5: "cfg5 batched 4096 x N=2048, n=7"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-5); 3 = the headline N=1e5")
+    args = ap.parse_args()
+    w = W.make(args.config)
+    if args.impl == "reference":
+        run_reference(args, w, CFG_NAMES[args.config])
+    else:
+        run_cuda(args, w, CFG_NAMES[args.config])
+
+
+if __name__ == "__main__":
+    main()

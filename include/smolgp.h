@@ -138,6 +138,16 @@ int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kernel, int32_t
 /* Launch accounting for bench.py: number of kernels this ctx has launched so far. */
 int64_t smolgp_launch_count(const smolgp_ctx* ctx);
 
+/* Per-kernel device timing for bench.py's roofline block.  smolgp_profile(ctx, 1) starts a window in
+ * which every kernel this ctx launches is bracketed by CUDA events on the ctx stream;
+ * smolgp_profile_read synchronises the stream, writes the summed milliseconds and launch counts per
+ * kernel id (HOST arrays of SMOLGP_NKERNELS entries; names from smolgp_kernel_name) and clears the
+ * window; smolgp_profile(ctx, 0) stops.  smolgp_kernel_name returns NULL outside [0, SMOLGP_NKERNELS). */
+#define SMOLGP_NKERNELS 15
+int smolgp_profile(smolgp_ctx* ctx, int32_t enable);
+int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launches);
+const char* smolgp_kernel_name(int32_t id);
+
 /* FP64 FMA throughput probe (roofline denominator): runs a register-only
  * DFMA kernel on the ctx stream and returns the achieved TFLOP/s in *tflops. */
 int smolgp_probe_fp64(smolgp_ctx* ctx, double* tflops);

@@ -14,7 +14,8 @@ STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
            "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
-           "smolgp_launch_count", "smolgp_probe_fp64"]
+           "smolgp_launch_count", "smolgp_probe_fp64", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name"]
+NKERNELS = 15
 
 
 class SmolgpError(RuntimeError):
@@ -61,6 +62,10 @@ def lib():
         L.smolgp_launch_count.argtypes = [vp]
         L.smolgp_launch_count.restype = i64
         L.smolgp_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
+        L.smolgp_profile.argtypes = [vp, i32]
+        L.smolgp_profile_read.argtypes = [vp, dp, dp]
+        L.smolgp_kernel_name.argtypes = [i32]
+        L.smolgp_kernel_name.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -129,6 +134,15 @@ class Context:
 
     def launch_count(self):
         return int(lib().smolgp_launch_count(self.handle))
+
+    def profile(self, enable):
+        self._check(lib().smolgp_profile(self.handle, int(bool(enable))))
+
+    def profile_read(self):
+        """{kernel name: (milliseconds, launches)} of the window since profile(True) / the last read"""
+        ms, cnt = np.zeros(NKERNELS), np.zeros(NKERNELS, dtype=np.int64)
+        self._check(lib().smolgp_profile_read(self.handle, _hptr(ms), _hptr(cnt)))
+        return {lib().smolgp_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(NKERNELS) if cnt[i]}
 
     def probe_fp64(self):
         v = C.c_double()

@@ -28,7 +28,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return SMOLGP_ECUDA; }
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
-  c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0;
+  c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0;
   c->opt_chunk = 0; c->opt_group = 8; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = new ModelDev();
   int v = 0;
   cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device); c->sm_count = v;
@@ -46,12 +46,41 @@ extern "C" void smolgp_destroy(smolgp_ctx* ctx) {
   cudaFree(ctx->arena);
   cudaFree(ctx->pers);
   cudaFree(ctx->d_flags);
+  for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto& e : ctx->evpool) cudaEventDestroy(e);
   delete ctx->hmodel;
   delete ctx;
 }
 
 extern "C" const char* smolgp_last_error(const smolgp_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 extern "C" int64_t smolgp_launch_count(const smolgp_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+static const char* const KNAMES[KID_COUNT] = {"k_ev_init", "k_rs_hist", "k_rs_scan", "k_rs_scatter", "k_ev_gather",
+                                               "k_xs_reduce", "k_xs_tiles", "k_ev_final", "k_disc", "k_fold0", "k_foldD",
+                                               "k_downD", "k_down0", "k_ll_reduce", "k_probe_dfma"};
+extern "C" const char* smolgp_kernel_name(int32_t id) { return (id >= 0 && id < KID_COUNT) ? KNAMES[id] : nullptr; }
+
+extern "C" int smolgp_profile(smolgp_ctx* ctx, int32_t enable) {
+  if (!ctx) return SMOLGP_EINVAL;
+  for (auto& r : ctx->prof) { ctx->evpool.push_back(r.a); ctx->evpool.push_back(r.b); }
+  ctx->prof.clear();
+  ctx->prof_on = enable ? 1 : 0;
+  return SMOLGP_OK;
+}
+
+extern "C" int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launches) {
+  if (!ctx || !ms || !launches) return SMOLGP_EINVAL;
+  SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  for (int i = 0; i < KID_COUNT; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  for (auto& r : ctx->prof) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) { ms[r.id] += t; launches[r.id]++; }
+    else cudaGetLastError();
+    ctx->evpool.push_back(r.a); ctx->evpool.push_back(r.b);
+  }
+  ctx->prof.clear();
+  return SMOLGP_OK;
+}
 
 extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value) {
   if (!ctx || !name) return SMOLGP_EINVAL;

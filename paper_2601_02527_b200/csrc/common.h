@@ -69,11 +69,19 @@ struct smolgp_events {
   double t_first, t_last;
 };
 
+// kernel ids for launch accounting / per-kernel timing (smolgp_profile_read)
+enum { KID_EV_INIT = 0, KID_RS_HIST, KID_RS_SCAN, KID_RS_SCATTER, KID_EV_GATHER, KID_XS_REDUCE, KID_XS_TILES,
+       KID_EV_FINAL, KID_DISC, KID_FOLD0, KID_FOLDD, KID_DOWND, KID_DOWN0, KID_LL_REDUCE, KID_PROBE, KID_COUNT };
+struct ProfRec { int id; cudaEvent_t a, b; };
+
 struct smolgp_ctx {
   int device;
   cudaStream_t stream;
   std::string err;
   int64_t launches;
+  int prof_on;
+  std::vector<ProfRec> prof;       // open records of the current profiling window
+  std::vector<cudaEvent_t> evpool; // recycled events
   int64_t opt_chunk, opt_group, opt_lanes;
   // workspace arena (grown on demand, reused across calls)
   void* arena;
@@ -85,6 +93,23 @@ struct smolgp_ctx {
   int sm_count;
   size_t smem_optin;
 };
+
+// bracket a kernel launch: counts it and, when profiling is on, times it with CUDA events on the ctx stream
+static inline void sg_launch_begin(smolgp_ctx* ctx, int id) {
+  ctx->launches++;
+  if (!ctx->prof_on) return;
+  ProfRec r; r.id = id;
+  cudaEvent_t* e[2] = {&r.a, &r.b};
+  for (int i = 0; i < 2; ++i) {
+    if (!ctx->evpool.empty()) { *e[i] = ctx->evpool.back(); ctx->evpool.pop_back(); }
+    else cudaEventCreate(e[i]);
+  }
+  cudaEventRecord(r.a, ctx->stream);
+  ctx->prof.push_back(r);
+}
+static inline void sg_launch_end(smolgp_ctx* ctx) {
+  if (ctx->prof_on && !ctx->prof.empty()) cudaEventRecord(ctx->prof.back().b, ctx->stream);
+}
 
 #define SG_CUDA(ctx, call)                                                            \
   do {                                                                                \

@@ -172,8 +172,9 @@ int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_m
                    int64_t K, double* disc) {
   const int64_t total = K * h_model->nblk;
   const int64_t blocks = (total + 127) / 128;
+  sg_launch_begin(ctx, KID_DISC);
   k_disc<<<(unsigned)blocks, 128, 0, ctx->stream>>>(d_model, dt, K, disc);
-  ctx->launches++;
+  sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
 }

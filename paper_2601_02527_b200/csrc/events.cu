@@ -106,10 +106,15 @@ int sg_sort_pairs(smolgp_ctx* ctx, uint64_t* keys, uint32_t* vals, uint64_t* key
   uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
   for (int pass = 0; pass < 8; ++pass) {
     const int shift = 8 * pass;
+    sg_launch_begin(ctx, KID_RS_HIST);
     k_rs_hist<<<ntiles, 32, 0, ctx->stream>>>(kin, n, shift, hist, ntiles);
+    sg_launch_end(ctx);
+    sg_launch_begin(ctx, KID_RS_SCAN);
     k_rs_scan<<<1, 1024, 0, ctx->stream>>>(hist, (int64_t)256 * ntiles);
+    sg_launch_end(ctx);
+    sg_launch_begin(ctx, KID_RS_SCATTER);
     k_rs_scatter<<<ntiles, 32, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles);
-    ctx->launches += 3;
+    sg_launch_end(ctx);
     uint64_t* tk = kin; kin = kout; kout = tk;
     uint32_t* tv = vin; vin = vout; vout = tv;
   }
@@ -213,15 +218,23 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   cudaStream_t st = ctx->stream;
   cudaMemsetAsync(ctx->d_flags, 0, sizeof(int), st);
   cudaMemsetAsync(maxdelta, 0, SG_MAXINST * 8, st);
+  sg_launch_begin(ctx, KID_EV_INIT);
   k_ev_init<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ts, te, inst, n_inst, keys, vals, ctx->d_flags, maxdelta);
-  ctx->launches++;
+  sg_launch_end(ctx);
   rc = sg_sort_pairs(ctx, keys, vals, keys_tmp, vals_tmp, K, hist);
   if (rc) return fail(rc);
+  sg_launch_begin(ctx, KID_EV_GATHER);
   k_ev_gather<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(K, vals, ts, te, inst, n_inst, ev->t, ev->delta, ev->obs, bits);
+  sg_launch_end(ctx);
+  sg_launch_begin(ctx, KID_XS_REDUCE);
   k_xs_reduce<<<ntiles_xs, 256, 0, st>>>(bits, K, tiles);
+  sg_launch_end(ctx);
+  sg_launch_begin(ctx, KID_XS_TILES);
   k_xs_tiles<<<1, 32, 0, st>>>(tiles, ntiles_xs);
+  sg_launch_end(ctx);
+  sg_launch_begin(ctx, KID_EV_FINAL);
   k_ev_final<<<ntiles_xs, 32, 0, st>>>(K, bits, tiles, vals, ev->t, n_inst, ev->meta, ev->dt, ctx->d_flags);
-  ctx->launches += 4;
+  sg_launch_end(ctx);
   int flags = 0;
   unsigned long long md[SG_MAXINST];
   double tfl[2];

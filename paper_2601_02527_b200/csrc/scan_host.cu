@@ -24,12 +24,14 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, int n, size_t tb, bo
   const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
   if (fold) {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_FOLD0);
     k_fold0<G><<<blocks, gpc * G, smem, ctx->stream>>>(P);
   } else {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_down0<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_DOWN0);
     k_down0<G><<<blocks, gpc * G, smem, ctx->stream>>>(P);
   }
-  ctx->launches++;
+  sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
 }
@@ -53,12 +55,14 @@ static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, size_t tb, b
   dim3 grid((unsigned)((groups + gpc - 1) / gpc), fold ? 1 : (D.want_suffix ? 2 : 1));
   if (fold) {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_FOLDD);
     k_foldD<<<grid, gpc * 32, smem, ctx->stream>>>(D);
   } else {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_downD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_DOWND);
     k_downD<<<grid, gpc * 32, smem, ctx->stream>>>(D);
   }
-  ctx->launches++;
+  sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
 }
@@ -152,8 +156,9 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   if (rc) return rc;
   if (a.loglik) {
     const int wpb = 4;
+    sg_launch_begin(ctx, KID_LL_REDUCE);
     k_ll_reduce<<<(unsigned)((batch + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(P.llpart, c1, batch, N, a.amp, a.loglik);
-    ctx->launches++;
+    sg_launch_end(ctx);
     SG_CUDA(ctx, cudaGetLastError());
   }
   return SMOLGP_OK;

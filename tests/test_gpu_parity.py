@@ -1,0 +1,208 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (ctypes binding), against the
+CPU oracle on the same seeded inputs.  Bars (north_star): event stream
+bit-exact; log-likelihood relative 1e-9; posterior mean and variance relative 1e-8 (the mean's
+error is scaled by |mean| + prior sd of the exposure average, reading c13)."""
+import numpy as np
+import pytest
+
+from paper_2601_02527_b200 import workloads as W
+import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2601_02527_b200 import binding as B
+    c = B.Context(0)
+    yield c
+    c.close()
+
+
+def _reset(ctx):
+    ctx.set_option("chunk", 0)
+    ctx.set_option("group", 8)
+    ctx.set_option("lanes", 0)
+
+
+SCAN_OPTS = {
+    "auto": (),
+    "sequential": (("chunk", 1 << 40),),                       # one chunk per series (row a8)
+    "deep": (("chunk", 16), ("group", 2)),                     # many dense levels
+    "ragged": (("chunk", 37), ("group", 3), ("lanes", 32)),    # chunk/group sizes dividing nothing
+}
+
+
+# ---------------------------------------------------------------------------------------------
+# a1: event build, bit-exact against the oracle's sort
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,N", [(1, 1000), (2, 20000), (3, 5000), (4, 4097), (5, 2048), ("fig2", 400), ("fig3", 600)])
+def test_events_bit_exact(ctx, oracle, cfg, N):
+    w = W.make(cfg, N=N, batch=(2 if cfg == 5 else None), n_features=4)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    t, kind, inst, idx = ev.export()
+    ot, ok, oi, ox = oracle.events(w["t_start"], w["t_end"], w["instrument"])
+    assert np.array_equal(t, ot)
+    assert np.array_equal(kind, ok)
+    assert np.array_equal(inst, oi)
+    assert np.array_equal(idx, ox)
+    ev.free()
+
+
+def test_events_device_pointers_and_shuffled_input(ctx, oracle):
+    """device-pointer entry point; exposures given in random order; negative and tied times"""
+    import torch
+    rng = np.random.default_rng(5)
+    w = W.make("fig2", N=300, n_features=4)            # back-to-back: every end ties with a start
+    ts, te = w["t_start"] - 20000.0, w["t_end"] - 20000.0  # times straddle zero
+    p = rng.permutation(ts.size)
+    ts, te, inst = ts[p], te[p], w["instrument"][p]
+    dev = torch.device("cuda:0")
+    ev = ctx.smolgp_build_events(torch.tensor(ts, device=dev), torch.tensor(te, device=dev),
+                                 torch.tensor(inst, device=dev), 1)
+    t, kind, ins, idx = ev.export()
+    ot, ok, oi, ox = oracle.events(ts, te, inst)
+    assert np.array_equal(t, ot) and np.array_equal(kind, ok) and np.array_equal(idx, ox)
+    # ties: the end comes first (reading R5)
+    tie = np.nonzero(t[1:] == t[:-1])[0]
+    assert tie.size > 100 and np.all(kind[tie] == 0) and np.all(kind[tie + 1] == 1)
+
+
+def test_events_validation(ctx):
+    from paper_2601_02527_b200.binding import SmolgpError
+    ts, te, ins = np.array([0.0, 10.0, 30.0]), np.array([5.0, 20.0, 40.0]), np.zeros(3, np.int32)
+    with pytest.raises(SmolgpError) as e:   # same-instrument overlap
+        ctx.smolgp_build_events_host(ts, np.array([5.0, 31.0, 40.0]), ins, 1)
+    assert e.value.rc == -2
+    ctx.smolgp_build_events_host(ts, np.array([10.0, 30.0, 40.0]), ins, 1).free()  # back-to-back is legal
+    ctx.smolgp_build_events_host(ts, np.array([5.0, 31.0, 40.0]), np.array([0, 1, 0], np.int32), 2).free()
+    for bad_te in (np.array([5.0, 10.0, 40.0]), np.array([5.0, np.nan, 40.0]), np.array([5.0, np.inf, 40.0])):
+        with pytest.raises(SmolgpError) as e:
+            ctx.smolgp_build_events_host(ts, bad_te, ins, 1)
+        assert e.value.rc == -1
+    with pytest.raises(SmolgpError) as e:
+        ctx.smolgp_build_events_host(ts, te, np.array([0, 2, 0], np.int32), 2)
+    assert e.value.rc == -1
+    with pytest.raises(SmolgpError) as e:
+        ctx.smolgp_build_events_host(ts, te, ins, 17)
+    assert e.value.rc == -3
+
+
+# ---------------------------------------------------------------------------------------------
+# a2: discretisation against the oracle's long-double Taylor + doubling
+# ---------------------------------------------------------------------------------------------
+KERNELS = {
+    "m32": [W.comp(W.MATERN32, 1.3, 600.0)],
+    "m52": [W.comp(W.MATERN52, 0.7, 86400.0)],
+    "sho": [W.comp(W.SHO, 1.0, 2 * np.pi / 330.0, 10.0)],
+    "sho_crit": [W.comp(W.SHO, 1.1, 0.02, 0.5)],
+    "sho_over": [W.comp(W.SHO, 0.9, 0.05, 0.3)],
+    "qp": [W.comp(W.MATERN32_X_PERIODIC, 1.0, 20 * W.DAY, 25 * W.DAY, 1.0, order=4)],
+    "cfg4": W.make(4, N=8, n_features=2)["kernel"],
+}
+
+
+@pytest.mark.parametrize("name", sorted(KERNELS))
+@pytest.mark.parametrize("dt", [0.0, 1e-3, 12.0, 55.0, 300.0, 5000.0, 57600.0, 3e6])
+def test_discretise_matches_oracle(ctx, oracle, name, dt):
+    kern = KERNELS[name]
+    ninst = 4 if name == "cfg4" else 2
+    A, Q = ctx.smolgp_discretise_host(kern, ninst, dt)
+    Ao, Qo = oracle.discretise(kern, ninst, dt)
+    n = A.shape[0]
+    d = n - ninst
+    # compare in equilibrated units: x rows by sqrt(Pinf_ii), z rows by dt * sd (so every entry is O(1))
+    _, _, Pinf, _ = oracle.ssm_matrices(kern, ninst)
+    s = np.concatenate([np.sqrt(np.diag(Pinf)), np.full(ninst, (dt if dt > 0 else 1.0) * np.sqrt(np.trace(Pinf)))])
+    As, Aos = A / s[:, None] * s[None, :], Ao / s[:, None] * s[None, :]
+    Qs, Qos = Q / np.outer(s, s), Qo / np.outer(s, s)
+    assert np.max(np.abs(As - Aos)) <= 1e-13 * max(1.0, np.max(np.abs(Aos)))
+    # Q entries span many orders of magnitude inside one matrix (q22 ~ dt^5 for short steps): each
+    # entry is compared relative to the geometric mean of its diagonal entries (Cauchy-Schwarz scale)
+    dg = np.sqrt(np.abs(np.diag(Qos)))
+    scale = np.outer(dg, dg) + 1e-300
+    assert np.max(np.abs(Qs - Qos) / scale) <= 2e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# a3-a6: log-likelihood and posterior at the observations, reduced-size versions of every config
+# (sizes the long-double oracle finishes in seconds; several chunks, several dense levels, ragged tails)
+# ---------------------------------------------------------------------------------------------
+CASES = [(1, 1000, None), (2, 3001, None), ("fig2", 400, None), ("fig3", 600, None), (3, 1500, None),
+         (4, 1203, None), (5, 300, 6)]
+
+
+@pytest.mark.parametrize("opt", sorted(SCAN_OPTS))
+@pytest.mark.parametrize("cfg,N,batch", CASES)
+def test_condition_matches_oracle(ctx, oracle, cfg, N, batch, opt):
+    w = W.make(cfg, N=N, batch=batch)
+    for k, v in SCAN_OPTS[opt]:
+        ctx.set_option(k, v)
+    try:
+        ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+        out = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"])
+        ll = ctx.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"])
+    finally:
+        _reset(ctx)
+    for s in ([None] if batch is None else range(batch)):
+        ref = PU.reference(oracle, w, series=s)
+        i = 0 if s is None else s
+        wk = w if s is None else dict(w, kernel=[dict(k, sigma=k["sigma"] * w["amp"][s]) for k in w["kernel"]])
+        floor = PU.prior_sd(oracle, wk) if N <= 1500 else None
+        e = PU.errors(ref, out["loglik"][i], out["mean"][i], out["var"][i], floor=floor)
+        assert e["ll"] <= PU.LL_RTOL, e
+        assert abs(ll[i] - ref["loglik"]) <= PU.LL_RTOL * abs(ref["loglik"])
+        assert e["mean"] <= PU.POST_RTOL, e
+        assert e["var"] <= PU.POST_RTOL, e
+
+
+def test_device_pointer_entry_points_match_host_ones(ctx):
+    import torch
+    w = W.make(2, N=2000)
+    dev = torch.device("cuda:0")
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    h = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])
+    y, sg = torch.tensor(w["y"], device=dev), torch.tensor(w["sigma"], device=dev)
+    d = ctx.smolgp_condition(ev, w["kernel"], y, sg)
+    ll = ctx.smolgp_loglik(ev, w["kernel"], y, sg)
+    torch.cuda.synchronize()
+    assert np.array_equal(d["mean"].cpu().numpy()[0], h["mean"][0])
+    assert np.array_equal(d["var"].cpu().numpy()[0], h["var"][0])
+    assert d["loglik"].cpu().numpy()[0] == h["loglik"][0] == ll.cpu().numpy()[0]
+
+
+def test_dense_definition_parity_tiny(ctx, oracle):
+    """the GPU path against the DEFINITION (dense integrated GP, Eq. 2.4 + 3.1) directly, N = 150"""
+    for cfg, batch in [(2, None), (3, None), (4, None), (5, 2)]:
+        w = W.make(cfg, N=150, batch=batch)
+        ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+        out = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"])
+        for s in ([None] if batch is None else range(batch)):
+            i = 0 if s is None else s
+            kern = w["kernel"] if s is None else [dict(k, sigma=k["sigma"] * w["amp"][s]) for k in w["kernel"]]
+            y = w["y"] if s is None else w["y"][s]
+            ref = oracle.dense(kern, w["t_start"], w["t_end"], w["instrument"], y, w["sigma"])
+            assert abs(out["loglik"][i] - ref["loglik"]) <= 1e-9 * abs(ref["loglik"])
+            floor = PU.prior_sd(oracle, dict(w, kernel=kern))
+            assert np.max(np.abs(out["mean"][i] - ref["mean"]) / (np.abs(ref["mean"]) + floor)) <= 1e-8
+            # the dense solver's own variance (K - K C^-1 K, cancellation) is good to ~1e-10 of the prior
+            assert np.max(np.abs(out["var"][i] - ref["var"]) / floor ** 2) <= 1e-8
+
+
+def test_numeric_errors_are_reported(ctx):
+    from paper_2601_02527_b200.binding import SmolgpError
+    w = W.make(1, N=64)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    y = w["y"].copy()
+    y[10] = np.nan
+    with pytest.raises(SmolgpError) as e:
+        ctx.smolgp_loglik_host(ev, w["kernel"], y, w["sigma"])
+    assert e.value.rc == -6
+    with pytest.raises(SmolgpError) as e:
+        ctx.smolgp_loglik_host(ev, [W.comp(7, 1.0, 1.0)], w["y"], w["sigma"])
+    assert e.value.rc == -3
+    # the context stays usable after an error
+    ll = ctx.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"])
+    assert np.isfinite(ll[0])
