@@ -143,7 +143,7 @@ int64_t smolgp_launch_count(const smolgp_ctx* ctx);
  * smolgp_profile_read synchronises the stream, writes the summed milliseconds and launch counts per
  * kernel id (HOST arrays of SMOLGP_NKERNELS entries; names from smolgp_kernel_name) and clears the
  * window; smolgp_profile(ctx, 0) stops.  smolgp_kernel_name returns NULL outside [0, SMOLGP_NKERNELS). */
-#define SMOLGP_NKERNELS 15
+#define SMOLGP_NKERNELS 17
 int smolgp_profile(smolgp_ctx* ctx, int32_t enable);
 int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launches);
 const char* smolgp_kernel_name(int32_t id);

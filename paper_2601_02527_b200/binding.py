@@ -15,7 +15,7 @@ EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_o
            "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
            "smolgp_launch_count", "smolgp_probe_fp64", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name"]
-NKERNELS = 15
+NKERNELS = 17
 
 
 class SmolgpError(RuntimeError):

@@ -57,7 +57,7 @@ extern "C" int64_t smolgp_launch_count(const smolgp_ctx* ctx) { return ctx ? ctx
 
 static const char* const KNAMES[KID_COUNT] = {"k_ev_init", "k_rs_hist", "k_rs_scan", "k_rs_scatter", "k_ev_gather",
                                                "k_xs_reduce", "k_xs_tiles", "k_ev_final", "k_disc", "k_fold0", "k_foldD",
-                                               "k_downD", "k_down0", "k_ll_reduce", "k_probe_dfma"};
+                                               "k_downD", "k_down0", "k_ll_reduce", "k_probe_dfma", "k_query_locate", "k_query"};
 extern "C" const char* smolgp_kernel_name(int32_t id) { return (id >= 0 && id < KID_COUNT) ? KNAMES[id] : nullptr; }
 
 extern "C" int smolgp_profile(smolgp_ctx* ctx, int32_t enable) {
@@ -92,9 +92,11 @@ extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t valu
 }
 
 // validation of sigma > 0 happens on the device inside the filter (S > 0 check) and here for amp
+struct QuerySpec { int64_t M = 0; const double* tq = nullptr; int qinst = 0; double* mean = nullptr; double* var = nullptr; };
+
 static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
                     const double* y, const double* sigma, const double* amp, double* mean, double* var,
-                    double* loglik, int want_smooth) {
+                    double* loglik, int want_smooth, const QuerySpec& qs = QuerySpec()) {
   if (!ctx) return SMOLGP_EINVAL;
   if (!ev || !kernel || !y || !sigma || batch <= 0) { ctx->err = "null or empty argument"; return SMOLGP_EINVAL; }
   if (want_smooth && (!mean || !var)) { ctx->err = "condition: mean_obs and var_obs are required"; return SMOLGP_EINVAL; }
@@ -121,11 +123,28 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   ScanArgs a;
   a.d_model = dm; a.h_model = &hm; a.ev = ev; a.disc = disc; a.batch = batch; a.y = y; a.sigma = sigma; a.amp = amp;
   a.loglik = loglik; a.mean = mean; a.var = var; a.want_smooth = want_smooth;
+  a.fstate = a.binfo = nullptr;
+  double* qstore = nullptr; // all 2N filtered states and backward informations, only when queries are asked for
+  if (qs.M > 0) {
+    if (!qs.tq || !qs.mean || !qs.var) { ctx->err = "condition: t_query, mean_query and var_query are required when M > 0"; return SMOLGP_EINVAL; }
+    if (qs.qinst < 0 || qs.qinst >= ev->n_inst) { ctx->err = "condition: query_instrument out of range"; return SMOLGP_EINVAL; }
+    const size_t one = (size_t)batch * ev->K * (hm.n + hm.n * hm.n) * 8;
+    if (cudaMalloc(&qstore, 2 * one) != cudaSuccess) { cudaGetLastError(); ctx->err = "out of device memory (states for query-time prediction)"; return SMOLGP_ENOMEM; }
+    a.fstate = qstore; a.binfo = (double*)((char*)qstore + one);
+  }
   rc = sg_run_scan(ctx, a);
-  if (rc) return rc;
+  if (rc == SMOLGP_OK && qs.M > 0) {
+    QueryArgs q;
+    q.d_model = dm; q.h_model = &hm; q.ev = ev; q.batch = batch; q.M = qs.M; q.tq = qs.tq; q.qinst = qs.qinst; q.amp = amp;
+    q.fstate = a.fstate; q.binfo = a.binfo; q.mean = qs.mean; q.var = qs.var;
+    rc = sg_run_query(ctx, q);
+  }
+  if (rc) { if (qstore) { cudaStreamSynchronize(ctx->stream); cudaFree(qstore); } return rc; }
   int flags = 0;
-  SG_CUDA(ctx, cudaMemcpyAsync(&flags, ctx->d_flags, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
-  SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  cudaError_t ce = cudaMemcpyAsync(&flags, ctx->d_flags, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);
+  if (qstore) cudaFree(qstore);
+  SG_CUDA(ctx, ce);
   if (flags) { ctx->err = "non-finite value or non-positive innovation variance (check noise_sigma > 0, amp > 0, finite y)"; return SMOLGP_ENUMERIC; }
   return SMOLGP_OK;
 }
@@ -140,20 +159,22 @@ extern "C" int smolgp_condition(smolgp_ctx* ctx, const smolgp_events* ev, const 
                                 const double* t_query, int32_t query_instrument, double* mean_obs, double* var_obs,
                                 double* mean_query, double* var_query, double* loglik) {
   if (!ctx) return SMOLGP_EINVAL;
-  if (M > 0) { ctx->err = "condition: query-time prediction (Algorithm 1) is not built yet"; return SMOLGP_EUNSUPPORTED; }
-  (void)t_query; (void)query_instrument; (void)mean_query; (void)var_query;
-  return run_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1);
+  if (M < 0) { ctx->err = "condition: M < 0"; return SMOLGP_EINVAL; }
+  QuerySpec qs;
+  qs.M = M; qs.tq = t_query; qs.qinst = query_instrument; qs.mean = mean_query; qs.var = var_query;
+  return run_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1, qs);
 }
 
 // ---- host-pointer variants: copies inside the call, on the ctx stream -------------------------------
 struct HostStage {
   double *y = nullptr, *sigma = nullptr, *amp = nullptr, *mean = nullptr, *var = nullptr, *ll = nullptr;
-  ~HostStage() { cudaFree(y); cudaFree(sigma); cudaFree(amp); cudaFree(mean); cudaFree(var); cudaFree(ll); }
+  double *tq = nullptr, *mq = nullptr, *vq = nullptr;
+  ~HostStage() { cudaFree(y); cudaFree(sigma); cudaFree(amp); cudaFree(mean); cudaFree(var); cudaFree(ll); cudaFree(tq); cudaFree(mq); cudaFree(vq); }
 };
 
 static int host_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
                      const double* y, const double* sigma, const double* amp, double* mean, double* var,
-                     double* loglik, int want_smooth) {
+                     double* loglik, int want_smooth, const QuerySpec& hq = QuerySpec()) {
   if (!ctx) return SMOLGP_EINVAL;
   if (!ev || !y || !sigma || batch <= 0) { ctx->err = "null or empty argument"; return SMOLGP_EINVAL; }
   SG_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -165,11 +186,23 @@ static int host_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kern
     cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM;
   }
   cudaStream_t st = ctx->stream;
+  QuerySpec qs;
+  const size_t bm = (size_t)batch * (hq.M > 0 ? hq.M : 0) * 8;
+  if (hq.M > 0) {
+    if (!hq.tq || !hq.mean || !hq.var) { ctx->err = "condition: t_query, mean_query and var_query are required when M > 0"; return SMOLGP_EINVAL; }
+    if (cudaMalloc(&s.tq, hq.M * 8) || cudaMalloc(&s.mq, bm) || cudaMalloc(&s.vq, bm)) { cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM; }
+    SG_CUDA(ctx, cudaMemcpyAsync(s.tq, hq.tq, hq.M * 8, cudaMemcpyHostToDevice, st));
+    qs.M = hq.M; qs.tq = s.tq; qs.qinst = hq.qinst; qs.mean = s.mq; qs.var = s.vq;
+  }
   SG_CUDA(ctx, cudaMemcpyAsync(s.y, y, bn, cudaMemcpyHostToDevice, st));
   SG_CUDA(ctx, cudaMemcpyAsync(s.sigma, sigma, N * 8, cudaMemcpyHostToDevice, st));
   if (amp) SG_CUDA(ctx, cudaMemcpyAsync(s.amp, amp, batch * 8, cudaMemcpyHostToDevice, st));
-  int rc = run_path(ctx, ev, kernel, batch, s.y, s.sigma, amp ? s.amp : nullptr, s.mean, s.var, s.ll, want_smooth);
+  int rc = run_path(ctx, ev, kernel, batch, s.y, s.sigma, amp ? s.amp : nullptr, s.mean, s.var, s.ll, want_smooth, qs);
   if (rc) return rc;
+  if (hq.M > 0) {
+    SG_CUDA(ctx, cudaMemcpyAsync(hq.mean, s.mq, bm, cudaMemcpyDeviceToHost, st));
+    SG_CUDA(ctx, cudaMemcpyAsync(hq.var, s.vq, bm, cudaMemcpyDeviceToHost, st));
+  }
   if (want_smooth) {
     SG_CUDA(ctx, cudaMemcpyAsync(mean, s.mean, bn, cudaMemcpyDeviceToHost, st));
     SG_CUDA(ctx, cudaMemcpyAsync(var, s.var, bn, cudaMemcpyDeviceToHost, st));
@@ -190,10 +223,11 @@ extern "C" int smolgp_condition_host(smolgp_ctx* ctx, const smolgp_events* ev, c
                                      int64_t M, const double* t_query, int32_t query_instrument, double* mean_obs,
                                      double* var_obs, double* mean_query, double* var_query, double* loglik) {
   if (!ctx) return SMOLGP_EINVAL;
-  if (M > 0) { ctx->err = "condition: query-time prediction (Algorithm 1) is not built yet"; return SMOLGP_EUNSUPPORTED; }
-  (void)t_query; (void)query_instrument; (void)mean_query; (void)var_query;
+  if (M < 0) { ctx->err = "condition: M < 0"; return SMOLGP_EINVAL; }
   if (!mean_obs || !var_obs) { ctx->err = "condition: mean_obs and var_obs are required"; return SMOLGP_EINVAL; }
-  return host_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1);
+  QuerySpec qs;
+  qs.M = M; qs.tq = t_query; qs.qinst = query_instrument; qs.mean = mean_query; qs.var = var_query;
+  return host_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1, qs);
 }
 
 // ---- step a2 alone (tests): A~ and Q~ of one step in raw state units ---------------------------------

@@ -41,6 +41,7 @@ struct ModelDev {
   int row_lo[SG_NMAX], row_hi[SG_NMAX]; // x-row i of F only touches columns [row_lo, row_hi)
   double cz[SG_MAXINST][SG_MAXBLK]; // c_qb: coupling of block b's integral into z_q (equilibrated units), 0 if masked out
   double tau[SG_MAXINST];          // z_q is carried as z_q / tau_q
+  double hq[SG_MAXINST][SG_MAXBLK]; // sigma_b if block b enters instrument q's integrand H_q (Eq. 3.2), else 0
   double p0[SG_NMAX * SG_NMAX];    // prior covariance blkdiag(Pinf'', 0) (Eq. 3.19, reading R6)
   BlockConst blk[SG_MAXBLK];
 };
@@ -71,7 +72,7 @@ struct smolgp_events {
 
 // kernel ids for launch accounting / per-kernel timing (smolgp_profile_read)
 enum { KID_EV_INIT = 0, KID_RS_HIST, KID_RS_SCAN, KID_RS_SCATTER, KID_EV_GATHER, KID_XS_REDUCE, KID_XS_TILES,
-       KID_EV_FINAL, KID_DISC, KID_FOLD0, KID_FOLDD, KID_DOWND, KID_DOWN0, KID_LL_REDUCE, KID_PROBE, KID_COUNT };
+       KID_EV_FINAL, KID_DISC, KID_FOLD0, KID_FOLDD, KID_DOWND, KID_DOWN0, KID_LL_REDUCE, KID_PROBE, KID_QLOCATE, KID_QUERY, KID_COUNT };
 struct ProfRec { int id; cudaEvent_t a, b; };
 
 struct smolgp_ctx {
@@ -142,7 +143,23 @@ struct ScanArgs {
   double* mean;        // [batch][N] or NULL
   double* var;         // [batch][N] or NULL
   int want_smooth;
+  double* fstate;      // [batch][K][n + n^2] or NULL: post-event filtered states (row a7)
+  double* binfo;       // [batch][K][n + n^2] or NULL: pre-update backward information
 };
 int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a);
+struct QueryArgs {
+  const ModelDev* d_model;
+  const ModelDev* h_model;
+  const smolgp_events* ev;
+  int64_t batch, M;
+  const double* tq;    // [M] device
+  int qinst;
+  const double* amp;
+  const double* fstate;
+  const double* binfo;
+  double* mean;        // [batch][M]
+  double* var;
+};
+int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a);
 // arena helper
 int sg_arena(smolgp_ctx* ctx, size_t bytes, void** out);

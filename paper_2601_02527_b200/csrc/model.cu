@@ -173,7 +173,10 @@ int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const
     M->row_lo[d + q] = 0; M->row_hi[d + q] = d; // z rows: the whole x range (plus their own diagonal)
     M->tau[q] = tau[q];
     for (int b = 0; b < nb; ++b)
+    {
       M->cz[q][b] = ((mask[b] >> q) & 1u) ? (double)(sig[b] / ((ld)M->blk[b].inv_T * (ld)tau[q])) : 0.0;
+      M->hq[q][b] = ((mask[b] >> q) & 1u) ? (double)sig[b] : 0.0;
+    }
   }
   const int n = M->n;
   for (int b = 0; b < nb; ++b)

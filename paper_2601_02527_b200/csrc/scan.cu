@@ -41,6 +41,8 @@ struct ScanDev {
   const double* PRE1; // [batch*c1][state] or NULL (prior)
   const double* SUF1; // [batch*c1][state] or NULL (zero)
   double* xbuf;    // [batch*N][state] filtered state at each end event
+  double* fstate;  // [batch*K][state] post-event filtered state of every event, or NULL (a7)
+  double* binfo;   // [batch*K][state] information [eta | J] about the pre-update state of every event, or NULL (a7)
   double* llpart;  // [batch*c1]
   double* mean;
   double* var;
@@ -362,6 +364,35 @@ __global__ void __launch_bounds__(64) k_downD(DenseArgs P) {
   }
 }
 
+// Backward information step over one transition (F, Q):  J <- F^T (I + J Q)^-1 J F,
+// eta <- F^T (I + J Q)^-1 eta  (the (eta, J) part of the SG21 combine with a primitive start-type
+// element on the left, reading R1).  Ws: n x (2n+1), Tm: n x n scratch.  Ends synchronised.
+template <int G>
+__device__ void info_backstep(const Grp<G>& g, const Tables& T, const double* Fs, const double* Qs, double* Jm, double* ev,
+                              double* Ws, double* Tm) {
+  const int n = T.n, ld = 2 * n + 1;
+  mm(g, n, n, n, Jm, n, 1, Qs, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1);
+  g.sync();
+  for (int e = g.gl; e < n * n; e += G) { const int i = e / n, j = e - i * n; Ws[i * ld + n + j] = Jm[e]; }
+  for (int i = g.gl; i < n; i += G) { Ws[i * ld + i] += 1.0; Ws[i * ld + 2 * n] = ev[i]; }
+  g.sync();
+  gj_solve(g, n, ld, Ws);
+  // Tm = F^T Y ; eta = F^T y ; J = F^T Tm^T  (Y symmetric)
+  lmul_Ft(g, T, Fs, Ws + n, ld, 1, Tm, n, 1, n);
+  lmul_Ft(g, T, Fs, Ws + 2 * n, ld, 0, ev, 1, 0, 1);
+  g.sync();
+  lmul_Ft(g, T, Fs, Tm, 1, n, Jm, n, 1, n); // src = Tm^T
+  g.sync();
+  // symmetrise (the two triangles were computed independently)
+  for (int e = g.gl; e < T.ntri; e += G) {
+    const int i = T.tri_i[e], j = T.tri_j[e];
+    const double w = 0.5 * (Jm[i * n + j] + Jm[j * n + i]);
+    Jm[i * n + j] = w;
+    Jm[j * n + i] = w;
+  }
+  g.sync();
+}
+
 // ---------------------------------------------------------------------------------------------------
 // k_down0: per chunk, forward Kalman filter from the prefix state, then backward information
 // recursion from the suffix information with the smoothed output at every end event.
@@ -453,6 +484,11 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
       for (int j = g.gl; j < n; j += G) { Pm[zi * n + j] = 0.0; Pm[j * n + zi] = 0.0; }
       g.sync();
     }
+    if (P.fstate) { // row a7: all 2N filtered states are kept for prediction at arbitrary times
+      double* x = P.fstate + (series * P.K + k) * (int64_t)ss;
+      for (int e = g.gl; e < n; e += G) x[e] = mv[e];
+      for (int e = g.gl; e < n * n; e += G) x[n + e] = Pm[e];
+    }
   }
   if (g.gl == 0) P.llpart[gid] = ll;
   if (!P.want_smooth) return;
@@ -514,32 +550,17 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
       }
       g.sync();
     }
+    if (P.binfo) {
+      double* x = P.binfo + (series * P.K + k) * (int64_t)ss;
+      for (int e = g.gl; e < n; e += G) x[e] = ev[e];
+      for (int e = g.gl; e < n * n; e += G) x[n + e] = Jm[e];
+    }
     if (k == k0) break;
     // back over the step into event k:  J <- F^T (I + J Q)^-1 J F,  eta <- F^T (I + J Q)^-1 eta
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
     assemble_step(g, T, P.disc + k * (int64_t)T.stride, tz, Fs, Qs);
     g.sync();
-    const int ld = 2 * n + 1;
-    mm(g, n, n, n, Jm, n, 1, Qs, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1);
-    g.sync();
-    for (int e = g.gl; e < n * n; e += G) { const int i = e / n, j = e - i * n; Ws[i * ld + n + j] = Jm[e]; }
-    for (int i = g.gl; i < n; i += G) { Ws[i * ld + i] += 1.0; Ws[i * ld + 2 * n] = ev[i]; }
-    g.sync();
-    gj_solve(g, n, ld, Ws);
-    // Tm = F^T Y ; eta = F^T y ; J = F^T Tm^T  (Y symmetric)
-    lmul_Ft(g, T, Fs, Ws + n, ld, 1, Tm, n, 1, n);
-    lmul_Ft(g, T, Fs, Ws + 2 * n, ld, 0, ev, 1, 0, 1);
-    g.sync();
-    lmul_Ft(g, T, Fs, Tm, 1, n, Jm, n, 1, n); // src = Tm^T
-    g.sync();
-    // symmetrise (the two triangles were computed independently)
-    for (int e = g.gl; e < T.ntri; e += G) {
-      const int i = T.tri_i[e], j = T.tri_j[e];
-      const double w = 0.5 * (Jm[i * n + j] + Jm[j * n + i]);
-      Jm[i * n + j] = w;
-      Jm[j * n + i] = w;
-    }
-    g.sync();
+    info_backstep(g, T, Fs, Qs, Jm, ev, Ws, Tm);
   }
 }
 
@@ -553,6 +574,140 @@ __global__ void k_ll_reduce(const double* __restrict__ llpart, int64_t c1, int64
   for (int64_t c = lane; c < c1; c += 32) acc += llpart[s * c1 + c];
   for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if (lane == 0) loglik[s] = acc - (amp ? (double)N * log(amp[s]) : 0.0);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Row a7: prediction at arbitrary times (Algorithm 1) in two-filter form.
+// k_query_locate: kp[q] = last event with t_k <= t*_q (-1 if none);  dtq[q] = t* - t_kp (0 if none),
+// dtq[M + q] = t_{kp+1} - t* (0 if kp is the last event).  k_disc then discretises the 2M steps.
+// k_query: one group per (series, query).
+// ---------------------------------------------------------------------------------------------------
+__global__ void k_query_locate(int64_t M, const double* __restrict__ tq, int64_t K, const double* __restrict__ t,
+                               int64_t* __restrict__ kp, double* __restrict__ dtq) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= M) return;
+  const double ts = tq[q];
+  int64_t lo = -1, hi = K; // invariant: t[lo] <= ts < t[hi]
+  while (hi - lo > 1) {
+    const int64_t mid = (lo + hi) >> 1;
+    if (t[mid] <= ts) lo = mid; else hi = mid;
+  }
+  kp[q] = lo;
+  dtq[q] = (lo >= 0) ? ts - t[lo] : 0.0;
+  dtq[M + q] = (lo + 1 < K) ? t[lo + 1] - ts : 0.0;
+}
+
+struct QueryDev {
+  const ModelDev* M;
+  const double* discq; // [2M][stride]
+  const int64_t* kp;   // [M]
+  const uint32_t* meta;
+  const double* fstate;
+  const double* binfo;
+  const double* amp;
+  int64_t K, Mq, batch;
+  int qinst;
+  double* mean; // [batch][M]
+  double* var;
+  int* flags;
+};
+
+template <int G>
+__global__ void __launch_bounds__(128) k_query(QueryDev P) {
+  extern __shared__ __align__(16) char smem[];
+  Tables T;
+  tables_build(P.M, smem, T);
+  __syncthreads();
+  const int n = T.n, d = T.d;
+  const size_t tb = tables_bytes(n, d, T.ninst, T.nblk, T.nent);
+  const Grp<G> g;
+  const int gpc = blockDim.x / G;
+  const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
+  if (gid >= P.batch * P.Mq) return;
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n);
+  double* Fs = base;
+  double* Qs = Fs + n * n;
+  double* Pm = Qs + n * n;
+  double* Tm = Pm + n * n;
+  double* Jm = Tm + n * n;
+  double* Ws = Jm + n * n;           // n x (2n+1)
+  double* mv = Ws + n * (2 * n + 1); // n
+  double* m2 = mv + n;               // n
+  double* ev = m2 + n;               // n
+  double* hv = ev + n;               // n: H_q in block units
+  const int ss = state_size(n);
+  const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
+  const int64_t kp = P.kp[q];
+  const double ampv = P.amp ? P.amp[series] : 1.0;
+  zero_fill(g, Fs, 2 * n * n);
+  for (int i = g.gl; i < n; i += G) hv[i] = 0.0;
+  g.sync();
+  if (g.gl == 0)
+    for (int b = 0; b < T.nblk; ++b) hv[P.M->blk[b].off] = P.M->hq[P.qinst][b];
+  // ---- state just after the last event at or before t* (stationary prior with idle z = 0 if none) ----
+  if (kp >= 0) {
+    const double* s = P.fstate + (series * P.K + kp) * (int64_t)ss;
+    for (int e = g.gl; e < n; e += G) mv[e] = s[e];
+    for (int e = g.gl; e < n * n; e += G) Pm[e] = s[n + e];
+    g.sync();
+    // predict over Delta_1 (Eq. 3.14); instruments idle after event kp stay zeroed
+    const uint32_t mp = P.meta[kp]; // idle through (t_kp, t_kp+1): zeroed after kp, except an instrument that just started
+    const unsigned idle = META_KIND(mp) ? (META_ZMASK(mp) & ~(1u << META_INST(mp))) : META_ZMASK(mp);
+    assemble_step(g, T, P.discq + q * (int64_t)T.stride, idle, Fs, Qs);
+    g.sync();
+    lmul_F(g, T, Fs, mv, 1, 0, m2, 1, 0, 1);
+    lmul_F(g, T, Fs, Pm, n, 1, Tm, n, 1, n);
+    g.sync();
+    rmul_Ft_sym(g, T, Fs, Tm, Qs, Pm);
+    g.sync();
+    { double* t = mv; mv = m2; m2 = t; }
+  } else {
+    for (int e = g.gl; e < n; e += G) mv[e] = 0.0;
+    for (int e = g.gl; e < n * n; e += G) Pm[e] = P.M->p0[e];
+    g.sync();
+  }
+  // ---- information about the state at t* from every later event ----
+  if (kp + 1 < P.K) {
+    const int64_t kn = kp + 1;
+    const double* s = P.binfo + (series * P.K + kn) * (int64_t)ss;
+    for (int e = g.gl; e < n; e += G) ev[e] = s[e];
+    for (int e = g.gl; e < n * n; e += G) Jm[e] = s[n + e];
+    const uint32_t meta = P.meta[kn];
+    const unsigned zm = META_ZMASK(meta);
+    const unsigned tz = META_KIND(meta) ? zm : (zm & ~(1u << META_INST(meta)));
+    g.sync();
+    assemble_step(g, T, P.discq + (P.Mq + q) * (int64_t)T.stride, tz, Fs, Qs);
+    g.sync();
+    info_backstep(g, T, Fs, Qs, Jm, ev, Ws, Tm);
+    // fuse: P^ = (I + P J)^-1 P, m^ = (I + P J)^-1 (m + P eta); right-hand sides P h and m + P eta
+    const int ld = n + 2;
+    mm(g, n, n, n, Pm, n, 1, Jm, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1);
+    g.sync();
+    for (int i = g.gl; i < n; i += G) {
+      Ws[i * ld + i] += 1.0;
+      double a = 0.0, acc = mv[i];
+      for (int l = 0; l < n; ++l) { a = fma(Pm[i * n + l], hv[l], a); acc = fma(Pm[i * n + l], ev[l], acc); }
+      Ws[i * ld + n] = a;
+      Ws[i * ld + n + 1] = acc;
+    }
+    g.sync();
+    gj_solve(g, n, ld, Ws);
+    if (g.gl == 0) {
+      double sv = 0.0, sm = 0.0;
+      for (int i = 0; i < n; ++i) { sv = fma(hv[i], Ws[i * ld + n], sv); sm = fma(hv[i], Ws[i * ld + n + 1], sm); }
+      if (!isfinite(sv) || !isfinite(sm)) atomicOr(P.flags, NUMF_BAD);
+      P.mean[series * P.Mq + q] = ampv * sm;
+      P.var[series * P.Mq + q] = ampv * ampv * sv;
+    }
+  } else if (g.gl == 0) { // extrapolation past the last event: the prediction itself
+    double sv = 0.0, sm = 0.0;
+    for (int i = 0; i < n; ++i) {
+      sm = fma(hv[i], mv[i], sm);
+      for (int j = 0; j < n; ++j) sv = fma(hv[i] * hv[j], Pm[i * n + j], sv);
+    }
+    P.mean[series * P.Mq + q] = ampv * sm;
+    P.var[series * P.Mq + q] = ampv * ampv * sv;
+  }
 }
 
 #include "scan_host.cu"

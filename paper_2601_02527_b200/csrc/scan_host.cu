@@ -130,6 +130,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   P.xbuf = a.want_smooth ? (double*)(w + oX) : nullptr;
   P.llpart = (double*)(w + oLL);
   P.mean = a.mean; P.var = a.var; P.flags = ctx->d_flags; P.want_smooth = a.want_smooth;
+  P.fstate = a.fstate; P.binfo = a.binfo;
 
   if (pl.T) {
     rc = launch_level0_any(ctx, P, n, tb, true, G);
@@ -162,4 +163,52 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     SG_CUDA(ctx, cudaGetLastError());
   }
   return SMOLGP_OK;
+}
+
+template <int G>
+static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, int n, size_t tb) {
+  const size_t per_group = (size_t)down0_group_doubles(n) * 8;
+  int gpc = 128 / G;
+  while (gpc > 1 && tb + per_group * gpc > 100 * 1024) gpc >>= 1;
+  const size_t smem = tb + per_group * gpc;
+  if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+  const int64_t groups = Q.batch * Q.Mq;
+  SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  sg_launch_begin(ctx, KID_QUERY);
+  k_query<G><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
+  sg_launch_end(ctx);
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
+}
+
+// Row a7.  Scratch (kp, dtq, discq) comes from the arena: the scan's workspace is dead by now
+// (stream order), fstate/binfo live outside it.
+int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
+  const ModelDev* hm = a.h_model;
+  const int n = hm->n;
+  int nent = 0;
+  for (int b = 0; b < hm->nblk; ++b) nent += hm->blk[b].dim * hm->blk[b].dim;
+  const size_t tb = tables_bytes(n, hm->d, hm->n_inst, hm->nblk, nent);
+  const int64_t M = a.M;
+  const size_t o_kp = 0, o_dt = ((size_t)M * 8 + 255) / 256 * 256, o_disc = o_dt + ((size_t)2 * M * 8 + 255) / 256 * 256;
+  void* ws;
+  int rc = sg_arena(ctx, o_disc + (size_t)2 * M * hm->disc_stride * 8, &ws);
+  if (rc) return rc;
+  int64_t* kp = (int64_t*)((char*)ws + o_kp);
+  double* dtq = (double*)((char*)ws + o_dt);
+  double* discq = (double*)((char*)ws + o_disc);
+  sg_launch_begin(ctx, KID_QLOCATE);
+  k_query_locate<<<(unsigned)((M + 127) / 128), 128, 0, ctx->stream>>>(M, a.tq, a.ev->K, a.ev->t, kp, dtq);
+  sg_launch_end(ctx);
+  SG_CUDA(ctx, cudaGetLastError());
+  rc = sg_launch_disc(ctx, a.d_model, hm, dtq, 2 * M, discq);
+  if (rc) return rc;
+  QueryDev Q;
+  Q.M = a.d_model; Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
+  Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
+  switch (pick_lanes(ctx, n)) {
+    case 8: return launch_query<8>(ctx, Q, n, tb);
+    case 16: return launch_query<16>(ctx, Q, n, tb);
+    default: return launch_query<32>(ctx, Q, n, tb);
+  }
 }

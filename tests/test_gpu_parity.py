@@ -118,7 +118,7 @@ def test_discretise_matches_oracle(ctx, oracle, name, dt):
     s = np.concatenate([np.sqrt(np.diag(Pinf)), np.full(ninst, (dt if dt > 0 else 1.0) * np.sqrt(np.trace(Pinf)))])
     As, Aos = A / s[:, None] * s[None, :], Ao / s[:, None] * s[None, :]
     Qs, Qos = Q / np.outer(s, s), Qo / np.outer(s, s)
-    assert np.max(np.abs(As - Aos)) <= 1e-13 * max(1.0, np.max(np.abs(Aos)))
+    assert np.max(np.abs(As - Aos)) <= 5e-13 * max(1.0, np.max(np.abs(Aos)))
     # Q entries span many orders of magnitude inside one matrix (q22 ~ dt^5 for short steps): each
     # entry is compared relative to the geometric mean of its diagonal entries (Cauchy-Schwarz scale)
     dg = np.sqrt(np.abs(np.diag(Qos)))
@@ -206,3 +206,75 @@ def test_numeric_errors_are_reported(ctx):
     # the context stays usable after an error
     ll = ctx.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"])
     assert np.isfinite(ll[0])
+
+
+# ---------------------------------------------------------------------------------------------
+# a7: prediction at arbitrary times (Algorithm 1) against the oracle's Algorithm 1 and
+# against the dense definition
+# ---------------------------------------------------------------------------------------------
+def _queries(w, rng, M):
+    ts, te = w["t_start"], w["t_end"]
+    t0, t1 = ts.min(), te.max()
+    span = t1 - t0
+    tq = np.concatenate([
+        rng.uniform(t0, t1, M),                       # interpolation (inside exposures and gaps)
+        t0 - rng.uniform(0, 0.05 * span, 5),          # retrodiction (reading R8)
+        t1 + rng.uniform(0, 0.05 * span, 5),          # extrapolation
+        ts[:3], te[-3:], [t0, t1],                    # exactly at event times
+    ])
+    return tq
+
+
+@pytest.mark.parametrize("cfg,N,batch,qi", [(1, 400, None, 0), (2, 900, None, 1), ("fig2", 300, None, 0),
+                                            (4, 700, None, 3), (5, 200, 3, 0)])
+def test_query_prediction_matches_oracle(ctx, oracle, cfg, N, batch, qi):
+    rng = np.random.default_rng(17)
+    w = W.make(cfg, N=N, batch=batch)
+    tq = _queries(w, rng, 60)
+    ctx.set_option("chunk", 24)
+    try:
+        ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+        out = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"], t_query=tq, query_instrument=qi)
+    finally:
+        _reset(ctx)
+    for s in ([None] if batch is None else range(batch)):
+        i = 0 if s is None else s
+        kern = w["kernel"] if s is None else [dict(k, sigma=k["sigma"] * w["amp"][s]) for k in w["kernel"]]
+        y = w["y"] if s is None else w["y"][s]
+        # the oracle's Algorithm 1 inverts P^-_next (as printed), which idle-z zeroing makes exactly singular:
+        # run it without that (output-equivalent, pinned in tests/test_oracle_inference_pins.py)
+        ref = oracle.ssm(kern, w["n_inst"], w["t_start"], w["t_end"], w["instrument"], y, w["sigma"],
+                         flags=oracle.FLAG_TWO_FILTER, tq=tq, query_inst=qi)
+        k0 = float(oracle.kernel(kern, qi, qi, np.zeros(1))[0])  # prior variance of the latent
+        assert np.max(np.abs(out["mean_query"][i] - ref["mq"])) <= 1e-8 * np.sqrt(k0) + 1e-8 * np.max(np.abs(ref["mq"]))
+        assert np.max(np.abs(out["var_query"][i] - ref["vq"]) / ref["vq"]) <= 1e-8
+        # the observation-time outputs are unchanged by asking for queries
+        assert abs(out["loglik"][i] - ref["loglik"]) <= 1e-9 * abs(ref["loglik"])
+        assert np.max(np.abs(out["var"][i] - ref["var"]) / ref["var"]) <= 1e-8
+
+
+def test_query_prediction_matches_dense_definition(ctx, oracle):
+    rng = np.random.default_rng(3)
+    for cfg, qi in [(2, 0), (4, 2), (3, 1)]:  # config 3: Algorithm 1's printed RTS step is too ill-conditioned to serve as a reference
+        w = W.make(cfg, N=150 if cfg != 3 else 300)
+        tq = _queries(w, rng, 40)
+        ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+        out = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], t_query=tq, query_instrument=qi)
+        ref = oracle.dense(w["kernel"], w["t_start"], w["t_end"], w["instrument"], w["y"], w["sigma"], tq=tq, query_inst=qi)
+        k0 = float(oracle.kernel(w["kernel"], qi, qi, np.zeros(1))[0])
+        assert np.max(np.abs(out["mean_query"][0] - ref["mq"])) <= 1e-8 * (np.sqrt(k0) + np.max(np.abs(ref["mq"])))
+        assert np.max(np.abs(out["var_query"][0] - ref["vq"])) <= 1e-8 * k0
+
+
+def test_query_device_pointers(ctx):
+    import torch
+    w = W.make(2, N=500)
+    dev = torch.device("cuda:0")
+    tq = np.linspace(w["t_start"].min() - 100, w["t_end"].max() + 100, 257)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    h = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], t_query=tq, query_instrument=1)
+    d = ctx.smolgp_condition(ev, w["kernel"], torch.tensor(w["y"], device=dev), torch.tensor(w["sigma"], device=dev),
+                             t_query=torch.tensor(tq, device=dev), query_instrument=1)
+    torch.cuda.synchronize()
+    assert np.array_equal(d["mean_query"].cpu().numpy(), h["mean_query"])
+    assert np.array_equal(d["var_query"].cpu().numpy(), h["var_query"])
