@@ -1,0 +1,217 @@
+// chunk_dev.cuh -- per-chunk sequential kernels' building blocks (k_fold0, k_down0, k_query).
+//
+// Layout: a group of G lanes (8, 16 or 32 lanes of one warp) works on one chunk.  Every n x n state
+// matrix (P, Lambda, C, A, J) lives in shared memory, row-major with an odd row stride ld >= n + 1
+// (column n carries the companion vector: [P | m], [Lambda | lambda], [A | b], [J | eta]), and lane j
+// OWNS column j: it computes whole columns, so a product with the transition needs no cross-lane
+// reduction.  The transition of one step is never assembled: it is applied straight from the step's
+// discretisation record (block-diagonal Phi_b, integral rows Phi-bar_b), so a
+// product F X costs sum_b (d_b^2 + d_b) + N_inst n_blk FMAs per column instead of n^2.
+//
+//   F  = R [Phi 0; Phi-bar I]  (Eq. 3.7, Eq. 3.17; R zeroes the z rows in `tz`,
+//                               the reset of Eq. 3.11/3.18 folded into the step, reading R2/R6)
+//   z_q row of [Phi-bar I]:  sum_b c_qb Phi-bar_b x_b + z_q   (c_qb = 0 if component b is not in
+//                               instrument q's integrand, Eq. 3.2)
+#pragma once
+#include "scan_dev.cuh"
+
+struct Tab {
+  int n, d, ninst, nblk, stride, ld, ntri;
+  unsigned char bdim[SG_MAXBLK], boff[SG_MAXBLK];
+  short roff[SG_MAXBLK];
+  unsigned char blk_of[SG_NMAX];
+  unsigned char tri_i[SG_NMAX * (SG_NMAX + 1) / 2], tri_j[SG_NMAX * (SG_NMAX + 1) / 2];
+  double cz[SG_MAXINST * SG_MAXBLK]; // [q * nblk + b]
+  double tau[SG_MAXINST];
+};
+
+__host__ __device__ inline int chunk_ld(int n) { return (n + 1) | 1; }
+
+// whole CTA participates; caller syncs afterwards
+__device__ inline void tab_build(const ModelDev* __restrict__ M, Tab* T) {
+  if (threadIdx.x == 0) {
+    const int n = M->n;
+    T->n = n; T->d = M->d; T->ninst = M->n_inst; T->nblk = M->nblk; T->stride = M->disc_stride; T->ld = chunk_ld(n);
+    T->ntri = n * (n + 1) / 2;
+    for (int b = 0; b < M->nblk; ++b) {
+      T->bdim[b] = (unsigned char)M->blk[b].dim; T->boff[b] = (unsigned char)M->blk[b].off; T->roff[b] = (short)M->disc_off[b];
+      for (int i = 0; i < M->blk[b].dim; ++i) T->blk_of[M->blk[b].off + i] = (unsigned char)b;
+      for (int q = 0; q < M->n_inst; ++q) T->cz[q * M->nblk + b] = M->cz[q][b];
+    }
+    for (int q = 0; q < M->n_inst; ++q) T->tau[q] = M->tau[q];
+    int e = 0;
+    for (int i = 0; i < n; ++i) for (int j = 0; j <= i; ++j) { T->tri_i[e] = (unsigned char)i; T->tri_j[e] = (unsigned char)j; ++e; }
+  }
+}
+
+// ---- record staging: global -> shared with cp.async (LDGSTS), one 8-byte copy per element ----------
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+template <int G>
+__device__ __forceinline__ void stage_rec(const Grp<G>& g, const Tab& T, const double* __restrict__ src, double* dst) {
+  for (int e = g.gl; e < T.stride; e += G) cp_async8(dst + e, src + e);
+  cp_async_commit();
+}
+
+// ---- one block of out = F v ------------------------------------------------------------------------
+template <int DB>
+__device__ __forceinline__ double blk_F(const double* __restrict__ r, const double* vp, int vs, double* op, int os, int off) {
+  double w[DB];
+#pragma unroll
+  for (int l = 0; l < DB; ++l) w[l] = vp[(off + l) * vs];
+#pragma unroll
+  for (int i = 0; i < DB; ++i) {
+    double acc = 0.0;
+#pragma unroll
+    for (int l = 0; l < DB; ++l) acc = fma(r[i * DB + l], w[l], acc);
+    op[(off + i) * os] = acc;
+  }
+  double u = 0.0;
+#pragma unroll
+  for (int l = 0; l < DB; ++l) u = fma(r[DB * DB + l], w[l], u); // Phi-bar_b . v_b
+  return u;
+}
+
+// out = F v for the calling lane's vector: v[i] = vp[i * vs], out[i] = op[i * os] (i < n).
+// U: lane-private scratch of nblk doubles at stride G.  `rec` in shared memory.
+template <int G>
+__device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigned tz, const double* vp, int vs, double* op, int os,
+                                        double* U) {
+  const int nblk = T.nblk, d = T.d;
+  for (int b = 0; b < nblk; ++b) {
+    const double* r = rec + T.roff[b];
+    const int off = T.boff[b];
+    double u;
+    switch (T.bdim[b]) {
+      case 2: u = blk_F<2>(r, vp, vs, op, os, off); break;
+      case 3: u = blk_F<3>(r, vp, vs, op, os, off); break;
+      default: u = blk_F<4>(r, vp, vs, op, os, off); break;
+    }
+    U[b * G] = u;
+  }
+  for (int q = 0; q < T.ninst; ++q) {
+    double acc = 0.0;
+    if (!((tz >> q) & 1u)) {
+      acc = vp[(d + q) * vs];
+      for (int b = 0; b < nblk; ++b) acc = fma(T.cz[q * nblk + b], U[b * G], acc);
+    }
+    op[(d + q) * os] = acc;
+  }
+}
+
+// ---- one block of out = F^T v ----------------------------------------------------------------------
+template <int DB>
+__device__ __forceinline__ void blk_Ft(const double* __restrict__ r, const double* vp, int vs, double* op, int os, int off, double s) {
+  double w[DB];
+#pragma unroll
+  for (int i = 0; i < DB; ++i) w[i] = vp[(off + i) * vs];
+#pragma unroll
+  for (int l = 0; l < DB; ++l) {
+    double acc = r[DB * DB + l] * s; // Phi-bar_b[l] * sum_q c_qb v_zq
+#pragma unroll
+    for (int i = 0; i < DB; ++i) acc = fma(r[i * DB + l], w[i], acc);
+    op[(off + l) * os] = acc;
+  }
+}
+
+template <int G>
+__device__ __forceinline__ void apply_Ft(const Tab& T, const double* rec, unsigned tz, const double* vp, int vs, double* op, int os) {
+  const int nblk = T.nblk, d = T.d;
+  for (int b = 0; b < nblk; ++b) {
+    double s = 0.0;
+    for (int q = 0; q < T.ninst; ++q)
+      if (!((tz >> q) & 1u)) s = fma(T.cz[q * nblk + b], vp[(d + q) * vs], s);
+    const double* r = rec + T.roff[b];
+    const int off = T.boff[b];
+    switch (T.bdim[b]) {
+      case 2: blk_Ft<2>(r, vp, vs, op, os, off, s); break;
+      case 3: blk_Ft<3>(r, vp, vs, op, os, off, s); break;
+      default: blk_Ft<4>(r, vp, vs, op, os, off, s); break;
+    }
+  }
+  for (int q = 0; q < T.ninst; ++q) op[(d + q) * os] = ((tz >> q) & 1u) ? 0.0 : vp[(d + q) * vs];
+}
+
+// column j of X += column j of Q = R Q~ R^T (Eq. 3.10 P:403-405 per block; z rows through c_qb)
+__device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsigned tz, int j, double* X) {
+  const int d = T.d, ld = T.ld, nblk = T.nblk;
+  if (j < d) {
+    const int b = T.blk_of[j], db = T.bdim[b], off = T.boff[b], jj = j - off;
+    const double* r = rec + T.roff[b];
+    const double* qxx = r + db * db + db;
+    for (int i = 0; i < db; ++i) X[(off + i) * ld + j] += qxx[i * db + jj];
+    const double q12 = r[2 * db * db + db + jj];
+    for (int q = 0; q < T.ninst; ++q)
+      if (!((tz >> q) & 1u)) X[(d + q) * ld + j] = fma(T.cz[q * nblk + b], q12, X[(d + q) * ld + j]);
+  } else if (j < T.n) {
+    const int q = j - d;
+    if ((tz >> q) & 1u) return;
+    for (int b = 0; b < nblk; ++b) {
+      const int db = T.bdim[b], off = T.boff[b];
+      const double* r = rec + T.roff[b];
+      const double c = T.cz[q * nblk + b];
+      if (c == 0.0) continue;
+      for (int l = 0; l < db; ++l) X[(off + l) * ld + j] = fma(c, r[2 * db * db + db + l], X[(off + l) * ld + j]);
+      const double q22 = r[2 * db * db + 2 * db];
+      for (int p = 0; p < T.ninst; ++p)
+        if (!((tz >> p) & 1u)) X[(d + p) * ld + j] = fma(c * T.cz[p * nblk + b], q22, X[(d + p) * ld + j]);
+    }
+  }
+}
+
+// X <- F X F^T (+ Q) for a symmetric X (columns 0..n-1) and x <- F x for the companion column n.
+// Tm: scratch of the same shape.  Two column-owned products:  Tm = F [X | x];  X[:, j] = F (Tm[j, :])^T.
+template <int G, bool ADDQ>
+__device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm, double* U) {
+  const int n = T.n, ld = T.ld;
+  for (int j = g.gl; j <= n; j += G) apply_F<G>(T, rec, tz, X + j, ld, Tm + j, ld, U);
+  g.sync();
+  for (int j = g.gl; j <= n; j += G) {
+    if (j < n) {
+      apply_F<G>(T, rec, tz, Tm + j * ld, 1, X + j, ld, U);
+      if (ADDQ) add_Q_col(T, rec, tz, j, X);
+    } else {
+      for (int i = 0; i < n; ++i) X[i * ld + n] = Tm[i * ld + n];
+    }
+  }
+  g.sync();
+}
+
+// X <- F^T X F, x <- F^T x (the adjoint / information direction)
+template <int G>
+__device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm) {
+  const int n = T.n, ld = T.ld;
+  for (int j = g.gl; j <= n; j += G) apply_Ft<G>(T, rec, tz, X + j, ld, Tm + j, ld);
+  g.sync();
+  for (int j = g.gl; j <= n; j += G) {
+    if (j < n) apply_Ft<G>(T, rec, tz, Tm + j * ld, 1, X + j, ld);
+    else for (int i = 0; i < n; ++i) X[i * ld + n] = Tm[i * ld + n];
+  }
+  g.sync();
+}
+
+// X <- (X + X^T) / 2 on columns 0..n-1
+template <int G>
+__device__ __forceinline__ void symmetrise(const Grp<G>& g, const Tab& T, double* X) {
+  const int ld = T.ld;
+  for (int e = g.gl; e < T.ntri; e += G) {
+    const int i = T.tri_i[e], j = T.tri_j[e];
+    const double w = 0.5 * (X[i * ld + j] + X[j * ld + i]);
+    X[i * ld + j] = w;
+    X[j * ld + i] = w;
+  }
+  g.sync();
+}
+
+// sum over the group's lanes
+template <int G>
+__device__ __forceinline__ double group_sum(const Grp<G>& g, double v) {
+#pragma unroll
+  for (int o = G / 2; o; o >>= 1) v += __shfl_xor_sync(g.mask, v, o);
+  return v;
+}

@@ -16,7 +16,7 @@
 // With one chunk per series (Lc >= K) only k_down0 runs: the sequential per-series filter (row a8).
 #include <math.h>
 
-#include "scan_dev.cuh"
+#include "chunk_dev.cuh"
 
 #define NUMF_BAD 1
 
@@ -40,7 +40,7 @@ struct ScanDev {
   double* E1;      // [batch*c1][elem]
   const double* PRE1; // [batch*c1][state] or NULL (prior)
   const double* SUF1; // [batch*c1][state] or NULL (zero)
-  double* xbuf;    // [batch*N][state] filtered state at each end event
+  double* kbuf;    // [batch*N][2n+4] per end event: gain K, filtered z-column p, S, v, filtered z mean
   double* fstate;  // [batch*K][state] post-event filtered state of every event, or NULL (a7)
   double* binfo;   // [batch*K][state] information [eta | J] about the pre-update state of every event, or NULL (a7)
   double* llpart;  // [batch*c1]
@@ -56,96 +56,100 @@ __device__ __forceinline__ void zero_fill(const Grp<G>& g, double* p, int cnt) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// k_fold0: chunk -> element
+// k_fold0: chunk -> element.  Column-owned layout of chunk_dev.cuh.
 // ---------------------------------------------------------------------------------------------------
-__host__ __device__ inline int fold0_group_doubles(int n) { return 7 * n * n + 5 * n + 2; }
+__host__ __device__ inline int fold0_group_doubles(int n, int stride, int nblk, int G) {
+  return 5 * n * chunk_ld(n) + 2 * stride + nblk * G + 2 * (n + 1) + 2;
+}
 
 template <int G>
 __global__ void __launch_bounds__(128) k_fold0(ScanDev P) {
   extern __shared__ __align__(16) char smem[];
-  Tables T;
-  tables_build(P.M, smem, T);
+  Tab& T = *(Tab*)smem;
+  tab_build(P.M, &T);
   __syncthreads();
-  const int n = T.n, d = T.d, n1 = n + 1;
-  const size_t tb = tables_bytes(n, d, T.ninst, T.nblk, T.nent);
+  const int n = T.n, d = T.d, ld = T.ld;
+  const size_t tb = (sizeof(Tab) + 15) / 16 * 16;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * fold0_group_doubles(n);
-  double* Fs = base;            // n*n
-  double* Qs = Fs + n * n;      // n*n
-  double* AB0 = Qs + n * n;     // n*(n+1)
-  double* AB1 = AB0 + n * n1;   // n*(n+1)
-  double* C = AB1 + n * n1;     // n*n
-  double* Tm = C + n * n;       // n*n
-  double* JE = Tm + n * n;      // n*(n+1)
-  double* av = JE + n * n1;     // n+1
-  double* cv = av + n1;         // n
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * fold0_group_doubles(n, T.stride, T.nblk, G);
+  double* AB0 = base;            // [A | b]
+  double* AB1 = AB0 + n * ld;
+  double* C = AB1 + n * ld;
+  double* Tm = C + n * ld;
+  double* JE = Tm + n * ld;      // [J | eta]
+  double* recs = JE + n * ld;    // 2 x stride
+  double* U = recs + 2 * T.stride + g.gl;
+  double* av = recs + 2 * T.stride + T.nblk * G; // n + 1
+  double* cv = av + n + 1;                        // n
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
 
-  zero_fill(g, Fs, 2 * n * n);
-  zero_fill(g, AB0, n * n1);
-  zero_fill(g, C, n * n);
-  zero_fill(g, JE, n * n1);
+  stage_rec(g, T, P.disc + k0 * (int64_t)T.stride, recs);
+  zero_fill(g, AB0, 5 * n * ld);
   g.sync();
-  for (int i = g.gl; i < n; i += G) AB0[i * n1 + i] = 1.0;
+  for (int i = g.gl; i < n; i += G) AB0[i * ld + i] = 1.0;
   g.sync();
 
   for (int64_t k = k0; k < k1; ++k) {
+    const double* rec = recs + ((k - k0) & 1) * T.stride;
+    cp_async_wait_all();
+    g.sync();
+    if (k + 1 < k1) stage_rec(g, T, P.disc + (k + 1) * (int64_t)T.stride, recs + ((k + 1 - k0) & 1) * T.stride);
     const uint32_t meta = P.meta[k];
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
-    assemble_step(g, T, P.disc + k * (int64_t)T.stride, tz, Fs, Qs);
-    g.sync();
-    lmul_F(g, T, Fs, AB0, n1, 1, AB1, n1, 1, n1); // [A | b] <- F [A | b]
-    lmul_F(g, T, Fs, C, n, 1, Tm, n, 1, n);       // T = F C
-    g.sync();
-    rmul_Ft_sym(g, T, Fs, Tm, Qs, C);             // C <- F C F^T + Q
-    g.sync();
+    // [A | b] <- F [A | b]
+    for (int j = g.gl; j <= n; j += G) apply_F<G>(T, rec, tz, AB0 + j, ld, AB1 + j, ld, U);
     { double* t = AB0; AB0 = AB1; AB1 = t; }
+    // C <- F C F^T + Q
+    sandwich_F<G, true>(g, T, rec, tz, C, Tm, U);
     if (!kind) {
-      // observe z_q / delta: h = hs e_z in equilibrated units (Eq. 3.12); SG21 Eq. 10 with
-      // the aggregate as the earlier element (rank-one J_j): Sherman-Morrison form of the combine
+      // observe z_q / delta: h = hs e_z in equilibrated units (Eq. 3.12); SG21 Eq. 10 with the
+      // aggregate as the earlier element (rank-one J_j): Sherman-Morrison form of the combine
       const int zi = d + q;
       const int32_t ob = P.obs[k];
       const double hs = T.tau[q] / P.delta[k];
       const double sg = P.sigma[ob] * ramp;
       const double yy = P.y[series * P.N + ob] * ramp;
-      const double S = hs * hs * C[zi * n + zi] + sg * sg;
+      const double S = hs * hs * C[zi * ld + zi] + sg * sg;
       if (!(S > 0.0) || !isfinite(S)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S;
-      for (int j = g.gl; j <= n; j += G) av[j] = hs * AB0[zi * n1 + j];
-      for (int i = g.gl; i < n; i += G) cv[i] = hs * C[i * n + zi];
+      for (int j = g.gl; j <= n; j += G) av[j] = hs * AB0[zi * ld + j];
+      for (int i = g.gl; i < n; i += G) cv[i] = hs * C[i * ld + zi];
       g.sync();
       const double resid = yy - av[n];
-      const float rn1 = 1.0f / (float)n1;
-      for (int e = g.gl; e < n * n1; e += G) {
-        int i, j;
-        divmod_small(e, n1, rn1, i, j);
-        const double aj = (j < n) ? av[j] : -resid; // last column: eta += a resid / S;  b += K resid
-        JE[e] = fma(av[i] * rS, (j < n) ? aj : resid, JE[e]);
-        AB0[e] = fma(-cv[i] * rS, aj, AB0[e]);
-      }
-      for (int e = g.gl; e < T.ntri; e += G) {
-        const int i = T.tri_i[e], j = T.tri_j[e];
-        const double v = fma(-cv[i] * rS, cv[j], C[i * n + j]);
-        C[i * n + j] = v;
-        C[j * n + i] = v;
+      for (int j = g.gl; j <= n; j += G) {
+        // column j of J += a a_j / S, of A -= c a_j / S; last column: eta += a resid / S, b += c resid / S
+        const double aj = (j < n) ? av[j] * rS : resid * rS;
+        const double sgn = (j < n) ? -1.0 : 1.0;
+        for (int i = 0; i < n; ++i) {
+          JE[i * ld + j] = fma(av[i], aj, JE[i * ld + j]);
+          AB0[i * ld + j] = fma(sgn * cv[i], aj, AB0[i * ld + j]);
+        }
+        if (j < n) {
+          const double cj = cv[j] * rS;
+          for (int i = 0; i < n; ++i) C[i * ld + j] = fma(-cv[i], cj, C[i * ld + j]);
+        }
       }
       g.sync();
       // the instrument is idle after its end: zero z_q (reading R6)
-      for (int j = g.gl; j <= n; j += G) AB0[zi * n1 + j] = 0.0;
-      for (int j = g.gl; j < n; j += G) { C[zi * n + j] = 0.0; C[j * n + zi] = 0.0; }
+      for (int j = g.gl; j <= n; j += G) { AB0[zi * ld + j] = 0.0; if (j < n) { C[zi * ld + j] = 0.0; C[j * ld + zi] = 0.0; } }
       g.sync();
     }
   }
   double* out = P.E1 + gid * (int64_t)elem_size(n);
-  for (int e = g.gl; e < n * n1; e += G) { out[e] = AB0[e]; out[n * n1 + n * n + e] = JE[e]; }
-  for (int e = g.gl; e < n * n; e += G) out[n * n1 + e] = C[e];
+  const int n1 = n + 1;
+  for (int j = g.gl; j <= n; j += G)
+    for (int i = 0; i < n; ++i) {
+      out[i * n1 + j] = AB0[i * ld + j];
+      out[n * n1 + n * n + i * n1 + j] = JE[i * ld + j];
+      if (j < n) out[n * n1 + i * n + j] = 0.5 * (C[i * ld + j] + C[j * ld + i]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -364,203 +368,203 @@ __global__ void __launch_bounds__(64) k_downD(DenseArgs P) {
   }
 }
 
-// Backward information step over one transition (F, Q):  J <- F^T (I + J Q)^-1 J F,
-// eta <- F^T (I + J Q)^-1 eta  (the (eta, J) part of the SG21 combine with a primitive start-type
-// element on the left, reading R1).  Ws: n x (2n+1), Tm: n x n scratch.  Ends synchronised.
-template <int G>
-__device__ void info_backstep(const Grp<G>& g, const Tables& T, const double* Fs, const double* Qs, double* Jm, double* ev,
-                              double* Ws, double* Tm) {
-  const int n = T.n, ld = 2 * n + 1;
-  mm(g, n, n, n, Jm, n, 1, Qs, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1);
-  g.sync();
-  for (int e = g.gl; e < n * n; e += G) { const int i = e / n, j = e - i * n; Ws[i * ld + n + j] = Jm[e]; }
-  for (int i = g.gl; i < n; i += G) { Ws[i * ld + i] += 1.0; Ws[i * ld + 2 * n] = ev[i]; }
-  g.sync();
-  gj_solve(g, n, ld, Ws);
-  // Tm = F^T Y ; eta = F^T y ; J = F^T Tm^T  (Y symmetric)
-  lmul_Ft(g, T, Fs, Ws + n, ld, 1, Tm, n, 1, n);
-  lmul_Ft(g, T, Fs, Ws + 2 * n, ld, 0, ev, 1, 0, 1);
-  g.sync();
-  lmul_Ft(g, T, Fs, Tm, 1, n, Jm, n, 1, n); // src = Tm^T
-  g.sync();
-  // symmetrise (the two triangles were computed independently)
-  for (int e = g.gl; e < T.ntri; e += G) {
-    const int i = T.tri_i[e], j = T.tri_j[e];
-    const double w = 0.5 * (Jm[i * n + j] + Jm[j * n + i]);
-    Jm[i * n + j] = w;
-    Jm[j * n + i] = w;
-  }
-  g.sync();
+// ---------------------------------------------------------------------------------------------------
+// k_down0: per chunk, (1) the plain integrated Kalman filter (Eq. 3.14 predict, 3.15 reset folded into
+// the step, 2.22 update) from the chunk's prefix state: innovations -> log-likelihood terms (Eq. 2.26),
+// and per end event the gain K, innovation (v, S) and the filtered z-column p kept in `kbuf`;
+// (2) the smoother as the adjoint (modified Bryson-Frazier) recursion of that same filter, started
+// from the chunk's suffix information (eta, J) of the reverse scan:
+//     Lambda^ = (I + J P)^-1 J,  lambda^ = (I + J P)^-1 (J m - eta)        at the chunk's last event,
+//     end event:  smoothed  m^ = m_f - P_f lambda^,  P^ = P_f - P_f Lambda^ P_f   (z entries only),
+//                 Lambda~ = C^T Lambda^ C + h h^T / S,  lambda~ = C^T lambda^ - h v / S,  C = I - K h^T,
+//     step:       Lambda^ <- F^T Lambda~ F,  lambda^ <- F^T lambda~.
+// It is the two-filter posterior of reading R7 written without any per-event inverse (Lambda^ =
+// (I + J P)^-1 J at every event): the only solves left are one per chunk here and those of the
+// dense levels.  DESIGN.md 5.
+// ---------------------------------------------------------------------------------------------------
+__host__ __device__ inline int kbuf_stride(int n) { return 2 * n + 4; }
+__host__ __device__ inline int down0_group_doubles(int n, int stride, int nblk, int G) {
+  return 2 * n * chunk_ld(n) + n * (2 * n + 1) + 2 * stride + nblk * G + 5 * (n + 1) + 1;
 }
 
-// ---------------------------------------------------------------------------------------------------
-// k_down0: per chunk, forward Kalman filter from the prefix state, then backward information
-// recursion from the suffix information with the smoothed output at every end event.
-// ---------------------------------------------------------------------------------------------------
-__host__ __device__ inline int down0_group_doubles(int n) { return 7 * n * n + 6 * n + 2; }
+// [vector | matrix(n x n)] in global memory  <->  column-owned [matrix | vector] with row stride ld
+template <int G>
+__device__ __forceinline__ void load_state(const Grp<G>& g, const Tab& T, const double* s, double* X) {
+  const int n = T.n, ld = T.ld;
+  for (int j = g.gl; j <= n; j += G)
+    for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? s[n + i * n + j] : s[i];
+}
+template <int G>
+__device__ __forceinline__ void store_state(const Grp<G>& g, const Tab& T, const double* X, double* s) {
+  const int n = T.n, ld = T.ld;
+  for (int j = g.gl; j <= n; j += G)
+    for (int i = 0; i < n; ++i) {
+      if (j < n) s[n + i * n + j] = X[i * ld + j];
+      else s[i] = X[i * ld + n];
+    }
+}
 
 template <int G>
 __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
   extern __shared__ __align__(16) char smem[];
-  Tables T;
-  tables_build(P.M, smem, T);
+  Tab& T = *(Tab*)smem;
+  tab_build(P.M, &T);
   __syncthreads();
-  const int n = T.n, d = T.d;
-  const size_t tb = tables_bytes(n, d, T.ninst, T.nblk, T.nent);
+  const int n = T.n, d = T.d, ld = T.ld;
+  const size_t tb = (sizeof(Tab) + 15) / 16 * 16;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n);
-  double* Fs = base;
-  double* Qs = Fs + n * n;
-  double* Pm = Qs + n * n;
-  double* Tm = Pm + n * n;
-  double* Jm = Tm + n * n;
-  double* Ws = Jm + n * n;           // n x (2n+1)
-  double* mv = Ws + n * (2 * n + 1); // n
-  double* m2 = mv + n;               // n
-  double* ev = m2 + n;               // n
-  double* cv = ev + n;               // n
-  const int ss = state_size(n);
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, T.stride, T.nblk, G);
+  double* X = base;                 // [P | m], later [Lambda | lambda]
+  double* Tm = X + n * ld;
+  double* Ws = Tm + n * ld;         // n x (2n+1)
+  double* recs = Ws + n * (2 * n + 1);
+  double* U = recs + 2 * T.stride + g.gl;
+  double* cv = recs + 2 * T.stride + T.nblk * G; // n
+  double* kv = cv + n + 1;
+  double* pv = kv + n + 1;
+  double* av = pv + n + 1;          // n + 1
+  double* gv = av + n + 1;          // n + 1
+  const int ss = state_size(n), ks = kbuf_stride(n);
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ampv = P.amp ? P.amp[series] : 1.0;
   const double ramp = 1.0 / ampv;
 
-  zero_fill(g, Fs, 2 * n * n);
-  if (P.PRE1) {
-    const double* s = P.PRE1 + gid * (int64_t)ss;
-    for (int e = g.gl; e < n; e += G) mv[e] = s[e];
-    for (int e = g.gl; e < n * n; e += G) Pm[e] = s[n + e];
-  } else {
-    for (int e = g.gl; e < n; e += G) mv[e] = 0.0;
-    for (int e = g.gl; e < n * n; e += G) Pm[e] = P.M->p0[e];
-  }
+  stage_rec(g, T, P.disc + k0 * (int64_t)T.stride, recs);
+  if (P.PRE1) load_state(g, T, P.PRE1 + gid * (int64_t)ss, X);
+  else
+    for (int j = g.gl; j <= n; j += G)
+      for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? P.M->p0[i * n + j] : 0.0;
   g.sync();
   double ll = 0.0;
-  // ---- forward: Eq. 3.14 (predict), 3.15 (reset, folded into the step), 2.22 (update), 2.26 ----
+  // ---- forward ----
   for (int64_t k = k0; k < k1; ++k) {
+    const double* rec = recs + ((k - k0) & 1) * T.stride;
+    cp_async_wait_all();
+    g.sync();
+    if (k + 1 < k1) stage_rec(g, T, P.disc + (k + 1) * (int64_t)T.stride, recs + ((k + 1 - k0) & 1) * T.stride);
     const uint32_t meta = P.meta[k];
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
-    assemble_step(g, T, P.disc + k * (int64_t)T.stride, tz, Fs, Qs);
-    g.sync();
-    lmul_F(g, T, Fs, mv, 1, 0, m2, 1, 0, 1);
-    lmul_F(g, T, Fs, Pm, n, 1, Tm, n, 1, n);
-    g.sync();
-    rmul_Ft_sym(g, T, Fs, Tm, Qs, Pm);
-    g.sync();
-    { double* t = mv; mv = m2; m2 = t; }
+    sandwich_F<G, true>(g, T, rec, tz, X, Tm, U);
     if (!kind) {
       const int zi = d + q;
       const int32_t ob = P.obs[k];
       const double hs = T.tau[q] / P.delta[k];
       const double sg = P.sigma[ob] * ramp;
       const double yy = P.y[series * P.N + ob] * ramp;
-      const double S = hs * hs * Pm[zi * n + zi] + sg * sg;
-      const double v = yy - hs * mv[zi];
+      const double S = hs * hs * X[zi * ld + zi] + sg * sg;
+      const double v = yy - hs * X[zi * ld + n];
       if (!(S > 0.0) || !isfinite(S) || !isfinite(v)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S;
       ll -= 0.5 * (log(6.283185307179586476925286766559 * S) + v * v * rS);
-      for (int i = g.gl; i < n; i += G) cv[i] = hs * Pm[i * n + zi];
+      for (int i = g.gl; i < n; i += G) cv[i] = hs * X[i * ld + zi];
       g.sync();
-      for (int i = g.gl; i < n; i += G) mv[i] = fma(cv[i] * rS, v, mv[i]);
-      for (int e = g.gl; e < T.ntri; e += G) {
-        const int i = T.tri_i[e], j = T.tri_j[e];
-        const double w = fma(-cv[i] * rS, cv[j], Pm[i * n + j]);
-        Pm[i * n + j] = w;
-        Pm[j * n + i] = w;
+      for (int j = g.gl; j <= n; j += G) {
+        const double cj = (j < n) ? -cv[j] * rS : v * rS;
+        for (int i = 0; i < n; ++i) X[i * ld + j] = fma(cv[i], cj, X[i * ld + j]);
       }
       g.sync();
-      if (P.want_smooth) { // X_k: filtered state at the end event (before z_q is dropped)
-        double* x = P.xbuf + (series * P.N + ob) * (int64_t)ss;
-        for (int e = g.gl; e < n; e += G) x[e] = mv[e];
-        for (int e = g.gl; e < n * n; e += G) x[n + e] = Pm[e];
+      if (P.want_smooth) {
+        double* kb = P.kbuf + (series * P.N + ob) * (int64_t)ks;
+        for (int i = g.gl; i < n; i += G) { kb[i] = cv[i] * rS; kb[n + i] = X[i * ld + zi]; }
+        if (g.gl == 0) { kb[2 * n] = S; kb[2 * n + 1] = v; kb[2 * n + 2] = X[zi * ld + n]; }
+        g.sync();
       }
+      // the instrument is idle after its end (reading R6)
+      for (int j = g.gl; j <= n; j += G) { X[zi * ld + j] = 0.0; if (j < n) X[j * ld + zi] = 0.0; }
       g.sync();
-      if (g.gl == 0) mv[zi] = 0.0;
-      for (int j = g.gl; j < n; j += G) { Pm[zi * n + j] = 0.0; Pm[j * n + zi] = 0.0; }
-      g.sync();
+      symmetrise(g, T, X); // the two triangles of F P F^T are rounded independently
     }
-    if (P.fstate) { // row a7: all 2N filtered states are kept for prediction at arbitrary times
-      double* x = P.fstate + (series * P.K + k) * (int64_t)ss;
-      for (int e = g.gl; e < n; e += G) x[e] = mv[e];
-      for (int e = g.gl; e < n * n; e += G) x[n + e] = Pm[e];
-    }
+    if (P.fstate) store_state(g, T, X, P.fstate + (series * P.K + k) * (int64_t)ss); // row a7
   }
   if (g.gl == 0) P.llpart[gid] = ll;
   if (!P.want_smooth) return;
 
-  // ---- backward: information (eta, J) about the state after event k held by all later data ----
+  // ---- adjoint at the chunk's last event from the suffix information ----
+  stage_rec(g, T, P.disc + (k1 - 1) * (int64_t)T.stride, recs);
   if (P.SUF1) {
-    const double* s = P.SUF1 + gid * (int64_t)ss;
-    for (int e = g.gl; e < n; e += G) ev[e] = s[e];
-    for (int e = g.gl; e < n * n; e += G) Jm[e] = s[n + e];
+    const int ld2 = 2 * n + 1;
+    load_state(g, T, P.SUF1 + gid * (int64_t)ss, Tm); // [J | eta]
+    g.sync();
+    for (int j = g.gl; j <= n; j += G)
+      for (int i = 0; i < n; ++i) {
+        double acc = 0.0;
+        for (int l = 0; l < n; ++l) acc = fma(Tm[i * ld + l], X[l * ld + j], acc);
+        if (j < n) { Ws[i * ld2 + j] = acc + (i == j ? 1.0 : 0.0); Ws[i * ld2 + n + j] = Tm[i * ld + j]; }
+        else Ws[i * ld2 + 2 * n] = acc - Tm[i * ld + n];
+      }
+    g.sync();
+    gj_solve(g, n, ld2, Ws);
+    for (int j = g.gl; j <= n; j += G)
+      for (int i = 0; i < n; ++i)
+        X[i * ld + j] = (j < n) ? 0.5 * (Ws[i * ld2 + n + j] + Ws[j * ld2 + n + i]) : Ws[i * ld2 + 2 * n];
   } else {
-    for (int e = g.gl; e < n; e += G) ev[e] = 0.0;
-    for (int e = g.gl; e < n * n; e += G) Jm[e] = 0.0;
+    zero_fill(g, X, n * ld);
   }
   g.sync();
+  // ---- backward ----
   for (int64_t k = k1 - 1; k >= k0; --k) {
+    const double* rec = recs + ((k1 - 1 - k) & 1) * T.stride;
+    cp_async_wait_all();
+    g.sync();
+    if (k > k0) stage_rec(g, T, P.disc + (k - 1) * (int64_t)T.stride, recs + ((k1 - k) & 1) * T.stride);
     const uint32_t meta = P.meta[k];
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
-    // components zeroed after event k carry no information backwards
+    // components zeroed after event k pass nothing backwards (adjoint of the zeroing)
     for (int r = 0; r < T.ninst; ++r)
       if ((zm >> r) & 1u) {
         const int zr = d + r;
-        if (g.gl == 0) ev[zr] = 0.0;
-        for (int j = g.gl; j < n; j += G) { Jm[zr * n + j] = 0.0; Jm[j * n + zr] = 0.0; }
+        for (int j = g.gl; j <= n; j += G) { X[zr * ld + j] = 0.0; if (j < n) X[j * ld + zr] = 0.0; }
       }
     g.sync();
     if (!kind) {
       const int zi = d + q;
       const int32_t ob = P.obs[k];
       const double hs = T.tau[q] / P.delta[k];
-      const double sg = P.sigma[ob] * ramp;
-      const double yy = P.y[series * P.N + ob] * ramp;
-      const double* x = P.xbuf + (series * P.N + ob) * (int64_t)ss;
-      for (int e = g.gl; e < n; e += G) m2[e] = x[e];
-      for (int e = g.gl; e < n * n; e += G) Pm[e] = x[n + e];
+      const double* kb = P.kbuf + (series * P.N + ob) * (int64_t)ks;
+      for (int i = g.gl; i < n; i += G) { kv[i] = kb[i]; pv[i] = kb[n + i]; }
+      const double S = kb[2 * n], v = kb[2 * n + 1], mfz = kb[2 * n + 2];
+      const double rS = 1.0 / S;
       g.sync();
-      // P^ = (I + P J)^-1 P,  m^ = (I + P J)^-1 (m + P eta): solve for the z_q column / the mean
-      const int ld = n + 2;
-      mm(g, n, n, n, Pm, n, 1, Jm, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1);
-      g.sync();
-      for (int i = g.gl; i < n; i += G) {
-        Ws[i * ld + i] += 1.0;
-        Ws[i * ld + n] = Pm[i * n + zi];
-        double acc = m2[i];
-        for (int l = 0; l < n; ++l) acc = fma(Pm[i * n + l], ev[l], acc);
-        Ws[i * ld + n + 1] = acc;
+      double quad = 0.0, kap = 0.0;
+      for (int j = g.gl; j <= n; j += G) {
+        double a = 0.0, b = 0.0;
+        for (int i = 0; i < n; ++i) { const double x = X[i * ld + j]; a = fma(x, pv[i], a); b = fma(x, kv[i], b); }
+        av[j] = a; gv[j] = b;
+        if (j < n) { quad = fma(pv[j], a, quad); kap = fma(kv[j], b, kap); }
       }
+      quad = group_sum(g, quad);
+      kap = group_sum(g, kap);
       g.sync();
-      gj_solve(g, n, ld, Ws);
       if (g.gl == 0) {
-        const double sv = Ws[zi * ld + n], sm = Ws[zi * ld + n + 1];
+        const double sm = mfz - av[n], sv = pv[zi] - quad;
         if (!isfinite(sv) || !isfinite(sm)) atomicOr(P.flags, NUMF_BAD);
-        P.mean[series * P.N + ob] = ampv * hs * sm;          // H~ m^
+        P.mean[series * P.N + ob] = ampv * hs * sm;            // H~ m^
         P.var[series * P.N + ob] = ampv * ampv * hs * hs * sv; // H~ P^ H~^T
-        // the observation's own information: h h^T / r, h y / r
-        const double rr = 1.0 / (sg * sg);
-        Jm[zi * n + zi] += hs * hs * rr;
-        ev[zi] += hs * yy * rr;
+      }
+      // Lambda~ = C^T Lambda^ C + h h^T / S: only row and column z change (h = hs e_z)
+      for (int j = g.gl; j <= n; j += G) {
+        if (j < n) {
+          X[zi * ld + j] -= hs * gv[j];
+          X[j * ld + zi] -= hs * gv[j];
+          if (j == zi) X[zi * ld + zi] += hs * hs * (kap + rS);
+        } else {
+          X[zi * ld + n] -= hs * (gv[n] + v * rS);
+        }
       }
       g.sync();
+      symmetrise(g, T, X);
     }
-    if (P.binfo) {
-      double* x = P.binfo + (series * P.K + k) * (int64_t)ss;
-      for (int e = g.gl; e < n; e += G) x[e] = ev[e];
-      for (int e = g.gl; e < n * n; e += G) x[n + e] = Jm[e];
-    }
+    if (P.binfo) store_state(g, T, X, P.binfo + (series * P.K + k) * (int64_t)ss);
     if (k == k0) break;
-    // back over the step into event k:  J <- F^T (I + J Q)^-1 J F,  eta <- F^T (I + J Q)^-1 eta
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
-    assemble_step(g, T, P.disc + k * (int64_t)T.stride, tz, Fs, Qs);
-    g.sync();
-    info_backstep(g, T, Fs, Qs, Jm, ev, Ws, Tm);
+    sandwich_Ft<G>(g, T, rec, tz, X, Tm);
   }
 }
 
@@ -615,96 +619,82 @@ struct QueryDev {
 template <int G>
 __global__ void __launch_bounds__(128) k_query(QueryDev P) {
   extern __shared__ __align__(16) char smem[];
-  Tables T;
-  tables_build(P.M, smem, T);
+  Tab& T = *(Tab*)smem;
+  tab_build(P.M, &T);
   __syncthreads();
-  const int n = T.n, d = T.d;
-  const size_t tb = tables_bytes(n, d, T.ninst, T.nblk, T.nent);
+  const int n = T.n, ld = T.ld;
+  const size_t tb = (sizeof(Tab) + 15) / 16 * 16;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.Mq) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n);
-  double* Fs = base;
-  double* Qs = Fs + n * n;
-  double* Pm = Qs + n * n;
-  double* Tm = Pm + n * n;
-  double* Jm = Tm + n * n;
-  double* Ws = Jm + n * n;           // n x (2n+1)
-  double* mv = Ws + n * (2 * n + 1); // n
-  double* m2 = mv + n;               // n
-  double* ev = m2 + n;               // n
-  double* hv = ev + n;               // n: H_q in block units
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, T.stride, T.nblk, G);
+  double* X = base;                 // [P* | m*]
+  double* Tm = X + n * ld;
+  double* Y = Tm + n * ld;          // [Lambda* | lambda*]  (the Ws region of k_down0)
+  double* recs = Y + n * (2 * n + 1);
+  double* U = recs + 2 * T.stride + g.gl;
+  double* hv = recs + 2 * T.stride + T.nblk * G; // n: H_q in block units
+  double* ph = hv + n + 1;                        // n: P* h
   const int ss = state_size(n);
   const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
   const int64_t kp = P.kp[q];
   const double ampv = P.amp ? P.amp[series] : 1.0;
-  zero_fill(g, Fs, 2 * n * n);
+  stage_rec(g, T, P.discq + q * (int64_t)T.stride, recs);
+  stage_rec(g, T, P.discq + (P.Mq + q) * (int64_t)T.stride, recs + T.stride);
   for (int i = g.gl; i < n; i += G) hv[i] = 0.0;
   g.sync();
   if (g.gl == 0)
-    for (int b = 0; b < T.nblk; ++b) hv[P.M->blk[b].off] = P.M->hq[P.qinst][b];
-  // ---- state just after the last event at or before t* (stationary prior with idle z = 0 if none) ----
+    for (int b = 0; b < T.nblk; ++b) hv[T.boff[b]] = P.M->hq[P.qinst][b];
+  cp_async_wait_all();
+  g.sync();
+  // ---- state just after the last event at or before t*, predicted over Delta_1 (Eq. 3.14) ----
   if (kp >= 0) {
-    const double* s = P.fstate + (series * P.K + kp) * (int64_t)ss;
-    for (int e = g.gl; e < n; e += G) mv[e] = s[e];
-    for (int e = g.gl; e < n * n; e += G) Pm[e] = s[n + e];
+    load_state(g, T, P.fstate + (series * P.K + kp) * (int64_t)ss, X);
     g.sync();
-    // predict over Delta_1 (Eq. 3.14); instruments idle after event kp stay zeroed
     const uint32_t mp = P.meta[kp]; // idle through (t_kp, t_kp+1): zeroed after kp, except an instrument that just started
     const unsigned idle = META_KIND(mp) ? (META_ZMASK(mp) & ~(1u << META_INST(mp))) : META_ZMASK(mp);
-    assemble_step(g, T, P.discq + q * (int64_t)T.stride, idle, Fs, Qs);
-    g.sync();
-    lmul_F(g, T, Fs, mv, 1, 0, m2, 1, 0, 1);
-    lmul_F(g, T, Fs, Pm, n, 1, Tm, n, 1, n);
-    g.sync();
-    rmul_Ft_sym(g, T, Fs, Tm, Qs, Pm);
-    g.sync();
-    { double* t = mv; mv = m2; m2 = t; }
-  } else {
-    for (int e = g.gl; e < n; e += G) mv[e] = 0.0;
-    for (int e = g.gl; e < n * n; e += G) Pm[e] = P.M->p0[e];
+    sandwich_F<G, true>(g, T, recs, idle, X, Tm, U);
+  } else { // before the first event: the stationary prior, idle z = 0 (retrodiction, reading R8)
+    for (int j = g.gl; j <= n; j += G)
+      for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? P.M->p0[i * n + j] : 0.0;
     g.sync();
   }
-  // ---- information about the state at t* from every later event ----
-  if (kp + 1 < P.K) {
+  // ---- adjoint at t*: the pre-update adjoint of the next event stepped back over Delta_2 ----
+  const bool have_next = kp + 1 < P.K;
+  if (have_next) {
     const int64_t kn = kp + 1;
-    const double* s = P.binfo + (series * P.K + kn) * (int64_t)ss;
-    for (int e = g.gl; e < n; e += G) ev[e] = s[e];
-    for (int e = g.gl; e < n * n; e += G) Jm[e] = s[n + e];
+    load_state(g, T, P.binfo + (series * P.K + kn) * (int64_t)ss, Y);
+    g.sync();
     const uint32_t meta = P.meta[kn];
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = META_KIND(meta) ? zm : (zm & ~(1u << META_INST(meta)));
-    g.sync();
-    assemble_step(g, T, P.discq + (P.Mq + q) * (int64_t)T.stride, tz, Fs, Qs);
-    g.sync();
-    info_backstep(g, T, Fs, Qs, Jm, ev, Ws, Tm);
-    // fuse: P^ = (I + P J)^-1 P, m^ = (I + P J)^-1 (m + P eta); right-hand sides P h and m + P eta
-    const int ld = n + 2;
-    mm(g, n, n, n, Pm, n, 1, Jm, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1);
-    g.sync();
-    for (int i = g.gl; i < n; i += G) {
-      Ws[i * ld + i] += 1.0;
-      double a = 0.0, acc = mv[i];
-      for (int l = 0; l < n; ++l) { a = fma(Pm[i * n + l], hv[l], a); acc = fma(Pm[i * n + l], ev[l], acc); }
-      Ws[i * ld + n] = a;
-      Ws[i * ld + n + 1] = acc;
+    sandwich_Ft<G>(g, T, recs + T.stride, tz, Y, Tm);
+  }
+  // ---- m^ = m* - P* lambda*,  P^ = P* - P* Lambda* P*, projected on H_q ----
+  for (int j = g.gl; j < n; j += G) {
+    double a = 0.0;
+    for (int l = 0; l < n; ++l) a = fma(X[l * ld + j], hv[l], a);
+    ph[j] = a;
+  }
+  g.sync();
+  double sm = 0.0, sv = 0.0;
+  for (int j = g.gl; j <= n; j += G) {
+    if (j < n) {
+      sm = fma(hv[j], X[j * ld + n], sm);
+      sv = fma(hv[j], ph[j], sv);
     }
-    g.sync();
-    gj_solve(g, n, ld, Ws);
-    if (g.gl == 0) {
-      double sv = 0.0, sm = 0.0;
-      for (int i = 0; i < n; ++i) { sv = fma(hv[i], Ws[i * ld + n], sv); sm = fma(hv[i], Ws[i * ld + n + 1], sm); }
-      if (!isfinite(sv) || !isfinite(sm)) atomicOr(P.flags, NUMF_BAD);
-      P.mean[series * P.Mq + q] = ampv * sm;
-      P.var[series * P.Mq + q] = ampv * ampv * sv;
+    if (have_next) {
+      double a = 0.0;
+      for (int i = 0; i < n; ++i) a = fma(Y[i * ld + j], ph[i], a);
+      if (j < n) sv = fma(-ph[j], a, sv);
+      else sm -= a;
     }
-  } else if (g.gl == 0) { // extrapolation past the last event: the prediction itself
-    double sv = 0.0, sm = 0.0;
-    for (int i = 0; i < n; ++i) {
-      sm = fma(hv[i], mv[i], sm);
-      for (int j = 0; j < n; ++j) sv = fma(hv[i] * hv[j], Pm[i * n + j], sv);
-    }
+  }
+  sm = group_sum(g, sm);
+  sv = group_sum(g, sv);
+  if (g.gl == 0) {
+    if (!isfinite(sv) || !isfinite(sm)) atomicOr(P.flags, NUMF_BAD);
     P.mean[series * P.Mq + q] = ampv * sm;
     P.var[series * P.Mq + q] = ampv * ampv * sv;
   }

@@ -8,17 +8,25 @@ struct LevelPlan {
 
 static int pick_lanes(const smolgp_ctx* ctx, int n) {
   if (ctx->opt_lanes == 8 || ctx->opt_lanes == 16 || ctx->opt_lanes == 32) return (int)ctx->opt_lanes;
-  return n <= 4 ? 8 : (n <= 8 ? 16 : 32);
+  return n + 1 <= 8 ? 8 : (n + 1 <= 16 ? 16 : 32); // one lane per column of [X | x]
+}
+
+static inline size_t tab_bytes() { return (sizeof(Tab) + 15) / 16 * 16; }
+
+// groups per CTA: as many as fit in ~72 KB (three CTAs per SM), at most 128 threads
+static int groups_per_cta(size_t per_group, int G) {
+  int gpc = 128 / G;
+  while (gpc > 1 && tab_bytes() + per_group * gpc > 72 * 1024) gpc >>= 1;
+  return gpc;
 }
 
 template <int G>
-static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, int n, size_t tb, bool fold) {
-  const int gd = fold ? fold0_group_doubles(n) : down0_group_doubles(n);
+static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold) {
+  const int n = hm->n;
+  const int gd = fold ? fold0_group_doubles(n, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, hm->disc_stride, hm->nblk, G);
   const size_t per_group = (size_t)gd * 8;
-  // groups per CTA: as many as fit in ~100 KB (two CTAs per SM), at most 128 threads
-  int gpc = 128 / G;
-  while (gpc > 1 && tb + per_group * gpc > 100 * 1024) gpc >>= 1;
-  const size_t smem = tb + per_group * gpc;
+  const int gpc = groups_per_cta(per_group, G);
+  const size_t smem = tab_bytes() + per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = P.batch * P.c1;
   const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
@@ -36,11 +44,11 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, int n, size_t tb, bo
   return SMOLGP_OK;
 }
 
-static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, int n, size_t tb, bool fold, int G) {
+static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G) {
   switch (G) {
-    case 8: return launch_level0<8>(ctx, P, n, tb, fold);
-    case 16: return launch_level0<16>(ctx, P, n, tb, fold);
-    default: return launch_level0<32>(ctx, P, n, tb, fold);
+    case 8: return launch_level0<8>(ctx, P, hm, fold);
+    case 16: return launch_level0<16>(ctx, P, hm, fold);
+    default: return launch_level0<32>(ctx, P, hm, fold);
   }
 }
 
@@ -78,14 +86,16 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   const int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 8;
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
-  // already fills it runs one chunk per series (the sequential filter)
+  // already fills it runs one chunk per series (the sequential filter, row a8)
   int64_t Lc = ctx->opt_chunk;
   if (Lc <= 0) {
-    const size_t per_group = (size_t)down0_group_doubles(n) * 8;
-    int64_t resident = (int64_t)ctx->sm_count * (int64_t)((200 * 1024) / (per_group ? per_group : 1));
-    const int64_t cap = (int64_t)ctx->sm_count * 64 * (32 / G);
-    if (resident > cap) resident = cap;
-    if (resident < ctx->sm_count) resident = ctx->sm_count;
+    const size_t per_group = (size_t)down0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8;
+    const int gpc = groups_per_cta(per_group, G);
+    const size_t cta = tab_bytes() + per_group * gpc;
+    int64_t ctas = (int64_t)((220 * 1024) / cta);
+    if (ctas > 16) ctas = 16;
+    if (ctas < 1) ctas = 1;
+    const int64_t resident = (int64_t)ctx->sm_count * ctas * gpc;
     const int64_t target = 2 * resident;
     if (batch >= target) Lc = K;
     else {
@@ -114,7 +124,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     oPRE[l] = add((size_t)batch * pl.cnt[l] * ss * 8);
     oSUF[l] = a.want_smooth ? add((size_t)batch * pl.cnt[l] * ss * 8) : 0;
   }
-  const size_t oX = a.want_smooth ? add((size_t)batch * N * ss * 8) : 0;
+  const size_t oX = a.want_smooth ? add((size_t)batch * N * kbuf_stride(n) * 8) : 0;
   const size_t oLL = add((size_t)batch * c1 * 8);
   void* ws;
   int rc = sg_arena(ctx, bytes, &ws);
@@ -127,13 +137,13 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   P.E1 = pl.T ? (double*)(w + oE[1]) : nullptr;
   P.PRE1 = pl.T ? (const double*)(w + oPRE[1]) : nullptr;
   P.SUF1 = (pl.T && a.want_smooth) ? (const double*)(w + oSUF[1]) : nullptr;
-  P.xbuf = a.want_smooth ? (double*)(w + oX) : nullptr;
+  P.kbuf = a.want_smooth ? (double*)(w + oX) : nullptr;
   P.llpart = (double*)(w + oLL);
   P.mean = a.mean; P.var = a.var; P.flags = ctx->d_flags; P.want_smooth = a.want_smooth;
   P.fstate = a.fstate; P.binfo = a.binfo;
 
   if (pl.T) {
-    rc = launch_level0_any(ctx, P, n, tb, true, G);
+    rc = launch_level0_any(ctx, P, hm, true, G);
     if (rc) return rc;
     for (int l = 1; l < pl.T; ++l) {
       DenseArgs D = {};
@@ -153,7 +163,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
       if (rc) return rc;
     }
   }
-  rc = launch_level0_any(ctx, P, n, tb, false, G);
+  rc = launch_level0_any(ctx, P, hm, false, G);
   if (rc) return rc;
   if (a.loglik) {
     const int wpb = 4;
@@ -166,11 +176,10 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
 }
 
 template <int G>
-static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, int n, size_t tb) {
-  const size_t per_group = (size_t)down0_group_doubles(n) * 8;
-  int gpc = 128 / G;
-  while (gpc > 1 && tb + per_group * gpc > 100 * 1024) gpc >>= 1;
-  const size_t smem = tb + per_group * gpc;
+static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
+  const size_t per_group = (size_t)down0_group_doubles(hm->n, hm->disc_stride, hm->nblk, G) * 8;
+  const int gpc = groups_per_cta(per_group, G);
+  const size_t smem = tab_bytes() + per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = Q.batch * Q.Mq;
   SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -207,8 +216,8 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   Q.M = a.d_model; Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
   Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
   switch (pick_lanes(ctx, n)) {
-    case 8: return launch_query<8>(ctx, Q, n, tb);
-    case 16: return launch_query<16>(ctx, Q, n, tb);
-    default: return launch_query<32>(ctx, Q, n, tb);
+    case 8: return launch_query<8>(ctx, Q, hm);
+    case 16: return launch_query<16>(ctx, Q, hm);
+    default: return launch_query<32>(ctx, Q, hm);
   }
 }
