@@ -33,6 +33,15 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   int v = 0;
   cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device); c->sm_count = v;
   cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device); c->smem_optin = (size_t)v;
+  {
+    // keep freed stream-ordered allocations in the pool instead of returning them at every synchronise
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+      unsigned long long thr = ~0ull;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    cudaGetLastError();
+  }
   if (cudaMalloc(&c->d_flags, 64) != cudaSuccess) { cudaGetLastError(); delete c->hmodel; delete c; return SMOLGP_ENOMEM; }
   cudaMemset(c->d_flags, 0, 64);
   *out = c;
@@ -129,7 +138,7 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
     if (!qs.tq || !qs.mean || !qs.var) { ctx->err = "condition: t_query, mean_query and var_query are required when M > 0"; return SMOLGP_EINVAL; }
     if (qs.qinst < 0 || qs.qinst >= ev->n_inst) { ctx->err = "condition: query_instrument out of range"; return SMOLGP_EINVAL; }
     const size_t one = (size_t)batch * ev->K * (hm.n + hm.n * hm.n) * 8;
-    if (cudaMalloc(&qstore, 2 * one) != cudaSuccess) { cudaGetLastError(); ctx->err = "out of device memory (states for query-time prediction)"; return SMOLGP_ENOMEM; }
+    if (cudaMallocAsync(&qstore, 2 * one, ctx->stream) != cudaSuccess) { cudaGetLastError(); ctx->err = "out of device memory (states for query-time prediction)"; return SMOLGP_ENOMEM; }
     a.fstate = qstore; a.binfo = (double*)((char*)qstore + one);
   }
   rc = sg_run_scan(ctx, a);
@@ -139,11 +148,11 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
     q.fstate = a.fstate; q.binfo = a.binfo; q.mean = qs.mean; q.var = qs.var;
     rc = sg_run_query(ctx, q);
   }
-  if (rc) { if (qstore) { cudaStreamSynchronize(ctx->stream); cudaFree(qstore); } return rc; }
+  if (rc) { if (qstore) cudaFreeAsync(qstore, ctx->stream); return rc; }
   int flags = 0;
   cudaError_t ce = cudaMemcpyAsync(&flags, ctx->d_flags, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);
-  if (qstore) cudaFree(qstore);
+  if (qstore) cudaFreeAsync(qstore, ctx->stream);
   SG_CUDA(ctx, ce);
   if (flags) { ctx->err = "non-finite value or non-positive innovation variance (check noise_sigma > 0, amp > 0, finite y)"; return SMOLGP_ENUMERIC; }
   return SMOLGP_OK;
@@ -169,7 +178,8 @@ extern "C" int smolgp_condition(smolgp_ctx* ctx, const smolgp_events* ev, const 
 struct HostStage {
   double *y = nullptr, *sigma = nullptr, *amp = nullptr, *mean = nullptr, *var = nullptr, *ll = nullptr;
   double *tq = nullptr, *mq = nullptr, *vq = nullptr;
-  ~HostStage() { cudaFree(y); cudaFree(sigma); cudaFree(amp); cudaFree(mean); cudaFree(var); cudaFree(ll); cudaFree(tq); cudaFree(mq); cudaFree(vq); }
+  cudaStream_t st = 0;
+  ~HostStage() { for (double* p : {y, sigma, amp, mean, var, ll, tq, mq, vq}) if (p) cudaFreeAsync(p, st); }
 };
 
 static int host_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
@@ -180,9 +190,11 @@ static int host_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kern
   SG_CUDA(ctx, cudaSetDevice(ctx->device));
   const int64_t N = ev->N;
   HostStage s;
+  s.st = ctx->stream;
   const size_t bn = (size_t)batch * N * 8;
-  if (cudaMalloc(&s.y, bn) || cudaMalloc(&s.sigma, N * 8) || (amp && cudaMalloc(&s.amp, batch * 8)) ||
-      (want_smooth && (cudaMalloc(&s.mean, bn) || cudaMalloc(&s.var, bn))) || cudaMalloc(&s.ll, batch * 8)) {
+  auto am = [&](double** p, size_t b) { return cudaMallocAsync(p, b, ctx->stream) != cudaSuccess; };
+  if (am(&s.y, bn) || am(&s.sigma, N * 8) || (amp && am(&s.amp, batch * 8)) ||
+      (want_smooth && (am(&s.mean, bn) || am(&s.var, bn))) || am(&s.ll, batch * 8)) {
     cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM;
   }
   cudaStream_t st = ctx->stream;
@@ -190,7 +202,7 @@ static int host_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kern
   const size_t bm = (size_t)batch * (hq.M > 0 ? hq.M : 0) * 8;
   if (hq.M > 0) {
     if (!hq.tq || !hq.mean || !hq.var) { ctx->err = "condition: t_query, mean_query and var_query are required when M > 0"; return SMOLGP_EINVAL; }
-    if (cudaMalloc(&s.tq, hq.M * 8) || cudaMalloc(&s.mq, bm) || cudaMalloc(&s.vq, bm)) { cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM; }
+    if (am(&s.tq, hq.M * 8) || am(&s.mq, bm) || am(&s.vq, bm)) { cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM; }
     SG_CUDA(ctx, cudaMemcpyAsync(s.tq, hq.tq, hq.M * 8, cudaMemcpyHostToDevice, st));
     qs.M = hq.M; qs.tq = s.tq; qs.qinst = hq.qinst; qs.mean = s.mq; qs.var = s.vq;
   }

@@ -67,6 +67,8 @@ struct smolgp_events {
   uint32_t* meta;  // [K]
   int32_t* obs;    // [K] exposure index
   double tau[SG_MAXINST]; // per-instrument power-of-two scale of z (host copy)
+  void* base;            // one stream-ordered allocation holds all five arrays
+  cudaStream_t stream;   // the ctx stream the allocation is ordered on
   double t_first, t_last;
 };
 

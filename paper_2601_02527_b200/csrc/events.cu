@@ -196,10 +196,16 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   const int64_t K = 2 * N;
   smolgp_events* ev = new smolgp_events();
   ev->device = ctx->device; ev->N = N; ev->K = K; ev->n_inst = n_inst;
-  ev->t = ev->dt = ev->delta = nullptr; ev->meta = nullptr; ev->obs = nullptr;
+  ev->t = ev->dt = ev->delta = nullptr; ev->meta = nullptr; ev->obs = nullptr; ev->base = nullptr; ev->stream = ctx->stream;
   auto fail = [&](int rc) { smolgp_free_events(ev); return rc; };
-  if (cudaMalloc(&ev->t, K * 8) || cudaMalloc(&ev->dt, K * 8) || cudaMalloc(&ev->delta, K * 8) ||
-      cudaMalloc(&ev->meta, K * 4) || cudaMalloc(&ev->obs, K * 4)) { cudaGetLastError(); ctx->err = "build_events: out of device memory"; return fail(SMOLGP_ENOMEM); }
+  // stream-ordered allocation (cudaMallocAsync): no device-wide synchronisation on alloc or free
+  const size_t k8 = ((size_t)K * 8 + 255) / 256 * 256, k4 = ((size_t)K * 4 + 255) / 256 * 256;
+  if (cudaMallocAsync(&ev->base, 3 * k8 + 2 * k4, ctx->stream) != cudaSuccess) { cudaGetLastError(); ev->base = nullptr; ctx->err = "build_events: out of device memory"; return fail(SMOLGP_ENOMEM); }
+  {
+    char* b = (char*)ev->base;
+    ev->t = (double*)b; ev->dt = (double*)(b + k8); ev->delta = (double*)(b + 2 * k8);
+    ev->meta = (uint32_t*)(b + 3 * k8); ev->obs = (int32_t*)(b + 3 * k8 + k4);
+  }
   // scratch: keys, keys_tmp (u64), vals, vals_tmp, bits (u32), hist, tiles, maxdelta
   const int ntiles_rs = (int)((K + RS_TILE - 1) / RS_TILE), ntiles_xs = (int)((K + XS_TILE - 1) / XS_TILE);
   size_t bytes = (size_t)K * (8 + 8 + 4 + 4 + 4) + (size_t)256 * ntiles_rs * 4 + (size_t)ntiles_xs * 4 + SG_MAXINST * 8 + 1024;
@@ -271,21 +277,23 @@ extern "C" int smolgp_build_events_host(smolgp_ctx* ctx, int64_t N, const double
   if (N <= 0 || !t_start || !t_end || !instrument) { ctx->err = "build_events_host: bad argument"; return SMOLGP_EINVAL; }
   SG_CUDA(ctx, cudaSetDevice(ctx->device));
   double *ds = nullptr, *de = nullptr; int32_t* di = nullptr;
-  if (cudaMalloc(&ds, N * 8) || cudaMalloc(&de, N * 8) || cudaMalloc(&di, N * 4)) {
-    cudaGetLastError(); cudaFree(ds); cudaFree(de); cudaFree(di); ctx->err = "build_events_host: out of device memory"; return SMOLGP_ENOMEM;
+  char* stage = nullptr;
+  const size_t n8 = ((size_t)N * 8 + 255) / 256 * 256;
+  if (cudaMallocAsync(&stage, 2 * n8 + (size_t)N * 4, ctx->stream) != cudaSuccess) {
+    cudaGetLastError(); ctx->err = "build_events_host: out of device memory"; return SMOLGP_ENOMEM;
   }
+  ds = (double*)stage; de = (double*)(stage + n8); di = (int32_t*)(stage + 2 * n8);
   cudaMemcpyAsync(ds, t_start, N * 8, cudaMemcpyHostToDevice, ctx->stream);
   cudaMemcpyAsync(de, t_end, N * 8, cudaMemcpyHostToDevice, ctx->stream);
   cudaMemcpyAsync(di, instrument, N * 4, cudaMemcpyHostToDevice, ctx->stream);
   int rc = build_events_impl(ctx, N, ds, de, di, n_inst, out);
-  cudaStreamSynchronize(ctx->stream);
-  cudaFree(ds); cudaFree(de); cudaFree(di);
+  cudaFreeAsync(stage, ctx->stream);
   return rc;
 }
 
 extern "C" void smolgp_free_events(smolgp_events* ev) {
   if (!ev) return;
-  cudaFree(ev->t); cudaFree(ev->dt); cudaFree(ev->delta); cudaFree(ev->meta); cudaFree(ev->obs);
+  if (ev->base) cudaFreeAsync(ev->base, ev->stream); // ordered after every kernel enqueued so far on that stream
   delete ev;
 }
 

@@ -7,13 +7,18 @@
 template <int G>
 struct Grp {
   int gl;        // lane inside the group
-  unsigned mask; // the group's lanes inside the warp
+  unsigned mask; // the group's lanes inside the warp (G <= 32)
   __device__ __forceinline__ Grp() {
-    const int lane = threadIdx.x & 31;
-    gl = lane & (G - 1);
-    mask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << (lane & ~(G - 1)));
+    if (G > 32) { gl = threadIdx.x; mask = 0xffffffffu; } // the group is the whole CTA (blockDim.x == G)
+    else {
+      const int lane = threadIdx.x & 31;
+      gl = lane & (G - 1);
+      mask = (G == 32) ? 0xffffffffu : (((1u << (G & 31)) - 1u) << (lane & ~(G - 1)));
+    }
   }
-  __device__ __forceinline__ void sync() const { __syncwarp(mask); }
+  __device__ __forceinline__ void sync() const {
+    if (G > 32) __syncthreads(); else __syncwarp(mask);
+  }
 };
 
 // e -> (e / nc, e % nc) for small non-negative e (exact: see DESIGN.md "index arithmetic")
@@ -219,19 +224,14 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, const Tables& T, int nk,
 template <int G>
 __device__ void gj_solve(const Grp<G>& g, int n, int ld, double* W) {
   for (int p = 0; p < n; ++p) {
-    // pivot search in column p, rows >= p
+    // pivot search in column p, rows >= p: every lane scans the column itself (broadcast reads)
     double best = -1.0;
     int bi = p;
-    for (int i = p + g.gl; i < n; i += G) {
+    for (int i = p; i < n; ++i) {
       const double v = fabs(W[i * ld + p]);
       if (v > best) { best = v; bi = i; }
     }
-#pragma unroll
-    for (int o = G / 2; o; o >>= 1) {
-      const double ob = __shfl_xor_sync(g.mask, best, o);
-      const int oi = __shfl_xor_sync(g.mask, bi, o);
-      if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
-    }
+    g.sync(); // all lanes have read column p before the swap touches it
     if (bi != p) {
       for (int j = p + g.gl; j < ld; j += G) {
         const double a = W[p * ld + j], b = W[bi * ld + j];

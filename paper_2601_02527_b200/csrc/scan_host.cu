@@ -52,23 +52,21 @@ static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* 
   }
 }
 
+#define SG_DENSE_NT 128 /* threads cooperating on one dense combine (one CTA per group of elements) */
 static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, size_t tb, bool fold) {
   const int gd = fold ? foldD_group_doubles(n) : downD_group_doubles(n);
-  const size_t per_group = (size_t)gd * 8;
-  int gpc = 2;
-  while (gpc > 1 && tb + per_group * gpc > 110 * 1024) gpc >>= 1;
-  const size_t smem = tb + per_group * gpc;
+  const size_t smem = tb + (size_t)gd * 8;
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = D.batch * D.cout;
-  dim3 grid((unsigned)((groups + gpc - 1) / gpc), fold ? 1 : (D.want_suffix ? 2 : 1));
+  dim3 grid((unsigned)groups, fold ? 1 : (D.want_suffix ? 2 : 1));
   if (fold) {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_FOLDD);
-    k_foldD<<<grid, gpc * 32, smem, ctx->stream>>>(D);
+    k_foldD<SG_DENSE_NT><<<grid, SG_DENSE_NT, smem, ctx->stream>>>(D);
   } else {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_downD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_downD<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_DOWND);
-    k_downD<<<grid, gpc * 32, smem, ctx->stream>>>(D);
+    k_downD<SG_DENSE_NT><<<grid, SG_DENSE_NT, smem, ctx->stream>>>(D);
   }
   sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
