@@ -13,35 +13,37 @@
 //   z_q row of [Phi-bar I]:  sum_b c_qb Phi-bar_b x_b + z_q   (c_qb = 0 if component b is not in
 //                               instrument q's integrand, Eq. 3.2)
 #pragma once
+#include <string.h>
+
 #include "scan_dev.cuh"
 
+// Model tables of the chunk kernels.  Passed BY VALUE inside the kernel parameter struct: kernel
+// parameters live in the constant bank, so every table look-up with a warp-uniform index is a
+// uniform load and the block loop's bookkeeping and branches run on the uniform datapath.
 struct Tab {
-  int n, d, ninst, nblk, stride, ld, ntri;
+  int n, d, ninst, nblk, stride, ld;
   unsigned char bdim[SG_MAXBLK], boff[SG_MAXBLK];
   short roff[SG_MAXBLK];
   unsigned char blk_of[SG_NMAX];
-  unsigned char tri_i[SG_NMAX * (SG_NMAX + 1) / 2], tri_j[SG_NMAX * (SG_NMAX + 1) / 2];
   double cz[SG_MAXINST * SG_MAXBLK]; // [q * nblk + b]
   double tau[SG_MAXINST];
+  double hq[SG_MAXINST * SG_MAXBLK]; // [q * nblk + b]: sigma_b if block b is in instrument q's integrand
 };
 
-__host__ __device__ inline int chunk_ld(int n) { return (n + 1) | 1; }
+// row stride of the chunk kernels' matrices: the smallest value = 1 (mod 4) that holds n + 1 columns
+// (odd: conflict-free row reads; a multiple-of-4 family keeps the number of compiled variants small)
+__host__ __device__ inline int chunk_ld(int n) { return ((n + 3) / 4) * 4 + 1; }
 
-// whole CTA participates; caller syncs afterwards
-__device__ inline void tab_build(const ModelDev* __restrict__ M, Tab* T) {
-  if (threadIdx.x == 0) {
-    const int n = M->n;
-    T->n = n; T->d = M->d; T->ninst = M->n_inst; T->nblk = M->nblk; T->stride = M->disc_stride; T->ld = chunk_ld(n);
-    T->ntri = n * (n + 1) / 2;
-    for (int b = 0; b < M->nblk; ++b) {
-      T->bdim[b] = (unsigned char)M->blk[b].dim; T->boff[b] = (unsigned char)M->blk[b].off; T->roff[b] = (short)M->disc_off[b];
-      for (int i = 0; i < M->blk[b].dim; ++i) T->blk_of[M->blk[b].off + i] = (unsigned char)b;
-      for (int q = 0; q < M->n_inst; ++q) T->cz[q * M->nblk + b] = M->cz[q][b];
-    }
-    for (int q = 0; q < M->n_inst; ++q) T->tau[q] = M->tau[q];
-    int e = 0;
-    for (int i = 0; i < n; ++i) for (int j = 0; j <= i; ++j) { T->tri_i[e] = (unsigned char)i; T->tri_j[e] = (unsigned char)j; ++e; }
+inline void tab_build(const ModelDev* M, Tab* T) {
+  memset(T, 0, sizeof(Tab));
+  const int n = M->n;
+  T->n = n; T->d = M->d; T->ninst = M->n_inst; T->nblk = M->nblk; T->stride = M->disc_stride; T->ld = chunk_ld(n);
+  for (int b = 0; b < M->nblk; ++b) {
+    T->bdim[b] = (unsigned char)M->blk[b].dim; T->boff[b] = (unsigned char)M->blk[b].off; T->roff[b] = (short)M->disc_off[b];
+    for (int i = 0; i < M->blk[b].dim; ++i) T->blk_of[M->blk[b].off + i] = (unsigned char)b;
+    for (int q = 0; q < M->n_inst; ++q) { T->cz[q * M->nblk + b] = M->cz[q][b]; T->hq[q * M->nblk + b] = M->hq[q][b]; }
   }
+  for (int q = 0; q < M->n_inst; ++q) T->tau[q] = M->tau[q];
 }
 
 // ---- record staging: global -> shared with cp.async (LDGSTS), one 8-byte copy per element ----------
@@ -59,17 +61,17 @@ __device__ __forceinline__ void stage_rec(const Grp<G>& g, const Tab& T, const d
 }
 
 // ---- one block of out = F v ------------------------------------------------------------------------
-template <int DB>
-__device__ __forceinline__ double blk_F(const double* __restrict__ r, const double* vp, int vs, double* op, int os, int off) {
+template <int DB, int VS, int OS>
+__device__ __forceinline__ double blk_F(const double* __restrict__ r, const double* vp, double* op, int off) {
   double w[DB];
 #pragma unroll
-  for (int l = 0; l < DB; ++l) w[l] = vp[(off + l) * vs];
+  for (int l = 0; l < DB; ++l) w[l] = vp[(off + l) * VS];
 #pragma unroll
   for (int i = 0; i < DB; ++i) {
     double acc = 0.0;
 #pragma unroll
     for (int l = 0; l < DB; ++l) acc = fma(r[i * DB + l], w[l], acc);
-    op[(off + i) * os] = acc;
+    op[(off + i) * OS] = acc;
   }
   double u = 0.0;
 #pragma unroll
@@ -79,67 +81,68 @@ __device__ __forceinline__ double blk_F(const double* __restrict__ r, const doub
 
 // out = F v for the calling lane's vector: v[i] = vp[i * vs], out[i] = op[i * os] (i < n).
 // U: lane-private scratch of nblk doubles at stride G.  `rec` in shared memory.
-template <int G>
-__device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigned tz, const double* vp, int vs, double* op, int os,
-                                        double* U) {
+template <int G, int VS, int OS>
+__device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigned tz, const double* vp, double* op, double* U) {
   const int nblk = T.nblk, d = T.d;
   for (int b = 0; b < nblk; ++b) {
     const double* r = rec + T.roff[b];
     const int off = T.boff[b];
     double u;
     switch (T.bdim[b]) {
-      case 2: u = blk_F<2>(r, vp, vs, op, os, off); break;
-      case 3: u = blk_F<3>(r, vp, vs, op, os, off); break;
-      default: u = blk_F<4>(r, vp, vs, op, os, off); break;
+      case 2: u = blk_F<2, VS, OS>(r, vp, op, off); break;
+      case 3: u = blk_F<3, VS, OS>(r, vp, op, off); break;
+      default: u = blk_F<4, VS, OS>(r, vp, op, off); break;
     }
     U[b * G] = u;
   }
   for (int q = 0; q < T.ninst; ++q) {
     double acc = 0.0;
     if (!((tz >> q) & 1u)) {
-      acc = vp[(d + q) * vs];
+      acc = vp[(d + q) * VS];
       for (int b = 0; b < nblk; ++b) acc = fma(T.cz[q * nblk + b], U[b * G], acc);
     }
-    op[(d + q) * os] = acc;
+    op[(d + q) * OS] = acc;
   }
 }
 
 // ---- one block of out = F^T v ----------------------------------------------------------------------
-template <int DB>
-__device__ __forceinline__ void blk_Ft(const double* __restrict__ r, const double* vp, int vs, double* op, int os, int off, double s) {
+template <int DB, int VS, int OS>
+__device__ __forceinline__ void blk_Ft(const double* __restrict__ r, const double* vp, double* op, int off, double s) {
   double w[DB];
 #pragma unroll
-  for (int i = 0; i < DB; ++i) w[i] = vp[(off + i) * vs];
+  for (int i = 0; i < DB; ++i) w[i] = vp[(off + i) * VS];
 #pragma unroll
   for (int l = 0; l < DB; ++l) {
     double acc = r[DB * DB + l] * s; // Phi-bar_b[l] * sum_q c_qb v_zq
 #pragma unroll
     for (int i = 0; i < DB; ++i) acc = fma(r[i * DB + l], w[i], acc);
-    op[(off + l) * os] = acc;
+    op[(off + l) * OS] = acc;
   }
 }
 
-template <int G>
-__device__ __forceinline__ void apply_Ft(const Tab& T, const double* rec, unsigned tz, const double* vp, int vs, double* op, int os) {
+template <int G, int VS, int OS>
+__device__ __forceinline__ void apply_Ft(const Tab& T, const double* rec, unsigned tz, const double* vp, double* op) {
   const int nblk = T.nblk, d = T.d;
   for (int b = 0; b < nblk; ++b) {
     double s = 0.0;
     for (int q = 0; q < T.ninst; ++q)
-      if (!((tz >> q) & 1u)) s = fma(T.cz[q * nblk + b], vp[(d + q) * vs], s);
+      if (!((tz >> q) & 1u)) s = fma(T.cz[q * nblk + b], vp[(d + q) * VS], s);
     const double* r = rec + T.roff[b];
     const int off = T.boff[b];
     switch (T.bdim[b]) {
-      case 2: blk_Ft<2>(r, vp, vs, op, os, off, s); break;
-      case 3: blk_Ft<3>(r, vp, vs, op, os, off, s); break;
-      default: blk_Ft<4>(r, vp, vs, op, os, off, s); break;
+      case 2: blk_Ft<2, VS, OS>(r, vp, op, off, s); break;
+      case 3: blk_Ft<3, VS, OS>(r, vp, op, off, s); break;
+      default: blk_Ft<4, VS, OS>(r, vp, op, off, s); break;
     }
   }
-  for (int q = 0; q < T.ninst; ++q) op[(d + q) * os] = ((tz >> q) & 1u) ? 0.0 : vp[(d + q) * vs];
+  for (int q = 0; q < T.ninst; ++q) op[(d + q) * OS] = ((tz >> q) & 1u) ? 0.0 : vp[(d + q) * VS];
 }
 
 // column j of X += column j of Q = R Q~ R^T (Eq. 3.10 P:403-405 per block; z rows through c_qb)
+template <int LD>
 __device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsigned tz, int j, double* X) {
-  const int d = T.d, ld = T.ld, nblk = T.nblk;
+  constexpr int ld = LD;
+  const int d = T.d, nblk = T.nblk;
   if (j < d) {
     const int b = T.blk_of[j], db = T.bdim[b], off = T.boff[b], jj = j - off;
     const double* r = rec + T.roff[b];
@@ -166,15 +169,16 @@ __device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsig
 
 // X <- F X F^T (+ Q) for a symmetric X (columns 0..n-1) and x <- F x for the companion column n.
 // Tm: scratch of the same shape.  Two column-owned products:  Tm = F [X | x];  X[:, j] = F (Tm[j, :])^T.
-template <int G, bool ADDQ>
+template <int G, int LD, bool ADDQ>
 __device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm, double* U) {
-  const int n = T.n, ld = T.ld;
-  for (int j = g.gl; j <= n; j += G) apply_F<G>(T, rec, tz, X + j, ld, Tm + j, ld, U);
+  constexpr int ld = LD;
+  const int n = T.n;
+  for (int j = g.gl; j <= n; j += G) apply_F<G, LD, LD>(T, rec, tz, X + j, Tm + j, U);
   g.sync();
   for (int j = g.gl; j <= n; j += G) {
     if (j < n) {
-      apply_F<G>(T, rec, tz, Tm + j * ld, 1, X + j, ld, U);
-      if (ADDQ) add_Q_col(T, rec, tz, j, X);
+      apply_F<G, 1, LD>(T, rec, tz, Tm + j * ld, X + j, U);
+      if (ADDQ) add_Q_col<LD>(T, rec, tz, j, X);
     } else {
       for (int i = 0; i < n; ++i) X[i * ld + n] = Tm[i * ld + n];
     }
@@ -183,28 +187,33 @@ __device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const 
 }
 
 // X <- F^T X F, x <- F^T x (the adjoint / information direction)
-template <int G>
+template <int G, int LD>
 __device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm) {
-  const int n = T.n, ld = T.ld;
-  for (int j = g.gl; j <= n; j += G) apply_Ft<G>(T, rec, tz, X + j, ld, Tm + j, ld);
+  constexpr int ld = LD;
+  const int n = T.n;
+  for (int j = g.gl; j <= n; j += G) apply_Ft<G, LD, LD>(T, rec, tz, X + j, Tm + j);
   g.sync();
   for (int j = g.gl; j <= n; j += G) {
-    if (j < n) apply_Ft<G>(T, rec, tz, Tm + j * ld, 1, X + j, ld);
+    if (j < n) apply_Ft<G, 1, LD>(T, rec, tz, Tm + j * ld, X + j);
     else for (int i = 0; i < n; ++i) X[i * ld + n] = Tm[i * ld + n];
   }
   g.sync();
 }
 
-// X <- (X + X^T) / 2 on columns 0..n-1
-template <int G>
+// X <- (X + X^T) / 2 on columns 0..n-1: lane j pairs with the n/2 columns after it (cyclically), so
+// every unordered pair is visited (twice for the antipodal pairs of an even n, with equal results)
+template <int G, int LD>
 __device__ __forceinline__ void symmetrise(const Grp<G>& g, const Tab& T, double* X) {
-  const int ld = T.ld;
-  for (int e = g.gl; e < T.ntri; e += G) {
-    const int i = T.tri_i[e], j = T.tri_j[e];
-    const double w = 0.5 * (X[i * ld + j] + X[j * ld + i]);
-    X[i * ld + j] = w;
-    X[j * ld + i] = w;
-  }
+  constexpr int ld = LD;
+  const int n = T.n, half = n >> 1;
+  for (int j = g.gl; j < n; j += G)
+    for (int s = 1; s <= half; ++s) {
+      int i = j + s;
+      if (i >= n) i -= n;
+      const double w = 0.5 * (X[i * ld + j] + X[j * ld + i]);
+      X[i * ld + j] = w;
+      X[j * ld + i] = w;
+    }
   g.sync();
 }
 

@@ -25,6 +25,7 @@ __host__ __device__ inline int elem_size(int n) { return 3 * n * n + 2 * n; }
 __host__ __device__ inline int state_size(int n) { return n * n + n; } // [vector | matrix]
 
 struct ScanDev {
+  Tab T;           // model tables (constant bank)
   const ModelDev* M;
   const double* disc;
   const double* dt;
@@ -59,25 +60,23 @@ __device__ __forceinline__ void zero_fill(const Grp<G>& g, double* p, int cnt) {
 // k_fold0: chunk -> element.  Column-owned layout of chunk_dev.cuh.
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int fold0_group_doubles(int n, int stride, int nblk, int G) {
-  return 5 * n * chunk_ld(n) + 2 * stride + nblk * G + 2 * (n + 1) + 2;
+  return 4 * n * chunk_ld(n) + 2 * stride + nblk * G + 2 * (n + 1) + 2;
 }
 
-template <int G>
-__global__ void __launch_bounds__(128) k_fold0(ScanDev P) {
+template <int G, int LD>
+__global__ void __launch_bounds__(128) k_fold0(const __grid_constant__ ScanDev P) {
   extern __shared__ __align__(16) char smem[];
-  Tab& T = *(Tab*)smem;
-  tab_build(P.M, &T);
-  __syncthreads();
-  const int n = T.n, d = T.d, ld = T.ld;
-  const size_t tb = (sizeof(Tab) + 15) / 16 * 16;
+  const Tab& T = P.T;
+  constexpr int ld = LD;
+  const int n = T.n, d = T.d;
+  const size_t tb = 0;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
   double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * fold0_group_doubles(n, T.stride, T.nblk, G);
   double* AB0 = base;            // [A | b]
-  double* AB1 = AB0 + n * ld;
-  double* C = AB1 + n * ld;
+  double* C = AB0 + n * ld;
   double* Tm = C + n * ld;
   double* JE = Tm + n * ld;      // [J | eta]
   double* recs = JE + n * ld;    // 2 x stride
@@ -89,7 +88,7 @@ __global__ void __launch_bounds__(128) k_fold0(ScanDev P) {
   const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
 
   stage_rec(g, T, P.disc + k0 * (int64_t)T.stride, recs);
-  zero_fill(g, AB0, 5 * n * ld);
+  zero_fill(g, AB0, 4 * n * ld);
   g.sync();
   for (int i = g.gl; i < n; i += G) AB0[i * ld + i] = 1.0;
   g.sync();
@@ -103,11 +102,11 @@ __global__ void __launch_bounds__(128) k_fold0(ScanDev P) {
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
-    // [A | b] <- F [A | b]
-    for (int j = g.gl; j <= n; j += G) apply_F<G>(T, rec, tz, AB0 + j, ld, AB1 + j, ld, U);
-    { double* t = AB0; AB0 = AB1; AB1 = t; }
+    // [A | b] <- F [A | b], in place: a lane reads a block of its column into registers before it
+    // writes that block, and the z rows read only z entries, which are written last
+    for (int j = g.gl; j <= n; j += G) apply_F<G, LD, LD>(T, rec, tz, AB0 + j, AB0 + j, U);
     // C <- F C F^T + Q
-    sandwich_F<G, true>(g, T, rec, tz, C, Tm, U);
+    sandwich_F<G, LD, true>(g, T, rec, tz, C, Tm, U);
     if (!kind) {
       // observe z_q / delta: h = hs e_z in equilibrated units (Eq. 3.12); SG21 Eq. 10 with the
       // aggregate as the earlier element (rank-one J_j): Sherman-Morrison form of the combine
@@ -383,19 +382,21 @@ __global__ void __launch_bounds__(NT) k_downD(DenseArgs P) {
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int kbuf_stride(int n) { return 2 * n + 4; }
 __host__ __device__ inline int down0_group_doubles(int n, int stride, int nblk, int G) {
-  return 2 * n * chunk_ld(n) + n * (2 * n + 1) + 2 * stride + nblk * G + 5 * (n + 1) + 1;
+  return n * chunk_ld(n) + n * (2 * n + 1) + 2 * stride + nblk * G + 5 * (n + 1) + 1; // Tm is the head of Ws
 }
 
 // [vector | matrix(n x n)] in global memory  <->  column-owned [matrix | vector] with row stride ld
-template <int G>
+template <int G, int LD>
 __device__ __forceinline__ void load_state(const Grp<G>& g, const Tab& T, const double* s, double* X) {
-  const int n = T.n, ld = T.ld;
+  constexpr int ld = LD;
+  const int n = T.n;
   for (int j = g.gl; j <= n; j += G)
     for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? s[n + i * n + j] : s[i];
 }
-template <int G>
+template <int G, int LD>
 __device__ __forceinline__ void store_state(const Grp<G>& g, const Tab& T, const double* X, double* s) {
-  const int n = T.n, ld = T.ld;
+  constexpr int ld = LD;
+  const int n = T.n;
   for (int j = g.gl; j <= n; j += G)
     for (int i = 0; i < n; ++i) {
       if (j < n) s[n + i * n + j] = X[i * ld + j];
@@ -403,14 +404,13 @@ __device__ __forceinline__ void store_state(const Grp<G>& g, const Tab& T, const
     }
 }
 
-template <int G>
-__global__ void __launch_bounds__(128) k_down0(ScanDev P) {
+template <int G, int LD>
+__global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P) {
   extern __shared__ __align__(16) char smem[];
-  Tab& T = *(Tab*)smem;
-  tab_build(P.M, &T);
-  __syncthreads();
-  const int n = T.n, d = T.d, ld = T.ld;
-  const size_t tb = (sizeof(Tab) + 15) / 16 * 16;
+  const Tab& T = P.T;
+  constexpr int ld = LD;
+  const int n = T.n, d = T.d;
+  const size_t tb = 0;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
@@ -418,7 +418,7 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
   double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, T.stride, T.nblk, G);
   double* X = base;                 // [P | m], later [Lambda | lambda]
   double* Tm = X + n * ld;
-  double* Ws = Tm + n * ld;         // n x (2n+1)
+  double* Ws = Tm;                  // n x (2n+1), used only for the one solve per chunk (Tm is dead there)
   double* recs = Ws + n * (2 * n + 1);
   double* U = recs + 2 * T.stride + g.gl;
   double* cv = recs + 2 * T.stride + T.nblk * G; // n
@@ -433,7 +433,7 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
   const double ramp = 1.0 / ampv;
 
   stage_rec(g, T, P.disc + k0 * (int64_t)T.stride, recs);
-  if (P.PRE1) load_state(g, T, P.PRE1 + gid * (int64_t)ss, X);
+  if (P.PRE1) load_state<G, LD>(g, T, P.PRE1 + gid * (int64_t)ss, X);
   else
     for (int j = g.gl; j <= n; j += G)
       for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? P.M->p0[i * n + j] : 0.0;
@@ -449,7 +449,7 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
-    sandwich_F<G, true>(g, T, rec, tz, X, Tm, U);
+    sandwich_F<G, LD, true>(g, T, rec, tz, X, Tm, U);
     if (!kind) {
       const int zi = d + q;
       const int32_t ob = P.obs[k];
@@ -477,9 +477,9 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
       // the instrument is idle after its end (reading R6)
       for (int j = g.gl; j <= n; j += G) { X[zi * ld + j] = 0.0; if (j < n) X[j * ld + zi] = 0.0; }
       g.sync();
-      symmetrise(g, T, X); // the two triangles of F P F^T are rounded independently
+      symmetrise<G, LD>(g, T, X); // the two triangles of F P F^T are rounded independently
     }
-    if (P.fstate) store_state(g, T, X, P.fstate + (series * P.K + k) * (int64_t)ss); // row a7
+    if (P.fstate) store_state<G, LD>(g, T, X, P.fstate + (series * P.K + k) * (int64_t)ss); // row a7
   }
   if (g.gl == 0) P.llpart[gid] = ll;
   if (!P.want_smooth) return;
@@ -488,14 +488,17 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
   stage_rec(g, T, P.disc + (k1 - 1) * (int64_t)T.stride, recs);
   if (P.SUF1) {
     const int ld2 = 2 * n + 1;
-    load_state(g, T, P.SUF1 + gid * (int64_t)ss, Tm); // [J | eta]
+    // Ws = [I + J P | J | J m - eta]: J goes straight to its place, eta is parked in column 2n
+    const double* sj = P.SUF1 + gid * (int64_t)ss;
+    for (int j = g.gl; j <= n; j += G)
+      for (int i = 0; i < n; ++i) Ws[i * ld2 + n + j] = (j < n) ? sj[n + i * n + j] : sj[i];
     g.sync();
     for (int j = g.gl; j <= n; j += G)
       for (int i = 0; i < n; ++i) {
         double acc = 0.0;
-        for (int l = 0; l < n; ++l) acc = fma(Tm[i * ld + l], X[l * ld + j], acc);
-        if (j < n) { Ws[i * ld2 + j] = acc + (i == j ? 1.0 : 0.0); Ws[i * ld2 + n + j] = Tm[i * ld + j]; }
-        else Ws[i * ld2 + 2 * n] = acc - Tm[i * ld + n];
+        for (int l = 0; l < n; ++l) acc = fma(Ws[i * ld2 + n + l], X[l * ld + j], acc);
+        if (j < n) Ws[i * ld2 + j] = acc + (i == j ? 1.0 : 0.0);
+        else Ws[i * ld2 + 2 * n] = acc - Ws[i * ld2 + 2 * n];
       }
     g.sync();
     gj_solve(g, n, ld2, Ws);
@@ -558,12 +561,12 @@ __global__ void __launch_bounds__(128) k_down0(ScanDev P) {
         }
       }
       g.sync();
-      symmetrise(g, T, X);
+      symmetrise<G, LD>(g, T, X);
     }
-    if (P.binfo) store_state(g, T, X, P.binfo + (series * P.K + k) * (int64_t)ss);
+    if (P.binfo) store_state<G, LD>(g, T, X, P.binfo + (series * P.K + k) * (int64_t)ss);
     if (k == k0) break;
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
-    sandwich_Ft<G>(g, T, rec, tz, X, Tm);
+    sandwich_Ft<G, LD>(g, T, rec, tz, X, Tm);
   }
 }
 
@@ -601,6 +604,7 @@ __global__ void k_query_locate(int64_t M, const double* __restrict__ tq, int64_t
 }
 
 struct QueryDev {
+  Tab T;
   const ModelDev* M;
   const double* discq; // [2M][stride]
   const int64_t* kp;   // [M]
@@ -615,23 +619,26 @@ struct QueryDev {
   int* flags;
 };
 
-template <int G>
-__global__ void __launch_bounds__(128) k_query(QueryDev P) {
+__host__ __device__ inline int query_group_doubles(int n, int stride, int nblk, int G) {
+  return 3 * n * chunk_ld(n) + 2 * stride + nblk * G + 2 * (n + 1) + 1;
+}
+
+template <int G, int LD>
+__global__ void __launch_bounds__(128) k_query(const __grid_constant__ QueryDev P) {
   extern __shared__ __align__(16) char smem[];
-  Tab& T = *(Tab*)smem;
-  tab_build(P.M, &T);
-  __syncthreads();
-  const int n = T.n, ld = T.ld;
-  const size_t tb = (sizeof(Tab) + 15) / 16 * 16;
+  const Tab& T = P.T;
+  constexpr int ld = LD;
+  const int n = T.n;
+  const size_t tb = 0;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.Mq) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, T.stride, T.nblk, G);
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * query_group_doubles(n, T.stride, T.nblk, G);
   double* X = base;                 // [P* | m*]
   double* Tm = X + n * ld;
-  double* Y = Tm + n * ld;          // [Lambda* | lambda*]  (the Ws region of k_down0)
-  double* recs = Y + n * (2 * n + 1);
+  double* Y = Tm + n * ld;          // [Lambda* | lambda*]
+  double* recs = Y + n * ld;
   double* U = recs + 2 * T.stride + g.gl;
   double* hv = recs + 2 * T.stride + T.nblk * G; // n: H_q in block units
   double* ph = hv + n + 1;                        // n: P* h
@@ -644,16 +651,16 @@ __global__ void __launch_bounds__(128) k_query(QueryDev P) {
   for (int i = g.gl; i < n; i += G) hv[i] = 0.0;
   g.sync();
   if (g.gl == 0)
-    for (int b = 0; b < T.nblk; ++b) hv[T.boff[b]] = P.M->hq[P.qinst][b];
+    for (int b = 0; b < T.nblk; ++b) hv[T.boff[b]] = T.hq[P.qinst * T.nblk + b];
   cp_async_wait_all();
   g.sync();
   // ---- state just after the last event at or before t*, predicted over Delta_1 (Eq. 3.14) ----
   if (kp >= 0) {
-    load_state(g, T, P.fstate + (series * P.K + kp) * (int64_t)ss, X);
+    load_state<G, LD>(g, T, P.fstate + (series * P.K + kp) * (int64_t)ss, X);
     g.sync();
     const uint32_t mp = P.meta[kp]; // idle through (t_kp, t_kp+1): zeroed after kp, except an instrument that just started
     const unsigned idle = META_KIND(mp) ? (META_ZMASK(mp) & ~(1u << META_INST(mp))) : META_ZMASK(mp);
-    sandwich_F<G, true>(g, T, recs, idle, X, Tm, U);
+    sandwich_F<G, LD, true>(g, T, recs, idle, X, Tm, U);
   } else { // before the first event: the stationary prior, idle z = 0 (retrodiction, reading R8)
     for (int j = g.gl; j <= n; j += G)
       for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? P.M->p0[i * n + j] : 0.0;
@@ -663,12 +670,12 @@ __global__ void __launch_bounds__(128) k_query(QueryDev P) {
   const bool have_next = kp + 1 < P.K;
   if (have_next) {
     const int64_t kn = kp + 1;
-    load_state(g, T, P.binfo + (series * P.K + kn) * (int64_t)ss, Y);
+    load_state<G, LD>(g, T, P.binfo + (series * P.K + kn) * (int64_t)ss, Y);
     g.sync();
     const uint32_t meta = P.meta[kn];
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = META_KIND(meta) ? zm : (zm & ~(1u << META_INST(meta)));
-    sandwich_Ft<G>(g, T, recs + T.stride, tz, Y, Tm);
+    sandwich_Ft<G, LD>(g, T, recs + T.stride, tz, Y, Tm);
   }
   // ---- m^ = m* - P* lambda*,  P^ = P* - P* Lambda* P*, projected on H_q ----
   for (int j = g.gl; j < n; j += G) {

@@ -7,20 +7,31 @@ struct LevelPlan {
 };
 
 static int pick_lanes(const smolgp_ctx* ctx, int n) {
-  if (ctx->opt_lanes == 8 || ctx->opt_lanes == 16 || ctx->opt_lanes == 32) return (int)ctx->opt_lanes;
-  return n + 1 <= 8 ? 8 : (n + 1 <= 16 ? 16 : 32); // one lane per column of [X | x]
+  const int need = n + 1 <= 8 ? 8 : (n + 1 <= 16 ? 16 : 32); // one lane per column of [X | x]
+  if ((ctx->opt_lanes == 8 || ctx->opt_lanes == 16 || ctx->opt_lanes == 32) && ctx->opt_lanes >= need) return (int)ctx->opt_lanes;
+  return need;
 }
 
-static inline size_t tab_bytes() { return (sizeof(Tab) + 15) / 16 * 16; }
+static inline size_t tab_bytes() { return 0; } // the chunk kernels' tables travel in the kernel parameters
 
-// groups per CTA: as many as fit in ~72 KB (three CTAs per SM), at most 128 threads
-static int groups_per_cta(size_t per_group, int G) {
-  int gpc = 128 / G;
-  while (gpc > 1 && tab_bytes() + per_group * gpc > 72 * 1024) gpc >>= 1;
-  return gpc;
+// groups per CTA: the count that puts the most groups on one SM (228 KB of shared memory per SM,
+// 1 KB reserved per CTA, at most 128 threads per CTA); ties go to the smaller CTA
+static int groups_per_cta(size_t per_group, int G, int* groups_per_sm = nullptr) {
+  int best = 1, best_sm = 0;
+  for (int gpc = 1; gpc <= 128 / G; ++gpc) {
+    const size_t cta = tab_bytes() + per_group * gpc;
+    if (cta > 227 * 1024) break;
+    int ctas = (int)((228 * 1024) / (cta + 1024));
+    if (ctas > 32) ctas = 32;
+    const int warps = (gpc * G + 31) / 32;
+    if (ctas * warps > 64) ctas = 64 / warps;
+    if (ctas * gpc > best_sm) { best_sm = ctas * gpc; best = gpc; }
+  }
+  if (groups_per_sm) *groups_per_sm = best_sm > 0 ? best_sm : 1;
+  return best;
 }
 
-template <int G>
+template <int G, int LD>
 static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold) {
   const int n = hm->n;
   const int gd = fold ? fold0_group_doubles(n, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, hm->disc_stride, hm->nblk, G);
@@ -31,25 +42,45 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
   const int64_t groups = P.batch * P.c1;
   const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
   if (fold) {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_FOLD0);
-    k_fold0<G><<<blocks, gpc * G, smem, ctx->stream>>>(P);
+    k_fold0<G, LD><<<blocks, gpc * G, smem, ctx->stream>>>(P);
   } else {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_down0<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_down0<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_DOWN0);
-    k_down0<G><<<blocks, gpc * G, smem, ctx->stream>>>(P);
+    k_down0<G, LD><<<blocks, gpc * G, smem, ctx->stream>>>(P);
   }
   sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
 }
 
+// (lanes, row stride) variants compiled: lanes = 8/16/32 for n + 1 <= 8/16/33 columns, stride = chunk_ld(n)
+#define SG_DISPATCH_GL(G, LD, CALL)                                                      \
+  do {                                                                                   \
+    if (G == 8 && LD == 5) { CALL(8, 5); }                                               \
+    else if (G == 8 && LD == 9) { CALL(8, 9); }                                          \
+    else if (G == 16 && LD == 5) { CALL(16, 5); }                                        \
+    else if (G == 16 && LD == 9) { CALL(16, 9); }                                        \
+    else if (G == 16 && LD == 13) { CALL(16, 13); }                                      \
+    else if (G == 16 && LD == 17) { CALL(16, 17); }                                      \
+    else if (G == 32 && LD == 5) { CALL(32, 5); }                                        \
+    else if (G == 32 && LD == 9) { CALL(32, 9); }                                        \
+    else if (G == 32 && LD == 13) { CALL(32, 13); }                                      \
+    else if (G == 32 && LD == 17) { CALL(32, 17); }                                      \
+    else if (G == 32 && LD == 21) { CALL(32, 21); }                                      \
+    else if (G == 32 && LD == 25) { CALL(32, 25); }                                      \
+    else if (G == 32 && LD == 29) { CALL(32, 29); }                                      \
+    else if (G == 32 && LD == 33) { CALL(32, 33); }                                      \
+    else { ctx->err = "scan: unsupported (lanes, n) combination"; return SMOLGP_EUNSUPPORTED; } \
+  } while (0)
+
 static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G) {
-  switch (G) {
-    case 8: return launch_level0<8>(ctx, P, hm, fold);
-    case 16: return launch_level0<16>(ctx, P, hm, fold);
-    default: return launch_level0<32>(ctx, P, hm, fold);
-  }
+  const int LD = chunk_ld(hm->n);
+#define SG_CALL_L0(g_, ld_) return launch_level0<g_, ld_>(ctx, P, hm, fold)
+  SG_DISPATCH_GL(G, LD, SG_CALL_L0);
+#undef SG_CALL_L0
+  return SMOLGP_EUNSUPPORTED;
 }
 
 #define SG_DENSE_NT 128 /* threads cooperating on one dense combine (one CTA per group of elements) */
@@ -81,25 +112,25 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   for (int b = 0; b < hm->nblk; ++b) nent += hm->blk[b].dim * hm->blk[b].dim;
   const size_t tb = tables_bytes(n, hm->d, hm->n_inst, hm->nblk, nent);
   const int G = pick_lanes(ctx, n);
-  const int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 8;
+  int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 0; // 0: automatic, set once the chunk count is known
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
   // already fills it runs one chunk per series (the sequential filter, row a8)
   int64_t Lc = ctx->opt_chunk;
   if (Lc <= 0) {
-    const size_t per_group = (size_t)down0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8;
-    const int gpc = groups_per_cta(per_group, G);
-    const size_t cta = tab_bytes() + per_group * gpc;
-    int64_t ctas = (int64_t)((220 * 1024) / cta);
-    if (ctas > 16) ctas = 16;
-    if (ctas < 1) ctas = 1;
-    const int64_t resident = (int64_t)ctx->sm_count * ctas * gpc;
-    const int64_t target = 2 * resident;
-    if (batch >= target) Lc = K;
+    // one full wave: as many chunks as groups can be resident at once (equal work per chunk, no tail);
+    // a batch that already fills the machine runs one chunk per series (the sequential filter, row a8)
+    int per_sm = 1;
+    groups_per_cta((size_t)down0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
+    int per_sm_f = 1;
+    groups_per_cta((size_t)fold0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
+    if (per_sm_f < per_sm) per_sm = per_sm_f;
+    const int64_t resident = (int64_t)ctx->sm_count * per_sm;
+    if (batch >= resident) Lc = K;
     else {
-      Lc = (batch * K + target - 1) / target;
+      const int64_t per_series = (resident + batch - 1) / batch; // chunks per series
+      Lc = (K + per_series - 1) / per_series;
       if (Lc < 16) Lc = 16;
-      if (Lc > 512) Lc = 512;
     }
   }
   if (Lc > K) Lc = K;
@@ -107,6 +138,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   LevelPlan pl;
   pl.T = 0;
   const int64_t c1 = (K + Lc - 1) / Lc;
+  if (g == 0) g = 8; // measured on config 3 (profiles/r01_accuracy_cfg3.md): neither deeper nor flatter trees are reliably more accurate
   if (c1 > 1) {
     pl.T = 1;
     pl.cnt[1] = c1;
@@ -130,6 +162,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   char* w = (char*)ws;
 
   ScanDev P;
+  tab_build(hm, &P.T);
   P.M = a.d_model; P.disc = a.disc; P.dt = a.ev->dt; P.delta = a.ev->delta; P.meta = a.ev->meta; P.obs = a.ev->obs;
   P.y = a.y; P.sigma = a.sigma; P.amp = a.amp; P.K = K; P.N = N; P.batch = batch; P.Lc = (int)Lc; P.c1 = c1;
   P.E1 = pl.T ? (double*)(w + oE[1]) : nullptr;
@@ -173,16 +206,16 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   return SMOLGP_OK;
 }
 
-template <int G>
+template <int G, int LD>
 static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
-  const size_t per_group = (size_t)down0_group_doubles(hm->n, hm->disc_stride, hm->nblk, G) * 8;
+  const size_t per_group = (size_t)query_group_doubles(hm->n, hm->disc_stride, hm->nblk, G) * 8;
   const int gpc = groups_per_cta(per_group, G);
   const size_t smem = tab_bytes() + per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = Q.batch * Q.Mq;
-  SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   sg_launch_begin(ctx, KID_QUERY);
-  k_query<G><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
+  k_query<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
   sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
@@ -211,11 +244,12 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   rc = sg_launch_disc(ctx, a.d_model, hm, dtq, 2 * M, discq);
   if (rc) return rc;
   QueryDev Q;
+  tab_build(hm, &Q.T);
   Q.M = a.d_model; Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
   Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
-  switch (pick_lanes(ctx, n)) {
-    case 8: return launch_query<8>(ctx, Q, hm);
-    case 16: return launch_query<16>(ctx, Q, hm);
-    default: return launch_query<32>(ctx, Q, hm);
-  }
+  const int G = pick_lanes(ctx, n), LD = chunk_ld(n);
+#define SG_CALL_Q(g_, ld_) return launch_query<g_, ld_>(ctx, Q, hm)
+  SG_DISPATCH_GL(G, LD, SG_CALL_Q);
+#undef SG_CALL_Q
+  return SMOLGP_EUNSUPPORTED;
 }

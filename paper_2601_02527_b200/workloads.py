@@ -204,7 +204,7 @@ def make(cfg, N=None, batch=None, seed=None, n_features=None):
         raise ValueError(cfg)
     n_inst = int(noise.size)
     sigma = noise[inst]
-    J = n_features if n_features is not None else (64 if batch else 256)
+    J = n_features if n_features is not None else (64 if batch else (32 if N > 200000 else 256))
     # y synthesis costs O(N J) sincos: chunk it for the large configs
     if batch is None and N > 50000:
         y = np.empty(N)
