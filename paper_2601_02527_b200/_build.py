@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsmolgp_b200.so")
 SOURCES = ["api.cu", "model.cu", "events.cu", "disc.cu", "scan.cu"]
-DEPS = SOURCES + ["common.h", "scan_dev.cuh", "chunk_dev.cuh", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
+DEPS = SOURCES + ["common.h", "dev_consts.h", "grp_dev.cuh", "scan_dev.cuh", "chunk_dev.cuh", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 

@@ -169,19 +169,17 @@ __device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsig
 
 // X <- F X F^T (+ Q) for a symmetric X (columns 0..n-1) and x <- F x for the companion column n.
 // Tm: scratch of the same shape.  Two column-owned products:  Tm = F [X | x];  X[:, j] = F (Tm[j, :])^T.
+// One lane per column (the group has at least n + 1 lanes: pick_lanes).
 template <int G, int LD, bool ADDQ>
 __device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm, double* U) {
   constexpr int ld = LD;
-  const int n = T.n;
-  for (int j = g.gl; j <= n; j += G) apply_F<G, LD, LD>(T, rec, tz, X + j, Tm + j, U);
+  const int n = T.n, j = g.gl;
+  if (j <= n) apply_F<G, LD, LD>(T, rec, tz, X + j, Tm + j, U);
   g.sync();
-  for (int j = g.gl; j <= n; j += G) {
-    if (j < n) {
-      apply_F<G, 1, LD>(T, rec, tz, Tm + j * ld, X + j, U);
-      if (ADDQ) add_Q_col<LD>(T, rec, tz, j, X);
-    } else {
-      for (int i = 0; i < n; ++i) X[i * ld + n] = Tm[i * ld + n];
-    }
+  if (j < n) {
+    apply_F<G, 1, LD>(T, rec, tz, Tm + j * ld, X + j, U);
+    if (ADDQ) add_Q_col<LD>(T, rec, tz, j, X);
+    X[j * ld + n] = Tm[j * ld + n]; // companion column: lane j moves entry j
   }
   g.sync();
 }
@@ -190,12 +188,12 @@ __device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const 
 template <int G, int LD>
 __device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm) {
   constexpr int ld = LD;
-  const int n = T.n;
-  for (int j = g.gl; j <= n; j += G) apply_Ft<G, LD, LD>(T, rec, tz, X + j, Tm + j);
+  const int n = T.n, j = g.gl;
+  if (j <= n) apply_Ft<G, LD, LD>(T, rec, tz, X + j, Tm + j);
   g.sync();
-  for (int j = g.gl; j <= n; j += G) {
-    if (j < n) apply_Ft<G, 1, LD>(T, rec, tz, Tm + j * ld, X + j);
-    else for (int i = 0; i < n; ++i) X[i * ld + n] = Tm[i * ld + n];
+  if (j < n) {
+    apply_Ft<G, 1, LD>(T, rec, tz, Tm + j * ld, X + j);
+    X[j * ld + n] = Tm[j * ld + n];
   }
   g.sync();
 }
@@ -205,22 +203,18 @@ __device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const
 template <int G, int LD>
 __device__ __forceinline__ void symmetrise(const Grp<G>& g, const Tab& T, double* X) {
   constexpr int ld = LD;
-  const int n = T.n, half = n >> 1;
-  for (int j = g.gl; j < n; j += G)
-    for (int s = 1; s <= half; ++s) {
-      int i = j + s;
-      if (i >= n) i -= n;
-      const double w = 0.5 * (X[i * ld + j] + X[j * ld + i]);
-      X[i * ld + j] = w;
-      X[j * ld + i] = w;
-    }
-  g.sync();
-}
-
-// sum over the group's lanes
-template <int G>
-__device__ __forceinline__ double group_sum(const Grp<G>& g, double v) {
+  const int n = T.n, half = n >> 1, j = g.gl;
+  if (j < n) {
 #pragma unroll
-  for (int o = G / 2; o; o >>= 1) v += __shfl_xor_sync(g.mask, v, o);
-  return v;
+    for (int s = 1; s <= (LD - 1) / 2; ++s) {
+      if (s <= half) {
+        int i = j + s;
+        if (i >= n) i -= n;
+        const double w = 0.5 * (X[i * ld + j] + X[j * ld + i]);
+        X[i * ld + j] = w;
+        X[j * ld + i] = w;
+      }
+    }
+  }
+  g.sync();
 }

@@ -8,11 +8,9 @@
 #include <vector>
 
 #include "../../include/smolgp.h"
+#include "dev_consts.h"
 
-#define SG_NMAX SMOLGP_MAX_DIM
-#define SG_MAXINST SMOLGP_MAX_INST
-#define SG_MAXBLK 16 /* max number of block-diagonal blocks of F (App. C.1 stacking) */
-#define SG_MAXBD 4   /* max block dimension */
+static_assert(SG_NMAX == SMOLGP_MAX_DIM && SG_MAXINST == SMOLGP_MAX_INST, "dev_consts.h out of step with smolgp.h");
 #define SG_KT 18     /* Taylor order of the small-step discretisation */
 #define SG_BE (SG_MAXBD + 1)
 
@@ -49,13 +47,6 @@ struct ModelDev {
 // per-event record layout inside the discretisation array, block b at disc_off[b]:
 //   Phi (dim*dim, row-major) | phibar (dim) | Qxx (dim*dim) | q12 (dim) | q22 (1)      [block units]
 static inline int disc_block_size(int dim) { return 2 * dim * dim + 2 * dim + 1; }
-
-// event meta word: bit 0 kind (1 = start/reset, 0 = end/observe), bits 1..5 instrument,
-// bits 8..23 zero-mask Z_k (instruments whose z is zeroed after event k: idle ones, and the
-// event's own instrument in both cases: reset at a start, idle after an end).
-#define META_KIND(m) ((m) & 1u)
-#define META_INST(m) (((m) >> 1) & 31u)
-#define META_ZMASK(m) (((m) >> 8) & 0xFFFFu)
 
 struct smolgp_events {
   int device;

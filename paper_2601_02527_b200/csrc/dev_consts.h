@@ -1,0 +1,15 @@
+// dev_consts.h -- constants and bit layouts shared by host code, the statically compiled kernels and
+// the run-time specialised (NVRTC) chunk kernels.  Macros only: no includes, no types.
+#pragma once
+#define SG_NMAX 32     /* max augmented state dimension n = d + N_inst (= SMOLGP_MAX_DIM) */
+#define SG_MAXINST 16  /* max number of instruments (= SMOLGP_MAX_INST) */
+#define SG_MAXBLK 16   /* max number of block-diagonal blocks of F (App. C.1 stacking) */
+#define SG_MAXBD 4     /* max block dimension */
+#define NUMF_BAD 1     /* numeric flag: non-finite value or non-positive innovation variance */
+
+// event meta word: bit 0 kind (1 = start/reset, 0 = end/observe), bits 1..5 instrument,
+// bits 8..23 zero-mask Z_k (instruments whose z is zeroed after event k: idle ones, and the
+// event's own instrument in both cases: reset at a start, idle after an end).
+#define META_KIND(m) ((m) & 1u)
+#define META_INST(m) (((m) >> 1) & 31u)
+#define META_ZMASK(m) (((m) >> 8) & 0xFFFFu)

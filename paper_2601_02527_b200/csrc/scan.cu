@@ -18,8 +18,6 @@
 
 #include "chunk_dev.cuh"
 
-#define NUMF_BAD 1
-
 // element layout in global memory: AB [n x (n+1)] = [A | b],  C [n x n],  JE [n x (n+1)] = [J | eta]
 __host__ __device__ inline int elem_size(int n) { return 3 * n * n + 2 * n; }
 __host__ __device__ inline int state_size(int n) { return n * n + n; } // [vector | matrix]
@@ -51,16 +49,12 @@ struct ScanDev {
   int want_smooth;
 };
 
-template <int G>
-__device__ __forceinline__ void zero_fill(const Grp<G>& g, double* p, int cnt) {
-  for (int e = g.gl; e < cnt; e += G) p[e] = 0.0;
-}
-
 // ---------------------------------------------------------------------------------------------------
 // k_fold0: chunk -> element.  Column-owned layout of chunk_dev.cuh.
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int fold0_group_doubles(int n, int stride, int nblk, int G) {
-  return 4 * n * chunk_ld(n) + 2 * stride + nblk * G + 2 * (n + 1) + 2;
+  const int ld = chunk_ld(n), nr = ld - 1; // nr >= n rows: the padding rows stay zero, so row loops run to the compile-time nr
+  return 4 * nr * ld + 2 * stride + nblk * G + 2 * ld + 2;
 }
 
 template <int G, int LD>
@@ -75,20 +69,22 @@ __global__ void __launch_bounds__(128) k_fold0(const __grid_constant__ ScanDev P
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
   double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * fold0_group_doubles(n, T.stride, T.nblk, G);
+  constexpr int NR = LD - 1;
   double* AB0 = base;            // [A | b]
-  double* C = AB0 + n * ld;
-  double* Tm = C + n * ld;
-  double* JE = Tm + n * ld;      // [J | eta]
-  double* recs = JE + n * ld;    // 2 x stride
+  double* C = AB0 + NR * ld;
+  double* Tm = C + NR * ld;
+  double* JE = Tm + NR * ld;     // [J | eta]
+  double* recs = JE + NR * ld;   // 2 x stride
   double* U = recs + 2 * T.stride + g.gl;
-  double* av = recs + 2 * T.stride + T.nblk * G; // n + 1
-  double* cv = av + n + 1;                        // n
+  double* av = recs + 2 * T.stride + T.nblk * G; // NR (zero padded) + 1: av[NR] = hs b_z
+  double* cv = av + ld;                           // NR (zero padded)
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
 
   stage_rec(g, T, P.disc + k0 * (int64_t)T.stride, recs);
-  zero_fill(g, AB0, 4 * n * ld);
+  zero_fill(g, AB0, 4 * NR * ld);
+  zero_fill(g, av, 2 * ld);
   g.sync();
   for (int i = g.gl; i < n; i += G) AB0[i * ld + i] = 1.0;
   g.sync();
@@ -104,7 +100,7 @@ __global__ void __launch_bounds__(128) k_fold0(const __grid_constant__ ScanDev P
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
     // [A | b] <- F [A | b], in place: a lane reads a block of its column into registers before it
     // writes that block, and the z rows read only z entries, which are written last
-    for (int j = g.gl; j <= n; j += G) apply_F<G, LD, LD>(T, rec, tz, AB0 + j, AB0 + j, U);
+    if (g.gl <= n) apply_F<G, LD, LD>(T, rec, tz, AB0 + g.gl, AB0 + g.gl, U);
     // C <- F C F^T + Q
     sandwich_F<G, LD, true>(g, T, rec, tz, C, Tm, U);
     if (!kind) {
@@ -118,26 +114,26 @@ __global__ void __launch_bounds__(128) k_fold0(const __grid_constant__ ScanDev P
       const double S = hs * hs * C[zi * ld + zi] + sg * sg;
       if (!(S > 0.0) || !isfinite(S)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S;
-      for (int j = g.gl; j <= n; j += G) av[j] = hs * AB0[zi * ld + j];
-      for (int i = g.gl; i < n; i += G) cv[i] = hs * C[i * ld + zi];
+      const int j = g.gl;
+      if (j < n) { av[j] = hs * AB0[zi * ld + j]; cv[j] = hs * C[j * ld + zi]; }
+      else if (j == n) av[NR] = hs * AB0[zi * ld + n];
       g.sync();
-      const double resid = yy - av[n];
-      for (int j = g.gl; j <= n; j += G) {
+      const double resid = yy - av[NR];
+      if (j <= n) {
         // column j of J += a a_j / S, of A -= c a_j / S; last column: eta += a resid / S, b += c resid / S
         const double aj = (j < n) ? av[j] * rS : resid * rS;
         const double sgn = (j < n) ? -1.0 : 1.0;
-        for (int i = 0; i < n; ++i) {
+        const double cj = (j < n) ? cv[j] * rS : 0.0;
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
           JE[i * ld + j] = fma(av[i], aj, JE[i * ld + j]);
           AB0[i * ld + j] = fma(sgn * cv[i], aj, AB0[i * ld + j]);
-        }
-        if (j < n) {
-          const double cj = cv[j] * rS;
-          for (int i = 0; i < n; ++i) C[i * ld + j] = fma(-cv[i], cj, C[i * ld + j]);
+          C[i * ld + j] = fma(-cv[i], cj, C[i * ld + j]); // column n of C is scratch (cj = 0 there)
         }
       }
       g.sync();
       // the instrument is idle after its end: zero z_q (reading R6)
-      for (int j = g.gl; j <= n; j += G) { AB0[zi * ld + j] = 0.0; if (j < n) { C[zi * ld + j] = 0.0; C[j * ld + zi] = 0.0; } }
+      if (j <= n) { AB0[zi * ld + j] = 0.0; if (j < n) { C[zi * ld + j] = 0.0; C[j * ld + zi] = 0.0; } }
       g.sync();
     }
   }
@@ -382,7 +378,8 @@ __global__ void __launch_bounds__(NT) k_downD(DenseArgs P) {
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int kbuf_stride(int n) { return 2 * n + 4; }
 __host__ __device__ inline int down0_group_doubles(int n, int stride, int nblk, int G) {
-  return n * chunk_ld(n) + n * (2 * n + 1) + 2 * stride + nblk * G + 5 * (n + 1) + 1; // Tm is the head of Ws
+  const int ld = chunk_ld(n), nr = ld - 1, ws = n * (2 * n + 1) > nr * ld ? n * (2 * n + 1) : nr * ld;
+  return nr * ld + ws + 2 * stride + nblk * G + 5 * ld + 1; // Tm is the head of Ws
 }
 
 // [vector | matrix(n x n)] in global memory  <->  column-owned [matrix | vector] with row stride ld
@@ -416,16 +413,17 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
   double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, T.stride, T.nblk, G);
+  constexpr int NR = LD - 1;        // rows allocated (>= n): padding rows and vector tails stay zero
   double* X = base;                 // [P | m], later [Lambda | lambda]
-  double* Tm = X + n * ld;
+  double* Tm = X + NR * ld;
   double* Ws = Tm;                  // n x (2n+1), used only for the one solve per chunk (Tm is dead there)
-  double* recs = Ws + n * (2 * n + 1);
+  double* recs = Ws + (n * (2 * n + 1) > NR * ld ? n * (2 * n + 1) : NR * ld);
   double* U = recs + 2 * T.stride + g.gl;
-  double* cv = recs + 2 * T.stride + T.nblk * G; // n
-  double* kv = cv + n + 1;
-  double* pv = kv + n + 1;
-  double* av = pv + n + 1;          // n + 1
-  double* gv = av + n + 1;          // n + 1
+  double* cv = recs + 2 * T.stride + T.nblk * G; // NR, zero padded
+  double* kv = cv + ld;
+  double* pv = kv + ld;
+  double* av = pv + ld;             // n + 1
+  double* gv = av + ld;             // n + 1
   const int ss = state_size(n), ks = kbuf_stride(n);
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
@@ -433,6 +431,9 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
   const double ramp = 1.0 / ampv;
 
   stage_rec(g, T, P.disc + k0 * (int64_t)T.stride, recs);
+  zero_fill(g, X, 2 * NR * ld);
+  zero_fill(g, cv, 5 * ld);
+  g.sync();
   if (P.PRE1) load_state<G, LD>(g, T, P.PRE1 + gid * (int64_t)ss, X);
   else
     for (int j = g.gl; j <= n; j += G)
@@ -463,9 +464,11 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
       ll -= 0.5 * (log(6.283185307179586476925286766559 * S) + v * v * rS);
       for (int i = g.gl; i < n; i += G) cv[i] = hs * X[i * ld + zi];
       g.sync();
-      for (int j = g.gl; j <= n; j += G) {
+      if (g.gl <= n) {
+        const int j = g.gl;
         const double cj = (j < n) ? -cv[j] * rS : v * rS;
-        for (int i = 0; i < n; ++i) X[i * ld + j] = fma(cv[i], cj, X[i * ld + j]);
+#pragma unroll
+        for (int i = 0; i < NR; ++i) X[i * ld + j] = fma(cv[i], cj, X[i * ld + j]);
       }
       g.sync();
       if (P.want_smooth) {
@@ -475,7 +478,7 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
         g.sync();
       }
       // the instrument is idle after its end (reading R6)
-      for (int j = g.gl; j <= n; j += G) { X[zi * ld + j] = 0.0; if (j < n) X[j * ld + zi] = 0.0; }
+      if (g.gl <= n) { const int j = g.gl; X[zi * ld + j] = 0.0; if (j < n) X[j * ld + zi] = 0.0; }
       g.sync();
       symmetrise<G, LD>(g, T, X); // the two triangles of F P F^T are rounded independently
     }
@@ -509,6 +512,8 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
     zero_fill(g, X, n * ld);
   }
   g.sync();
+  zero_fill(g, Tm, NR * ld); // the solve used this region as Ws
+  g.sync();
   // ---- backward ----
   for (int64_t k = k1 - 1; k >= k0; --k) {
     const double* rec = recs + ((k1 - 1 - k) & 1) * T.stride;
@@ -522,7 +527,7 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
     for (int r = 0; r < T.ninst; ++r)
       if ((zm >> r) & 1u) {
         const int zr = d + r;
-        for (int j = g.gl; j <= n; j += G) { X[zr * ld + j] = 0.0; if (j < n) X[j * ld + zr] = 0.0; }
+        if (g.gl <= n) { const int j = g.gl; X[zr * ld + j] = 0.0; if (j < n) X[j * ld + zr] = 0.0; }
       }
     g.sync();
     if (!kind) {
@@ -535,11 +540,13 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
       const double rS = 1.0 / S;
       g.sync();
       double quad = 0.0, kap = 0.0;
-      for (int j = g.gl; j <= n; j += G) {
+      if (g.gl <= n) {
+        const int j = g.gl;
         double a = 0.0, b = 0.0;
-        for (int i = 0; i < n; ++i) { const double x = X[i * ld + j]; a = fma(x, pv[i], a); b = fma(x, kv[i], b); }
+#pragma unroll
+        for (int i = 0; i < NR; ++i) { const double x = X[i * ld + j]; a = fma(x, pv[i], a); b = fma(x, kv[i], b); }
         av[j] = a; gv[j] = b;
-        if (j < n) { quad = fma(pv[j], a, quad); kap = fma(kv[j], b, kap); }
+        if (j < n) { quad = pv[j] * a; kap = kv[j] * b; }
       }
       quad = group_sum(g, quad);
       kap = group_sum(g, kap);
@@ -551,7 +558,8 @@ __global__ void __launch_bounds__(128) k_down0(const __grid_constant__ ScanDev P
         P.var[series * P.N + ob] = ampv * ampv * hs * hs * sv; // H~ P^ H~^T
       }
       // Lambda~ = C^T Lambda^ C + h h^T / S: only row and column z change (h = hs e_z)
-      for (int j = g.gl; j <= n; j += G) {
+      if (g.gl <= n) {
+        const int j = g.gl;
         if (j < n) {
           X[zi * ld + j] -= hs * gv[j];
           X[j * ld + zi] -= hs * gv[j];
@@ -620,7 +628,8 @@ struct QueryDev {
 };
 
 __host__ __device__ inline int query_group_doubles(int n, int stride, int nblk, int G) {
-  return 3 * n * chunk_ld(n) + 2 * stride + nblk * G + 2 * (n + 1) + 1;
+  const int ld = chunk_ld(n);
+  return 3 * (ld - 1) * ld + 2 * stride + nblk * G + 2 * ld + 1;
 }
 
 template <int G, int LD>
@@ -636,12 +645,13 @@ __global__ void __launch_bounds__(128) k_query(const __grid_constant__ QueryDev 
   if (gid >= P.batch * P.Mq) return;
   double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * query_group_doubles(n, T.stride, T.nblk, G);
   double* X = base;                 // [P* | m*]
-  double* Tm = X + n * ld;
-  double* Y = Tm + n * ld;          // [Lambda* | lambda*]
-  double* recs = Y + n * ld;
+  constexpr int NR = LD - 1;
+  double* Tm = X + NR * ld;
+  double* Y = Tm + NR * ld;         // [Lambda* | lambda*]
+  double* recs = Y + NR * ld;
   double* U = recs + 2 * T.stride + g.gl;
   double* hv = recs + 2 * T.stride + T.nblk * G; // n: H_q in block units
-  double* ph = hv + n + 1;                        // n: P* h
+  double* ph = hv + ld;                           // n: P* h
   const int ss = state_size(n);
   const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
   const int64_t kp = P.kp[q];

@@ -3,29 +3,7 @@
 // all matrices are n x n (n <= 32, run time) row-major in shared memory.
 #pragma once
 #include "common.h"
-
-template <int G>
-struct Grp {
-  int gl;        // lane inside the group
-  unsigned mask; // the group's lanes inside the warp (G <= 32)
-  __device__ __forceinline__ Grp() {
-    if (G > 32) { gl = threadIdx.x; mask = 0xffffffffu; } // the group is the whole CTA (blockDim.x == G)
-    else {
-      const int lane = threadIdx.x & 31;
-      gl = lane & (G - 1);
-      mask = (G == 32) ? 0xffffffffu : (((1u << (G & 31)) - 1u) << (lane & ~(G - 1)));
-    }
-  }
-  __device__ __forceinline__ void sync() const {
-    if (G > 32) __syncthreads(); else __syncwarp(mask);
-  }
-};
-
-// e -> (e / nc, e % nc) for small non-negative e (exact: see DESIGN.md "index arithmetic")
-__device__ __forceinline__ void divmod_small(int e, int nc, float rnc, int& i, int& j) {
-  i = __float2int_rz(((float)e + 0.5f) * rnc);
-  j = e - i * nc;
-}
+#include "grp_dev.cuh"
 
 // per-CTA tables derived from the model
 struct Tables {
@@ -218,48 +196,3 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, const Tables& T, int nk,
   }
 }
 
-// Gauss-Jordan elimination with partial pivoting on the augmented matrix W = [M | R] (n rows,
-// ld = n + m columns) in place; on return R holds M^-1 R.  M = I + (PSD)(PSD) in every use here
-// (eigenvalues >= 1), so a zero pivot cannot occur for finite input.
-template <int G>
-__device__ void gj_solve(const Grp<G>& g, int n, int ld, double* W) {
-  for (int p = 0; p < n; ++p) {
-    // pivot search in column p, rows >= p: every lane scans the column itself (broadcast reads)
-    double best = -1.0;
-    int bi = p;
-    for (int i = p; i < n; ++i) {
-      const double v = fabs(W[i * ld + p]);
-      if (v > best) { best = v; bi = i; }
-    }
-    g.sync(); // all lanes have read column p before the swap touches it
-    if (bi != p) {
-      for (int j = p + g.gl; j < ld; j += G) {
-        const double a = W[p * ld + j], b = W[bi * ld + j];
-        W[p * ld + j] = b;
-        W[bi * ld + j] = a;
-      }
-    }
-    g.sync();
-    const double rpv = 1.0 / W[p * ld + p];
-    const int nc = ld - p - 1;
-    const float rnc = 1.0f / (float)nc;
-    const int tot = (n - 1) * nc;
-    for (int e = g.gl; e < tot; e += G) {
-      int i, j;
-      divmod_small(e, nc, rnc, i, j);
-      if (i >= p) ++i;
-      j += p + 1;
-      W[i * ld + j] = fma(-W[i * ld + p] * rpv, W[p * ld + j], W[i * ld + j]);
-    }
-    g.sync();
-  }
-  // scale by the diagonal
-  const int m = ld - n;
-  const float rm = 1.0f / (float)m;
-  for (int e = g.gl; e < n * m; e += G) {
-    int i, j;
-    divmod_small(e, m, rm, i, j);
-    W[i * ld + n + j] = W[i * ld + n + j] / W[i * ld + i];
-  }
-  g.sync();
-}
