@@ -139,6 +139,25 @@ def run_reference(args, w, cfgname):
 
 
 # ----------------------------------------------------------------------------------------------
+# multi-rank plumbing: replicas only -- no data-path collective; the only exchange is
+# the max over ranks of the timed milliseconds
+# ----------------------------------------------------------------------------------------------
+def max_over_ranks(values, world, device):
+    if world <= 1:
+        return list(values)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def aggregate_throughput(events_per_replica, steps, ms_max, world):
+    """whole-job events/s: every rank processed the same number of events, in the slowest rank's time"""
+    return world * events_per_replica * steps / (ms_max * 1e-3)
+
+
+# ----------------------------------------------------------------------------------------------
 # CUDA arm
 # ----------------------------------------------------------------------------------------------
 def run_cuda(args, w, cfgname):
@@ -225,16 +244,13 @@ def run_cuda(args, w, cfgname):
     clocks = sampler.stop() if rank == 0 else None
     fp64_probe = ctx.probe_fp64() if rank == 0 else None
 
-    if world > 1:  # max over ranks
-        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, ms_e2e = t.tolist()
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    value = world * K_events * args.steps / (ms * 1e-3)
-    e2e_value = world * K_events * args.steps / (ms_e2e * 1e-3)
+    value = aggregate_throughput(K_events, args.steps, ms, world)
+    e2e_value = aggregate_throughput(K_events, args.steps, ms_e2e, world)
     # ---- roofline of the dominant kernel (device time from the ctx's own CUDA events) ----
     top = max(prof, key=lambda k: prof[k][0])
     t_top_ms = prof[top][0] / prof[top][1]           # average launch duration
