@@ -121,7 +121,7 @@ int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_m
                    int64_t K, double* disc);
 // events.cu
 int sg_sort_pairs(smolgp_ctx* ctx, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
-                  int64_t n, uint32_t* hist);
+                  int64_t n, uint32_t* hist, uint32_t* gcnt);
 // scan.cu
 struct ScanArgs {
   const ModelDev* d_model;

@@ -13,7 +13,7 @@
 //      CLOSED FORM of the family (B10, and its Matern analogues) instead of a repeated
 //      square, so the error grows like s eps, not 2^s eps;
 //   3. Phi(Delta) itself from the closed form.
-// One thread per (event, block); output record layout in common.h.
+// One thread per (event, block), blocks along grid.y; output record layout in common.h.
 #include "common.h"
 
 template <int DB>
@@ -75,12 +75,21 @@ __device__ void disc_block(const BlockConst& B, double dts, double* __restrict__
     double x = B.rho * dts;
     while (x > 0.25 && s < 64) { x *= 0.5; h *= 0.5; ++s; }
   }
+  // Taylor order.  The slowest-starting entry of Q~ (the integral's own variance) begins at order
+  // kmin = 2 DB + 1 in h; keep terms until they fall below 2^-58 of THAT leading term, so that every
+  // entry keeps full relative accuracy: x^j kmin! / (kmin + j)! < 2^-58 with x = rho h <= 1/4.
+  int kt = 2 * DB + 1;
+  {
+    const double x = B.rho * h;
+    double rel = 1.0;
+    while (rel > 3.5e-18 && kt < SG_KT) { ++kt; rel *= x / (double)kt; }
+  }
   double A[M][M], Q[M][M];
 #pragma unroll
   for (int i = 0; i < M; ++i)
 #pragma unroll
-    for (int j = 0; j < M; ++j) { A[i][j] = B.tayA[SG_KT][i * SG_BE + j]; Q[i][j] = B.tayQ[SG_KT][i * SG_BE + j]; }
-  for (int k = SG_KT - 1; k >= 0; --k) {
+    for (int j = 0; j < M; ++j) { A[i][j] = B.tayA[kt][i * SG_BE + j]; Q[i][j] = B.tayQ[kt][i * SG_BE + j]; }
+  for (int k = kt - 1; k >= 0; --k) {
 #pragma unroll
     for (int i = 0; i < M; ++i)
 #pragma unroll
@@ -151,13 +160,13 @@ __device__ void disc_block(const BlockConst& B, double dts, double* __restrict__
   out[2 * DB * DB + 2 * DB] = Q[DB][DB];
 }
 
+// blockIdx.y = block of the model: every thread of a CTA works on the same block, so the Taylor
+// coefficients and closed-form constants are warp-uniform loads and the family switch does not diverge
 __global__ void __launch_bounds__(128) k_disc(const ModelDev* __restrict__ Mp, const double* __restrict__ dt, int64_t K,
                                               double* __restrict__ disc) {
-  const int nblk = Mp->nblk;
-  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= K * nblk) return;
-  const int64_t k = gid / nblk;
-  const int b = (int)(gid - k * nblk);
+  const int b = blockIdx.y;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= K) return;
   const BlockConst& B = Mp->blk[b];
   const double dts = dt[k] * B.inv_T;
   double* out = disc + k * (int64_t)Mp->disc_stride + Mp->disc_off[b];
@@ -170,10 +179,9 @@ __global__ void __launch_bounds__(128) k_disc(const ModelDev* __restrict__ Mp, c
 
 int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_model, const double* dt,
                    int64_t K, double* disc) {
-  const int64_t total = K * h_model->nblk;
-  const int64_t blocks = (total + 127) / 128;
+  dim3 grid((unsigned)((K + 127) / 128), (unsigned)h_model->nblk);
   sg_launch_begin(ctx, KID_DISC);
-  k_disc<<<(unsigned)blocks, 128, 0, ctx->stream>>>(d_model, dt, K, disc);
+  k_disc<<<grid, 128, 0, ctx->stream>>>(d_model, dt, K, disc);
   sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;

@@ -39,49 +39,74 @@ __global__ void k_ev_init(int64_t N, const double* __restrict__ ts, const double
   if (!bad) atomicMax(maxdelta + q, (unsigned long long)__double_as_longlong(e - s)); // positive doubles order like their bits
 }
 
-// ---- LSD radix sort, 8 bits per pass.  One warp per tile of RS_TILE keys. -------------------------
-#define RS_TILE 2048
-__global__ void __launch_bounds__(32) k_rs_hist(const uint64_t* __restrict__ keys, int64_t n, int shift,
-                                                uint32_t* __restrict__ hist, int ntiles) {
-  __shared__ uint32_t cnt[256];
-  const int lane = threadIdx.x;
+// ---- LSD radix sort, 8 bits per pass.  One warp per tile of RS_TILE keys, RS_WPB tiles per CTA. ----
+// hist: per-tile digit counts (digit-major) + global digit totals; scan: one CTA per digit turns its
+// row into global positions (base = total of the smaller digits); scatter: stable, warp-serial
+// ranking with match_any (equal keys keep their order: ends stay before starts, reading R5).
+#define RS_TILE 512
+#define RS_WPB 4
+__global__ void __launch_bounds__(32 * RS_WPB) k_rs_hist(const uint64_t* __restrict__ keys, int64_t n, int shift,
+                                                         uint32_t* __restrict__ hist, int ntiles, uint32_t* __restrict__ gcnt) {
+  __shared__ uint32_t cnt_all[RS_WPB][256];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int tile = blockIdx.x * RS_WPB + w;
+  uint32_t* cnt = cnt_all[w];
   for (int b = lane; b < 256; b += 32) cnt[b] = 0;
   __syncwarp();
-  const int64_t base = (int64_t)blockIdx.x * RS_TILE;
-  for (int i = lane; i < RS_TILE; i += 32) {
-    const int64_t p = base + i;
-    if (p < n) atomicAdd(&cnt[(keys[p] >> shift) & 255u], 1u);
+  if (tile < ntiles) {
+    const int64_t base = (int64_t)tile * RS_TILE;
+    for (int i = lane; i < RS_TILE; i += 32) {
+      const int64_t p = base + i;
+      if (p < n) atomicAdd(&cnt[(keys[p] >> shift) & 255u], 1u);
+    }
+    __syncwarp();
+    for (int b = lane; b < 256; b += 32) {
+      const uint32_t c = cnt[b];
+      hist[(int64_t)b * ntiles + tile] = c; // digit-major
+      if (c) atomicAdd(&gcnt[b], c);
+    }
   }
-  __syncwarp();
-  for (int b = lane; b < 256; b += 32) hist[(int64_t)b * ntiles + blockIdx.x] = cnt[b]; // digit-major
 }
-// exclusive scan of the digit-major histogram (256 * ntiles entries), one block
-__global__ void __launch_bounds__(1024) k_rs_scan(uint32_t* __restrict__ hist, int64_t total) {
-  __shared__ uint32_t part[1024];
-  const int tid = threadIdx.x;
-  const int64_t per = (total + 1023) / 1024;
-  const int64_t lo = tid * per, hi = (lo + per < total) ? lo + per : total;
-  uint32_t s = 0;
-  for (int64_t i = lo; i < hi; ++i) s += hist[i];
-  part[tid] = s;
+// exclusive scan of the digit-major histogram: CTA d scans row d, starting at the total of digits < d
+__global__ void __launch_bounds__(256) k_rs_scan(uint32_t* __restrict__ hist, int ntiles, const uint32_t* __restrict__ gcnt) {
+  __shared__ uint32_t sm[256];
+  __shared__ uint32_t carry;
+  const int d = blockIdx.x, tid = threadIdx.x;
+  sm[tid] = (tid < d) ? gcnt[tid] : 0u;
   __syncthreads();
-  for (int off = 1; off < 1024; off <<= 1) {
-    uint32_t v = (tid >= off) ? part[tid - off] : 0;
+  for (int off = 128; off; off >>= 1) { if (tid < off) sm[tid] += sm[tid + off]; __syncthreads(); }
+  if (tid == 0) carry = sm[0];
+  __syncthreads();
+  uint32_t* row = hist + (int64_t)d * ntiles;
+  for (int t0 = 0; t0 < ntiles; t0 += 256) {
+    const int t = t0 + tid;
+    const uint32_t v = (t < ntiles) ? row[t] : 0u;
+    const uint32_t run0 = carry;
     __syncthreads();
-    part[tid] += v;
+    sm[tid] = v;
+    __syncthreads();
+    for (int off = 1; off < 256; off <<= 1) {
+      const uint32_t x = (tid >= off) ? sm[tid - off] : 0u;
+      __syncthreads();
+      sm[tid] += x;
+      __syncthreads();
+    }
+    if (t < ntiles) row[t] = run0 + sm[tid] - v;
+    if (tid == 255) carry = run0 + sm[255];
     __syncthreads();
   }
-  uint32_t run = part[tid] - s;
-  for (int64_t i = lo; i < hi; ++i) { uint32_t v = hist[i]; hist[i] = run; run += v; }
 }
-__global__ void __launch_bounds__(32) k_rs_scatter(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals,
-                                                   uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                                                   int64_t n, int shift, const uint32_t* __restrict__ hist, int ntiles) {
-  __shared__ uint32_t pos[256];
-  const int lane = threadIdx.x;
-  for (int b = lane; b < 256; b += 32) pos[b] = hist[(int64_t)b * ntiles + blockIdx.x];
+__global__ void __launch_bounds__(32 * RS_WPB) k_rs_scatter(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals,
+                                                            uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
+                                                            int64_t n, int shift, const uint32_t* __restrict__ hist, int ntiles) {
+  __shared__ uint32_t pos_all[RS_WPB][256];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int tile = blockIdx.x * RS_WPB + w;
+  if (tile >= ntiles) return;
+  uint32_t* pos = pos_all[w];
+  for (int b = lane; b < 256; b += 32) pos[b] = hist[(int64_t)b * ntiles + tile];
   __syncwarp();
-  const int64_t base = (int64_t)blockIdx.x * RS_TILE;
+  const int64_t base = (int64_t)tile * RS_TILE;
   for (int i0 = 0; i0 < RS_TILE; i0 += 32) {
     const int64_t p = base + i0 + lane;
     const bool live = p < n;
@@ -100,20 +125,24 @@ __global__ void __launch_bounds__(32) k_rs_scatter(const uint64_t* __restrict__ 
   }
 }
 
+// gcnt: 8 x 256 counters (one slice per pass)
 int sg_sort_pairs(smolgp_ctx* ctx, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
-                  int64_t n, uint32_t* hist) {
+                  int64_t n, uint32_t* hist, uint32_t* gcnt) {
   const int ntiles = (int)((n + RS_TILE - 1) / RS_TILE);
+  const unsigned blocks = (unsigned)((ntiles + RS_WPB - 1) / RS_WPB);
   uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
+  cudaMemsetAsync(gcnt, 0, 8 * 256 * sizeof(uint32_t), ctx->stream);
   for (int pass = 0; pass < 8; ++pass) {
     const int shift = 8 * pass;
+    uint32_t* gc = gcnt + pass * 256;
     sg_launch_begin(ctx, KID_RS_HIST);
-    k_rs_hist<<<ntiles, 32, 0, ctx->stream>>>(kin, n, shift, hist, ntiles);
+    k_rs_hist<<<blocks, 32 * RS_WPB, 0, ctx->stream>>>(kin, n, shift, hist, ntiles, gc);
     sg_launch_end(ctx);
     sg_launch_begin(ctx, KID_RS_SCAN);
-    k_rs_scan<<<1, 1024, 0, ctx->stream>>>(hist, (int64_t)256 * ntiles);
+    k_rs_scan<<<256, 256, 0, ctx->stream>>>(hist, ntiles, gc);
     sg_launch_end(ctx);
     sg_launch_begin(ctx, KID_RS_SCATTER);
-    k_rs_scatter<<<ntiles, 32, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles);
+    k_rs_scatter<<<blocks, 32 * RS_WPB, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles);
     sg_launch_end(ctx);
     uint64_t* tk = kin; kin = kout; kout = tk;
     uint32_t* tv = vin; vin = vout; vout = tv;
@@ -208,7 +237,7 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   }
   // scratch: keys, keys_tmp (u64), vals, vals_tmp, bits (u32), hist, tiles, maxdelta
   const int ntiles_rs = (int)((K + RS_TILE - 1) / RS_TILE), ntiles_xs = (int)((K + XS_TILE - 1) / XS_TILE);
-  size_t bytes = (size_t)K * (8 + 8 + 4 + 4 + 4) + (size_t)256 * ntiles_rs * 4 + (size_t)ntiles_xs * 4 + SG_MAXINST * 8 + 1024;
+  size_t bytes = (size_t)K * (8 + 8 + 4 + 4 + 4) + (size_t)256 * ntiles_rs * 4 + (size_t)ntiles_xs * 4 + SG_MAXINST * 8 + 8 * 256 * 4 + 1024;
   void* scratch;
   int rc = sg_arena(ctx, bytes, &scratch);
   if (rc) return fail(rc);
@@ -220,6 +249,7 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   uint32_t* vals_tmp = (uint32_t*)p; p += K * 4;
   uint32_t* bits = (uint32_t*)p; p += K * 4;
   uint32_t* hist = (uint32_t*)p; p += (size_t)256 * ntiles_rs * 4;
+  uint32_t* gcnt = (uint32_t*)p; p += 8 * 256 * 4;
   uint32_t* tiles = (uint32_t*)p;
   cudaStream_t st = ctx->stream;
   cudaMemsetAsync(ctx->d_flags, 0, sizeof(int), st);
@@ -227,7 +257,7 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   sg_launch_begin(ctx, KID_EV_INIT);
   k_ev_init<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ts, te, inst, n_inst, keys, vals, ctx->d_flags, maxdelta);
   sg_launch_end(ctx);
-  rc = sg_sort_pairs(ctx, keys, vals, keys_tmp, vals_tmp, K, hist);
+  rc = sg_sort_pairs(ctx, keys, vals, keys_tmp, vals_tmp, K, hist, gcnt);
   if (rc) return fail(rc);
   sg_launch_begin(ctx, KID_EV_GATHER);
   k_ev_gather<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(K, vals, ts, te, inst, n_inst, ev->t, ev->delta, ev->obs, bits);

@@ -138,7 +138,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   LevelPlan pl;
   pl.T = 0;
   const int64_t c1 = (K + Lc - 1) / Lc;
-  if (g == 0) g = 8; // measured on config 3 (profiles/r01_accuracy_cfg3.md): neither deeper nor flatter trees are reliably more accurate
+  if (g == 0) g = 4; // measured on config 3 (profiles/r01_accuracy_cfg3.md): fastest; neither deeper nor flatter trees are reliably more accurate
   if (c1 > 1) {
     pl.T = 1;
     pl.cnt[1] = c1;
