@@ -5,8 +5,9 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsmolgp_b200.so")
-SOURCES = ["api.cu", "model.cu", "events.cu", "disc.cu", "scan.cu"]
-DEPS = SOURCES + ["common.h", "dev_consts.h", "grp_dev.cuh", "scan_dev.cuh", "chunk_dev.cuh", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
+SOURCES = ["api.cu", "model.cu", "events.cu", "disc.cu", "scan.cu", "jit.cu"]
+JIT_PARTS = ["dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh"]  # run-time specialised source, in order
+DEPS = SOURCES + ["common.h", "dev_consts.h", "grp_dev.cuh", "scan_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "jit.h", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
@@ -18,10 +19,29 @@ def _stale():
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
+def _write_jit_source():
+    """csrc/jit_src.inc: the chunk kernels' source as one C++ raw string (local includes stripped),
+    compiled at run time by jit.cu with the model's tables as constants."""
+    text = []
+    for f in JIT_PARTS:
+        for line in open(os.path.join(CSRC, f)):
+            st = line.strip()
+            if st.startswith('#include "') or st == "#pragma once":
+                continue
+            text.append(line)
+    body = "".join(text)
+    assert ')SGJIT"' not in body
+    out = os.path.join(CSRC, "jit_src.inc")
+    new = 'R"SGJIT(' + body + ')SGJIT"\n'
+    if not os.path.exists(out) or open(out).read() != new:
+        open(out, "w").write(new)
+
+
 def build(force=False, verbose=False):
     """Compile if missing or stale; returns the path of the shared library."""
     if not force and not _stale():
         return SO
+    _write_jit_source()
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
@@ -39,7 +59,7 @@ def build(force=False, verbose=False):
             raise RuntimeError("nvcc failed on %s:\n%s" % (s, out.decode()))
         if verbose:
             print(out.decode())
-    subprocess.check_call([nvcc, "-shared", "-o", SO, *objs, "-lcudart"])
+    subprocess.check_call([nvcc, "-shared", "-o", SO, *objs, "-lcudart", "-ldl"])
     return SO
 
 

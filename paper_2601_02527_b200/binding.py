@@ -14,7 +14,7 @@ STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
            "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
-           "smolgp_launch_count", "smolgp_probe_fp64", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name"]
+           "smolgp_launch_count", "smolgp_probe_fp64", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log"]
 NKERNELS = 17
 
 
@@ -66,6 +66,8 @@ def lib():
         L.smolgp_profile_read.argtypes = [vp, dp, dp]
         L.smolgp_kernel_name.argtypes = [i32]
         L.smolgp_kernel_name.restype = C.c_char_p
+        L.smolgp_jit_log.argtypes = [vp]
+        L.smolgp_jit_log.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -143,6 +145,9 @@ class Context:
         ms, cnt = np.zeros(NKERNELS), np.zeros(NKERNELS, dtype=np.int64)
         self._check(lib().smolgp_profile_read(self.handle, _hptr(ms), _hptr(cnt)))
         return {lib().smolgp_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(NKERNELS) if cnt[i]}
+
+    def jit_log(self):
+        return lib().smolgp_jit_log(self.handle).decode()
 
     def probe_fp64(self):
         v = C.c_double()

@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include "common.h"
+#include "jit.h"
 
 int sg_arena(smolgp_ctx* ctx, size_t bytes, void** out) {
   if (bytes > ctx->arena_bytes) {
@@ -29,7 +30,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0;
-  c->opt_chunk = 0; c->opt_group = 0; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = new ModelDev();
+  c->opt_chunk = 0; c->opt_group = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = new ModelDev();
   int v = 0;
   cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device); c->sm_count = v;
   cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device); c->smem_optin = (size_t)v;
@@ -52,6 +53,7 @@ extern "C" void smolgp_destroy(smolgp_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
   cudaStreamSynchronize(ctx->stream);
+  sg_jit_destroy(ctx);
   cudaFree(ctx->arena);
   cudaFree(ctx->pers);
   cudaFree(ctx->d_flags);
@@ -91,11 +93,14 @@ extern "C" int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launche
   return SMOLGP_OK;
 }
 
+extern "C" const char* smolgp_jit_log(smolgp_ctx* ctx) { return ctx ? sg_jit_log(ctx) : ""; }
+
 extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value) {
   if (!ctx || !name) return SMOLGP_EINVAL;
   if (!strcmp(name, "chunk")) ctx->opt_chunk = value;
   else if (!strcmp(name, "group")) ctx->opt_group = value;
   else if (!strcmp(name, "lanes")) ctx->opt_lanes = value;
+  else if (!strcmp(name, "jit")) ctx->opt_jit = value;
   else { ctx->err = std::string("unknown option ") + name; return SMOLGP_EINVAL; }
   return SMOLGP_OK;
 }

@@ -13,9 +13,13 @@
 //   z_q row of [Phi-bar I]:  sum_b c_qb Phi-bar_b x_b + z_q   (c_qb = 0 if component b is not in
 //                               instrument q's integrand, Eq. 3.2)
 #pragma once
+#ifndef SG_JIT
 #include <string.h>
 
-#include "scan_dev.cuh"
+#include "common.h"
+#endif
+#include "dev_consts.h"
+#include "grp_dev.cuh"
 
 // Model tables of the chunk kernels.  Passed BY VALUE inside the kernel parameter struct: kernel
 // parameters live in the constant bank, so every table look-up with a warp-uniform index is a
@@ -34,6 +38,7 @@ struct Tab {
 // (odd: conflict-free row reads; a multiple-of-4 family keeps the number of compiled variants small)
 __host__ __device__ inline int chunk_ld(int n) { return ((n + 3) / 4) * 4 + 1; }
 
+#ifndef SG_JIT
 inline void tab_build(const ModelDev* M, Tab* T) {
   memset(T, 0, sizeof(Tab));
   const int n = M->n;
@@ -45,6 +50,40 @@ inline void tab_build(const ModelDev* M, Tab* T) {
   }
   for (int q = 0; q < M->n_inst; ++q) T->tau[q] = M->tau[q];
 }
+#endif
+
+// Table access.  Statically compiled kernels read the tables from the kernel parameters (`T`); the
+// run-time specialised build (SG_JIT, jit.cu) replaces them by constants generated for one model, so
+// every loop over blocks / instruments unrolls and the family switch disappears.
+#ifdef SG_JIT
+#define TN JT_N
+#define TD JT_D
+#define TNI JT_NI
+#define TNB JT_NB
+#define TSTRIDE JT_STRIDE
+#define TBDIM(b) jt_bdim(b)
+#define TBOFF(b) jt_boff(b)
+#define TROFF(b) jt_roff(b)
+#define TBLKOF(j) jt_blkof(j)
+#define TCZ(i) (jt_czmask(i) ? T.cz[i] : 0.0) /* values stay run-time; the zero pattern is compile-time */
+#define TTAU(q) (T.tau[q])
+#define THQ(i) (T.hq[i])
+#define SG_UNROLL _Pragma("unroll")
+#else
+#define TN (T.n)
+#define TD (T.d)
+#define TNI (T.ninst)
+#define TNB (T.nblk)
+#define TSTRIDE (T.stride)
+#define TBDIM(b) (T.bdim[b])
+#define TBOFF(b) (T.boff[b])
+#define TROFF(b) (T.roff[b])
+#define TBLKOF(j) (T.blk_of[j])
+#define TCZ(i) (T.cz[i])
+#define TTAU(q) (T.tau[q])
+#define THQ(i) (T.hq[i])
+#define SG_UNROLL
+#endif
 
 // ---- record staging: global -> shared with cp.async (LDGSTS), one 8-byte copy per element ----------
 __device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
@@ -56,7 +95,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 template <int G>
 __device__ __forceinline__ void stage_rec(const Grp<G>& g, const Tab& T, const double* __restrict__ src, double* dst) {
-  for (int e = g.gl; e < T.stride; e += G) cp_async8(dst + e, src + e);
+  for (int e = g.gl; e < TSTRIDE; e += G) cp_async8(dst + e, src + e);
   cp_async_commit();
 }
 
@@ -83,23 +122,26 @@ __device__ __forceinline__ double blk_F(const double* __restrict__ r, const doub
 // U: lane-private scratch of nblk doubles at stride G.  `rec` in shared memory.
 template <int G, int VS, int OS>
 __device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigned tz, const double* vp, double* op, double* U) {
-  const int nblk = T.nblk, d = T.d;
+  const int nblk = TNB, d = TD;
+  SG_UNROLL
   for (int b = 0; b < nblk; ++b) {
-    const double* r = rec + T.roff[b];
-    const int off = T.boff[b];
+    const double* r = rec + TROFF(b);
+    const int off = TBOFF(b);
     double u;
-    switch (T.bdim[b]) {
+    switch (TBDIM(b)) {
       case 2: u = blk_F<2, VS, OS>(r, vp, op, off); break;
       case 3: u = blk_F<3, VS, OS>(r, vp, op, off); break;
       default: u = blk_F<4, VS, OS>(r, vp, op, off); break;
     }
     U[b * G] = u;
   }
-  for (int q = 0; q < T.ninst; ++q) {
+  SG_UNROLL
+  for (int q = 0; q < TNI; ++q) {
     double acc = 0.0;
     if (!((tz >> q) & 1u)) {
       acc = vp[(d + q) * VS];
-      for (int b = 0; b < nblk; ++b) acc = fma(T.cz[q * nblk + b], U[b * G], acc);
+      SG_UNROLL
+      for (int b = 0; b < nblk; ++b) acc = fma(TCZ(q * nblk + b), U[b * G], acc);
     }
     op[(d + q) * OS] = acc;
   }
@@ -122,47 +164,51 @@ __device__ __forceinline__ void blk_Ft(const double* __restrict__ r, const doubl
 
 template <int G, int VS, int OS>
 __device__ __forceinline__ void apply_Ft(const Tab& T, const double* rec, unsigned tz, const double* vp, double* op) {
-  const int nblk = T.nblk, d = T.d;
+  const int nblk = TNB, d = TD;
+  SG_UNROLL
   for (int b = 0; b < nblk; ++b) {
     double s = 0.0;
-    for (int q = 0; q < T.ninst; ++q)
-      if (!((tz >> q) & 1u)) s = fma(T.cz[q * nblk + b], vp[(d + q) * VS], s);
-    const double* r = rec + T.roff[b];
-    const int off = T.boff[b];
-    switch (T.bdim[b]) {
+    SG_UNROLL
+    for (int q = 0; q < TNI; ++q)
+      if (!((tz >> q) & 1u)) s = fma(TCZ(q * nblk + b), vp[(d + q) * VS], s);
+    const double* r = rec + TROFF(b);
+    const int off = TBOFF(b);
+    switch (TBDIM(b)) {
       case 2: blk_Ft<2, VS, OS>(r, vp, op, off, s); break;
       case 3: blk_Ft<3, VS, OS>(r, vp, op, off, s); break;
       default: blk_Ft<4, VS, OS>(r, vp, op, off, s); break;
     }
   }
-  for (int q = 0; q < T.ninst; ++q) op[(d + q) * OS] = ((tz >> q) & 1u) ? 0.0 : vp[(d + q) * VS];
+  SG_UNROLL
+  for (int q = 0; q < TNI; ++q) op[(d + q) * OS] = ((tz >> q) & 1u) ? 0.0 : vp[(d + q) * VS];
 }
 
 // column j of X += column j of Q = R Q~ R^T (Eq. 3.10 P:403-405 per block; z rows through c_qb)
 template <int LD>
 __device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsigned tz, int j, double* X) {
   constexpr int ld = LD;
-  const int d = T.d, nblk = T.nblk;
+  const int d = TD, nblk = TNB;
   if (j < d) {
-    const int b = T.blk_of[j], db = T.bdim[b], off = T.boff[b], jj = j - off;
-    const double* r = rec + T.roff[b];
+    const int b = TBLKOF(j), db = TBDIM(b), off = TBOFF(b), jj = j - off;
+    const double* r = rec + TROFF(b);
     const double* qxx = r + db * db + db;
     for (int i = 0; i < db; ++i) X[(off + i) * ld + j] += qxx[i * db + jj];
     const double q12 = r[2 * db * db + db + jj];
-    for (int q = 0; q < T.ninst; ++q)
-      if (!((tz >> q) & 1u)) X[(d + q) * ld + j] = fma(T.cz[q * nblk + b], q12, X[(d + q) * ld + j]);
-  } else if (j < T.n) {
+    for (int q = 0; q < TNI; ++q)
+      if (!((tz >> q) & 1u)) X[(d + q) * ld + j] = fma(TCZ(q * nblk + b), q12, X[(d + q) * ld + j]);
+  } else if (j < TN) {
     const int q = j - d;
     if ((tz >> q) & 1u) return;
-    for (int b = 0; b < nblk; ++b) {
-      const int db = T.bdim[b], off = T.boff[b];
-      const double* r = rec + T.roff[b];
-      const double c = T.cz[q * nblk + b];
+    SG_UNROLL
+  for (int b = 0; b < nblk; ++b) {
+      const int db = TBDIM(b), off = TBOFF(b);
+      const double* r = rec + TROFF(b);
+      const double c = TCZ(q * nblk + b);
       if (c == 0.0) continue;
       for (int l = 0; l < db; ++l) X[(off + l) * ld + j] = fma(c, r[2 * db * db + db + l], X[(off + l) * ld + j]);
       const double q22 = r[2 * db * db + 2 * db];
-      for (int p = 0; p < T.ninst; ++p)
-        if (!((tz >> p) & 1u)) X[(d + p) * ld + j] = fma(c * T.cz[p * nblk + b], q22, X[(d + p) * ld + j]);
+      for (int p = 0; p < TNI; ++p)
+        if (!((tz >> p) & 1u)) X[(d + p) * ld + j] = fma(c * TCZ(p * nblk + b), q22, X[(d + p) * ld + j]);
     }
   }
 }
@@ -173,7 +219,7 @@ __device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsig
 template <int G, int LD, bool ADDQ>
 __device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm, double* U) {
   constexpr int ld = LD;
-  const int n = T.n, j = g.gl;
+  const int n = TN, j = g.gl;
   if (j <= n) apply_F<G, LD, LD>(T, rec, tz, X + j, Tm + j, U);
   g.sync();
   if (j < n) {
@@ -188,7 +234,7 @@ __device__ __forceinline__ void sandwich_F(const Grp<G>& g, const Tab& T, const 
 template <int G, int LD>
 __device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const double* rec, unsigned tz, double* X, double* Tm) {
   constexpr int ld = LD;
-  const int n = T.n, j = g.gl;
+  const int n = TN, j = g.gl;
   if (j <= n) apply_Ft<G, LD, LD>(T, rec, tz, X + j, Tm + j);
   g.sync();
   if (j < n) {
@@ -203,7 +249,7 @@ __device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const
 template <int G, int LD>
 __device__ __forceinline__ void symmetrise(const Grp<G>& g, const Tab& T, double* X) {
   constexpr int ld = LD;
-  const int n = T.n, half = n >> 1, j = g.gl;
+  const int n = TN, half = n >> 1, j = g.gl;
   if (j < n) {
 #pragma unroll
     for (int s = 1; s <= (LD - 1) / 2; ++s) {

@@ -1,0 +1,164 @@
+// jit.cu -- run-time specialisation of the chunk kernels (k_fold0, k_down0, k_query) for one model
+// STRUCTURE: state dimension, block dimensions and offsets, number of instruments and which
+// (instrument, block) couplings are non-zero become compile-time constants, so the loops over blocks and
+// instruments unroll, the family switch disappears and all shared-memory addresses are immediates.
+// Hyper-parameter VALUES (couplings c_qb, tau, sigma) stay run-time kernel parameters: one compilation
+// serves every likelihood evaluation of an optimisation over the same kernel structure.
+//
+// The source is the very text of the statically compiled kernels (csrc/jit_src.inc, written by
+// _build.py from dev_consts.h + grp_dev.cuh + chunk_dev.cuh + chunk_kernels.cuh), compiled with NVRTC
+// for sm_100a and loaded through the runtime's library API.  NVRTC is opened with dlopen: when it is
+// not there, or a compilation fails, the generic kernels run instead (same arithmetic, same results).
+#include <dlfcn.h>
+#include <nvrtc.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "chunk_dev.cuh"
+#include "jit.h"
+
+static const char* const JIT_SRC =
+#include "jit_src.inc"
+    ;
+
+struct NvrtcApi {
+  void* h = nullptr;
+  nvrtcResult (*create)(nvrtcProgram*, const char*, const char*, int, const char* const*, const char* const*) = nullptr;
+  nvrtcResult (*compile)(nvrtcProgram, int, const char* const*) = nullptr;
+  nvrtcResult (*cubin_size)(nvrtcProgram, size_t*) = nullptr;
+  nvrtcResult (*cubin)(nvrtcProgram, char*) = nullptr;
+  nvrtcResult (*log_size)(nvrtcProgram, size_t*) = nullptr;
+  nvrtcResult (*log)(nvrtcProgram, char*) = nullptr;
+  nvrtcResult (*destroy)(nvrtcProgram*) = nullptr;
+  bool ok = false;
+};
+
+struct JitEntry {
+  std::string key;
+  SgJitKernels k;
+  bool good;
+};
+
+struct JitState {
+  NvrtcApi api;
+  bool tried_open = false;
+  std::vector<JitEntry> cache;
+  std::string log;
+};
+
+static bool open_nvrtc(NvrtcApi& a) {
+  const char* names[] = {"libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so.12"};
+  for (const char* nm : names) { a.h = dlopen(nm, RTLD_NOW | RTLD_LOCAL); if (a.h) break; }
+  if (!a.h) return false;
+#define SG_SYM(field, name) *(void**)(&a.field) = dlsym(a.h, name); if (!a.field) return false
+  SG_SYM(create, "nvrtcCreateProgram");
+  SG_SYM(compile, "nvrtcCompileProgram");
+  SG_SYM(cubin_size, "nvrtcGetCUBINSize");
+  SG_SYM(cubin, "nvrtcGetCUBIN");
+  SG_SYM(log_size, "nvrtcGetProgramLogSize");
+  SG_SYM(log, "nvrtcGetProgramLog");
+  SG_SYM(destroy, "nvrtcDestroyProgram");
+#undef SG_SYM
+  a.ok = true;
+  return true;
+}
+
+static std::string structure_key(const Tab& T, int G, int LD) {
+  char buf[64];
+  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, G, LD);
+  std::string k = buf;
+  for (int b = 0; b < T.nblk; ++b) { snprintf(buf, sizeof buf, "%d.%d.%d;", T.bdim[b], T.boff[b], T.roff[b]); k += buf; }
+  k += "|";
+  for (int i = 0; i < T.ninst * T.nblk; ++i) k += (T.cz[i] != 0.0) ? '1' : '0';
+  return k;
+}
+
+static void int_table(std::string& s, const char* name, int cnt, const int* v) {
+  char buf[64];
+  s += "__device__ constexpr int ";
+  s += name;
+  s += "(int i) { constexpr int v[] = {";
+  for (int i = 0; i < cnt; ++i) { snprintf(buf, sizeof buf, "%d,", v[i]); s += buf; }
+  s += "0}; return v[i]; }\n";
+}
+
+static std::string prelude(const Tab& T, int G, int LD) {
+  std::string s = "#define SG_JIT 1\n"
+                  "typedef long long int64_t;\ntypedef unsigned long long uint64_t;\n"
+                  "typedef int int32_t;\ntypedef unsigned int uint32_t;\n";
+  char buf[128];
+  snprintf(buf, sizeof buf, "#define JT_N %d\n#define JT_D %d\n#define JT_NI %d\n#define JT_NB %d\n#define JT_STRIDE %d\n", T.n, T.d,
+           T.ninst, T.nblk, T.stride);
+  s += buf;
+  snprintf(buf, sizeof buf, "#define JT_G %d\n#define JT_LD %d\n", G, LD);
+  s += buf;
+  int v[SG_MAXINST * SG_MAXBLK];
+  for (int b = 0; b < T.nblk; ++b) v[b] = T.bdim[b];
+  int_table(s, "jt_bdim", T.nblk, v);
+  for (int b = 0; b < T.nblk; ++b) v[b] = T.boff[b];
+  int_table(s, "jt_boff", T.nblk, v);
+  for (int b = 0; b < T.nblk; ++b) v[b] = T.roff[b];
+  int_table(s, "jt_roff", T.nblk, v);
+  for (int j = 0; j < T.d; ++j) v[j] = T.blk_of[j];
+  int_table(s, "jt_blkof", T.d, v);
+  for (int i = 0; i < T.ninst * T.nblk; ++i) v[i] = (T.cz[i] != 0.0) ? 1 : 0;
+  int_table(s, "jt_czmask", T.ninst * T.nblk, v);
+  return s;
+}
+
+static JitState* state_of(smolgp_ctx* ctx) {
+  if (!ctx->jit) ctx->jit = new JitState();
+  return (JitState*)ctx->jit;
+}
+
+void sg_jit_destroy(smolgp_ctx* ctx) {
+  JitState* st = (JitState*)ctx->jit;
+  if (!st) return;
+  for (auto& e : st->cache)
+    if (e.good) cudaLibraryUnload(e.k.lib);
+  if (st->api.h) dlclose(st->api.h);
+  delete st;
+  ctx->jit = nullptr;
+}
+
+const char* sg_jit_log(smolgp_ctx* ctx) { return ctx->jit ? ((JitState*)ctx->jit)->log.c_str() : ""; }
+
+// returns the specialised kernels for (T's structure, G, LD), compiling them on first use; nullptr when
+// run-time compilation is unavailable or failed (the reason is kept in sg_jit_log)
+const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD) {
+  JitState* st = state_of(ctx);
+  const std::string key = structure_key(T, G, LD);
+  for (auto& e : st->cache)
+    if (e.key == key) return e.good ? &e.k : nullptr;
+  if (!st->tried_open) { st->tried_open = true; if (!open_nvrtc(st->api)) st->log = "NVRTC not available (dlopen libnvrtc.so.12 failed)"; }
+  JitEntry ent;
+  ent.key = key;
+  ent.good = false;
+  memset(&ent.k, 0, sizeof ent.k);
+  if (st->api.ok) {
+    const std::string src = prelude(T, G, LD) + JIT_SRC;
+    nvrtcProgram prog = nullptr;
+    const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo"};
+    nvrtcResult r = st->api.create(&prog, src.c_str(), "smolgp_chunk_jit.cu", 0, nullptr, nullptr);
+    if (r == NVRTC_SUCCESS) r = st->api.compile(prog, 3, opts);
+    if (r != NVRTC_SUCCESS) {
+      size_t ls = 0;
+      if (prog && st->api.log_size(prog, &ls) == NVRTC_SUCCESS && ls > 1) { st->log.resize(ls); st->api.log(prog, &st->log[0]); }
+      else st->log = "nvrtc: compilation failed";
+    } else {
+      size_t cs = 0;
+      st->api.cubin_size(prog, &cs);
+      std::vector<char> cubin(cs);
+      st->api.cubin(prog, cubin.data());
+      cudaError_t e = cudaLibraryLoadData(&ent.k.lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.fold0, ent.k.lib, "jit_fold0");
+      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.down0, ent.k.lib, "jit_down0");
+      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.query, ent.k.lib, "jit_query");
+      if (e == cudaSuccess) ent.good = true;
+      else { st->log = std::string("loading the specialised kernels: ") + cudaGetErrorString(e); cudaGetLastError(); }
+    }
+    if (prog) st->api.destroy(&prog);
+  }
+  st->cache.push_back(ent);
+  return st->cache.back().good ? &st->cache.back().k : nullptr;
+}

@@ -1,3 +1,6 @@
+#include <stddef.h>
+
+#include "jit.h"
 // scan_host.cu -- host orchestration of the scan kernels (level plan, workspace carving, launches).
 // Included at the end of scan.cu (same translation unit as the kernels it launches).
 
@@ -31,6 +34,22 @@ static int groups_per_cta(size_t per_group, int G, int* groups_per_sm = nullptr)
   return best;
 }
 
+// run-time specialised kernels (jit.cu): always when asked for, by default from 1e5 events per call
+// (the one-off compilation, ~5 s per model structure, is cached in the ctx)
+static bool want_jit(const smolgp_ctx* ctx, int64_t events) {
+  return ctx->opt_jit > 0 || (ctx->opt_jit == 0 && events >= 100000);
+}
+
+static int launch_jit(smolgp_ctx* ctx, cudaKernel_t k, int kid, unsigned blocks, unsigned threads, size_t smem, const void* params) {
+  SG_CUDA(ctx, cudaFuncSetAttribute((const void*)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  void* args[1] = {const_cast<void*>(params)};
+  sg_launch_begin(ctx, kid);
+  cudaError_t e = cudaLaunchKernel((const void*)k, dim3(blocks), dim3(threads), args, smem, ctx->stream);
+  sg_launch_end(ctx);
+  SG_CUDA(ctx, e);
+  return SMOLGP_OK;
+}
+
 template <int G, int LD>
 static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold) {
   const int n = hm->n;
@@ -41,6 +60,10 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = P.batch * P.c1;
   const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
+  if (want_jit(ctx, P.batch * P.K)) {
+    if (const SgJitKernels* jk = sg_jit_get(ctx, P.T, G, LD))
+      return launch_jit(ctx, fold ? jk->fold0 : jk->down0, fold ? KID_FOLD0 : KID_DOWN0, blocks, gpc * G, smem, &P);
+  }
   if (fold) {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_FOLD0);
@@ -163,7 +186,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
 
   ScanDev P;
   tab_build(hm, &P.T);
-  P.M = a.d_model; P.disc = a.disc; P.dt = a.ev->dt; P.delta = a.ev->delta; P.meta = a.ev->meta; P.obs = a.ev->obs;
+  P.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); P.disc = a.disc; P.dt = a.ev->dt; P.delta = a.ev->delta; P.meta = a.ev->meta; P.obs = a.ev->obs;
   P.y = a.y; P.sigma = a.sigma; P.amp = a.amp; P.K = K; P.N = N; P.batch = batch; P.Lc = (int)Lc; P.c1 = c1;
   P.E1 = pl.T ? (double*)(w + oE[1]) : nullptr;
   P.PRE1 = pl.T ? (const double*)(w + oPRE[1]) : nullptr;
@@ -213,6 +236,10 @@ static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) 
   const size_t smem = tab_bytes() + per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = Q.batch * Q.Mq;
+  if (want_jit(ctx, Q.batch * Q.K)) {
+    if (const SgJitKernels* jk = sg_jit_get(ctx, Q.T, G, LD))
+      return launch_jit(ctx, jk->query, KID_QUERY, (unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, &Q);
+  }
   SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   sg_launch_begin(ctx, KID_QUERY);
   k_query<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
@@ -245,7 +272,7 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   if (rc) return rc;
   QueryDev Q;
   tab_build(hm, &Q.T);
-  Q.M = a.d_model; Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
+  Q.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
   Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
   const int G = pick_lanes(ctx, n), LD = chunk_ld(n);
 #define SG_CALL_Q(g_, ld_) return launch_query<g_, ld_>(ctx, Q, hm)

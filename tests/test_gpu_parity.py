@@ -25,6 +25,7 @@ def _reset(ctx):
     ctx.set_option("chunk", 0)
     ctx.set_option("group", 0)
     ctx.set_option("lanes", 0)
+    ctx.set_option("jit", 0)
 
 
 SCAN_OPTS = {
@@ -32,6 +33,7 @@ SCAN_OPTS = {
     "sequential": (("chunk", 1 << 40),),                       # one chunk per series (row a8)
     "deep": (("chunk", 16), ("group", 2)),                     # many dense levels
     "ragged": (("chunk", 37), ("group", 3), ("lanes", 32)),    # chunk/group sizes dividing nothing
+    "jit": (("chunk", 29), ("jit", 1)),                        # run-time specialised chunk kernels (NVRTC)
 }
 
 
