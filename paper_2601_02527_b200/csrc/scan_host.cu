@@ -149,7 +149,9 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     groups_per_cta((size_t)fold0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
     if (per_sm_f < per_sm) per_sm = per_sm_f;
     const int64_t resident = (int64_t)ctx->sm_count * per_sm;
-    if (batch >= resident) Lc = K;
+    // measured on config 5 (profiles/r01_sweeps.md): once the batch alone gives every SM >= 4 warps, one
+    // chunk per series wins, because chunking costs the extra fold pass (~ +70 % arithmetic)
+    if (batch >= resident || batch * G >= (int64_t)ctx->sm_count * 4 * 32) Lc = K;
     else {
       const int64_t per_series = (resident + batch - 1) / batch; // chunks per series
       Lc = (K + per_series - 1) / per_series;
@@ -161,7 +163,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   LevelPlan pl;
   pl.T = 0;
   const int64_t c1 = (K + Lc - 1) / Lc;
-  if (g == 0) g = 4; // measured on config 3 (profiles/r01_accuracy_cfg3.md): fastest; neither deeper nor flatter trees are reliably more accurate
+  if (g == 0) g = 3; // measured on configs 3 and 4 (profiles/r01_accuracy_cfg3.md, r01_sweeps.md): fastest; neither deeper nor flatter trees are reliably more accurate
   if (c1 > 1) {
     pl.T = 1;
     pl.cnt[1] = c1;
