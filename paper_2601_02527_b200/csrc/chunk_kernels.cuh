@@ -76,15 +76,23 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
   for (int i = g.gl; i < n; i += G) AB0[i * ld + i] = 1.0;
   g.sync();
 
+  uint32_t meta_nx = P.meta[k0];
+  int32_t ob_nx = P.obs[k0];
   for (int64_t k = k0; k < k1; ++k) {
     const double* rec = recs + ((k - k0) & 1) * TSTRIDE;
     cp_async_wait_all();
     g.sync();
     if (k + 1 < k1) stage_rec(g, T, P.disc + (k + 1) * (int64_t)TSTRIDE, recs + ((k + 1 - k0) & 1) * TSTRIDE);
-    const uint32_t meta = P.meta[k];
+    // event k's scalars were requested one iteration ago; the data of an end event are requested now
+    // and consumed after the products, so no global latency sits on the per-event critical path
+    const uint32_t meta = meta_nx;
+    const int32_t ob = ob_nx;
+    if (k + 1 < k1) { meta_nx = P.meta[k + 1]; ob_nx = P.obs[k + 1]; }
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
+    double dl_r = 1.0, sg_r = 0.0, y_r = 0.0;
+    if (!kind) { dl_r = P.delta[k]; sg_r = P.sigma[ob]; y_r = P.y[series * P.N + ob]; }
     // [A | b] <- F [A | b], in place: a lane reads a block of its column into registers before it
     // writes that block, and the z rows read only z entries, which are written last
     if (g.gl <= n) apply_F<G, LD, LD>(T, rec, tz, AB0 + g.gl, AB0 + g.gl, U);
@@ -94,10 +102,9 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
       // observe z_q / delta: h = hs e_z in equilibrated units (Eq. 3.12); SG21 Eq. 10 with the
       // aggregate as the earlier element (rank-one J_j): Sherman-Morrison form of the combine
       const int zi = d + q;
-      const int32_t ob = P.obs[k];
-      const double hs = TTAU(q) / P.delta[k];
-      const double sg = P.sigma[ob] * ramp;
-      const double yy = P.y[series * P.N + ob] * ramp;
+      const double hs = TTAU(q) / dl_r;
+      const double sg = sg_r * ramp;
+      const double yy = y_r * ramp;
       const double S = hs * hs * C[zi * ld + zi] + sg * sg;
       if (!(S > 0.0) || !isfinite(S)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S;
@@ -213,22 +220,27 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   g.sync();
   double ll = 0.0;
   // ---- forward ----
+  uint32_t meta_nx = P.meta[k0];
+  int32_t ob_nx = P.obs[k0];
   for (int64_t k = k0; k < k1; ++k) {
     const double* rec = recs + ((k - k0) & 1) * TSTRIDE;
     cp_async_wait_all();
     g.sync();
     if (k + 1 < k1) stage_rec(g, T, P.disc + (k + 1) * (int64_t)TSTRIDE, recs + ((k + 1 - k0) & 1) * TSTRIDE);
-    const uint32_t meta = P.meta[k];
+    const uint32_t meta = meta_nx; // prefetched: see k_fold0
+    const int32_t ob = ob_nx;
+    if (k + 1 < k1) { meta_nx = P.meta[k + 1]; ob_nx = P.obs[k + 1]; }
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
+    double dl_r = 1.0, sg_r = 0.0, y_r = 0.0;
+    if (!kind) { dl_r = P.delta[k]; sg_r = P.sigma[ob]; y_r = P.y[series * P.N + ob]; }
     sandwich_F<G, LD, true>(g, T, rec, tz, X, Tm, U);
     if (!kind) {
       const int zi = d + q;
-      const int32_t ob = P.obs[k];
-      const double hs = TTAU(q) / P.delta[k];
-      const double sg = P.sigma[ob] * ramp;
-      const double yy = P.y[series * P.N + ob] * ramp;
+      const double hs = TTAU(q) / dl_r;
+      const double sg = sg_r * ramp;
+      const double yy = y_r * ramp;
       const double S = hs * hs * X[zi * ld + zi] + sg * sg;
       const double v = yy - hs * X[zi * ld + n];
       if (!(S > 0.0) || !isfinite(S) || !isfinite(v)) atomicOr(P.flags, NUMF_BAD);
@@ -287,12 +299,25 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   zero_fill(g, Tm, NR * ld); // the solve used this region as Ws
   g.sync();
   // ---- backward ----
+  // backward prefetch: meta / exposure index one event ahead, the end event's kbuf record (one entry of
+  // K and of p per lane, S, v, filtered z mean) and exposure length requested before the previous step
+  meta_nx = P.meta[k1 - 1];
+  ob_nx = P.obs[k1 - 1];
+  double kv_r = 0.0, pv_r = 0.0, S_r = 1.0, v_r = 0.0, m_r = 0.0, dlb_r = 1.0;
+  if (!META_KIND(meta_nx)) {
+    const double* kb = P.kbuf + (series * P.N + ob_nx) * (int64_t)ks;
+    if (g.gl < n) { kv_r = kb[g.gl]; pv_r = kb[n + g.gl]; }
+    S_r = kb[2 * n]; v_r = kb[2 * n + 1]; m_r = kb[2 * n + 2]; dlb_r = P.delta[k1 - 1];
+  }
   for (int64_t k = k1 - 1; k >= k0; --k) {
     const double* rec = recs + ((k1 - 1 - k) & 1) * TSTRIDE;
     cp_async_wait_all();
     g.sync();
     if (k > k0) stage_rec(g, T, P.disc + (k - 1) * (int64_t)TSTRIDE, recs + ((k1 - k) & 1) * TSTRIDE);
-    const uint32_t meta = P.meta[k];
+    const uint32_t meta = meta_nx;
+    const int32_t ob = ob_nx;
+    const double kv_c = kv_r, pv_c = pv_r, S = S_r, v = v_r, mfz = m_r, dl_c = dlb_r;
+    if (k > k0) { meta_nx = P.meta[k - 1]; ob_nx = P.obs[k - 1]; }
     const int kind = META_KIND(meta), q = META_INST(meta);
     const unsigned zm = META_ZMASK(meta);
     // components zeroed after event k pass nothing backwards (adjoint of the zeroing)
@@ -304,11 +329,8 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
     g.sync();
     if (!kind) {
       const int zi = d + q;
-      const int32_t ob = P.obs[k];
-      const double hs = TTAU(q) / P.delta[k];
-      const double* kb = P.kbuf + (series * P.N + ob) * (int64_t)ks;
-      for (int i = g.gl; i < n; i += G) { kv[i] = kb[i]; pv[i] = kb[n + i]; }
-      const double S = kb[2 * n], v = kb[2 * n + 1], mfz = kb[2 * n + 2];
+      const double hs = TTAU(q) / dl_c;
+      if (g.gl < n) { kv[g.gl] = kv_c; pv[g.gl] = pv_c; }
       const double rS = 1.0 / S;
       g.sync();
       double quad = 0.0, kap = 0.0;
@@ -345,6 +367,11 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
     }
     if (P.binfo) store_state<G, LD>(g, T, X, P.binfo + (series * P.K + k) * (int64_t)ss);
     if (k == k0) break;
+    if (!META_KIND(meta_nx)) { // request event k-1's record now: it arrives during the step below
+      const double* kb = P.kbuf + (series * P.N + ob_nx) * (int64_t)ks;
+      if (g.gl < n) { kv_r = kb[g.gl]; pv_r = kb[n + g.gl]; }
+      S_r = kb[2 * n]; v_r = kb[2 * n + 1]; m_r = kb[2 * n + 2]; dlb_r = P.delta[k - 1];
+    }
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
     sandwich_Ft<G, LD>(g, T, rec, tz, X, Tm);
   }
