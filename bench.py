@@ -41,6 +41,16 @@ def min_bytes(n):
     return 32 + 2 * 8 * (n + n * (n + 1) // 2)
 
 
+def ncu_traffic(kernel, cfg):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/r01_top_kernel_traffic.json; config 3 only), else None"""
+    try:
+        rec = json.load(open(os.path.join(ROOT, "profiles", "r01_top_kernel_traffic.json")))
+        return rec["traffic_bytes_per_launch"] if (rec["kernel"] == kernel and cfg == 3) else None
+    except (OSError, ValueError, KeyError):
+        return None
+
+
 def model_dim(w):
     d = 0
     for c in w["kernel"]:
@@ -59,7 +69,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -258,7 +268,7 @@ def run_cuda(args, w, cfgname):
     flops_launch = K_events * w_useful_flops(n) / launches_per_step
     achieved = flops_launch / (t_top_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(top, args.config),
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md); register-only DFMA probe measured %.1f TFLOP/s in this run" % fp64_probe,
                 "work_model": "W_useful = 10.3 n^3 + 9 n^2 flop/event (SURVEY 8(d)), n = %d" % n,
                 "kernel_share_of_step": prof[top][0] / ms,
