@@ -39,8 +39,8 @@ struct ScanDev {
 // ---------------------------------------------------------------------------------------------------
 // k_fold0: chunk -> element.  Column-owned layout of chunk_dev.cuh.
 // ---------------------------------------------------------------------------------------------------
-__host__ __device__ inline int fold0_group_doubles(int n, int stride, int nblk, int G) {
-  const int ld = chunk_ld(n), nr = ld - 1; // nr >= n rows: the padding rows stay zero, so row loops run to the compile-time nr
+__host__ __device__ inline int fold0_group_doubles(int n, int ld, int stride, int nblk, int G) {
+  const int nr = ld - 1; // nr >= n rows: the padding rows stay zero, so row loops run to the compile-time nr
   return 4 * nr * ld + 2 * stride + nblk * G + 2 * ld + 2;
 }
 
@@ -55,7 +55,7 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * fold0_group_doubles(n, TSTRIDE, TNB, G);
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * fold0_group_doubles(n, LD, TSTRIDE, TNB, G);
   constexpr int NR = LD - 1;
   double* AB0 = base;            // [A | b]
   double* C = AB0 + NR * ld;
@@ -156,8 +156,8 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
 // dense levels.  DESIGN.md 5.
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int kbuf_stride(int n) { return 2 * n + 4; }
-__host__ __device__ inline int down0_group_doubles(int n, int stride, int nblk, int G) {
-  const int ld = chunk_ld(n), nr = ld - 1, ws = n * (2 * n + 1) > nr * ld ? n * (2 * n + 1) : nr * ld;
+__host__ __device__ inline int down0_group_doubles(int n, int ld, int stride, int nblk, int G) {
+  const int nr = ld - 1, ws = n * (2 * n + 1) > nr * ld ? n * (2 * n + 1) : nr * ld;
   return nr * ld + ws + 2 * stride + nblk * G + 5 * ld + 1; // Tm is the head of Ws
 }
 
@@ -191,7 +191,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, TSTRIDE, TNB, G);
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * down0_group_doubles(n, LD, TSTRIDE, TNB, G);
   constexpr int NR = LD - 1;        // rows allocated (>= n): padding rows and vector tails stay zero
   double* X = base;                 // [P | m], later [Lambda | lambda]
   double* Tm = X + NR * ld;
@@ -393,8 +393,7 @@ struct QueryDev {
   int* flags;
 };
 
-__host__ __device__ inline int query_group_doubles(int n, int stride, int nblk, int G) {
-  const int ld = chunk_ld(n);
+__host__ __device__ inline int query_group_doubles(int n, int ld, int stride, int nblk, int G) {
   return 3 * (ld - 1) * ld + 2 * stride + nblk * G + 2 * ld + 1;
 }
 
@@ -409,7 +408,7 @@ __device__ __forceinline__ void query_body(const QueryDev& P) {
   const int gpc = blockDim.x / G;
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.Mq) return;
-  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * query_group_doubles(n, TSTRIDE, TNB, G);
+  double* base = (double*)(smem + tb) + (size_t)(threadIdx.x / G) * query_group_doubles(n, LD, TSTRIDE, TNB, G);
   double* X = base;                 // [P* | m*]
   constexpr int NR = LD - 1;
   double* Tm = X + NR * ld;

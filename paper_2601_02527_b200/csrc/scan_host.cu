@@ -50,20 +50,28 @@ static int launch_jit(smolgp_ctx* ctx, cudaKernel_t k, int kid, unsigned blocks,
   return SMOLGP_OK;
 }
 
+// row stride in effect: the specialised kernels take the tightest odd stride (n + 1) | 1 (less shared
+// memory per group => more groups per SM); the static variants are compiled for chunk_ld(n) only
+static int eff_ld(smolgp_ctx* ctx, const Tab& T, int G, int64_t events, const SgJitKernels** jk) {
+  *jk = nullptr;
+  if (want_jit(ctx, events)) {
+    const int ldj = (T.n + 1) | 1;
+    *jk = sg_jit_get(ctx, T, G, ldj);
+    if (*jk) return ldj;
+  }
+  return chunk_ld(T.n);
+}
+
 template <int G, int LD>
 static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold) {
   const int n = hm->n;
-  const int gd = fold ? fold0_group_doubles(n, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, hm->disc_stride, hm->nblk, G);
+  const int gd = fold ? fold0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G);
   const size_t per_group = (size_t)gd * 8;
   const int gpc = groups_per_cta(per_group, G);
   const size_t smem = tab_bytes() + per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = P.batch * P.c1;
   const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
-  if (want_jit(ctx, P.batch * P.K)) {
-    if (const SgJitKernels* jk = sg_jit_get(ctx, P.T, G, LD))
-      return launch_jit(ctx, fold ? jk->fold0 : jk->down0, fold ? KID_FOLD0 : KID_DOWN0, blocks, gpc * G, smem, &P);
-  }
   if (fold) {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_FOLD0);
@@ -99,7 +107,18 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
   } while (0)
 
 static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G) {
-  const int LD = chunk_ld(hm->n);
+  const SgJitKernels* jk;
+  const int LD = eff_ld(ctx, P.T, G, P.batch * P.K, &jk);
+  if (jk) {
+    const int n = hm->n;
+    const int gd = fold ? fold0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G);
+    const size_t per_group = (size_t)gd * 8;
+    const int gpc = groups_per_cta(per_group, G);
+    const size_t smem = per_group * gpc;
+    if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+    const int64_t groups = P.batch * P.c1;
+    return launch_jit(ctx, fold ? jk->fold0 : jk->down0, fold ? KID_FOLD0 : KID_DOWN0, (unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, &P);
+  }
 #define SG_CALL_L0(g_, ld_) return launch_level0<g_, ld_>(ctx, P, hm, fold)
   SG_DISPATCH_GL(G, LD, SG_CALL_L0);
 #undef SG_CALL_L0
@@ -143,10 +162,14 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   if (Lc <= 0) {
     // one full wave: as many chunks as groups can be resident at once (equal work per chunk, no tail);
     // a batch that already fills the machine runs one chunk per series (the sequential filter, row a8)
+    Tab T0;
+    tab_build(hm, &T0);
+    const SgJitKernels* jk0;
+    const int ld0 = eff_ld(ctx, T0, G, batch * K, &jk0);
     int per_sm = 1;
-    groups_per_cta((size_t)down0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
+    groups_per_cta((size_t)down0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
     int per_sm_f = 1;
-    groups_per_cta((size_t)fold0_group_doubles(n, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
+    groups_per_cta((size_t)fold0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
     if (per_sm_f < per_sm) per_sm = per_sm_f;
     const int64_t resident = (int64_t)ctx->sm_count * per_sm;
     // measured on config 5 (profiles/r01_sweeps.md): once the batch alone gives every SM >= 4 warps, one
@@ -233,15 +256,11 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
 
 template <int G, int LD>
 static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
-  const size_t per_group = (size_t)query_group_doubles(hm->n, hm->disc_stride, hm->nblk, G) * 8;
+  const size_t per_group = (size_t)query_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
   const int gpc = groups_per_cta(per_group, G);
   const size_t smem = tab_bytes() + per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = Q.batch * Q.Mq;
-  if (want_jit(ctx, Q.batch * Q.K)) {
-    if (const SgJitKernels* jk = sg_jit_get(ctx, Q.T, G, LD))
-      return launch_jit(ctx, jk->query, KID_QUERY, (unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, &Q);
-  }
   SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   sg_launch_begin(ctx, KID_QUERY);
   k_query<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
@@ -276,7 +295,15 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   tab_build(hm, &Q.T);
   Q.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
   Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
-  const int G = pick_lanes(ctx, n), LD = chunk_ld(n);
+  const int G = pick_lanes(ctx, n);
+  const SgJitKernels* jk;
+  const int LD = eff_ld(ctx, Q.T, G, Q.batch * Q.K, &jk);
+  if (jk) {
+    const size_t per_group = (size_t)query_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) * 8;
+    const int gpc = groups_per_cta(per_group, G);
+    const int64_t groups = Q.batch * Q.Mq;
+    return launch_jit(ctx, jk->query, KID_QUERY, (unsigned)((groups + gpc - 1) / gpc), gpc * G, per_group * gpc, &Q);
+  }
 #define SG_CALL_Q(g_, ld_) return launch_query<g_, ld_>(ctx, Q, hm)
   SG_DISPATCH_GL(G, LD, SG_CALL_Q);
 #undef SG_CALL_Q
