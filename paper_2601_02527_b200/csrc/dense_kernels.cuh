@@ -1,0 +1,262 @@
+// dense_kernels.cuh -- the dense levels of the scan: combine of chunk aggregates (k_foldD) and the
+// down-sweep of prefix states / suffix information (k_downD).  One CTA of NT threads per group of
+// elements; all matrices n x n in shared memory.  Device-safe text on top of dev_consts.h and
+// grp_dev.cuh: compiled statically with a run-time n and, specialised, with n as a constant (jit.cu).
+#pragma once
+#include "chunk_kernels.cuh"
+
+#ifdef SG_JIT
+#define DN JT_N
+#else
+#define DN (P.n)
+#endif
+
+// general dense product  D[i,j] = (C ? C[i,j] : 0) + sum_l A[i,l] B[l,j],  strided operands
+template <int G>
+__device__ __forceinline__ void mm(const Grp<G>& g, int nr, int nc, int nk, const double* A, int ar, int ac,
+                                   const double* B, int br, int bc, const double* C, int cr, int cc, double* D, int dr, int dc) {
+  const float rnc = 1.0f / (float)nc;
+  for (int e = g.gl; e < nr * nc; e += G) {
+    int i, j;
+    divmod_small(e, nc, rnc, i, j);
+    double acc = C ? C[i * cr + j * cc] : 0.0;
+    for (int l = 0; l < nk; ++l) acc = fma(A[i * ar + l * ac], B[l * br + j * bc], acc);
+    D[i * dr + j * dc] = acc;
+  }
+}
+// symmetric result: D[i,j] = D[j,i] = (C ? C[i,j] : 0) + sum_l A[i,l] B[l,j] for i >= j (n x n, row stride n)
+template <int G>
+__device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const double* A, int ar, int ac,
+                                       const double* B, int br, int bc, const double* C, double* D) {
+  for (int e = g.gl; e < n * n; e += G) {
+    const int i = e / n, j = e - i * n;
+    if (j > i) continue;
+    double acc = C ? C[i * n + j] : 0.0;
+    for (int l = 0; l < nk; ++l) acc = fma(A[i * ar + l * ac], B[l * br + j * bc], acc);
+    D[i * n + j] = acc;
+    D[j * n + i] = acc;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// dense combine (SG21 Eq. 11 as cited P:502; the paper prints neither): with
+// M = (I + C_i J_j)^-1,
+//   A = A_j M A_i,  b = A_j M (b_i + C_i eta_j) + b_j,  C = A_j M C_i A_j^T + C_j,
+//   eta = A_i^T M^T (eta_j - J_j b_i) + eta_i,           J = A_i^T M^T J_j A_i + J_i.
+// One warp per group.  ei, ej, eo: elements in shared memory (layout above); Ws: n x (3n+1); Tm: n x n.
+// ---------------------------------------------------------------------------------------------------
+template <int G>
+__device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const double* ej, double* eo,
+                              double* Ws, double* Tm, double* uv) {
+  const int n1 = n + 1, ld = 3 * n + 1;
+  const double *Ai = ei, *Ci = ei + n * n1, *Ji = Ci + n * n;
+  const double *Aj = ej, *Cj = ej + n * n1, *Jj = Cj + n * n;
+  double *Ao = eo, *Co = eo + n * n1, *Jo = Co + n * n;
+  // Ws = [I + C_i J_j | A_i | b_i + C_i eta_j | C_i]
+  mm(g, n, n1, n, Ci, n, 1, Jj, n1, 1, (const double*)nullptr, 0, 0, Tm, n1, 1); // n x (n+1): C_i [J_j | eta_j]  (Tm has room: see caller)
+  g.sync();
+  for (int e = g.gl; e < n * n; e += G) {
+    const int i = e / n, j = e - i * n;
+    Ws[i * ld + j] = Tm[i * n1 + j] + (i == j ? 1.0 : 0.0);
+    Ws[i * ld + n + j] = Ai[i * n1 + j];
+    Ws[i * ld + 2 * n + 1 + j] = Ci[i * n + j];
+  }
+  for (int i = g.gl; i < n; i += G) Ws[i * ld + 2 * n] = Ai[i * n1 + n] + Tm[i * n1 + n];
+  // u = eta_j - J_j b_i
+  for (int i = g.gl; i < n; i += G) {
+    double acc = Jj[i * n1 + n];
+    for (int l = 0; l < n; ++l) acc = fma(-Jj[i * n1 + l], Ai[l * n1 + n], acc);
+    uv[i] = acc;
+  }
+  g.sync();
+  gj_solve(g, n, ld, Ws);
+  const double* X1 = Ws + n;         // M A_i           (row stride ld)
+  const double* X2 = Ws + 2 * n;     // M (b_i + C_i eta_j), then X3 = M C_i follows
+  // [A | b] = A_j [X1 | x2] (+ b_j in the last column)
+  mm(g, n, n1, n, Aj, n1, 1, X1, ld, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
+  // Tm = A_j X3
+  mm(g, n, n, n, Aj, n1, 1, X2 + 1, ld, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+  g.sync();
+  for (int i = g.gl; i < n; i += G) Ao[i * n1 + n] += Aj[i * n1 + n];
+  // C = Tm A_j^T + C_j
+  mm_sym(g, n, n, Tm, n, 1, Aj, 1, n1, Cj, Co);
+  // eta = X1^T u + eta_i
+  for (int i = g.gl; i < n; i += G) {
+    double acc = Ji[i * n1 + n];
+    for (int l = 0; l < n; ++l) acc = fma(X1[l * ld + i], uv[l], acc);
+    Jo[i * n1 + n] = acc;
+  }
+  g.sync();
+  // Tm = J_j A_i ; J = X1^T Tm + J_i
+  mm(g, n, n, n, Jj, n1, 1, Ai, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+  g.sync();
+  for (int e = g.gl; e < n * n; e += G) {
+    const int i = e / n, j = e - i * n;
+    if (j > i) continue;
+    double acc = Ji[i * n1 + j];
+    for (int l = 0; l < n; ++l) acc = fma(X1[l * ld + i], Tm[l * n + j], acc);
+    Jo[i * n1 + j] = acc;
+    Jo[j * n1 + i] = acc;
+  }
+  g.sync();
+}
+
+__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 1) + n * (n + 1) + n; }
+
+struct DenseArgs {
+  int n;              // augmented state dimension
+  const double* p0;   // [n][n] prior covariance
+  const double* Ein;  // [batch*cin][elem]
+  double* Eout;       // [batch*cout][elem]
+  int64_t cin, cout, batch;
+  int g;              // fan-in
+  // down-sweep
+  const double* PREup; // [batch*cout][state] or NULL -> prior
+  const double* SUFup; // [batch*cout][state] or NULL -> zero
+  double* PRE;         // [batch*cin][state]
+  double* SUF;         // [batch*cin][state]
+  int want_suffix;
+};
+
+template <int NT>
+__device__ __forceinline__ void foldD_body(const DenseArgs& P) {
+  extern __shared__ __align__(16) char smem[];
+  const int n = DN, es = elem_size(n);
+  const size_t tb = 0;
+  const Grp<NT> g;
+  const int64_t gid = blockIdx.x;
+  if (gid >= P.batch * P.cout) return;
+  double* base = (double*)(smem + tb);
+  double* e0 = base; double* e1 = e0 + es; double* e2 = e1 + es;
+  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 1); double* uv = Tm + n * (n + 1);
+  const int64_t series = gid / P.cout, grp = gid - series * P.cout;
+  const int64_t m0 = grp * P.g, m1 = (m0 + P.g < P.cin) ? m0 + P.g : P.cin;
+  const double* src = P.Ein + (series * P.cin + m0) * (int64_t)es;
+  for (int e = g.gl; e < es; e += NT) e0[e] = src[e];
+  g.sync();
+  double* acc = e0; double* nxt = e1; double* out = e2;
+  for (int64_t m = m0 + 1; m < m1; ++m) {
+    src += es;
+    for (int e = g.gl; e < es; e += NT) nxt[e] = src[e];
+    g.sync();
+    dense_combine(g, n, acc, nxt, out, Ws, Tm, uv);
+    double* t = acc; acc = out; out = t;
+  }
+  double* dst = P.Eout + gid * (int64_t)es;
+  for (int e = g.gl; e < es; e += NT) dst[e] = acc[e];
+}
+
+// ---------------------------------------------------------------------------------------------------
+// down-sweep over dense elements.  blockIdx.y = 0: prefix states; 1: suffix information.
+//   forward : (m,P) (x) element:  M = (I + P J)^-1;  m' = A M (m + P eta) + b;  P' = A M P A^T + C
+//   backward: element (x) (eta_e, J_e):  M = (I + C J_e)^-1;  eta' = A^T M^T (eta_e - J_e b) + eta;
+//             J' = A^T M^T J_e A + J
+// ---------------------------------------------------------------------------------------------------
+__host__ __device__ inline int downD_group_doubles(int n) { return elem_size(n) + 2 * state_size(n) + n * (2 * n + 1) + n * n + n; }
+
+template <int NT>
+__device__ __forceinline__ void downD_body(const DenseArgs& P) {
+  extern __shared__ __align__(16) char smem[];
+  const int n = DN, n1 = n + 1, es = elem_size(n), ss = state_size(n), ld = 2 * n + 1;
+  const size_t tb = 0;
+  const Grp<NT> g;
+  const int64_t gid = blockIdx.x;
+  if (gid >= P.batch * P.cout) return;
+  const int backward = blockIdx.y;
+  double* base = (double*)(smem + tb);
+  double* el = base; double* st = el + es; double* st2 = st + ss; double* Ws = st2 + ss; double* Tm = Ws + n * ld; double* uv = Tm + n * n;
+  const int64_t series = gid / P.cout, grp = gid - series * P.cout;
+  const int64_t m0 = grp * P.g, m1 = (m0 + P.g < P.cin) ? m0 + P.g : P.cin;
+  const double *A = el, *C = el + n * n1, *J = C + n * n; // [A|b], C, [J|eta]
+  if (!backward) {
+    // st = [m | P]
+    if (P.PREup) { const double* s = P.PREup + gid * (int64_t)ss; for (int e = g.gl; e < ss; e += NT) st[e] = s[e]; }
+    else { for (int e = g.gl; e < n; e += NT) st[e] = 0.0; for (int e = g.gl; e < n * n; e += NT) st[n + e] = P.p0[e]; }
+    g.sync();
+    for (int64_t m = m0; m < m1; ++m) {
+      double* dst = P.PRE + (series * P.cin + m) * (int64_t)ss;
+      for (int e = g.gl; e < ss; e += NT) dst[e] = st[e];
+      if (m + 1 == m1) break;
+      const double* src = P.Ein + (series * P.cin + m) * (int64_t)es;
+      for (int e = g.gl; e < es; e += NT) el[e] = src[e];
+      g.sync();
+      const double *mv = st, *Pm = st + n;
+      // Ws = [I + P J | m + P eta | P]
+      mm(g, n, n1, n, Pm, n, 1, J, n1, 1, (const double*)nullptr, 0, 0, Ws, ld, 1); // cols 0..n: P [J | eta]
+      g.sync();
+      for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n1 + j] = Pm[e]; }
+      for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + n] += mv[i]; }
+      g.sync();
+      gj_solve(g, n, ld, Ws);
+      // m' = A x + b ; Tm = A X ; P' = Tm A^T + C
+      for (int i = g.gl; i < n; i += NT) {
+        double acc = A[i * n1 + n];
+        for (int l = 0; l < n; ++l) acc = fma(A[i * n1 + l], Ws[l * ld + n], acc);
+        st2[i] = acc;
+      }
+      mm(g, n, n, n, A, n1, 1, Ws + n1, ld, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+      g.sync();
+      mm_sym(g, n, n, Tm, n, 1, A, 1, n1, C, st2 + n);
+      g.sync();
+      double* t = st; st = st2; st2 = t;
+    }
+  } else {
+    if (!P.want_suffix) return;
+    // st = [eta | J]
+    if (P.SUFup) { const double* s = P.SUFup + gid * (int64_t)ss; for (int e = g.gl; e < ss; e += NT) st[e] = s[e]; }
+    else { for (int e = g.gl; e < ss; e += NT) st[e] = 0.0; }
+    g.sync();
+    for (int64_t m = m1 - 1; m >= m0; --m) {
+      double* dst = P.SUF + (series * P.cin + m) * (int64_t)ss;
+      for (int e = g.gl; e < ss; e += NT) dst[e] = st[e];
+      if (m == m0) break;
+      const double* src = P.Ein + (series * P.cin + m) * (int64_t)es;
+      for (int e = g.gl; e < es; e += NT) el[e] = src[e];
+      g.sync();
+      const double *ev = st, *Je = st + n;
+      const int ld2 = 2 * n;
+      // Ws = [I + C J_e | A]
+      mm(g, n, n, n, C, n, 1, Je, n, 1, (const double*)nullptr, 0, 0, Ws, ld2, 1);
+      g.sync();
+      for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld2 + n + j] = A[i * n1 + j]; }
+      for (int i = g.gl; i < n; i += NT) Ws[i * ld2 + i] += 1.0;
+      // u = eta_e - J_e b
+      for (int i = g.gl; i < n; i += NT) {
+        double acc = ev[i];
+        for (int l = 0; l < n; ++l) acc = fma(-Je[i * n + l], A[l * n1 + n], acc);
+        uv[i] = acc;
+      }
+      g.sync();
+      gj_solve(g, n, ld2, Ws);
+      const double* X = Ws + n; // M A, row stride ld2
+      for (int i = g.gl; i < n; i += NT) {
+        double acc = J[i * n1 + n];
+        for (int l = 0; l < n; ++l) acc = fma(X[l * ld2 + i], uv[l], acc);
+        st2[i] = acc;
+      }
+      mm(g, n, n, n, Je, n, 1, A, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1); // Tm = J_e A
+      g.sync();
+      for (int e = g.gl; e < n * n; e += NT) {
+        const int i = e / n, j = e - i * n;
+        if (j > i) continue;
+        double acc = J[i * n1 + j];
+        for (int l = 0; l < n; ++l) acc = fma(X[l * ld2 + i], Tm[l * n + j], acc);
+        st2[n + i * n + j] = acc;
+        st2[n + j * n + i] = acc;
+      }
+      g.sync();
+      double* t = st; st = st2; st2 = t;
+    }
+  }
+}
+
+
+#ifdef SG_JIT
+extern "C" __global__ void __launch_bounds__(SG_DENSE_NT) jit_foldD(const __grid_constant__ DenseArgs P) { foldD_body<SG_DENSE_NT>(P); }
+extern "C" __global__ void __launch_bounds__(SG_DENSE_NT) jit_downD(const __grid_constant__ DenseArgs P) { downD_body<SG_DENSE_NT>(P); }
+#else
+template <int NT>
+__global__ void __launch_bounds__(NT) k_foldD(const __grid_constant__ DenseArgs P) { foldD_body<NT>(P); }
+template <int NT>
+__global__ void __launch_bounds__(NT) k_downD(const __grid_constant__ DenseArgs P) { downD_body<NT>(P); }
+#endif

@@ -5,6 +5,7 @@
 #define SG_MAXINST 16  /* max number of instruments (= SMOLGP_MAX_INST) */
 #define SG_MAXBLK 16   /* max number of block-diagonal blocks of F (App. C.1 stacking) */
 #define SG_MAXBD 4     /* max block dimension */
+#define SG_DENSE_NT 256 /* threads of the CTA that works on one dense combine */
 #define NUMF_BAD 1     /* numeric flag: non-finite value or non-positive innovation variance */
 
 // event meta word: bit 0 kind (1 = start/reset, 0 = end/observe), bits 1..5 instrument,

@@ -1,4 +1,4 @@
-// jit.cu -- run-time specialisation of the chunk kernels (k_fold0, k_down0, k_query) for one model
+// jit.cu -- run-time specialisation of the scan kernels (k_fold0, k_down0, k_query, k_foldD, k_downD) for one model
 // STRUCTURE: state dimension, block dimensions and offsets, number of instruments and which
 // (instrument, block) couplings are non-zero become compile-time constants, so the loops over blocks and
 // instruments unroll, the family switch disappears and all shared-memory addresses are immediates.
@@ -6,7 +6,7 @@
 // serves every likelihood evaluation of an optimisation over the same kernel structure.
 //
 // The source is the very text of the statically compiled kernels (csrc/jit_src.inc, written by
-// _build.py from dev_consts.h + grp_dev.cuh + chunk_dev.cuh + chunk_kernels.cuh), compiled with NVRTC
+// _build.py from dev_consts.h + grp_dev.cuh + chunk_dev.cuh + chunk_kernels.cuh + dense_kernels.cuh), compiled with NVRTC
 // for sm_100a and loaded through the runtime's library API.  NVRTC is opened with dlopen: when it is
 // not there, or a compilation fails, the generic kernels run instead (same arithmetic, same results).
 #include <dlfcn.h>
@@ -154,6 +154,8 @@ const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD) {
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.fold0, ent.k.lib, "jit_fold0");
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.down0, ent.k.lib, "jit_down0");
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.query, ent.k.lib, "jit_query");
+      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.foldD, ent.k.lib, "jit_foldD");
+      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.downD, ent.k.lib, "jit_downD");
       if (e == cudaSuccess) ent.good = true;
       else { st->log = std::string("loading the specialised kernels: ") + cudaGetErrorString(e); cudaGetLastError(); }
     }

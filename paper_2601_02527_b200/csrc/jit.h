@@ -5,7 +5,7 @@
 struct Tab;
 struct SgJitKernels {
   cudaLibrary_t lib;
-  cudaKernel_t fold0, down0, query;
+  cudaKernel_t fold0, down0, query, foldD, downD;
 };
 const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD);
 void sg_jit_destroy(smolgp_ctx* ctx);

@@ -125,13 +125,22 @@ static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* 
   return SMOLGP_EUNSUPPORTED;
 }
 
-#define SG_DENSE_NT 128 /* threads cooperating on one dense combine (one CTA per group of elements) */
-static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, size_t tb, bool fold) {
+static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, const SgJitKernels* jk, bool fold) {
   const int gd = fold ? foldD_group_doubles(n) : downD_group_doubles(n);
-  const size_t smem = tb + (size_t)gd * 8;
+  const size_t smem = (size_t)gd * 8;
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = D.batch * D.cout;
   dim3 grid((unsigned)groups, fold ? 1 : (D.want_suffix ? 2 : 1));
+  if (jk) {
+    cudaKernel_t k = fold ? jk->foldD : jk->downD;
+    SG_CUDA(ctx, cudaFuncSetAttribute((const void*)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    void* args[1] = {const_cast<DenseArgs*>(&D)};
+    sg_launch_begin(ctx, fold ? KID_FOLDD : KID_DOWND);
+    cudaError_t e = cudaLaunchKernel((const void*)k, grid, dim3(SG_DENSE_NT), args, smem, ctx->stream);
+    sg_launch_end(ctx);
+    SG_CUDA(ctx, e);
+    return SMOLGP_OK;
+  }
   if (fold) {
     SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     sg_launch_begin(ctx, KID_FOLDD);
@@ -150,10 +159,11 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   const ModelDev* hm = a.h_model;
   const int n = hm->n;
   const int64_t K = a.ev->K, N = a.ev->N, batch = a.batch;
-  int nent = 0;
-  for (int b = 0; b < hm->nblk; ++b) nent += hm->blk[b].dim * hm->blk[b].dim;
-  const size_t tb = tables_bytes(n, hm->d, hm->n_inst, hm->nblk, nent);
   const int G = pick_lanes(ctx, n);
+  Tab T0;
+  tab_build(hm, &T0);
+  const SgJitKernels* jk0; // specialised kernels for this model's structure, or nullptr (generic kernels)
+  const int ld0 = eff_ld(ctx, T0, G, batch * K, &jk0);
   int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 0; // 0: automatic, set once the chunk count is known
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
@@ -162,10 +172,6 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   if (Lc <= 0) {
     // one full wave: as many chunks as groups can be resident at once (equal work per chunk, no tail);
     // a batch that already fills the machine runs one chunk per series (the sequential filter, row a8)
-    Tab T0;
-    tab_build(hm, &T0);
-    const SgJitKernels* jk0;
-    const int ld0 = eff_ld(ctx, T0, G, batch * K, &jk0);
     int per_sm = 1;
     groups_per_cta((size_t)down0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
     int per_sm_f = 1;
@@ -210,7 +216,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   char* w = (char*)ws;
 
   ScanDev P;
-  tab_build(hm, &P.T);
+  P.T = T0;
   P.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); P.disc = a.disc; P.dt = a.ev->dt; P.delta = a.ev->delta; P.meta = a.ev->meta; P.obs = a.ev->obs;
   P.y = a.y; P.sigma = a.sigma; P.amp = a.amp; P.K = K; P.N = N; P.batch = batch; P.Lc = (int)Lc; P.c1 = c1;
   P.E1 = pl.T ? (double*)(w + oE[1]) : nullptr;
@@ -226,19 +232,19 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     if (rc) return rc;
     for (int l = 1; l < pl.T; ++l) {
       DenseArgs D = {};
-      D.M = a.d_model; D.Ein = (const double*)(w + oE[l]); D.Eout = (double*)(w + oE[l + 1]);
+      D.n = n; D.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); D.Ein = (const double*)(w + oE[l]); D.Eout = (double*)(w + oE[l + 1]);
       D.cin = pl.cnt[l]; D.cout = pl.cnt[l + 1]; D.batch = batch; D.g = g;
-      rc = launch_dense(ctx, D, n, tb, true);
+      rc = launch_dense(ctx, D, n, jk0, true);
       if (rc) return rc;
     }
     for (int l = pl.T; l >= 1; --l) {
       DenseArgs D = {};
-      D.M = a.d_model; D.Ein = (const double*)(w + oE[l]); D.cin = pl.cnt[l]; D.batch = batch;
+      D.n = n; D.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); D.Ein = (const double*)(w + oE[l]); D.cin = pl.cnt[l]; D.batch = batch;
       D.want_suffix = a.want_smooth;
       if (l == pl.T) { D.cout = 1; D.g = (int)pl.cnt[l]; D.PREup = nullptr; D.SUFup = nullptr; }
       else { D.cout = pl.cnt[l + 1]; D.g = g; D.PREup = (const double*)(w + oPRE[l + 1]); D.SUFup = a.want_smooth ? (const double*)(w + oSUF[l + 1]) : nullptr; }
       D.PRE = (double*)(w + oPRE[l]); D.SUF = a.want_smooth ? (double*)(w + oSUF[l]) : nullptr;
-      rc = launch_dense(ctx, D, n, tb, false);
+      rc = launch_dense(ctx, D, n, jk0, false);
       if (rc) return rc;
     }
   }
@@ -274,9 +280,6 @@ static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) 
 int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   const ModelDev* hm = a.h_model;
   const int n = hm->n;
-  int nent = 0;
-  for (int b = 0; b < hm->nblk; ++b) nent += hm->blk[b].dim * hm->blk[b].dim;
-  const size_t tb = tables_bytes(n, hm->d, hm->n_inst, hm->nblk, nent);
   const int64_t M = a.M;
   const size_t o_kp = 0, o_dt = ((size_t)M * 8 + 255) / 256 * 256, o_disc = o_dt + ((size_t)2 * M * 8 + 255) / 256 * 256;
   void* ws;
