@@ -164,16 +164,27 @@ __device__ void disc_block(const BlockConst& B, double dts, double* __restrict__
 // coefficients and closed-form constants are warp-uniform loads and the family switch does not diverge
 __global__ void __launch_bounds__(128) k_disc(const ModelDev* __restrict__ Mp, const double* __restrict__ dt, int64_t K,
                                               double* __restrict__ disc) {
+  extern __shared__ double stage[]; // [128][bs]: each thread's record, then written out in coalesced runs
   const int b = blockIdx.y;
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= K) return;
+  const int64_t k0 = (int64_t)blockIdx.x * blockDim.x, k = k0 + threadIdx.x;
   const BlockConst& B = Mp->blk[b];
-  const double dts = dt[k] * B.inv_T;
-  double* out = disc + k * (int64_t)Mp->disc_stride + Mp->disc_off[b];
-  switch (B.dim) {
-    case 2: disc_block<2>(B, dts, out); break;
-    case 3: disc_block<3>(B, dts, out); break;
-    default: disc_block<4>(B, dts, out); break;
+  const int bs = 2 * B.dim * B.dim + 2 * B.dim + 1; // odd: conflict-free per-thread rows
+  if (k < K) {
+    const double dts = dt[k] * B.inv_T;
+    double* out = stage + threadIdx.x * bs;
+    switch (B.dim) {
+      case 2: disc_block<2>(B, dts, out); break;
+      case 3: disc_block<3>(B, dts, out); break;
+      default: disc_block<4>(B, dts, out); break;
+    }
+  }
+  __syncthreads();
+  const int64_t nev = (K - k0 < blockDim.x) ? (K - k0) : blockDim.x;
+  const int stride = Mp->disc_stride, off = Mp->disc_off[b];
+  const float rbs = 1.0f / (float)bs;
+  for (int e = threadIdx.x; e < (int)nev * bs; e += blockDim.x) {
+    const int ev = __float2int_rz(((float)e + 0.5f) * rbs), j = e - ev * bs;
+    disc[(k0 + ev) * (int64_t)stride + off + j] = stage[e];
   }
 }
 
@@ -181,7 +192,7 @@ int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_m
                    int64_t K, double* disc) {
   dim3 grid((unsigned)((K + 127) / 128), (unsigned)h_model->nblk);
   sg_launch_begin(ctx, KID_DISC);
-  k_disc<<<grid, 128, 0, ctx->stream>>>(d_model, dt, K, disc);
+  k_disc<<<grid, 128, 128 * (2 * SG_MAXBD * SG_MAXBD + 2 * SG_MAXBD + 1) * sizeof(double), ctx->stream>>>(d_model, dt, K, disc);
   sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
