@@ -99,22 +99,39 @@ __device__ __forceinline__ void stage_rec(const Grp<G>& g, const Tab& T, const d
   cp_async_commit();
 }
 
+// Phi_b (DB x DB, row-major) and Phi-bar_b (DB) of one block, contiguous in the staged record.  Records
+// are laid out so that every block starts on a 16-byte boundary (even block sizes, even buffer offsets):
+// for even DB the rows come in as 128-bit shared-memory loads -- all lanes read the same address, so a
+// wider broadcast load halves the number of LSU wavefronts.
+template <int DB>
+__device__ __forceinline__ void load_block(const double* __restrict__ r, double (&m)[DB * DB + DB]) {
+  if constexpr (DB % 2 == 0) {
+    const double2* r2 = reinterpret_cast<const double2*>(r);
+#pragma unroll
+    for (int k = 0; k < (DB * DB + DB) / 2; ++k) { const double2 t = r2[k]; m[2 * k] = t.x; m[2 * k + 1] = t.y; }
+  } else {
+#pragma unroll
+    for (int k = 0; k < DB * DB + DB; ++k) m[k] = r[k];
+  }
+}
+
 // ---- one block of out = F v ------------------------------------------------------------------------
 template <int DB, int VS, int OS>
 __device__ __forceinline__ double blk_F(const double* __restrict__ r, const double* vp, double* op, int off) {
-  double w[DB];
+  double w[DB], m[DB * DB + DB];
 #pragma unroll
   for (int l = 0; l < DB; ++l) w[l] = vp[(off + l) * VS];
+  load_block<DB>(r, m);
 #pragma unroll
   for (int i = 0; i < DB; ++i) {
     double acc = 0.0;
 #pragma unroll
-    for (int l = 0; l < DB; ++l) acc = fma(r[i * DB + l], w[l], acc);
+    for (int l = 0; l < DB; ++l) acc = fma(m[i * DB + l], w[l], acc);
     op[(off + i) * OS] = acc;
   }
   double u = 0.0;
 #pragma unroll
-  for (int l = 0; l < DB; ++l) u = fma(r[DB * DB + l], w[l], u); // Phi-bar_b . v_b
+  for (int l = 0; l < DB; ++l) u = fma(m[DB * DB + l], w[l], u); // Phi-bar_b . v_b
   return u;
 }
 
@@ -150,14 +167,15 @@ __device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigne
 // ---- one block of out = F^T v ----------------------------------------------------------------------
 template <int DB, int VS, int OS>
 __device__ __forceinline__ void blk_Ft(const double* __restrict__ r, const double* vp, double* op, int off, double s) {
-  double w[DB];
+  double w[DB], m[DB * DB + DB];
 #pragma unroll
   for (int i = 0; i < DB; ++i) w[i] = vp[(off + i) * VS];
+  load_block<DB>(r, m);
 #pragma unroll
   for (int l = 0; l < DB; ++l) {
-    double acc = r[DB * DB + l] * s; // Phi-bar_b[l] * sum_q c_qb v_zq
+    double acc = m[DB * DB + l] * s; // Phi-bar_b[l] * sum_q c_qb v_zq
 #pragma unroll
-    for (int i = 0; i < DB; ++i) acc = fma(r[i * DB + l], w[i], acc);
+    for (int i = 0; i < DB; ++i) acc = fma(m[i * DB + l], w[i], acc);
     op[(off + l) * OS] = acc;
   }
 }

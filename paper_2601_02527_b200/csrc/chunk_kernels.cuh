@@ -41,7 +41,7 @@ struct ScanDev {
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int fold0_group_doubles(int n, int ld, int stride, int nblk, int G) {
   const int nr = ld - 1; // nr >= n rows: the padding rows stay zero, so row loops run to the compile-time nr
-  return 4 * nr * ld + 2 * stride + nblk * G + 2 * ld + 2;
+  return (4 * nr * ld + 2 * stride + nblk * G + 2 * ld + 2 + 1) & ~1; // even: record buffers stay 16-byte aligned
 }
 
 template <int G, int LD>
@@ -157,8 +157,8 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int kbuf_stride(int n) { return 2 * n + 4; }
 __host__ __device__ inline int down0_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  const int nr = ld - 1, ws = n * (2 * n + 1) > nr * ld ? n * (2 * n + 1) : nr * ld;
-  return nr * ld + ws + 2 * stride + nblk * G + 5 * ld + 1; // Tm is the head of Ws
+  const int nr = ld - 1, ws = ((n * (2 * n + 1) > nr * ld ? n * (2 * n + 1) : nr * ld) + 1) & ~1;
+  return (nr * ld + ws + 2 * stride + nblk * G + 5 * ld + 1 + 1) & ~1; // Tm is the head of Ws; even sizes keep the record buffers aligned
 }
 
 // [vector | matrix(n x n)] in global memory  <->  column-owned [matrix | vector] with row stride ld
@@ -196,7 +196,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   double* X = base;                 // [P | m], later [Lambda | lambda]
   double* Tm = X + NR * ld;
   double* Ws = Tm;                  // n x (2n+1), used only for the one solve per chunk (Tm is dead there)
-  double* recs = Ws + (n * (2 * n + 1) > NR * ld ? n * (2 * n + 1) : NR * ld);
+  double* recs = Ws + (((n * (2 * n + 1) > NR * ld ? n * (2 * n + 1) : NR * ld) + 1) & ~1);
   double* U = recs + 2 * TSTRIDE + g.gl;
   double* cv = recs + 2 * TSTRIDE + TNB * G; // NR, zero padded
   double* kv = cv + ld;
@@ -394,7 +394,7 @@ struct QueryDev {
 };
 
 __host__ __device__ inline int query_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  return 3 * (ld - 1) * ld + 2 * stride + nblk * G + 2 * ld + 1;
+  return (3 * (ld - 1) * ld + 2 * stride + nblk * G + 2 * ld + 1 + 1) & ~1;
 }
 
 template <int G, int LD>

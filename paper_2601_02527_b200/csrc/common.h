@@ -45,8 +45,8 @@ struct ModelDev {
 };
 
 // per-event record layout inside the discretisation array, block b at disc_off[b]:
-//   Phi (dim*dim, row-major) | phibar (dim) | Qxx (dim*dim) | q12 (dim) | q22 (1)      [block units]
-static inline int disc_block_size(int dim) { return 2 * dim * dim + 2 * dim + 1; }
+//   Phi (dim*dim, row-major) | phibar (dim) | Qxx (dim*dim) | q12 (dim) | q22 (1) | pad (1)      [block units]
+static inline int disc_block_size(int dim) { return 2 * dim * dim + 2 * dim + 2; } // + 1 pad: every block 16-byte aligned
 
 struct smolgp_events {
   int device;
