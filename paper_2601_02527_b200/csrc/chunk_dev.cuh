@@ -140,6 +140,12 @@ __device__ __forceinline__ double blk_F(const double* __restrict__ r, const doub
 template <int G, int VS, int OS>
 __device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigned tz, const double* vp, double* op, double* U) {
   const int nblk = TNB, d = TD;
+#ifdef SG_JIT
+  double ul[JT_NB]; // the specialised build unrolls the block loops: the per-block integrals stay in registers
+#define SG_UREF(b) ul[b]
+#else
+#define SG_UREF(b) U[(b) * G]
+#endif
   SG_UNROLL
   for (int b = 0; b < nblk; ++b) {
     const double* r = rec + TROFF(b);
@@ -150,7 +156,7 @@ __device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigne
       case 3: u = blk_F<3, VS, OS>(r, vp, op, off); break;
       default: u = blk_F<4, VS, OS>(r, vp, op, off); break;
     }
-    U[b * G] = u;
+    SG_UREF(b) = u;
   }
   SG_UNROLL
   for (int q = 0; q < TNI; ++q) {
@@ -158,10 +164,11 @@ __device__ __forceinline__ void apply_F(const Tab& T, const double* rec, unsigne
     if (!((tz >> q) & 1u)) {
       acc = vp[(d + q) * VS];
       SG_UNROLL
-      for (int b = 0; b < nblk; ++b) acc = fma(TCZ(q * nblk + b), U[b * G], acc);
+      for (int b = 0; b < nblk; ++b) acc = fma(TCZ(q * nblk + b), SG_UREF(b), acc);
     }
     op[(d + q) * OS] = acc;
   }
+#undef SG_UREF
 }
 
 // ---- one block of out = F^T v ----------------------------------------------------------------------
