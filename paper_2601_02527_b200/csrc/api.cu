@@ -30,7 +30,9 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0;
-  c->opt_chunk = 0; c->opt_group = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = new ModelDev();
+  c->opt_chunk = 0; c->opt_group = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
+  // pinned: the per-call model upload is a true asynchronous copy
+  if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
   int v = 0;
   cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device); c->sm_count = v;
   cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device); c->smem_optin = (size_t)v;
@@ -43,7 +45,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
     }
     cudaGetLastError();
   }
-  if (cudaMalloc(&c->d_flags, 64) != cudaSuccess) { cudaGetLastError(); delete c->hmodel; delete c; return SMOLGP_ENOMEM; }
+  if (cudaMalloc(&c->d_flags, 64) != cudaSuccess) { cudaGetLastError(); cudaFreeHost(c->hmodel); delete c; return SMOLGP_ENOMEM; }
   cudaMemset(c->d_flags, 0, 64);
   *out = c;
   return SMOLGP_OK;
@@ -59,7 +61,7 @@ extern "C" void smolgp_destroy(smolgp_ctx* ctx) {
   cudaFree(ctx->d_flags);
   for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto& e : ctx->evpool) cudaEventDestroy(e);
-  delete ctx->hmodel;
+  cudaFreeHost(ctx->hmodel);
   delete ctx;
 }
 
