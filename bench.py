@@ -208,12 +208,12 @@ def run_cuda(args, w, cfgname):
             dist.barrier()
             torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()  # nvidia-smi needs a moment to come up: started before the warm-up, read after the timed loops
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     ctx.profile(True)
     l0 = ctx.launch_count()
     evs = []

@@ -161,6 +161,7 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);
   if (qstore) cudaFreeAsync(qstore, ctx->stream);
   SG_CUDA(ctx, ce);
+  if (flags & NUMF_SIGMA) { ctx->err = "noise_sigma must be finite and > 0 at every exposure"; return SMOLGP_EINVAL; }
   if (flags) { ctx->err = "non-finite value or non-positive innovation variance (check noise_sigma > 0, amp > 0, finite y)"; return SMOLGP_ENUMERIC; }
   return SMOLGP_OK;
 }

@@ -243,6 +243,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
       const double yy = y_r * ramp;
       const double S = hs * hs * X[zi * ld + zi] + sg * sg;
       const double v = yy - hs * X[zi * ld + n];
+      if (!(sg_r > 0.0) || !isfinite(sg_r)) atomicOr(P.flags, NUMF_SIGMA);
       if (!(S > 0.0) || !isfinite(S) || !isfinite(v)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S;
       ll -= 0.5 * (log(6.283185307179586476925286766559 * S) + v * v * rS);

@@ -205,6 +205,11 @@ def test_numeric_errors_are_reported(ctx):
     with pytest.raises(SmolgpError) as e:
         ctx.smolgp_loglik_host(ev, [W.comp(7, 1.0, 1.0)], w["y"], w["sigma"])
     assert e.value.rc == -3
+    sg = w["sigma"].copy()
+    sg[5] = 0.0
+    with pytest.raises(SmolgpError) as e:   # sigma_n <= 0 is an invalid argument
+        ctx.smolgp_loglik_host(ev, w["kernel"], w["y"], sg)
+    assert e.value.rc == -1
     # the context stays usable after an error
     ll = ctx.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"])
     assert np.isfinite(ll[0])
