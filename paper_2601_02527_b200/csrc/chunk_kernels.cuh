@@ -283,8 +283,9 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
     g.sync();
     for (int j = g.gl; j <= n; j += G)
       for (int i = 0; i < n; ++i) {
-        double acc = 0.0;
-        for (int l = 0; l < n; ++l) acc = fma(Ws[i * ld2 + n + l], X[l * ld + j], acc);
+        double acc = 0.0, cmp = 0.0; // J P cancels like the products of the dense levels: compensated (Dot2)
+        for (int l = 0; l < n; ++l) dot2_step(Ws[i * ld2 + n + l], X[l * ld + j], acc, cmp);
+        acc += cmp;
         if (j < n) Ws[i * ld2 + j] = acc + (i == j ? 1.0 : 0.0);
         else Ws[i * ld2 + 2 * n] = acc - Ws[i * ld2 + 2 * n];
       }

@@ -20,7 +20,7 @@ __device__ __forceinline__ void mm(const Grp<G>& g, int nr, int nc, int nk, cons
     int i, j;
     divmod_small(e, nc, rnc, i, j);
     double acc = C ? C[i * cr + j * cc] : 0.0;
-    for (int l = 0; l < nk; ++l) acc = fma(A[i * ar + l * ac], B[l * br + j * bc], acc);
+    { double cmp = 0.0; for (int l = 0; l < nk; ++l) dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp); acc += cmp; }
     D[i * dr + j * dc] = acc;
   }
 }
@@ -32,7 +32,7 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const dou
     const int i = e / n, j = e - i * n;
     if (j > i) continue;
     double acc = C ? C[i * n + j] : 0.0;
-    for (int l = 0; l < nk; ++l) acc = fma(A[i * ar + l * ac], B[l * br + j * bc], acc);
+    { double cmp = 0.0; for (int l = 0; l < nk; ++l) dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp); acc += cmp; }
     D[i * n + j] = acc;
     D[j * n + i] = acc;
   }
@@ -65,7 +65,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   // u = eta_j - J_j b_i
   for (int i = g.gl; i < n; i += G) {
     double acc = Jj[i * n1 + n];
-    for (int l = 0; l < n; ++l) acc = fma(-Jj[i * n1 + l], Ai[l * n1 + n], acc);
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(-Jj[i * n1 + l], Ai[l * n1 + n], acc, cmp); acc += cmp; }
     uv[i] = acc;
   }
   g.sync();
@@ -83,7 +83,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   // eta = X1^T u + eta_i
   for (int i = g.gl; i < n; i += G) {
     double acc = Ji[i * n1 + n];
-    for (int l = 0; l < n; ++l) acc = fma(X1[l * ld + i], uv[l], acc);
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * ld + i], uv[l], acc, cmp); acc += cmp; }
     Jo[i * n1 + n] = acc;
   }
   g.sync();
@@ -94,7 +94,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
     const int i = e / n, j = e - i * n;
     if (j > i) continue;
     double acc = Ji[i * n1 + j];
-    for (int l = 0; l < n; ++l) acc = fma(X1[l * ld + i], Tm[l * n + j], acc);
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * ld + i], Tm[l * n + j], acc, cmp); acc += cmp; }
     Jo[i * n1 + j] = acc;
     Jo[j * n1 + i] = acc;
   }
@@ -191,7 +191,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       // m' = A x + b ; Tm = A X ; P' = Tm A^T + C
       for (int i = g.gl; i < n; i += NT) {
         double acc = A[i * n1 + n];
-        for (int l = 0; l < n; ++l) acc = fma(A[i * n1 + l], Ws[l * ld + n], acc);
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(A[i * n1 + l], Ws[l * ld + n], acc, cmp); acc += cmp; }
         st2[i] = acc;
       }
       mm(g, n, n, n, A, n1, 1, Ws + n1, ld, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
@@ -223,7 +223,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       // u = eta_e - J_e b
       for (int i = g.gl; i < n; i += NT) {
         double acc = ev[i];
-        for (int l = 0; l < n; ++l) acc = fma(-Je[i * n + l], A[l * n1 + n], acc);
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(-Je[i * n + l], A[l * n1 + n], acc, cmp); acc += cmp; }
         uv[i] = acc;
       }
       g.sync();
@@ -231,7 +231,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       const double* X = Ws + n; // M A, row stride ld2
       for (int i = g.gl; i < n; i += NT) {
         double acc = J[i * n1 + n];
-        for (int l = 0; l < n; ++l) acc = fma(X[l * ld2 + i], uv[l], acc);
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * ld2 + i], uv[l], acc, cmp); acc += cmp; }
         st2[i] = acc;
       }
       mm(g, n, n, n, Je, n, 1, A, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1); // Tm = J_e A
@@ -240,7 +240,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
         const int i = e / n, j = e - i * n;
         if (j > i) continue;
         double acc = J[i * n1 + j];
-        for (int l = 0; l < n; ++l) acc = fma(X[l * ld2 + i], Tm[l * n + j], acc);
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * ld2 + i], Tm[l * n + j], acc, cmp); acc += cmp; }
         st2[n + i * n + j] = acc;
         st2[n + j * n + i] = acc;
       }

@@ -38,6 +38,20 @@ __device__ __forceinline__ double group_sum(const Grp<G>& g, double v) {
   return v;
 }
 
+// Compensated dot product (Ogita-Rump-Oishi "Dot2"): the products and the running sum carry their exact
+// rounding errors (one FMA and one TwoSum per term), so a sum of terms that cancel by many orders of
+// magnitude is as accurate as if it had been formed in twice the working precision.  The dense levels
+// multiply covariances whose large entries lie in the weakly determined directions with informations
+// whose large entries lie in the strongly determined ones: the products cancel.
+__device__ __forceinline__ void dot2_step(double a, double b, double& s, double& c) {
+  const double p = __dmul_rn(a, b); // _rn intrinsics: never contracted into an FMA, the error terms stay exact
+  const double pe = fma(a, b, -p);
+  const double t = __dadd_rn(s, p);
+  const double z = __dadd_rn(t, -s);
+  c += __dadd_rn(__dadd_rn(__dadd_rn(s, -__dadd_rn(t, -z)), __dadd_rn(p, -z)), pe);
+  s = t;
+}
+
 // Gauss-Jordan elimination with partial pivoting on the augmented matrix W = [M | R] (n rows,
 // ld = n + m columns) in place; on return R holds M^-1 R.  M = I + (PSD)(PSD) in every use here
 // (eigenvalues >= 1), so a zero pivot cannot occur for finite input.
