@@ -219,6 +219,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
       for (int i = 0; i < n; ++i) X[i * ld + j] = (j < n) ? P.p0[i * n + j] : 0.0;
   g.sync();
   double ll = 0.0;
+  int nend = 0; // end events seen by this chunk (forward, then backward)
   // ---- forward ----
   uint32_t meta_nx = P.meta[k0];
   int32_t ob_nx = P.obs[k0];
@@ -265,7 +266,9 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
       // the instrument is idle after its end (reading R6)
       if (g.gl <= n) { const int j = g.gl; X[zi * ld + j] = 0.0; if (j < n) X[j * ld + zi] = 0.0; }
       g.sync();
-      symmetrise<G, LD>(g, T, X); // the two triangles of F P F^T are rounded independently
+      // the two triangles of F P F^T are rounded independently: re-symmetrised every 4th end event (the
+      // asymmetry is pure rounding and grows slowly; the transposed accesses conflict in shared memory)
+      if ((++nend & 3) == 0) symmetrise<G, LD>(g, T, X);
     }
     if (P.fstate) store_state<G, LD>(g, T, X, P.fstate + (series * P.K + k) * (int64_t)ss); // row a7
   }
@@ -365,7 +368,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
         }
       }
       g.sync();
-      symmetrise<G, LD>(g, T, X);
+      if ((++nend & 3) == 0) symmetrise<G, LD>(g, T, X);
     }
     if (P.binfo) store_state<G, LD>(g, T, X, P.binfo + (series * P.K + k) * (int64_t)ss);
     if (k == k0) break;
