@@ -273,6 +273,25 @@ def test_query_prediction_matches_dense_definition(ctx, oracle):
         assert np.max(np.abs(out["var_query"][0] - ref["vq"])) <= 1e-8 * k0
 
 
+def test_query_prediction_specialised_kernels_match_generic(ctx):
+    """the NVRTC-specialised query kernel against the statically compiled one (bitwise: same source)"""
+    rng = np.random.default_rng(9)
+    w = W.make(4, N=400)
+    tq = _queries(w, rng, 50)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    outs = []
+    try:
+        for jit in (-1, 1):
+            ctx.set_option("jit", jit)
+            ctx.set_option("chunk", 40)
+            outs.append(ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], t_query=tq, query_instrument=1))
+    finally:
+        _reset(ctx)
+    assert ctx.jit_log() == "", ctx.jit_log()
+    for k in ("mean_query", "var_query", "mean", "var", "loglik"):
+        np.testing.assert_allclose(outs[0][k], outs[1][k], rtol=1e-11, atol=1e-13)
+
+
 def test_query_device_pointers(ctx):
     import torch
     w = W.make(2, N=500)
