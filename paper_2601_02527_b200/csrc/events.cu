@@ -25,18 +25,27 @@ __global__ void k_ev_init(int64_t N, const double* __restrict__ ts, const double
                           uint32_t* __restrict__ vals, int* __restrict__ flags,
                           unsigned long long* __restrict__ maxdelta) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  const double s = ts[i], e = te[i];
-  const int q = inst[i];
-  int bad = 0;
-  if (!isfinite(s) || !isfinite(e) || !(e > s)) bad |= EVF_BADTIME;
-  if (q < 0 || q >= n_inst) bad |= EVF_BADINST;
-  if (bad) { atomicOr(flags, bad); }
-  keys[i] = time_key(e);
-  vals[i] = (uint32_t)(2 * i);
-  keys[N + i] = time_key(s);
-  vals[N + i] = (uint32_t)(2 * i + 1);
-  if (!bad) atomicMax(maxdelta + q, (unsigned long long)__double_as_longlong(e - s)); // positive doubles order like their bits
+  unsigned long long dbits = 0ull; // bits of this exposure's length (0 for dead / invalid lanes)
+  int q = -1;
+  if (i < N) {
+    const double s = ts[i], e = te[i];
+    q = inst[i];
+    int bad = 0;
+    if (!isfinite(s) || !isfinite(e) || !(e > s)) bad |= EVF_BADTIME;
+    if (q < 0 || q >= n_inst) bad |= EVF_BADINST;
+    if (bad) { atomicOr(flags, bad); q = -1; }
+    keys[i] = time_key(e);
+    vals[i] = (uint32_t)(2 * i);
+    keys[N + i] = time_key(s);
+    vals[N + i] = (uint32_t)(2 * i + 1);
+    if (!bad) dbits = (unsigned long long)__double_as_longlong(e - s); // positive doubles order like their bits
+  }
+  // longest exposure per instrument: one atomic per (warp, instrument) instead of one per exposure
+  for (int r = 0; r < n_inst; ++r) {
+    unsigned long long m = (q == r) ? dbits : 0ull;
+    for (int o = 16; o; o >>= 1) { const unsigned long long x = __shfl_xor_sync(0xffffffffu, m, o); m = x > m ? x : m; }
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(maxdelta + r, m);
+  }
 }
 
 // ---- LSD radix sort, 8 bits per pass.  One warp per tile of RS_TILE keys, RS_WPB tiles per CTA. ----
