@@ -41,7 +41,7 @@ typedef enum {
   SMOLGP_ENUMERIC = -6      /* a non-finite value or a non-positive innovation variance was met */
 } smolgp_status;
 
-#define SMOLGP_MAX_DIM 32  /* max augmented state dimension n = d + N_inst */
+#define SMOLGP_MAX_DIM 31  /* max augmented state dimension n = d + N_inst (n + 1 columns, one lane each) */
 #define SMOLGP_MAX_INST 16 /* max number of instruments */
 
 /* kernel families (state-space forms: DESIGN.md "Models"; SHO: App. B) */

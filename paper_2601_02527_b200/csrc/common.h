@@ -10,7 +10,7 @@
 #include "../../include/smolgp.h"
 #include "dev_consts.h"
 
-static_assert(SG_NMAX == SMOLGP_MAX_DIM && SG_MAXINST == SMOLGP_MAX_INST, "dev_consts.h out of step with smolgp.h");
+static_assert(SG_NMAX >= SMOLGP_MAX_DIM + 1 && SG_MAXINST == SMOLGP_MAX_INST, "dev_consts.h out of step with smolgp.h");
 #define SG_KT 18     /* Taylor order of the small-step discretisation */
 #define SG_BE (SG_MAXBD + 1)
 

@@ -1,7 +1,7 @@
 // dev_consts.h -- constants and bit layouts shared by host code, the statically compiled kernels and
 // the run-time specialised (NVRTC) chunk kernels.  Macros only: no includes, no types.
 #pragma once
-#define SG_NMAX 32     /* max augmented state dimension n = d + N_inst (= SMOLGP_MAX_DIM) */
+#define SG_NMAX 32     /* table size: SMOLGP_MAX_DIM (31) + 1; the chunk kernels give each of the n + 1 columns a lane */
 #define SG_MAXINST 16  /* max number of instruments (= SMOLGP_MAX_INST) */
 #define SG_MAXBLK 16   /* max number of block-diagonal blocks of F (App. C.1 stacking) */
 #define SG_MAXBD 4     /* max block dimension */

@@ -165,7 +165,7 @@ int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const
   }
   int off = 0;
   for (int b = 0; b < nb; ++b) { M->blk[b].off = d; d += M->blk[b].dim; M->disc_off[b] = off; off += disc_block_size(M->blk[b].dim); }
-  if (d + n_inst > SG_NMAX) { ctx->err = "augmented state dimension above SMOLGP_MAX_DIM"; return SMOLGP_EUNSUPPORTED; }
+  if (d + n_inst > SMOLGP_MAX_DIM) { ctx->err = "augmented state dimension above SMOLGP_MAX_DIM"; return SMOLGP_EUNSUPPORTED; }
   M->n = d + n_inst; M->d = d; M->n_inst = n_inst; M->nblk = nb; M->disc_stride = off;
   for (int b = 0; b < nb; ++b)
     for (int i = 0; i < M->blk[b].dim; ++i) { M->row_lo[M->blk[b].off + i] = M->blk[b].off; M->row_hi[M->blk[b].off + i] = M->blk[b].off + M->blk[b].dim; }

@@ -354,3 +354,67 @@ def test_full_size_cfg5_sampled_series(ctx, oracle):
         e = PU.errors(ref, out["loglik"][s], out["mean"][s], out["var"][s])
         assert e["ll"] <= PU.LL_RTOL and e["mean"] <= PU.POST_RTOL and e["var"] <= PU.POST_RTOL, (s, e)
     assert np.all(np.isfinite(out["loglik"])) and np.all(out["var"] > 0)
+
+
+def test_largest_state_dimension(ctx, oracle):
+    """n = SMOLGP_MAX_DIM = 31: periodic product of order 6 (d = 26) seen by 5 overlapping instruments;
+    n = 32 is refused"""
+    from paper_2601_02527_b200.binding import SmolgpError
+    rng = np.random.default_rng(21)
+    N, ninst = 240, 5
+    ts = np.sort(rng.uniform(0, 40000.0, N))
+    inst = np.arange(N, dtype=np.int32) % ninst
+    te = ts + rng.uniform(20.0, 120.0, N)
+    for q in range(ninst):  # no self-overlap: clip each exposure at the instrument's next start
+        idx = np.nonzero(inst == q)[0]
+        te[idx[:-1]] = np.minimum(te[idx[:-1]], ts[idx[1:]] - 1.0)
+    kern = [W.comp(W.MATERN32_X_PERIODIC, 1.2, 5000.0, 9000.0, 0.8, order=6)]
+    sigma = np.full(N, 0.2)
+    y = W.synth_y(rng, kern, ts, te, inst, sigma)
+    w = dict(kernel=kern, n_inst=ninst, t_start=ts, t_end=te, instrument=inst, y=y, sigma=sigma, amp=None)
+    ev = ctx.smolgp_build_events_host(ts, te, inst, ninst)
+    for jit in (-1, 1):
+        ctx.set_option("jit", jit)
+        ctx.set_option("chunk", 48)
+        try:
+            out = ctx.smolgp_condition_host(ev, kern, y, sigma)
+        finally:
+            _reset(ctx)
+        ref = PU.reference(oracle, w)
+        e = PU.errors(ref, out["loglik"][0], out["mean"][0], out["var"][0], floor=PU.prior_sd(oracle, w))
+        assert e["ll"] <= PU.LL_RTOL and e["mean"] <= PU.POST_RTOL and e["var"] <= PU.POST_RTOL, (jit, e)
+    ev6 = ctx.smolgp_build_events_host(ts, te, np.arange(N, dtype=np.int32) % 6, 6)  # n would be 32
+    with pytest.raises(SmolgpError) as ex:
+        ctx.smolgp_loglik_host(ev6, kern, y, sigma)
+    assert ex.value.rc == -3
+
+
+def test_degenerate_inputs(ctx, oracle):
+    """N = 1, N = 2, exact ties between instruments (start/start, end/start, end/end), one query"""
+    kern = [W.comp(W.SHO, 1.0, 2 * np.pi / 330.0, 10.0), W.comp(W.MATERN32, 0.5, 900.0, inst_mask=2)]
+    cases = [
+        (np.array([5.0]), np.array([60.0]), np.array([0], np.int32), 1),
+        (np.array([5.0, 100.0]), np.array([60.0, 130.0]), np.array([0, 0], np.int32), 1),
+        # two instruments: equal starts, an end tied with a start, equal ends
+        (np.array([0.0, 0.0, 50.0, 80.0, 120.0]), np.array([50.0, 80.0, 120.0, 120.0, 200.0]),
+         np.array([0, 1, 0, 1, 0], np.int32), 2),
+    ]
+    rng = np.random.default_rng(2)
+    for ts, te, inst, ninst in cases:
+        y = rng.standard_normal(ts.size)
+        sigma = np.full(ts.size, 0.3)
+        tq = np.array([0.5 * (ts[0] + te[-1])])
+        for opts in ((), (("chunk", 2), ("group", 2))):
+            for k, v in opts:
+                ctx.set_option(k, v)
+            try:
+                ev = ctx.smolgp_build_events_host(ts, te, inst, ninst)
+                out = ctx.smolgp_condition_host(ev, kern, y, sigma, t_query=tq, query_instrument=ninst - 1)
+            finally:
+                _reset(ctx)
+            ref = oracle.dense(kern, ts, te, inst, y, sigma, tq=tq, query_inst=ninst - 1)
+            assert abs(out["loglik"][0] - ref["loglik"]) <= 1e-9 * abs(ref["loglik"])
+            np.testing.assert_allclose(out["mean"][0], ref["mean"], rtol=1e-8, atol=1e-9)
+            np.testing.assert_allclose(out["var"][0], ref["var"], rtol=1e-8, atol=1e-10)
+            np.testing.assert_allclose(out["mean_query"][0], ref["mq"], rtol=1e-8, atol=1e-9)
+            np.testing.assert_allclose(out["var_query"][0], ref["vq"], rtol=1e-8, atol=1e-10)
