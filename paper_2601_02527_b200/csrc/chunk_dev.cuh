@@ -214,26 +214,38 @@ __device__ __forceinline__ void add_Q_col(const Tab& T, const double* rec, unsig
   constexpr int ld = LD;
   const int d = TD, nblk = TNB;
   if (j < d) {
-    const int b = TBLKOF(j), db = TBDIM(b), off = TBOFF(b), jj = j - off;
-    const double* r = rec + TROFF(b);
-    const double* qxx = r + db * db + db;
-    for (int i = 0; i < db; ++i) X[(off + i) * ld + j] += qxx[i * db + jj];
-    const double q12 = r[2 * db * db + db + jj];
-    for (int q = 0; q < TNI; ++q)
-      if (!((tz >> q) & 1u)) X[(d + q) * ld + j] = fma(TCZ(q * nblk + b), q12, X[(d + q) * ld + j]);
-  } else if (j < TN) {
-    const int q = j - d;
-    if ((tz >> q) & 1u) return;
+    // the block of column j is found by a loop over the blocks with compile-time bounds in the specialised
+    // build (no table look-up with a lane-dependent index, which would live in local memory there)
     SG_UNROLL
-  for (int b = 0; b < nblk; ++b) {
-      const int db = TBDIM(b), off = TBOFF(b);
+    for (int b = 0; b < nblk; ++b) {
+      const int db = TBDIM(b), off = TBOFF(b), jj = j - off;
+      if (jj < 0 || jj >= db) continue;
       const double* r = rec + TROFF(b);
-      const double c = TCZ(q * nblk + b);
-      if (c == 0.0) continue;
-      for (int l = 0; l < db; ++l) X[(off + l) * ld + j] = fma(c, r[2 * db * db + db + l], X[(off + l) * ld + j]);
-      const double q22 = r[2 * db * db + 2 * db];
-      for (int p = 0; p < TNI; ++p)
-        if (!((tz >> p) & 1u)) X[(d + p) * ld + j] = fma(c * TCZ(p * nblk + b), q22, X[(d + p) * ld + j]);
+      const double* qxx = r + db * db + db;
+      SG_UNROLL
+      for (int i = 0; i < db; ++i) X[(off + i) * ld + j] += qxx[i * db + jj];
+      const double q12 = r[2 * db * db + db + jj];
+      SG_UNROLL
+      for (int q = 0; q < TNI; ++q)
+        if (!((tz >> q) & 1u)) X[(d + q) * ld + j] = fma(TCZ(q * nblk + b), q12, X[(d + q) * ld + j]);
+    }
+  } else if (j < TN) {
+    SG_UNROLL
+    for (int q = 0; q < TNI; ++q) { // the lane's own instrument, found with compile-time indices (see above)
+      if (j != d + q || ((tz >> q) & 1u)) continue;
+      SG_UNROLL
+      for (int b = 0; b < nblk; ++b) {
+        const int db = TBDIM(b), off = TBOFF(b);
+        const double* r = rec + TROFF(b);
+        const double c = TCZ(q * nblk + b);
+        if (c == 0.0) continue;
+        SG_UNROLL
+        for (int l = 0; l < db; ++l) X[(off + l) * ld + j] = fma(c, r[2 * db * db + db + l], X[(off + l) * ld + j]);
+        const double q22 = r[2 * db * db + 2 * db];
+        SG_UNROLL
+        for (int p = 0; p < TNI; ++p)
+          if (!((tz >> p) & 1u)) X[(d + p) * ld + j] = fma(c * TCZ(p * nblk + b), q22, X[(d + p) * ld + j]);
+      }
     }
   }
 }
