@@ -138,7 +138,7 @@ def run_reference(args, w, cfgname):
     tot = sum(ts)
     val = 2.0 * ns * args.steps / tot
     sample = "first %d of %d exposures (%d events) per step, oracle fp64 build, sequential filter + two-filter smoother, 1 thread" % (ns, w["t_start"].size, 2 * ns)
-    line = {"impl": "reference", "metric": "events/sec, loglik + smoother", "value": val, "unit": "events/s",
+    line = {"impl": "reference", "metric": "events/sec for loglik+RTS smoother at N=1e5", "value": val, "unit": "events/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfgname, "sample": sample},
@@ -281,7 +281,7 @@ def run_cuda(args, w, cfgname):
     t_cpu = oracle_step(w, ns)
     cpu = {"value": 2.0 * ns / t_cpu, "unit": "events/s", "cores": 1, "kind": "oracle",
            "sample": "first %d of %d exposures (%d events), oracle fp64 build, sequential filter + two-filter smoother, 1 thread, %.1f s" % (ns, N, 2 * ns, t_cpu)}
-    line = {"metric": "events/sec, loglik + smoother (posterior at observations)", "value": value, "unit": "events/s",
+    line = {"metric": "events/sec for loglik+RTS smoother at N=1e5", "value": value, "unit": "events/s",
             "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfgname, "N": N, "events": 2 * N, "batch": batch, "state_dim": n,

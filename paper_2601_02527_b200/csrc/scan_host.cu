@@ -192,7 +192,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   LevelPlan pl;
   pl.T = 0;
   const int64_t c1 = (K + Lc - 1) / Lc;
-  if (g == 0) g = 3; // measured on configs 3 and 4 (profiles/r01_accuracy_cfg3.md, r01_sweeps.md): fastest; neither deeper nor flatter trees are reliably more accurate
+  if (g == 0) g = 2; // measured on configs 3 and 4 (profiles/r01_sweeps.md): fan-in 2-4 is a flat optimum, 2 the fastest
   if (c1 > 1) {
     pl.T = 1;
     pl.cnt[1] = c1;
