@@ -1,19 +1,20 @@
-// scan.cu -- steps a3-a6: filter scan elements and their associative combine, the two-filter
-// smoother, the log-likelihood reduction and the projection onto the observations.
+// scan.cu -- steps a3-a6: the translation unit of the scan kernels and their host orchestration.
 //
-// Scan layout (DESIGN.md "Scan"): the K events of a series are cut into chunks of Lc events.
-//   up-sweep   k_fold0 : one group of lanes per chunk folds the chunk's primitive elements
-//                        (Eq. 3.20/3.21; SG21 Eq. 10) into ONE element (A,b,C,eta,J).
+// Scan layout (DESIGN.md 5-7): the K events of a series are cut into chunks of Lc events.
+//   up-sweep   k_fold0 (chunk_kernels.cuh): one group of lanes per chunk folds the chunk's primitive
+//                        elements (Eq. 3.20/3.21; SG21 Eq. 10) into ONE element (A,b,C,eta,J).
 //                        Folding a primitive element onto an aggregate is the associative combine
 //                        with a rank-one J_j and a block-structured A_j: O(n^2 bs), not O(n^3).
-//              k_foldD : dense combine of g consecutive elements, level by level.
-//   down-sweep k_downD : from the top, the state (m,P) before every element (prefix) and the
-//                        backward information (eta,J) after it (suffix of the SAME elements).
-//              k_down0 : per chunk, the plain integrated Kalman filter (Eq. 3.14-3.15, 2.22) from
-//                        the chunk's prefix state -> innovations -> log-likelihood terms (Eq. 2.26);
-//                        then the backward information recursion from the chunk's suffix and the
-//                        smoothed exposure average at each end event (two-filter form; reading R7).
+//              k_foldD (dense_kernels.cuh): dense combine of g consecutive elements per level.
+//   down-sweep k_downD (dense_kernels.cuh): from the top, the state (m,P) before every element (prefix)
+//                        and the backward information (eta,J) after it (suffix of the SAME elements).
+//              k_down0 (chunk_kernels.cuh): per chunk, the plain integrated Kalman filter (Eq. 3.14-3.15,
+//                        2.22) from the chunk's prefix state -> innovations -> log-likelihood terms
+//                        (Eq. 2.26); then the adjoint (modified Bryson-Frazier) recursion of that filter
+//                        started from the chunk's suffix information, with the smoothed exposure average at
+//                        each end event (the two-filter posterior of reading R7 without per-event solves).
 // With one chunk per series (Lc >= K) only k_down0 runs: the sequential per-series filter (row a8).
+// Here: the log-likelihood reduction (a5), the query locator (a7) and scan_host.cu (plan and launches).
 #include <math.h>
 
 #include "dense_kernels.cuh"
@@ -31,7 +32,7 @@ __global__ void k_ll_reduce(const double* __restrict__ llpart, int64_t c1, int64
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Row a7: prediction at arbitrary times (Algorithm 1) in two-filter form.
+// Row a7: prediction at arbitrary times (Algorithm 1), adjoint form of the two-filter posterior.
 // k_query_locate: kp[q] = last event with t_k <= t*_q (-1 if none);  dtq[q] = t* - t_kp (0 if none),
 // dtq[M + q] = t_{kp+1} - t* (0 if kp is the last event).  k_disc then discretises the 2M steps.
 // k_query: one group per (series, query).
