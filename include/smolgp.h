@@ -122,7 +122,11 @@ int smolgp_loglik_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_ke
 /* Steps a2-a6 (+ a7 when M > 0).  As smolgp_loglik, plus the posterior of the noise-free exposure
  * average at every observation (mean_obs, var_obs: [batch][N]; H~ m^, H~ P^ H~^T of P:460) and,
  * when M > 0, the posterior of the instantaneous latent of instrument query_instrument at the
- * M query times (Algorithm 1; mean_query, var_query: [batch][M]).  loglik may be NULL. */
+ * M query times (Algorithm 1; mean_query, var_query: [batch][M]).  loglik may be NULL.
+ * query_instrument is a bit of the components' inst_mask: a bit < n_inst selects that instrument's
+ * integrand H_q (Eq. 3.2); a bit in [n_inst, 32) is a VIRTUAL instrument that takes no data: setting it
+ * on some components and querying it gives the component-wise predictive mean and variance of
+ * App. C.3 (H^m of Eq. C13-C14). */
 int smolgp_condition(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
                      int64_t batch, const double* y, const double* noise_sigma, const double* amp,
                      int64_t M, const double* t_query, int32_t query_instrument,

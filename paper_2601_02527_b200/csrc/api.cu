@@ -143,7 +143,7 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   double* qstore = nullptr; // all 2N filtered states and backward informations, only when queries are asked for
   if (qs.M > 0) {
     if (!qs.tq || !qs.mean || !qs.var) { ctx->err = "condition: t_query, mean_query and var_query are required when M > 0"; return SMOLGP_EINVAL; }
-    if (qs.qinst < 0 || qs.qinst >= ev->n_inst) { ctx->err = "condition: query_instrument out of range"; return SMOLGP_EINVAL; }
+    if (qs.qinst < 0 || qs.qinst >= 32) { ctx->err = "condition: query_instrument must be a mask bit in [0, 32)"; return SMOLGP_EINVAL; }
     const size_t one = (size_t)batch * ev->K * (hm.n + hm.n * hm.n) * 8;
     if (cudaMallocAsync(&qstore, 2 * one, ctx->stream) != cudaSuccess) { cudaGetLastError(); ctx->err = "out of device memory (states for query-time prediction)"; return SMOLGP_ENOMEM; }
     a.fstate = qstore; a.binfo = (double*)((char*)qstore + one);

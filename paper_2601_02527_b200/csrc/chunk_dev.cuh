@@ -31,7 +31,8 @@ struct Tab {
   unsigned char blk_of[SG_NMAX];
   double cz[SG_MAXINST * SG_MAXBLK]; // [q * nblk + b]
   double tau[SG_MAXINST];
-  double hq[SG_MAXINST * SG_MAXBLK]; // [q * nblk + b]: sigma_b if block b is in instrument q's integrand
+  double bsig[SG_MAXBLK];            // sigma_b
+  unsigned bmask[SG_MAXBLK];         // inst_mask of block b's component (bits >= n_inst: virtual instruments, C13-C14)
 };
 
 // row stride of the chunk kernels' matrices: the smallest value = 1 (mod 4) that holds n + 1 columns
@@ -46,7 +47,8 @@ inline void tab_build(const ModelDev* M, Tab* T) {
   for (int b = 0; b < M->nblk; ++b) {
     T->bdim[b] = (unsigned char)M->blk[b].dim; T->boff[b] = (unsigned char)M->blk[b].off; T->roff[b] = (short)M->disc_off[b];
     for (int i = 0; i < M->blk[b].dim; ++i) T->blk_of[M->blk[b].off + i] = (unsigned char)b;
-    for (int q = 0; q < M->n_inst; ++q) { T->cz[q * M->nblk + b] = M->cz[q][b]; T->hq[q * M->nblk + b] = M->hq[q][b]; }
+    for (int q = 0; q < M->n_inst; ++q) T->cz[q * M->nblk + b] = M->cz[q][b];
+    T->bsig[b] = M->bsig[b]; T->bmask[b] = M->bmask[b];
   }
   for (int q = 0; q < M->n_inst; ++q) T->tau[q] = M->tau[q];
 }
@@ -67,7 +69,6 @@ inline void tab_build(const ModelDev* M, Tab* T) {
 #define TBLKOF(j) jt_blkof(j)
 #define TCZ(i) (jt_czmask(i) ? T.cz[i] : 0.0) /* values stay run-time; the zero pattern is compile-time */
 #define TTAU(q) (T.tau[q])
-#define THQ(i) (T.hq[i])
 #define SG_UNROLL _Pragma("unroll")
 #else
 #define TN (T.n)
@@ -81,7 +82,6 @@ inline void tab_build(const ModelDev* M, Tab* T) {
 #define TBLKOF(j) (T.blk_of[j])
 #define TCZ(i) (T.cz[i])
 #define TTAU(q) (T.tau[q])
-#define THQ(i) (T.hq[i])
 #define SG_UNROLL
 #endif
 

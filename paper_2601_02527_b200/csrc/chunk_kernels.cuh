@@ -431,7 +431,7 @@ __device__ __forceinline__ void query_body(const QueryDev& P) {
   for (int i = g.gl; i < n; i += G) hv[i] = 0.0;
   g.sync();
   if (g.gl == 0)
-    for (int b = 0; b < TNB; ++b) hv[TBOFF(b)] = THQ(P.qinst * TNB + b);
+    for (int b = 0; b < TNB; ++b) hv[TBOFF(b)] = ((P.T.bmask[b] >> P.qinst) & 1u) ? P.T.bsig[b] : 0.0; // H of the queried (virtual) instrument
   cp_async_wait_all();
   g.sync();
   // ---- state just after the last event at or before t*, predicted over Delta_1 (Eq. 3.14) ----

@@ -39,7 +39,8 @@ struct ModelDev {
   int row_lo[SG_NMAX], row_hi[SG_NMAX]; // x-row i of F only touches columns [row_lo, row_hi)
   double cz[SG_MAXINST][SG_MAXBLK]; // c_qb: coupling of block b's integral into z_q (equilibrated units), 0 if masked out
   double tau[SG_MAXINST];          // z_q is carried as z_q / tau_q
-  double hq[SG_MAXINST][SG_MAXBLK]; // sigma_b if block b enters instrument q's integrand H_q (Eq. 3.2), else 0
+  double bsig[SG_MAXBLK];          // amplitude sigma_b of block b (H_b = sigma_b e_0 in block units)
+  uint32_t bmask[SG_MAXBLK];       // the component's inst_mask: bit v set <=> block b is in the integrand of (virtual) instrument v
   double p0[SG_NMAX * SG_NMAX];    // prior covariance blkdiag(Pinf'', 0) (Eq. 3.19, reading R6)
   BlockConst blk[SG_MAXBLK];
 };

@@ -175,9 +175,9 @@ int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const
     for (int b = 0; b < nb; ++b)
     {
       M->cz[q][b] = ((mask[b] >> q) & 1u) ? (double)(sig[b] / ((ld)M->blk[b].inv_T * (ld)tau[q])) : 0.0;
-      M->hq[q][b] = ((mask[b] >> q) & 1u) ? (double)sig[b] : 0.0;
     }
   }
+  for (int b = 0; b < nb; ++b) { M->bsig[b] = (double)sig[b]; M->bmask[b] = mask[b]; }
   const int n = M->n;
   for (int b = 0; b < nb; ++b)
     for (int i = 0; i < M->blk[b].dim; ++i)

@@ -418,3 +418,39 @@ def test_degenerate_inputs(ctx, oracle):
             np.testing.assert_allclose(out["var"][0], ref["var"], rtol=1e-8, atol=1e-10)
             np.testing.assert_allclose(out["mean_query"][0], ref["mq"], rtol=1e-8, atol=1e-9)
             np.testing.assert_allclose(out["var_query"][0], ref["vq"], rtol=1e-8, atol=1e-10)
+
+
+def test_component_wise_prediction(ctx, oracle):
+    """App. C.3 (C13-C14): a virtual instrument (mask bit >= n_inst) selects the component(s)
+    whose latent is predicted; GPU against the oracle's dense definition and sequential algorithm"""
+    rng = np.random.default_rng(8)
+    w = W.make(2, N=400)                                   # two overlapping instruments
+    w0 = 2 * np.pi / 330.0
+    kern = [W.comp(W.SHO, 1.0, w0, 10.0, inst_mask=0b0111),            # seen by both; bit 2: the SHO alone
+            W.comp(W.MATERN52, 0.6, 3000.0, inst_mask=0b1011),          # seen by both; bit 3: the Matern alone
+            W.comp(W.MATERN32, 0.4, 900.0, inst_mask=0b0010)]           # systematic of instrument 1 only
+    ts, te, inst, sig = w["t_start"], w["t_end"], w["instrument"], w["sigma"]
+    y = W.synth_y(rng, kern, ts, te, inst, sig)
+    tq = _queries(w, rng, 40)
+    ev = ctx.smolgp_build_events_host(ts, te, inst, 2)
+    got = {}
+    for v in (0, 1, 2, 3):
+        ctx.set_option("chunk", 40)
+        try:
+            got[v] = ctx.smolgp_condition_host(ev, kern, y, sig, t_query=tq, query_instrument=v)
+        finally:
+            _reset(ctx)
+        ref = oracle.ssm(kern, 2, ts, te, inst, y, sig, flags=oracle.FLAG_TWO_FILTER, tq=tq, query_inst=v)
+        k0 = float(oracle.kernel(kern, v, v, np.zeros(1))[0])
+        assert np.max(np.abs(got[v]["mean_query"][0] - ref["mq"])) <= 1e-8 * (np.sqrt(k0) + np.max(np.abs(ref["mq"])))
+        assert np.max(np.abs(got[v]["var_query"][0] - ref["vq"]) / ref["vq"]) <= 1e-8
+    # C12: instrument 1's latent = SHO + Matern-5/2 + its own systematic
+    sub = W.make(2, N=120)
+    y2 = W.synth_y(rng, kern, sub["t_start"], sub["t_end"], sub["instrument"], sub["sigma"])
+    tq2 = _queries(sub, rng, 20)
+    ev2 = ctx.smolgp_build_events_host(sub["t_start"], sub["t_end"], sub["instrument"], 2)
+    for v in (2, 3):
+        out = ctx.smolgp_condition_host(ev2, kern, y2, sub["sigma"], t_query=tq2, query_instrument=v)
+        ref = oracle.dense(kern, sub["t_start"], sub["t_end"], sub["instrument"], y2, sub["sigma"], tq=tq2, query_inst=v)
+        np.testing.assert_allclose(out["mean_query"][0], ref["mq"], rtol=1e-8, atol=1e-9)
+        np.testing.assert_allclose(out["var_query"][0], ref["vq"], rtol=1e-8, atol=1e-11)

@@ -234,3 +234,43 @@ def test_query_prediction_matches_dense(oracle, cfg, N, flags):
         s = oracle.ssm(kern, ni, ts, te, inst, y, sig, flags=flags, tq=tq, query_inst=qi)
         np.testing.assert_allclose(s["mq"], d["mq"], rtol=0, atol=1e-11)
         np.testing.assert_allclose(s["vq"], d["vq"], rtol=1e-10, atol=1e-13)
+
+
+# ---------------------------------------------------------------------------------------------
+# component-wise prediction (App. C.3, Eq. C10-C14): a VIRTUAL instrument (a mask bit
+# >= n_inst that takes no data) selects H^m
+# ---------------------------------------------------------------------------------------------
+def test_component_wise_prediction(oracle):
+    rng = np.random.default_rng(4)
+    N = 40
+    ts = np.sort(rng.uniform(0, 6000.0, N))
+    te = ts + rng.uniform(20.0, 100.0, N)
+    te[:-1] = np.minimum(te[:-1], ts[1:] - 1.0)
+    inst = np.zeros(N, np.int32)
+    w0, Q, s0, ell, s1 = 2 * np.pi / 330.0, 4.0, 1.1, 900.0, 0.7
+    # both components are seen by instrument 0; bit 1 marks the SHO alone, bit 2 the Matern alone
+    kern = [W.comp(W.SHO, s0, w0, Q, inst_mask=0b011), W.comp(W.MATERN52, s1, ell, inst_mask=0b101)]
+    y, sig = rng.standard_normal(N), np.full(N, 0.25)
+    tq = np.concatenate([[ts[0] - 200.0], rng.uniform(ts[0], te[-1], 12), [te[-1] + 300.0]])
+    tot = oracle.dense(kern, ts, te, inst, y, sig, tq=tq, query_inst=0)
+    parts = [oracle.dense(kern, ts, te, inst, y, sig, tq=tq, query_inst=v) for v in (1, 2)]
+    # C12: the component means add up to the mean of the sum; the data likelihood is untouched
+    np.testing.assert_allclose(parts[0]["mq"] + parts[1]["mq"], tot["mq"], rtol=0, atol=1e-12)
+    assert parts[0]["loglik"] == tot["loglik"] == parts[1]["loglik"]
+    # C13-C14 typed out independently: mu_m = k_m*^T C^-1 y, var_m = k_m(0) - k_m*^T C^-1 k_m*, with the
+    # exposure average of the component's kernel by quadrature
+    C = oracle.kff(kern, ts, te, inst) + np.diag(sig ** 2)
+    a = np.linalg.solve(C, y)
+    ks = [lambda tau: k_sho(tau, w0, Q, s0), lambda tau: k_matern(tau, ell, s1, 2.5)]
+    for m in range(2):
+        for qi in (0, 5, len(tq) - 1):
+            col = np.array([integrate.quad(lambda u: ks[m](tq[qi] - u), ts[j], te[j], epsabs=0, epsrel=1e-12,
+                                           points=[tq[qi]] if ts[j] < tq[qi] < te[j] else None)[0] / (te[j] - ts[j])
+                            for j in range(N)])
+            assert parts[m]["mq"][qi] == pytest.approx(col @ a, rel=1e-9, abs=1e-11)
+            assert parts[m]["vq"][qi] == pytest.approx(ks[m](0.0) - col @ np.linalg.solve(C, col), rel=1e-8)
+    # the sequential algorithm with H^m (C13-C14) agrees with the dense definition
+    for v in (1, 2):
+        s = oracle.ssm(kern, 1, ts, te, inst, y, sig, flags=2, tq=tq, query_inst=v)
+        np.testing.assert_allclose(s["mq"], parts[v - 1]["mq"], rtol=0, atol=1e-11)
+        np.testing.assert_allclose(s["vq"], parts[v - 1]["vq"], rtol=1e-10, atol=1e-13)
