@@ -184,7 +184,11 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     else {
       const int64_t per_series = (resident + batch - 1) / batch; // chunks per series
       Lc = (K + per_series - 1) / per_series;
-      if (Lc < 16) Lc = 16;
+      // floor of 16 events per chunk (below it the dense levels cost more than the chunks save: config 2),
+      // relaxed down to 4 for series so short that 16 would leave most SMs idle (config 1)
+      int64_t lc_min = (batch * K) / (2 * (int64_t)ctx->sm_count);
+      lc_min = lc_min < 4 ? 4 : (lc_min > 16 ? 16 : lc_min);
+      if (Lc < lc_min) Lc = lc_min;
     }
   }
   if (Lc > K) Lc = K;
@@ -192,7 +196,9 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   LevelPlan pl;
   pl.T = 0;
   const int64_t c1 = (K + Lc - 1) / Lc;
-  if (g == 0) g = 2; // measured on configs 3 and 4 (profiles/r01_sweeps.md): fan-in 2-4 is a flat optimum, 2 the fastest
+  // measured (profiles/r01_sweeps.md): fan-in 2-4 is a flat optimum; 2 where a combine is long (n >= 12:
+  // the chain length matters), 4 where it is short and the launches dominate
+  if (g == 0) g = (n >= 12) ? 2 : 4;
   if (c1 > 1) {
     pl.T = 1;
     pl.cnt[1] = c1;
