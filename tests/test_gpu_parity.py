@@ -454,3 +454,26 @@ def test_component_wise_prediction(ctx, oracle):
         ref = oracle.dense(kern, sub["t_start"], sub["t_end"], sub["instrument"], y2, sub["sigma"], tq=tq2, query_inst=v)
         np.testing.assert_allclose(out["mean_query"][0], ref["mq"], rtol=1e-8, atol=1e-9)
         np.testing.assert_allclose(out["var_query"][0], ref["vq"], rtol=1e-8, atol=1e-11)
+
+
+def test_specialised_kernels_are_reused_across_hyperparameters(ctx, oracle):
+    """the run-time specialisation depends on the kernel STRUCTURE only: new hyper-parameter values reuse
+    the compiled module (no second compilation) and still match the oracle"""
+    import time
+    w = W.make(4, N=500)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    ctx.set_option("jit", 1)
+    ctx.set_option("chunk", 50)
+    try:
+        ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])          # compiles (or finds) the structure
+        kern2 = [dict(k, sigma=k["sigma"] * 1.7, p0=k["p0"] * 0.6) for k in w["kernel"]]
+        t0 = time.perf_counter()
+        out = ctx.smolgp_condition_host(ev, kern2, w["y"], w["sigma"])
+        dt = time.perf_counter() - t0
+    finally:
+        _reset(ctx)
+    assert ctx.jit_log() == ""
+    assert dt < 0.5, "second call with new hyper-parameters took %.2f s: recompiled?" % dt
+    ref = PU.reference(oracle, dict(w, kernel=kern2))
+    e = PU.errors(ref, out["loglik"][0], out["mean"][0], out["var"][0])
+    assert e["ll"] <= PU.LL_RTOL and e["mean"] <= PU.POST_RTOL and e["var"] <= PU.POST_RTOL, e
