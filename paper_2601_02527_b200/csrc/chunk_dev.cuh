@@ -85,17 +85,18 @@ inline void tab_build(const ModelDev* M, Tab* T) {
 #define SG_UNROLL
 #endif
 
-// ---- record staging: global -> shared with cp.async (LDGSTS), one 8-byte copy per element ----------
-__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
+// ---- record staging: global -> shared with cp.async (LDGSTS), 16 bytes per copy -------------------
+// (records have an even number of doubles and start on 16-byte boundaries in both memories)
+__device__ __forceinline__ void cp_async16(double* dst_smem, const double* src) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src));
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(src));
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
 template <int G>
 __device__ __forceinline__ void stage_rec(const Grp<G>& g, const Tab& T, const double* __restrict__ src, double* dst) {
-  for (int e = g.gl; e < TSTRIDE; e += G) cp_async8(dst + e, src + e);
+  for (int e = 2 * g.gl; e < TSTRIDE; e += 2 * G) cp_async16(dst + e, src + e);
   cp_async_commit();
 }
 
