@@ -82,7 +82,8 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * SURVEY 8(a) row a8); "group": dense-combine fan-in of the upper scan levels (default 8);
  * "lanes": threads cooperating on one chunk (0 = automatic; 8, 16 or 32);
  * "jit": run-time specialisation of the chunk kernels for the kernel's structure with NVRTC
- * (0 = automatic: from 1e5 events per call; 1 = always; -1 = never).  A structure is compiled once
+ * (0 = automatic: from 1e5 events per call, or after 32 calls with the same structure; 1 = always;
+ * -1 = never).  A structure is compiled once
  * per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);

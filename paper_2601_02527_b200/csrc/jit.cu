@@ -43,6 +43,7 @@ struct JitState {
   NvrtcApi api;
   bool tried_open = false;
   std::vector<JitEntry> cache;
+  std::vector<std::pair<std::string, int64_t>> calls; // calls seen per structure (tiered compilation)
   std::string log;
 };
 
@@ -109,6 +110,21 @@ static std::string prelude(const Tab& T, int G, int LD) {
 static JitState* state_of(smolgp_ctx* ctx) {
   if (!ctx->jit) ctx->jit = new JitState();
   return (JitState*)ctx->jit;
+}
+
+// Tiered compilation: counts the calls made with this structure (when `count`) and says whether it is
+// "hot": already compiled, or seen SG_JIT_HOT_CALLS times -- a hyper-parameter optimisation over a small
+// series then gets the specialised kernels after a few dozen evaluations, a one-off call never pays for them.
+#define SG_JIT_HOT_CALLS 32
+bool sg_jit_hot(smolgp_ctx* ctx, const Tab& T, int G, int LD, bool count) {
+  JitState* st = state_of(ctx);
+  const std::string key = structure_key(T, G, LD);
+  for (auto& e : st->cache)
+    if (e.key == key) return e.good;
+  for (auto& c : st->calls)
+    if (c.first == key) { if (count) ++c.second; return c.second >= SG_JIT_HOT_CALLS; }
+  st->calls.emplace_back(key, count ? 1 : 0);
+  return false;
 }
 
 void sg_jit_destroy(smolgp_ctx* ctx) {

@@ -34,10 +34,13 @@ static int groups_per_cta(size_t per_group, int G, int* groups_per_sm = nullptr)
   return best;
 }
 
-// run-time specialised kernels (jit.cu): always when asked for, by default from 1e5 events per call
-// (the one-off compilation, ~5 s per model structure, is cached in the ctx)
-static bool want_jit(const smolgp_ctx* ctx, int64_t events) {
-  return ctx->opt_jit > 0 || (ctx->opt_jit == 0 && events >= 100000);
+// run-time specialised kernels (jit.cu): always when asked for; by default from 1e5 events per call, or
+// once the same structure has been evaluated a few dozen times (tiered: sg_jit_hot).  The one-off
+// compilation (~6 s per model structure) is cached in the ctx.
+static bool want_jit(smolgp_ctx* ctx, int64_t events, const Tab& T, int G, int ld, bool count) {
+  if (ctx->opt_jit != 0) return ctx->opt_jit > 0;
+  const bool hot = sg_jit_hot(ctx, T, G, ld, count); // counted once per API call (sg_run_scan)
+  return events >= 100000 || hot;
 }
 
 static int launch_jit(smolgp_ctx* ctx, cudaKernel_t k, int kid, unsigned blocks, unsigned threads, size_t smem, const void* params) {
@@ -52,10 +55,10 @@ static int launch_jit(smolgp_ctx* ctx, cudaKernel_t k, int kid, unsigned blocks,
 
 // row stride in effect: the specialised kernels take the tightest odd stride (n + 1) | 1 (less shared
 // memory per group => more groups per SM); the static variants are compiled for chunk_ld(n) only
-static int eff_ld(smolgp_ctx* ctx, const Tab& T, int G, int64_t events, const SgJitKernels** jk) {
+static int eff_ld(smolgp_ctx* ctx, const Tab& T, int G, int64_t events, const SgJitKernels** jk, bool count = false) {
   *jk = nullptr;
-  if (want_jit(ctx, events)) {
-    const int ldj = (T.n + 1) | 1;
+  const int ldj = (T.n + 1) | 1;
+  if (want_jit(ctx, events, T, G, ldj, count)) {
     *jk = sg_jit_get(ctx, T, G, ldj);
     if (*jk) return ldj;
   }
@@ -163,7 +166,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   Tab T0;
   tab_build(hm, &T0);
   const SgJitKernels* jk0; // specialised kernels for this model's structure, or nullptr (generic kernels)
-  const int ld0 = eff_ld(ctx, T0, G, batch * K, &jk0);
+  const int ld0 = eff_ld(ctx, T0, G, batch * K, &jk0, true);
   int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 0; // 0: automatic, set once the chunk count is known
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that

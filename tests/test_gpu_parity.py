@@ -477,3 +477,21 @@ def test_specialised_kernels_are_reused_across_hyperparameters(ctx, oracle):
     ref = PU.reference(oracle, dict(w, kernel=kern2))
     e = PU.errors(ref, out["loglik"][0], out["mean"][0], out["var"][0])
     assert e["ll"] <= PU.LL_RTOL and e["mean"] <= PU.POST_RTOL and e["var"] <= PU.POST_RTOL, e
+
+
+def test_tiered_specialisation_keeps_results(ctx, oracle):
+    """automatic mode: after 32 calls with one kernel structure the specialised kernels take over
+    (include/smolgp.h, option "jit"); results before and after agree and match the oracle"""
+    w = W.make("fig3", N=300)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    first = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])
+    for i in range(40):
+        kern = [dict(k, sigma=k["sigma"] * (1.0 + 0.01 * i)) for k in w["kernel"]]
+        ctx.smolgp_loglik_host(ev, kern, w["y"], w["sigma"])
+    last = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])
+    assert ctx.jit_log() == ""
+    for k in ("loglik", "mean", "var"):
+        np.testing.assert_allclose(first[k], last[k], rtol=1e-11, atol=1e-13)
+    ref = PU.reference(oracle, w)
+    e = PU.errors(ref, last["loglik"][0], last["mean"][0], last["var"][0])
+    assert e["ll"] <= PU.LL_RTOL and e["mean"] <= PU.POST_RTOL and e["var"] <= PU.POST_RTOL, e
