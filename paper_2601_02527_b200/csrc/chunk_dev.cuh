@@ -5,7 +5,7 @@
 // (column n carries the companion vector: [P | m], [Lambda | lambda], [A | b], [J | eta]), and lane j
 // OWNS column j: it computes whole columns, so a product with the transition needs no cross-lane
 // reduction.  The transition of one step is never assembled: it is applied straight from the step's
-// discretisation record (block-diagonal Phi_b, integral rows Phi-bar_b), so a
+// discretisation record (staged by a TMA bulk copy; block-diagonal Phi_b, integral rows Phi-bar_b), so a
 // product F X costs sum_b (d_b^2 + d_b) + N_inst n_blk FMAs per column instead of n^2.
 //
 //   F  = R [Phi 0; Phi-bar I]  (Eq. 3.7, Eq. 3.17; R zeroes the z rows in `tz`,
@@ -85,20 +85,52 @@ inline void tab_build(const ModelDev* M, Tab* T) {
 #define SG_UNROLL
 #endif
 
-// ---- record staging: global -> shared with cp.async (LDGSTS), 16 bytes per copy -------------------
-// (records have an even number of doubles and start on 16-byte boundaries in both memories)
-__device__ __forceinline__ void cp_async16(double* dst_smem, const double* src) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(src));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+// ---- record staging: global -> shared with the TMA bulk copy (cp.async.bulk, UBLKCP) ----------------
+// One lane of the group arms an mbarrier with the record's byte count and issues ONE bulk copy per
+// event (records have an even number of doubles and start on 16-byte boundaries in both memories);
+// every lane then waits on the barrier's phase.  Two buffers, two barriers: event k + 1 is in flight
+// while event k is being used.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-template <int G>
-__device__ __forceinline__ void stage_rec(const Grp<G>& g, const Tab& T, const double* __restrict__ src, double* dst) {
-  for (int e = 2 * g.gl; e < TSTRIDE; e += 2 * G) cp_async16(dst + e, src + e);
-  cp_async_commit();
-}
+struct RecStage {
+  double* buf;               // 2 x stride doubles
+  unsigned long long* bar;   // 2 mbarriers (right after the buffers)
+  unsigned phase;            // bit b = parity to wait for on barrier b
+  int stride;
+
+  template <int G>
+  __device__ __forceinline__ void init(const Grp<G>& g, double* recs, int stride_) {
+    buf = recs; stride = stride_; phase = 0u;
+    bar = reinterpret_cast<unsigned long long*>(recs + 2 * stride_);
+    if (g.gl == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(bar)));
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(bar + 1)));
+      asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    g.sync();
+  }
+  // request the record at `src` into buffer b (all lanes call it; one issues)
+  template <int G>
+  __device__ __forceinline__ void issue(const Grp<G>& g, const double* __restrict__ src, int b) {
+    if (g.gl == 0) {
+      const unsigned bytes = (unsigned)stride * 8u, mb = smem_u32(bar + b);
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(mb), "r"(bytes) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(buf + b * stride)),
+                   "l"(src), "r"(bytes), "r"(mb)
+                   : "memory");
+    }
+  }
+  // wait until buffer b holds its record; returns it
+  __device__ __forceinline__ const double* wait(int b) {
+    const unsigned mb = smem_u32(bar + b), par = (phase >> b) & 1u;
+    unsigned ok = 0;
+    while (!ok) {
+      asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok) : "r"(mb), "r"(par) : "memory");
+    }
+    phase ^= (1u << b);
+    return buf + b * stride;
+  }
+};
 
 // Phi_b (DB x DB, row-major) and Phi-bar_b (DB) of one block, contiguous in the staged record.  Records
 // are laid out so that every block starts on a 16-byte boundary (even block sizes, even buffer offsets):

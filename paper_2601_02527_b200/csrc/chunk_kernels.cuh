@@ -41,7 +41,7 @@ struct ScanDev {
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int fold0_group_doubles(int n, int ld, int stride, int nblk, int G) {
   const int nr = ld - 1; // nr >= n rows: the padding rows stay zero, so row loops run to the compile-time nr
-  return (4 * nr * ld + 2 * stride + nblk * G + 2 * ld + 2 + 1) & ~1; // even: record buffers stay 16-byte aligned
+  return (4 * nr * ld + 2 * stride + 2 + nblk * G + 2 * ld + 2 + 1) & ~1; // even: record buffers stay 16-byte aligned; + 2 mbarriers
 }
 
 template <int G, int LD>
@@ -62,14 +62,16 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
   double* Tm = C + NR * ld;
   double* JE = Tm + NR * ld;     // [J | eta]
   double* recs = JE + NR * ld;   // 2 x stride
-  double* U = recs + 2 * TSTRIDE + g.gl;
-  double* av = recs + 2 * TSTRIDE + TNB * G; // NR (zero padded) + 1: av[NR] = hs b_z
+  double* U = recs + 2 * TSTRIDE + 2 + g.gl;
+  double* av = recs + 2 * TSTRIDE + 2 + TNB * G; // NR (zero padded) + 1: av[NR] = hs b_z
   double* cv = av + ld;                           // NR (zero padded)
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
 
-  stage_rec(g, T, P.disc + k0 * (int64_t)TSTRIDE, recs);
+  RecStage rs;
+  rs.init(g, recs, TSTRIDE);
+  rs.issue(g, P.disc + k0 * (int64_t)TSTRIDE, 0);
   zero_fill(g, AB0, 4 * NR * ld);
   zero_fill(g, av, 2 * ld);
   g.sync();
@@ -79,10 +81,9 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
   uint32_t meta_nx = P.meta[k0];
   int32_t ob_nx = P.obs[k0];
   for (int64_t k = k0; k < k1; ++k) {
-    const double* rec = recs + ((k - k0) & 1) * TSTRIDE;
-    cp_async_wait_all();
+    const double* rec = rs.wait((int)((k - k0) & 1));
     g.sync();
-    if (k + 1 < k1) stage_rec(g, T, P.disc + (k + 1) * (int64_t)TSTRIDE, recs + ((k + 1 - k0) & 1) * TSTRIDE);
+    if (k + 1 < k1) rs.issue(g, P.disc + (k + 1) * (int64_t)TSTRIDE, (int)((k + 1 - k0) & 1));
     // event k's scalars were requested one iteration ago; the data of an end event are requested now
     // and consumed after the products, so no global latency sits on the per-event critical path
     const uint32_t meta = meta_nx;
@@ -158,7 +159,7 @@ __device__ __forceinline__ void fold0_body(const ScanDev& P) {
 __host__ __device__ inline int kbuf_stride(int n) { return 2 * n + 4; }
 __host__ __device__ inline int down0_group_doubles(int n, int ld, int stride, int nblk, int G) {
   const int nr = ld - 1, ws = ((n * (2 * n + 1) > nr * ld ? n * (2 * n + 1) : nr * ld) + 1) & ~1;
-  return (nr * ld + ws + 2 * stride + nblk * G + 5 * ld + 1 + 1) & ~1; // Tm is the head of Ws; even sizes keep the record buffers aligned
+  return (nr * ld + ws + 2 * stride + 2 + nblk * G + 5 * ld + 1 + 1) & ~1; // Tm is the head of Ws; even sizes keep the record buffers aligned
 }
 
 // [vector | matrix(n x n)] in global memory  <->  column-owned [matrix | vector] with row stride ld
@@ -197,8 +198,8 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   double* Tm = X + NR * ld;
   double* Ws = Tm;                  // n x (2n+1), used only for the one solve per chunk (Tm is dead there)
   double* recs = Ws + (((n * (2 * n + 1) > NR * ld ? n * (2 * n + 1) : NR * ld) + 1) & ~1);
-  double* U = recs + 2 * TSTRIDE + g.gl;
-  double* cv = recs + 2 * TSTRIDE + TNB * G; // NR, zero padded
+  double* U = recs + 2 * TSTRIDE + 2 + g.gl;
+  double* cv = recs + 2 * TSTRIDE + 2 + TNB * G; // NR, zero padded
   double* kv = cv + ld;
   double* pv = kv + ld;
   double* av = pv + ld;             // n + 1
@@ -209,7 +210,9 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   const double ampv = P.amp ? P.amp[series] : 1.0;
   const double ramp = 1.0 / ampv;
 
-  stage_rec(g, T, P.disc + k0 * (int64_t)TSTRIDE, recs);
+  RecStage rs;
+  rs.init(g, recs, TSTRIDE);
+  rs.issue(g, P.disc + k0 * (int64_t)TSTRIDE, 0);
   zero_fill(g, X, 2 * NR * ld);
   zero_fill(g, cv, 5 * ld);
   g.sync();
@@ -224,10 +227,9 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   uint32_t meta_nx = P.meta[k0];
   int32_t ob_nx = P.obs[k0];
   for (int64_t k = k0; k < k1; ++k) {
-    const double* rec = recs + ((k - k0) & 1) * TSTRIDE;
-    cp_async_wait_all();
+    const double* rec = rs.wait((int)((k - k0) & 1));
     g.sync();
-    if (k + 1 < k1) stage_rec(g, T, P.disc + (k + 1) * (int64_t)TSTRIDE, recs + ((k + 1 - k0) & 1) * TSTRIDE);
+    if (k + 1 < k1) rs.issue(g, P.disc + (k + 1) * (int64_t)TSTRIDE, (int)((k + 1 - k0) & 1));
     const uint32_t meta = meta_nx; // prefetched: see k_fold0
     const int32_t ob = ob_nx;
     if (k + 1 < k1) { meta_nx = P.meta[k + 1]; ob_nx = P.obs[k + 1]; }
@@ -276,7 +278,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   if (!P.want_smooth) return;
 
   // ---- adjoint at the chunk's last event from the suffix information ----
-  stage_rec(g, T, P.disc + (k1 - 1) * (int64_t)TSTRIDE, recs);
+  rs.issue(g, P.disc + (k1 - 1) * (int64_t)TSTRIDE, 0);
   if (P.SUF1) {
     const int ld2 = 2 * n + 1;
     // Ws = [I + J P | J | J m - eta]: J goes straight to its place, eta is parked in column 2n
@@ -315,10 +317,9 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
     S_r = kb[2 * n]; v_r = kb[2 * n + 1]; m_r = kb[2 * n + 2]; dlb_r = P.delta[k1 - 1];
   }
   for (int64_t k = k1 - 1; k >= k0; --k) {
-    const double* rec = recs + ((k1 - 1 - k) & 1) * TSTRIDE;
-    cp_async_wait_all();
+    const double* rec = rs.wait((int)((k1 - 1 - k) & 1));
     g.sync();
-    if (k > k0) stage_rec(g, T, P.disc + (k - 1) * (int64_t)TSTRIDE, recs + ((k1 - k) & 1) * TSTRIDE);
+    if (k > k0) rs.issue(g, P.disc + (k - 1) * (int64_t)TSTRIDE, (int)((k1 - k) & 1));
     const uint32_t meta = meta_nx;
     const int32_t ob = ob_nx;
     const double kv_c = kv_r, pv_c = pv_r, S = S_r, v = v_r, mfz = m_r, dl_c = dlb_r;
@@ -399,7 +400,7 @@ struct QueryDev {
 };
 
 __host__ __device__ inline int query_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  return (3 * (ld - 1) * ld + 2 * stride + nblk * G + 2 * ld + 1 + 1) & ~1;
+  return (3 * (ld - 1) * ld + 2 * stride + 2 + nblk * G + 2 * ld + 1 + 1) & ~1;
 }
 
 template <int G, int LD>
@@ -419,20 +420,23 @@ __device__ __forceinline__ void query_body(const QueryDev& P) {
   double* Tm = X + NR * ld;
   double* Y = Tm + NR * ld;         // [Lambda* | lambda*]
   double* recs = Y + NR * ld;
-  double* U = recs + 2 * TSTRIDE + g.gl;
-  double* hv = recs + 2 * TSTRIDE + TNB * G; // n: H_q in block units
+  double* U = recs + 2 * TSTRIDE + 2 + g.gl;
+  double* hv = recs + 2 * TSTRIDE + 2 + TNB * G; // n: H_q in block units
   double* ph = hv + ld;                           // n: P* h
   const int ss = state_size(n);
   const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
   const int64_t kp = P.kp[q];
   const double ampv = P.amp ? P.amp[series] : 1.0;
-  stage_rec(g, T, P.discq + q * (int64_t)TSTRIDE, recs);
-  stage_rec(g, T, P.discq + (P.Mq + q) * (int64_t)TSTRIDE, recs + TSTRIDE);
+  RecStage rs;
+  rs.init(g, recs, TSTRIDE);
+  rs.issue(g, P.discq + q * (int64_t)TSTRIDE, 0);
+  rs.issue(g, P.discq + (P.Mq + q) * (int64_t)TSTRIDE, 1);
   for (int i = g.gl; i < n; i += G) hv[i] = 0.0;
   g.sync();
   if (g.gl == 0)
     for (int b = 0; b < TNB; ++b) hv[TBOFF(b)] = ((P.T.bmask[b] >> P.qinst) & 1u) ? P.T.bsig[b] : 0.0; // H of the queried (virtual) instrument
-  cp_async_wait_all();
+  rs.wait(0);
+  rs.wait(1);
   g.sync();
   // ---- state just after the last event at or before t*, predicted over Delta_1 (Eq. 3.14) ----
   if (kp >= 0) {
