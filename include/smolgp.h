@@ -79,12 +79,11 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
 
 /* Tuning knobs (all optional).  name = "chunk": events per scan chunk at the leaf level
  * (0 = automatic; >= the series length selects the sequential one-group-per-series filter of
- * SURVEY 8(a) row a8); "group": dense-combine fan-in of the upper scan levels (default 8);
+ * SURVEY 8(a) row a8); "group": dense-combine fan-in of the upper scan levels (0 = automatic: 2 for n >= 12, else 4);
  * "lanes": threads cooperating on one chunk (0 = automatic; 8, 16 or 32);
  * "jit": run-time specialisation of the chunk kernels for the kernel's structure with NVRTC
  * (0 = automatic: from 1e5 events per call, or after 32 calls with the same structure; 1 = always;
- * -1 = never).  A structure is compiled once
- * per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
+ * -1 = never).  A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);
 const char* smolgp_jit_log(smolgp_ctx* ctx);
@@ -96,7 +95,8 @@ const char* smolgp_jit_log(smolgp_ctx* ctx);
  * order-preserving 64-bit image of the times; the reset/observe flags, the per-event set of idle
  * instruments and the validation that no instrument overlaps itself come from an
  * exclusive XOR scan of the instrument bits.  The three inputs are DEVICE pointers; the result
- * is owned by the caller (smolgp_free_events) and can be reused across kernels and data.
+ * is owned by the caller (smolgp_free_events; free it before destroying the ctx whose stream it was
+ * allocated on) and can be reused across kernels and data.
  * Errors: EINVAL, EOVERLAP, EUNSUPPORTED (n_inst > SMOLGP_MAX_INST), ENOMEM, ECUDA. */
 int smolgp_build_events(smolgp_ctx* ctx, int64_t N, const double* t_start, const double* t_end,
                         const int32_t* instrument, int32_t n_inst, smolgp_events** out);
