@@ -80,6 +80,8 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
 /* Tuning knobs (all optional).  name = "chunk": events per scan chunk at the leaf level
  * (0 = automatic; >= the series length selects the sequential one-group-per-series filter of
  * SURVEY 8(a) row a8); "group": dense-combine fan-in of the upper scan levels (0 = automatic: 2 for n >= 12, else 4);
+ * "top": the level tree of the scan stops once a level holds <= top elements, which the top down-sweep
+ * walks sequentially (0 = automatic: 4 for n >= 12, else 8; values below the fan-in act as the fan-in);
  * "lanes": threads cooperating on one chunk (0 = automatic; 8, 16 or 32);
  * "jit": run-time specialisation of the chunk kernels for the kernel's structure with NVRTC
  * (0 = automatic: from 1e5 events per call, or after 32 calls with the same structure; 1 = always;

@@ -30,7 +30,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0;
-  c->opt_chunk = 0; c->opt_group = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
+  c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
   // pinned: the per-call model upload is a true asynchronous copy
   if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
   int v = 0;
@@ -101,6 +101,7 @@ extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t valu
   if (!ctx || !name) return SMOLGP_EINVAL;
   if (!strcmp(name, "chunk")) ctx->opt_chunk = value;
   else if (!strcmp(name, "group")) ctx->opt_group = value;
+  else if (!strcmp(name, "top")) ctx->opt_top = value;
   else if (!strcmp(name, "lanes")) ctx->opt_lanes = value;
   else if (!strcmp(name, "jit")) ctx->opt_jit = value;
   else { ctx->err = std::string("unknown option ") + name; return SMOLGP_EINVAL; }

@@ -77,7 +77,7 @@ struct smolgp_ctx {
   int prof_on;
   std::vector<ProfRec> prof;       // open records of the current profiling window
   std::vector<cudaEvent_t> evpool; // recycled events
-  int64_t opt_chunk, opt_group, opt_lanes, opt_jit; // opt_jit: 0 automatic, 1 always, -1 never
+  int64_t opt_chunk, opt_group, opt_lanes, opt_top, opt_jit; // opt_jit: 0 automatic, 1 always, -1 never
   void* jit;       // run-time specialised kernels (jit.cu)
   // workspace arena (grown on demand, reused across calls)
   void* arena;

@@ -43,12 +43,13 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const dou
 // M = (I + C_i J_j)^-1,
 //   A = A_j M A_i,  b = A_j M (b_i + C_i eta_j) + b_j,  C = A_j M C_i A_j^T + C_j,
 //   eta = A_i^T M^T (eta_j - J_j b_i) + eta_i,           J = A_i^T M^T J_j A_i + J_i.
-// One warp per group.  ei, ej, eo: elements in shared memory (layout above); Ws: n x (3n+1); Tm: n x n.
+// One CTA per group.  ei, ej, eo: elements in shared memory (layout above); Ws: n x (3n+1); Tm: n x (n+1);
+// Xs: n x (2n+1), receives M^-1 [A_i | b_i + C_i eta_j | C_i].
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const double* ej, double* eo,
-                              double* Ws, double* Tm, double* uv) {
-  const int n1 = n + 1, ld = 3 * n + 1;
+                              double* Ws, double* Tm, double* uv, double* Xs) {
+  const int n1 = n + 1, ld = 3 * n + 1, lx = 2 * n + 1;
   const double *Ai = ei, *Ci = ei + n * n1, *Ji = Ci + n * n;
   const double *Aj = ej, *Cj = ej + n * n1, *Jj = Cj + n * n;
   double *Ao = eo, *Co = eo + n * n1, *Jo = Co + n * n;
@@ -69,13 +70,13 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
     uv[i] = acc;
   }
   g.sync();
-  gj_solve(g, n, ld, Ws);
-  const double* X1 = Ws + n;         // M A_i           (row stride ld)
-  const double* X2 = Ws + 2 * n;     // M (b_i + C_i eta_j), then X3 = M C_i follows
+  gj_solve_np(g, n, ld, Ws, Xs);
+  const double* X1 = Xs;             // M A_i           (row stride lx)
+  const double* X2 = Xs + n;         // M (b_i + C_i eta_j), then X3 = M C_i follows
   // [A | b] = A_j [X1 | x2] (+ b_j in the last column)
-  mm(g, n, n1, n, Aj, n1, 1, X1, ld, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
+  mm(g, n, n1, n, Aj, n1, 1, X1, lx, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
   // Tm = A_j X3
-  mm(g, n, n, n, Aj, n1, 1, X2 + 1, ld, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+  mm(g, n, n, n, Aj, n1, 1, X2 + 1, lx, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
   g.sync();
   for (int i = g.gl; i < n; i += G) Ao[i * n1 + n] += Aj[i * n1 + n];
   // C = Tm A_j^T + C_j
@@ -83,7 +84,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   // eta = X1^T u + eta_i
   for (int i = g.gl; i < n; i += G) {
     double acc = Ji[i * n1 + n];
-    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * ld + i], uv[l], acc, cmp); acc += cmp; }
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * lx + i], uv[l], acc, cmp); acc += cmp; }
     Jo[i * n1 + n] = acc;
   }
   g.sync();
@@ -94,14 +95,14 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
     const int i = e / n, j = e - i * n;
     if (j > i) continue;
     double acc = Ji[i * n1 + j];
-    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * ld + i], Tm[l * n + j], acc, cmp); acc += cmp; }
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * lx + i], Tm[l * n + j], acc, cmp); acc += cmp; }
     Jo[i * n1 + j] = acc;
     Jo[j * n1 + i] = acc;
   }
   g.sync();
 }
 
-__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 1) + n * (n + 1) + n; }
+__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 1) + n * (n + 1) + n + n * (2 * n + 1); }
 
 struct DenseArgs {
   int n;              // augmented state dimension
@@ -128,18 +129,22 @@ __device__ __forceinline__ void foldD_body(const DenseArgs& P) {
   if (gid >= P.batch * P.cout) return;
   double* base = (double*)(smem + tb);
   double* e0 = base; double* e1 = e0 + es; double* e2 = e1 + es;
-  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 1); double* uv = Tm + n * (n + 1);
+  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 1); double* uv = Tm + n * (n + 1); double* Xs = uv + n;
   const int64_t series = gid / P.cout, grp = gid - series * P.cout;
   const int64_t m0 = grp * P.g, m1 = (m0 + P.g < P.cin) ? m0 + P.g : P.cin;
   const double* src = P.Ein + (series * P.cin + m0) * (int64_t)es;
-  for (int e = g.gl; e < es; e += NT) e0[e] = src[e];
+  // the first two elements of the group are consecutive in memory (e0, e1 too): one pass of loads for both
+  const int first = (m0 + 1 < m1) ? 2 * es : es;
+  for (int e = g.gl; e < first; e += NT) e0[e] = src[e];
   g.sync();
   double* acc = e0; double* nxt = e1; double* out = e2;
   for (int64_t m = m0 + 1; m < m1; ++m) {
     src += es;
-    for (int e = g.gl; e < es; e += NT) nxt[e] = src[e];
-    g.sync();
-    dense_combine(g, n, acc, nxt, out, Ws, Tm, uv);
+    if (m > m0 + 1) {
+      for (int e = g.gl; e < es; e += NT) nxt[e] = src[e];
+      g.sync();
+    }
+    dense_combine(g, n, acc, nxt, out, Ws, Tm, uv, Xs);
     double* t = acc; acc = out; out = t;
   }
   double* dst = P.Eout + gid * (int64_t)es;
@@ -152,7 +157,7 @@ __device__ __forceinline__ void foldD_body(const DenseArgs& P) {
 //   backward: element (x) (eta_e, J_e):  M = (I + C J_e)^-1;  eta' = A^T M^T (eta_e - J_e b) + eta;
 //             J' = A^T M^T J_e A + J
 // ---------------------------------------------------------------------------------------------------
-__host__ __device__ inline int downD_group_doubles(int n) { return elem_size(n) + 2 * state_size(n) + n * (2 * n + 1) + n * n + n; }
+__host__ __device__ inline int downD_group_doubles(int n) { return elem_size(n) + 2 * state_size(n) + n * (2 * n + 1) + n * n + n + n * (n + 1); }
 
 template <int NT>
 __device__ __forceinline__ void downD_body(const DenseArgs& P) {
@@ -164,7 +169,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
   if (gid >= P.batch * P.cout) return;
   const int backward = blockIdx.y;
   double* base = (double*)(smem + tb);
-  double* el = base; double* st = el + es; double* st2 = st + ss; double* Ws = st2 + ss; double* Tm = Ws + n * ld; double* uv = Tm + n * n;
+  double* el = base; double* st = el + es; double* st2 = st + ss; double* Ws = st2 + ss; double* Tm = Ws + n * ld; double* uv = Tm + n * n; double* Xs = uv + n;
   const int64_t series = gid / P.cout, grp = gid - series * P.cout;
   const int64_t m0 = grp * P.g, m1 = (m0 + P.g < P.cin) ? m0 + P.g : P.cin;
   const double *A = el, *C = el + n * n1, *J = C + n * n; // [A|b], C, [J|eta]
@@ -187,14 +192,14 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n1 + j] = Pm[e]; }
       for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + n] += mv[i]; }
       g.sync();
-      gj_solve(g, n, ld, Ws);
+      gj_solve_np(g, n, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
       // m' = A x + b ; Tm = A X ; P' = Tm A^T + C
       for (int i = g.gl; i < n; i += NT) {
         double acc = A[i * n1 + n];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(A[i * n1 + l], Ws[l * ld + n], acc, cmp); acc += cmp; }
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(A[i * n1 + l], Xs[l * n1], acc, cmp); acc += cmp; }
         st2[i] = acc;
       }
-      mm(g, n, n, n, A, n1, 1, Ws + n1, ld, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+      mm(g, n, n, n, A, n1, 1, Xs + 1, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
       g.sync();
       mm_sym(g, n, n, Tm, n, 1, A, 1, n1, C, st2 + n);
       g.sync();
@@ -227,11 +232,11 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
         uv[i] = acc;
       }
       g.sync();
-      gj_solve(g, n, ld2, Ws);
-      const double* X = Ws + n; // M A, row stride ld2
+      gj_solve_np(g, n, ld2, Ws, Xs);
+      const double* X = Xs; // M A, row stride n
       for (int i = g.gl; i < n; i += NT) {
         double acc = J[i * n1 + n];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * ld2 + i], uv[l], acc, cmp); acc += cmp; }
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * n + i], uv[l], acc, cmp); acc += cmp; }
         st2[i] = acc;
       }
       mm(g, n, n, n, Je, n, 1, A, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1); // Tm = J_e A
@@ -240,7 +245,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
         const int i = e / n, j = e - i * n;
         if (j > i) continue;
         double acc = J[i * n1 + j];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * ld2 + i], Tm[l * n + j], acc, cmp); acc += cmp; }
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * n + i], Tm[l * n + j], acc, cmp); acc += cmp; }
         st2[n + i * n + j] = acc;
         st2[n + j * n + i] = acc;
       }

@@ -97,3 +97,52 @@ __device__ void gj_solve(const Grp<G>& g, int n, int ld, double* W) {
   }
   g.sync();
 }
+
+// Gauss-Jordan with partial pivoting and NO row exchange, for a group that is a whole CTA (G > 32, n <= 32):
+// the dense levels run one solve per combine on the latency-critical path, so the barriers per pivot count.
+// The pivot of column p is the largest entry among the rows not yet used as a pivot; it is found by every
+// warp on its own (lane l holds row l, shuffle arg-max, ties to the lower row, so all warps agree without
+// a barrier), the row stays where it is and only its index is recorded.  Elimination p writes columns > p of
+// the other rows and reads column p and row r only, so ONE barrier per pivot (before the next search) is
+// enough, against three in gj_solve.  Same pivots, hence the same arithmetic per entry, as gj_solve.
+// W = [M | R] (n rows, ld = n + m columns) is destroyed; X (n x m, row stride m) receives M^-1 R.
+template <int G>
+__device__ void gj_solve_np(const Grp<G>& g, int n, int ld, double* W, double* X) {
+  __shared__ int rowof[32];
+  const int lane = threadIdx.x & 31;
+  unsigned used = 0u;
+  for (int p = 0; p < n; ++p) {
+    double v = (lane < n && !((used >> lane) & 1u)) ? fabs(W[lane * ld + p]) : -1.0;
+    int r = lane;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+      const double ov = __shfl_xor_sync(0xffffffffu, v, o);
+      const int orow = __shfl_xor_sync(0xffffffffu, r, o);
+      if (ov > v || (ov == v && orow < r)) { v = ov; r = orow; }
+    }
+    r = min(__shfl_sync(0xffffffffu, r, 0), n - 1); // non-finite input: still one in-range row for the whole CTA
+    used |= 1u << r;
+    if (g.gl == 0) rowof[p] = r;
+    const double rpv = 1.0 / W[r * ld + p];
+    const int nc = ld - p - 1;
+    const float rnc = 1.0f / (float)nc;
+    const int tot = (n - 1) * nc;
+    for (int e = g.gl; e < tot; e += G) {
+      int i, j;
+      divmod_small(e, nc, rnc, i, j);
+      if (i >= r) ++i;
+      j += p + 1;
+      W[i * ld + j] = fma(-W[i * ld + p] * rpv, W[r * ld + j], W[i * ld + j]);
+    }
+    g.sync();
+  }
+  const int m = ld - n;
+  const float rm = 1.0f / (float)m;
+  for (int e = g.gl; e < n * m; e += G) {
+    int i, j;
+    divmod_small(e, m, rm, i, j);
+    const int r = rowof[i];
+    X[e] = W[r * ld + n + j] / W[r * ld + i];
+  }
+  g.sync();
+}

@@ -205,7 +205,12 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   if (c1 > 1) {
     pl.T = 1;
     pl.cnt[1] = c1;
-    while (pl.cnt[pl.T] > g) { pl.cnt[pl.T + 1] = (pl.cnt[pl.T] + g - 1) / g; pl.T++; }
+    // the tree stops once a level holds <= gtop elements: the top down-sweep walks them sequentially in one
+    // CTA per direction.  A level costs two latency-bound launches, a step of the walk about one; measured
+    // (profiles/r01_sweeps.md, sweep "top"): 3-8 is a flat optimum at n = 21 / 17, 8-16 for short series of small n
+    int gtop = (ctx->opt_top >= 2) ? (int)ctx->opt_top : ((n >= 12) ? 4 : 8);
+    if (gtop < g) gtop = g;
+    while (pl.cnt[pl.T] > gtop) { pl.cnt[pl.T + 1] = (pl.cnt[pl.T] + g - 1) / g; pl.T++; }
   }
   const int es = elem_size(n), ss = state_size(n);
   // workspace

@@ -2,7 +2,7 @@
 min of several runs) over the scan-plan knobs of smolgp_set_option, so that the automatic choices in
 csrc/scan_host.cu can be checked against measurement on a given GPU.
 
-    python -m paper_2601_02527_b200.tune --config 3 [--sweep group|chunks|jit|lanes|predict] [--reps 7]
+    python -m paper_2601_02527_b200.tune --config 3 [--sweep group|top|chunks|jit|lanes|predict] [--reps 7]
 
 Prints markdown table rows.  No oracle involved (accuracy sweeps: tests/accuracy_sweep.py)."""
 import argparse
@@ -25,7 +25,7 @@ def main():
     from . import binding as B, workloads as W
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--sweep", default="group", choices=["group", "chunks", "jit", "lanes", "predict"])
+    ap.add_argument("--sweep", default="group", choices=["group", "top", "chunks", "jit", "lanes", "predict"])
     ap.add_argument("--reps", type=int, default=7)
     ap.add_argument("--predict-mult", type=int, default=10, help="queries per exposure for --sweep predict")
     args = ap.parse_args()
@@ -54,6 +54,10 @@ def main():
         for g in (2, 3, 4, 6, 8, 16):
             ctx.set_option("group", g)
             run("group %d" % g)
+    elif args.sweep == "top":
+        for t in (2, 3, 4, 6, 8, 12, 16, 24):
+            ctx.set_option("top", t)
+            run("top %d" % t)
     elif args.sweep == "chunks":
         for per_sm in (0, 4, 6, 8, 10, 12, 16, 20):
             ctx.set_option("chunk", 0 if per_sm == 0 else -(-(2 * N) // (sm * per_sm)))

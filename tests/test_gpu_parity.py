@@ -24,6 +24,7 @@ def ctx():
 def _reset(ctx):
     ctx.set_option("chunk", 0)
     ctx.set_option("group", 0)
+    ctx.set_option("top", 0)
     ctx.set_option("lanes", 0)
     ctx.set_option("jit", 0)
 
@@ -31,7 +32,8 @@ def _reset(ctx):
 SCAN_OPTS = {
     "auto": (),
     "sequential": (("chunk", 1 << 40),),                       # one chunk per series (row a8)
-    "deep": (("chunk", 16), ("group", 2)),                     # many dense levels
+    "deep": (("chunk", 16), ("group", 2), ("top", 2)),         # many dense levels, tree up to the root
+    "walk": (("chunk", 16), ("group", 2), ("top", 13)),        # long sequential walk at the top level
     "ragged": (("chunk", 37), ("group", 3), ("lanes", 32)),    # chunk/group sizes dividing nothing
     "jit": (("chunk", 29), ("jit", 1)),                        # run-time specialised chunk kernels (NVRTC)
 }
