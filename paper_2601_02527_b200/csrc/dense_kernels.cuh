@@ -11,30 +11,64 @@
 #define DN (P.n)
 #endif
 
-// general dense product  D[i,j] = (C ? C[i,j] : 0) + sum_l A[i,l] B[l,j],  strided operands
+// general dense product  D[i,j] = (C ? C[i,j] : 0) + sum_l A[i,l] B[l,j],  strided operands.  A thread works on
+// two outputs at a time: the two compensated chains are independent, so their fixed-latency FP64 dependencies
+// overlap (the dense levels are latency-bound, profiles/r01_dense_level_ncu.md).  skew: number of work items the
+// group has already been dealt in this phase (the next item goes to lane skew % G), so that several products
+// between two barriers load the lanes evenly.
 template <int G>
 __device__ __forceinline__ void mm(const Grp<G>& g, int nr, int nc, int nk, const double* A, int ar, int ac,
-                                   const double* B, int br, int bc, const double* C, int cr, int cc, double* D, int dr, int dc) {
+                                   const double* B, int br, int bc, const double* C, int cr, int cc, double* D, int dr, int dc,
+                                   int skew = 0) {
   const float rnc = 1.0f / (float)nc;
-  for (int e = g.gl; e < nr * nc; e += G) {
-    int i, j;
+  const int tot = nr * nc;
+  int e0 = g.gl - skew % G;
+  if (e0 < 0) e0 += G;
+  for (int e = e0; e < tot; e += 2 * G) {
+    const int eb = (e + G < tot) ? e + G : e; // no second output left: the first one is computed twice
+    int i, j, ib, jb;
     divmod_small(e, nc, rnc, i, j);
-    double acc = C ? C[i * cr + j * cc] : 0.0;
-    { double cmp = 0.0; for (int l = 0; l < nk; ++l) dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp); acc += cmp; }
-    D[i * dr + j * dc] = acc;
+    divmod_small(eb, nc, rnc, ib, jb);
+    double acc = C ? C[i * cr + j * cc] : 0.0, accb = C ? C[ib * cr + jb * cc] : 0.0;
+    double cmp = 0.0, cmpb = 0.0;
+    for (int l = 0; l < nk; ++l) {
+      dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp);
+      dot2_step(A[ib * ar + l * ac], B[l * br + jb * bc], accb, cmpb);
+    }
+    D[i * dr + j * dc] = acc + cmp;
+    if (eb != e) D[ib * dr + jb * dc] = accb + cmpb;
   }
 }
-// symmetric result: D[i,j] = D[j,i] = (C ? C[i,j] : 0) + sum_l A[i,l] B[l,j] for i >= j (n x n, row stride n)
+// e -> (i, j), j <= i, of the e-th entry of the lower triangle in row order (e < 2^20)
+__device__ __forceinline__ void tri_index(int e, int& i, int& j) {
+  i = (int)((sqrtf((float)(8 * e + 1)) - 1.0f) * 0.5f);
+  if (i * (i + 1) / 2 > e) --i;
+  if ((i + 1) * (i + 2) / 2 <= e) ++i;
+  j = e - i * (i + 1) / 2;
+}
+// symmetric result: D[i,j] = D[j,i] = C[i,j] + sum_l A[i,l] B[l,j] for i >= j (n x n; row strides cr, dr);
+// the n (n + 1) / 2 entries of the lower triangle are the work items, two at a time as in mm
 template <int G>
 __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const double* A, int ar, int ac,
-                                       const double* B, int br, int bc, const double* C, double* D) {
-  for (int e = g.gl; e < n * n; e += G) {
-    const int i = e / n, j = e - i * n;
-    if (j > i) continue;
-    double acc = C ? C[i * n + j] : 0.0;
-    { double cmp = 0.0; for (int l = 0; l < nk; ++l) dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp); acc += cmp; }
-    D[i * n + j] = acc;
-    D[j * n + i] = acc;
+                                       const double* B, int br, int bc, const double* C, int cr, double* D, int dr, int skew = 0) {
+  const int tot = n * (n + 1) / 2;
+  int e0 = g.gl - skew % G;
+  if (e0 < 0) e0 += G;
+  for (int e = e0; e < tot; e += 2 * G) {
+    const int eb = (e + G < tot) ? e + G : e;
+    int i, j, ib, jb;
+    tri_index(e, i, j);
+    tri_index(eb, ib, jb);
+    double acc = C[i * cr + j], accb = C[ib * cr + jb];
+    double cmp = 0.0, cmpb = 0.0;
+    for (int l = 0; l < nk; ++l) {
+      dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp);
+      dot2_step(A[ib * ar + l * ac], B[l * br + jb * bc], accb, cmpb);
+    }
+    acc += cmp;
+    D[i * dr + j] = acc;
+    D[j * dr + i] = acc;
+    if (eb != e) { accb += cmpb; D[ib * dr + jb] = accb; D[jb * dr + ib] = accb; }
   }
 }
 
@@ -48,14 +82,21 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const dou
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const double* ej, double* eo,
-                              double* Ws, double* Tm, double* uv, double* Xs) {
-  const int n1 = n + 1, ld = 3 * n + 1, lx = 2 * n + 1;
+                              double* Ws, double* Tm, double* uv, double* Xs, double* T2) {
+  const int n1 = n + 1, ld = 3 * n + 1, lx = 2 * n + 1, ntri = n * (n + 1) / 2;
   const double *Ai = ei, *Ci = ei + n * n1, *Ji = Ci + n * n;
   const double *Aj = ej, *Cj = ej + n * n1, *Jj = Cj + n * n;
   double *Ao = eo, *Co = eo + n * n1, *Jo = Co + n * n;
-  // Ws = [I + C_i J_j | A_i | b_i + C_i eta_j | C_i]
-  mm(g, n, n1, n, Ci, n, 1, Jj, n1, 1, (const double*)nullptr, 0, 0, Tm, n1, 1); // n x (n+1): C_i [J_j | eta_j]  (Tm has room: see caller)
+  // phase 1 (everything that needs no solve): Tm = C_i [J_j | eta_j] (n x (n+1)); T2 = J_j A_i; u = eta_j - J_j b_i
+  mm(g, n, n1, n, Ci, n, 1, Jj, n1, 1, (const double*)nullptr, 0, 0, Tm, n1, 1);
+  mm(g, n, n, n, Jj, n1, 1, Ai, n1, 1, (const double*)nullptr, 0, 0, T2, n, 1, n * n1);
+  for (int i = G - 1 - g.gl; i < n; i += G) { // dealt from the last lane down: those have the fewest items above
+    double acc = Jj[i * n1 + n];
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(-Jj[i * n1 + l], Ai[l * n1 + n], acc, cmp); acc += cmp; }
+    uv[i] = acc;
+  }
   g.sync();
+  // Ws = [I + C_i J_j | A_i | b_i + C_i eta_j | C_i]
   for (int e = g.gl; e < n * n; e += G) {
     const int i = e / n, j = e - i * n;
     Ws[i * ld + j] = Tm[i * n1 + j] + (i == j ? 1.0 : 0.0);
@@ -63,46 +104,27 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
     Ws[i * ld + 2 * n + 1 + j] = Ci[i * n + j];
   }
   for (int i = g.gl; i < n; i += G) Ws[i * ld + 2 * n] = Ai[i * n1 + n] + Tm[i * n1 + n];
-  // u = eta_j - J_j b_i
-  for (int i = g.gl; i < n; i += G) {
-    double acc = Jj[i * n1 + n];
-    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(-Jj[i * n1 + l], Ai[l * n1 + n], acc, cmp); acc += cmp; }
-    uv[i] = acc;
-  }
   g.sync();
   gj_solve_np(g, n, ld, Ws, Xs);
   const double* X1 = Xs;             // M A_i           (row stride lx)
   const double* X2 = Xs + n;         // M (b_i + C_i eta_j), then X3 = M C_i follows
-  // [A | b] = A_j [X1 | x2] (+ b_j in the last column)
+  // phase 2: [A | b] = A_j [X1 | x2] (b_j is added in phase 3); Tm = A_j X3
   mm(g, n, n1, n, Aj, n1, 1, X1, lx, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
-  // Tm = A_j X3
-  mm(g, n, n, n, Aj, n1, 1, X2 + 1, lx, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+  mm(g, n, n, n, Aj, n1, 1, X2 + 1, lx, 1, (const double*)nullptr, 0, 0, Tm, n, 1, n * n1);
   g.sync();
-  for (int i = g.gl; i < n; i += G) Ao[i * n1 + n] += Aj[i * n1 + n];
-  // C = Tm A_j^T + C_j
-  mm_sym(g, n, n, Tm, n, 1, Aj, 1, n1, Cj, Co);
-  // eta = X1^T u + eta_i
-  for (int i = g.gl; i < n; i += G) {
+  // phase 3: C = Tm A_j^T + C_j;  J = X1^T T2 + J_i;  eta = X1^T u + eta_i;  b += b_j
+  mm_sym(g, n, n, Tm, n, 1, Aj, 1, n1, Cj, n, Co, n);
+  mm_sym(g, n, n, X1, 1, lx, T2, n, 1, Ji, n1, Jo, n1, ntri);
+  for (int i = G - 1 - g.gl; i < n; i += G) {
     double acc = Ji[i * n1 + n];
     { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * lx + i], uv[l], acc, cmp); acc += cmp; }
     Jo[i * n1 + n] = acc;
-  }
-  g.sync();
-  // Tm = J_j A_i ; J = X1^T Tm + J_i
-  mm(g, n, n, n, Jj, n1, 1, Ai, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
-  g.sync();
-  for (int e = g.gl; e < n * n; e += G) {
-    const int i = e / n, j = e - i * n;
-    if (j > i) continue;
-    double acc = Ji[i * n1 + j];
-    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * lx + i], Tm[l * n + j], acc, cmp); acc += cmp; }
-    Jo[i * n1 + j] = acc;
-    Jo[j * n1 + i] = acc;
+    Ao[i * n1 + n] += Aj[i * n1 + n];
   }
   g.sync();
 }
 
-__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 1) + n * (n + 1) + n + n * (2 * n + 1); }
+__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 1) + n * (n + 1) + n + n * (2 * n + 1) + n * n; }
 
 struct DenseArgs {
   int n;              // augmented state dimension
@@ -129,7 +151,7 @@ __device__ __forceinline__ void foldD_body(const DenseArgs& P) {
   if (gid >= P.batch * P.cout) return;
   double* base = (double*)(smem + tb);
   double* e0 = base; double* e1 = e0 + es; double* e2 = e1 + es;
-  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 1); double* uv = Tm + n * (n + 1); double* Xs = uv + n;
+  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 1); double* uv = Tm + n * (n + 1); double* Xs = uv + n; double* T2 = Xs + n * (2 * n + 1);
   const int64_t series = gid / P.cout, grp = gid - series * P.cout;
   const int64_t m0 = grp * P.g, m1 = (m0 + P.g < P.cin) ? m0 + P.g : P.cin;
   const double* src = P.Ein + (series * P.cin + m0) * (int64_t)es;
@@ -144,7 +166,7 @@ __device__ __forceinline__ void foldD_body(const DenseArgs& P) {
       for (int e = g.gl; e < es; e += NT) nxt[e] = src[e];
       g.sync();
     }
-    dense_combine(g, n, acc, nxt, out, Ws, Tm, uv, Xs);
+    dense_combine(g, n, acc, nxt, out, Ws, Tm, uv, Xs, T2);
     double* t = acc; acc = out; out = t;
   }
   double* dst = P.Eout + gid * (int64_t)es;
@@ -201,7 +223,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       }
       mm(g, n, n, n, A, n1, 1, Xs + 1, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
       g.sync();
-      mm_sym(g, n, n, Tm, n, 1, A, 1, n1, C, st2 + n);
+      mm_sym(g, n, n, Tm, n, 1, A, 1, n1, C, n, st2 + n, n);
       g.sync();
       double* t = st; st = st2; st2 = t;
     }
@@ -241,14 +263,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       }
       mm(g, n, n, n, Je, n, 1, A, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1); // Tm = J_e A
       g.sync();
-      for (int e = g.gl; e < n * n; e += NT) {
-        const int i = e / n, j = e - i * n;
-        if (j > i) continue;
-        double acc = J[i * n1 + j];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * n + i], Tm[l * n + j], acc, cmp); acc += cmp; }
-        st2[n + i * n + j] = acc;
-        st2[n + j * n + i] = acc;
-      }
+      mm_sym(g, n, n, X, 1, n, Tm, n, 1, J, n1, st2 + n, n); // J' = X^T (J_e A) + J
       g.sync();
       double* t = st; st = st2; st2 = t;
     }
