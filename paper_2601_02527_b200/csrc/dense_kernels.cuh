@@ -83,7 +83,7 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const dou
 template <int G>
 __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const double* ej, double* eo,
                               double* Ws, double* Tm, double* uv, double* Xs, double* T2) {
-  const int n1 = n + 1, ld = 3 * n + 1, lx = 2 * n + 1, ntri = n * (n + 1) / 2;
+  const int n1 = n + 1, ld = (3 * n + 1) | 1, lx = 2 * n + 1, ntri = n * (n + 1) / 2; // ld: odd row stride of Ws
   const double *Ai = ei, *Ci = ei + n * n1, *Ji = Ci + n * n;
   const double *Aj = ej, *Cj = ej + n * n1, *Jj = Cj + n * n;
   double *Ao = eo, *Co = eo + n * n1, *Jo = Co + n * n;
@@ -105,7 +105,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   }
   for (int i = g.gl; i < n; i += G) Ws[i * ld + 2 * n] = Ai[i * n1 + n] + Tm[i * n1 + n];
   g.sync();
-  gj_solve_np(g, n, ld, Ws, Xs);
+  gj_solve_np(g, n, 3 * n + 1, ld, Ws, Xs);
   const double* X1 = Xs;             // M A_i           (row stride lx)
   const double* X2 = Xs + n;         // M (b_i + C_i eta_j), then X3 = M C_i follows
   // phase 2: [A | b] = A_j [X1 | x2] (b_j is added in phase 3); Tm = A_j X3
@@ -124,7 +124,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   g.sync();
 }
 
-__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 1) + n * (n + 1) + n + n * (2 * n + 1) + n * n; }
+__host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 2) + n * (n + 1) + n + n * (2 * n + 1) + n * n; }
 
 struct DenseArgs {
   int n;              // augmented state dimension
@@ -151,7 +151,7 @@ __device__ __forceinline__ void foldD_body(const DenseArgs& P) {
   if (gid >= P.batch * P.cout) return;
   double* base = (double*)(smem + tb);
   double* e0 = base; double* e1 = e0 + es; double* e2 = e1 + es;
-  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 1); double* uv = Tm + n * (n + 1); double* Xs = uv + n; double* T2 = Xs + n * (2 * n + 1);
+  double* Ws = e2 + es; double* Tm = Ws + n * (3 * n + 2); double* uv = Tm + n * (n + 1); double* Xs = uv + n; double* T2 = Xs + n * (2 * n + 1);
   const int64_t series = gid / P.cout, grp = gid - series * P.cout;
   const int64_t m0 = grp * P.g, m1 = (m0 + P.g < P.cin) ? m0 + P.g : P.cin;
   const double* src = P.Ein + (series * P.cin + m0) * (int64_t)es;
@@ -214,7 +214,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n1 + j] = Pm[e]; }
       for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + n] += mv[i]; }
       g.sync();
-      gj_solve_np(g, n, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
+      gj_solve_np(g, n, ld, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
       // m' = A x + b ; Tm = A X ; P' = Tm A^T + C
       for (int i = g.gl; i < n; i += NT) {
         double acc = A[i * n1 + n];
@@ -241,7 +241,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       for (int e = g.gl; e < es; e += NT) el[e] = src[e];
       g.sync();
       const double *ev = st, *Je = st + n;
-      const int ld2 = 2 * n;
+      const int ld2 = 2 * n + 1; // odd row stride, 2n columns in use
       // Ws = [I + C J_e | A]
       mm(g, n, n, n, C, n, 1, Je, n, 1, (const double*)nullptr, 0, 0, Ws, ld2, 1);
       g.sync();
@@ -254,7 +254,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
         uv[i] = acc;
       }
       g.sync();
-      gj_solve_np(g, n, ld2, Ws, Xs);
+      gj_solve_np(g, n, 2 * n, ld2, Ws, Xs);
       const double* X = Xs; // M A, row stride n
       for (int i = g.gl; i < n; i += NT) {
         double acc = J[i * n1 + n];

@@ -105,9 +105,10 @@ __device__ void gj_solve(const Grp<G>& g, int n, int ld, double* W) {
 // a barrier), the row stays where it is and only its index is recorded.  Elimination p writes columns > p of
 // the other rows and reads column p and row r only, so ONE barrier per pivot (before the next search) is
 // enough, against three in gj_solve.  Same pivots, hence the same arithmetic per entry, as gj_solve.
-// W = [M | R] (n rows, ld = n + m columns) is destroyed; X (n x m, row stride m) receives M^-1 R.
+// W = [M | R] (n rows, nc_all = n + m columns, row stride ld >= nc_all: an odd ld keeps the column reads of the
+// pivot search and the row pairs of a warp off the same banks) is destroyed; X (n x m, row stride m) receives M^-1 R.
 template <int G>
-__device__ void gj_solve_np(const Grp<G>& g, int n, int ld, double* W, double* X) {
+__device__ void gj_solve_np(const Grp<G>& g, int n, int nc_all, int ld, double* W, double* X) {
   __shared__ int rowof[32];
   const int lane = threadIdx.x & 31;
   unsigned used = 0u;
@@ -124,7 +125,7 @@ __device__ void gj_solve_np(const Grp<G>& g, int n, int ld, double* W, double* X
     used |= 1u << r;
     if (g.gl == 0) rowof[p] = r;
     const double rpv = 1.0 / W[r * ld + p];
-    const int nc = ld - p - 1;
+    const int nc = nc_all - p - 1;
     const float rnc = 1.0f / (float)nc;
     const int tot = (n - 1) * nc;
     for (int e = g.gl; e < tot; e += G) {
@@ -136,7 +137,7 @@ __device__ void gj_solve_np(const Grp<G>& g, int n, int ld, double* W, double* X
     }
     g.sync();
   }
-  const int m = ld - n;
+  const int m = nc_all - n;
   const float rm = 1.0f / (float)m;
   for (int e = g.gl; e < n * m; e += G) {
     int i, j;
