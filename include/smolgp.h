@@ -151,7 +151,9 @@ int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kernel, int32_t
 int64_t smolgp_launch_count(const smolgp_ctx* ctx);
 
 /* Per-kernel device timing for bench.py's roofline block.  smolgp_profile(ctx, 1) starts a window in
- * which every kernel this ctx launches is bracketed by CUDA events on the ctx stream;
+ * which every kernel this ctx launches is bracketed by CUDA events on the ctx stream (two event records per
+ * launch: about 0.25 ms per step of config 3, so a headline is not timed in this mode);
+ * smolgp_profile(ctx, 2 + id) brackets only the launches of kernel id (EINVAL outside [0, SMOLGP_NKERNELS));
  * smolgp_profile_read synchronises the stream, writes the summed milliseconds and launch counts per
  * kernel id (HOST arrays of SMOLGP_NKERNELS entries; names from smolgp_kernel_name) and clears the
  * window; smolgp_profile(ctx, 0) stops.  smolgp_kernel_name returns NULL outside [0, SMOLGP_NKERNELS). */

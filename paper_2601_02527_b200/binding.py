@@ -138,7 +138,10 @@ class Context:
         return int(lib().smolgp_launch_count(self.handle))
 
     def profile(self, enable):
-        self._check(lib().smolgp_profile(self.handle, int(bool(enable))))
+        """False/0: off; True/1: every kernel; a kernel name: only that kernel's launches"""
+        if isinstance(enable, str):
+            enable = 2 + [lib().smolgp_kernel_name(i).decode() for i in range(NKERNELS)].index(enable)
+        self._check(lib().smolgp_profile(self.handle, int(enable)))
 
     def profile_read(self):
         """{kernel name: (milliseconds, launches)} of the window since profile(True) / the last read"""

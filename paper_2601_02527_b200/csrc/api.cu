@@ -29,7 +29,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return SMOLGP_ECUDA; }
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
-  c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0;
+  c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0; c->prof_cur = 0;
   c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
   // pinned: the per-call model upload is a true asynchronous copy
   if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
@@ -77,7 +77,8 @@ extern "C" int smolgp_profile(smolgp_ctx* ctx, int32_t enable) {
   if (!ctx) return SMOLGP_EINVAL;
   for (auto& r : ctx->prof) { ctx->evpool.push_back(r.a); ctx->evpool.push_back(r.b); }
   ctx->prof.clear();
-  ctx->prof_on = enable ? 1 : 0;
+  if (enable < 0 || enable >= 2 + KID_COUNT) return SMOLGP_EINVAL;
+  ctx->prof_on = enable;
   return SMOLGP_OK;
 }
 

@@ -74,7 +74,8 @@ struct smolgp_ctx {
   cudaStream_t stream;
   std::string err;
   int64_t launches;
-  int prof_on;
+  int prof_on;   // 0 off, 1 every kernel, 2 + id: only kernel id (smolgp_profile)
+  int prof_cur;  // the launch in flight is being timed
   std::vector<ProfRec> prof;       // open records of the current profiling window
   std::vector<cudaEvent_t> evpool; // recycled events
   int64_t opt_chunk, opt_group, opt_lanes, opt_top, opt_jit; // opt_jit: 0 automatic, 1 always, -1 never
@@ -93,7 +94,8 @@ struct smolgp_ctx {
 // bracket a kernel launch: counts it and, when profiling is on, times it with CUDA events on the ctx stream
 static inline void sg_launch_begin(smolgp_ctx* ctx, int id) {
   ctx->launches++;
-  if (!ctx->prof_on) return;
+  ctx->prof_cur = ctx->prof_on == 1 || ctx->prof_on == 2 + id;
+  if (!ctx->prof_cur) return;
   ProfRec r; r.id = id;
   cudaEvent_t* e[2] = {&r.a, &r.b};
   for (int i = 0; i < 2; ++i) {
@@ -104,7 +106,8 @@ static inline void sg_launch_begin(smolgp_ctx* ctx, int id) {
   ctx->prof.push_back(r);
 }
 static inline void sg_launch_end(smolgp_ctx* ctx) {
-  if (ctx->prof_on && !ctx->prof.empty()) cudaEventRecord(ctx->prof.back().b, ctx->stream);
+  if (ctx->prof_cur && !ctx->prof.empty()) cudaEventRecord(ctx->prof.back().b, ctx->stream);
+  ctx->prof_cur = 0;
 }
 
 #define SG_CUDA(ctx, call)                                                            \
