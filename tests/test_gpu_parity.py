@@ -497,3 +497,31 @@ def test_tiered_specialisation_keeps_results(ctx, oracle):
     ref = PU.reference(oracle, w)
     e = PU.errors(ref, last["loglik"][0], last["mean"][0], last["var"][0])
     assert e["ll"] <= PU.LL_RTOL and e["mean"] <= PU.POST_RTOL and e["var"] <= PU.POST_RTOL, e
+
+
+def test_profile_modes(ctx):
+    """smolgp_profile (include/smolgp.h): 1 brackets every launch, 2 + id only the launches of kernel id (what
+    bench.py uses inside its timed region), 0 none; the launch counter counts in every mode"""
+    w = W.make(2, N=2000)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    try:
+        ctx.set_option("chunk", 32)
+        ctx.profile(True)
+        l0 = ctx.launch_count()
+        ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])
+        n_launch = ctx.launch_count() - l0
+        every = ctx.profile_read()
+        assert {"k_disc", "k_fold0", "k_foldD", "k_downD", "k_down0"} <= set(every)
+        assert sum(c for _, c in every.values()) == n_launch
+        ctx.profile("k_down0")
+        ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])
+        one = ctx.profile_read()
+        assert set(one) == {"k_down0"} and one["k_down0"][1] == every["k_down0"][1] and one["k_down0"][0] > 0.0
+        ctx.profile(False)
+        ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"])
+        assert ctx.profile_read() == {}
+        with pytest.raises(Exception):
+            ctx.profile(2 + 1000)
+    finally:
+        ctx.profile(False)
+        _reset(ctx)
