@@ -113,15 +113,16 @@ __device__ void gj_solve_np(const Grp<G>& g, int n, int nc_all, int ld, double* 
   const int lane = threadIdx.x & 31;
   unsigned used = 0u;
   for (int p = 0; p < n; ++p) {
-    double v = (lane < n && !((used >> lane) & 1u)) ? fabs(W[lane * ld + p]) : -1.0;
-    int r = lane;
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-      const double ov = __shfl_xor_sync(0xffffffffu, v, o);
-      const int orow = __shfl_xor_sync(0xffffffffu, r, o);
-      if (ov > v || (ov == v && orow < r)) { v = ov; r = orow; }
-    }
-    r = min(__shfl_sync(0xffffffffu, r, 0), n - 1); // non-finite input: still one in-range row for the whole CTA
+    // arg-max of |W[., p]| over the unused rows: the bit pattern of a non-negative double orders like the value,
+    // so the maximum is two 32-bit warp reductions (high word, then low word among the lanes that hold the
+    // maximal high word) and a ballot; ties go to the lowest row
+    const bool cand = lane < n && !((used >> lane) & 1u);
+    const unsigned long long key = cand ? (unsigned long long)__double_as_longlong(fabs(W[lane * ld + p])) + 1ull : 0ull;
+    const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+    const unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
+    const unsigned hit = __ballot_sync(0xffffffffu, hi == mhi && lo == mlo);
+    int r = min(__ffs(hit) - 1, n - 1); // non-finite input: still one in-range row for the whole CTA
     used |= 1u << r;
     if (g.gl == 0) rowof[p] = r;
     const double rpv = 1.0 / W[r * ld + p];
