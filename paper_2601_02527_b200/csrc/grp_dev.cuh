@@ -101,7 +101,7 @@ __device__ void gj_solve(const Grp<G>& g, int n, int ld, double* W) {
 // Gauss-Jordan with partial pivoting and NO row exchange, for a group that is a whole CTA (G > 32, n <= 32):
 // the dense levels run one solve per combine on the latency-critical path, so the barriers per pivot count.
 // The pivot of column p is the largest entry among the rows not yet used as a pivot; it is found by every
-// warp on its own (lane l holds row l, shuffle arg-max, ties to the lower row, so all warps agree without
+// warp on its own (lane l holds row l, warp-reduction arg-max, ties to the lower row, so all warps agree without
 // a barrier), the row stays where it is and only its index is recorded.  Elimination p writes columns > p of
 // the other rows and reads column p and row r only, so ONE barrier per pivot (before the next search) is
 // enough, against three in gj_solve.  Same pivots, hence the same arithmetic per entry, as gj_solve.
