@@ -26,7 +26,40 @@ sys.path.insert(0, ROOT)
 
 from paper_2601_02527_b200 import workloads as W  # noqa: E402
 
-FP64_PEAK_TFLOPS = 37.2  # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz
+FP64_PEAK_DERIVED_TFLOPS = 37.2  # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz; the line's `peak` is MEASURED
+
+
+def fp64_probe(device):
+    """plain-ALU FP64 FMA throughput of this device, measured now (TFLOP/s): the roofline denominator.
+    MEASURED_PEAKS.json has no FP64 entry; the probe is bench.py's own tool (csrc/probe_fp64.cu)."""
+    import ctypes
+    from paper_2601_02527_b200 import _build
+    L = ctypes.CDLL(_build.build_probe())
+    v = ctypes.c_double()
+    rc = L.sgprobe_fp64(int(device), 5, ctypes.byref(v))
+    if rc != 0:
+        raise RuntimeError("fp64 probe failed: cuda error %d" % rc)
+    return v.value
+
+
+def hbm_peak_gbs():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except (OSError, ValueError, KeyError):
+        return 6545.9, "fallback (SURVEY 0: 6545.9 GB/s)"
+
+
+def kernel_source_hash():
+    """hash of the chunk / dense kernel sources: an ncu capture under profiles/ is only quoted for the
+    build it was taken from"""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "chunk_reg.cuh", "dense_kernels.cuh", "scan_host.cu"):
+        try:
+            h.update(open(os.path.join(ROOT, "paper_2601_02527_b200", "csrc", f), "rb").read())
+        except OSError:
+            pass
+    return h.hexdigest()[:16]
 
 
 def w_useful_flops(n):
@@ -41,14 +74,20 @@ def min_bytes(n):
     return 32 + 2 * 8 * (n + n * (n + 1) // 2)
 
 
-def ncu_traffic(kernel, cfg):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/r01_top_kernel_traffic.json; config 3 only), else None"""
+def ncu_capture(kernel, cfg):
+    """(dram bytes per launch, executed-DFMA fraction of the FP64 peak, source) of the dominant kernel from the
+    committed ncu --set full capture of THIS build (profiles/r02_top_kernel_capture.json: config 3 only; the
+    capture records the hash of the kernel sources it was taken from), else (None, None, why)"""
+    path = os.path.join(ROOT, "profiles", "r02_top_kernel_capture.json")
     try:
-        rec = json.load(open(os.path.join(ROOT, "profiles", "r01_top_kernel_traffic.json")))
-        return rec["traffic_bytes_per_launch"] if (rec["kernel"] == kernel and cfg == 3) else None
-    except (OSError, ValueError, KeyError):
-        return None
+        rec = json.load(open(path))
+    except (OSError, ValueError):
+        return None, None, "no capture file"
+    if cfg != 3 or rec.get("kernel") != kernel:
+        return None, None, "capture is of %s on config 3" % rec.get("kernel")
+    if rec.get("source_hash") != kernel_source_hash():
+        return None, None, "capture is stale (kernel sources changed since profiles/r02_top_kernel_capture.json)"
+    return rec.get("traffic_bytes_per_launch"), rec.get("dfma_frac_of_peak"), "profiles/r02_top_kernel_capture.json"
 
 
 def model_dim(w):
@@ -104,17 +143,32 @@ class ClockSampler:
 # as it stands, single thread (the recursion is sequential in k), on a bounded sample = the first
 # `n_sample` exposures of the workload.
 # ----------------------------------------------------------------------------------------------
-def oracle_step(w, n_sample):
+def oracle_step(w, n_sample, series=0, split=False):
+    """one pass of the fp64 oracle over the first n_sample exposures of series `series`; seconds (and, with
+    split, the seconds of that pass spent in the discretisation: oracle instrumentation)"""
     import oracle
     sl = slice(0, n_sample)
-    y = w["y"][0, sl] if w["y"].ndim == 2 else w["y"][sl]
+    y = w["y"][series, sl] if w["y"].ndim == 2 else w["y"][sl]
     kern = w["kernel"]
     if w.get("amp") is not None:
-        kern = [dict(k, sigma=k["sigma"] * float(w["amp"][0])) for k in kern]
+        kern = [dict(k, sigma=k["sigma"] * float(w["amp"][series])) for k in kern]
     t0 = time.perf_counter()
-    oracle.ssm(kern, w["n_inst"], w["t_start"][sl], w["t_end"][sl], w["instrument"][sl], y, w["sigma"][sl],
-               flags=oracle.FLAG_IDLE_ZERO | oracle.FLAG_TWO_FILTER, prec="f64")
-    return time.perf_counter() - t0
+    r = oracle.ssm(kern, w["n_inst"], w["t_start"][sl], w["t_end"][sl], w["instrument"][sl], y, w["sigma"][sl],
+                   flags=oracle.FLAG_IDLE_ZERO | oracle.FLAG_TWO_FILTER, prec="f64")
+    dt = time.perf_counter() - t0
+    return (dt, r["disc_seconds"]) if split else dt
+
+
+def oracle_all_cores(w, n_series, n_sample):
+    """batched workloads on all host cores, one series per thread (the C call releases the GIL).
+    Returns (events/s, threads used, seconds)."""
+    from concurrent.futures import ThreadPoolExecutor
+    threads = min(os.cpu_count() or 1, n_series)
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(lambda s: oracle_step(w, n_sample, series=s), range(n_series)))
+    dt = time.perf_counter() - t0
+    return 2.0 * n_sample * n_series / dt, threads, dt
 
 
 def oracle_sample_size(w, target_s):
@@ -269,7 +323,9 @@ def run_cuda(args, w, cfgname):
     barrier()
     ms_e2e = sum(a.elapsed_time(b) for a, b in evs2)
     clocks = sampler.stop() if rank == 0 else None
-    fp64_probe = ctx.probe_fp64() if rank == 0 else None
+    peak = fp64_probe(local) if rank == 0 else None
+    plan = ctx.plan_info()
+    jit_log = ctx.jit_log()
 
     ms, ms_e2e = max_over_ranks([ms, ms_e2e], world, dev)
     if rank != 0:
@@ -278,39 +334,61 @@ def run_cuda(args, w, cfgname):
         return
     value = aggregate_throughput(K_events, args.steps, ms, world)
     e2e_value = aggregate_throughput(K_events, args.steps, ms_e2e, world)
-    # ---- roofline of the dominant kernel (device time from the ctx's own CUDA events) ----
+    # ---- roofline.  Three fractions, none to be mistaken for another:
+    #   frac            : the dominant kernel credited with the whole path's USEFUL work, W_useful x the
+    #                     events of one launch / its average duration (CUDA events on the ctx stream, timed region);
+    #   frac_whole_step : SURVEY 8(d)'s headline fraction T_roof / t_measured over the WHOLE step;
+    #   frac_executed_dfma : DFMA actually executed by that kernel (ncu capture of this build under profiles/).
     t_top_ms = prof_top[0] / prof_top[1]             # average launch duration over the timed region
     launches_per_step = prof_top[1] / args.steps
     flops_launch = K_events * w_useful_flops(n) / launches_per_step
     achieved = flops_launch / (t_top_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(top, args.config),
-                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md); register-only DFMA probe measured %.1f TFLOP/s in this run" % fp64_probe,
-                "work_model": "W_useful = 10.3 n^3 + 9 n^2 flop/event (SURVEY 8(d)), n = %d" % n,
+    hbm_gbs, hbm_src = hbm_peak_gbs()
+    t_step = ms / args.steps * 1e-3
+    t_roof = max(K_events * w_useful_flops(n) / (peak * 1e12), K_events * min_bytes(n) / (hbm_gbs * 1e9))
+    traffic, dfma_frac, cap_src = ncu_capture(top, args.config)
+    roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": traffic,
+                "frac_whole_step": t_roof / t_step, "frac_executed_dfma": dfma_frac, "capture": cap_src,
+                "peak_source": "measured in this run: register-only FP64 FMA probe (csrc/probe_fp64.cu), best of 5; "
+                               "derived figure 148 SM x 64 FMA/clk x 2 x 1.965 GHz = %.1f TFLOP/s" % FP64_PEAK_DERIVED_TFLOPS,
+                "work_model": "W_useful = 10.3 n^3 + 9 n^2 flop/event (SURVEY 8(d)), n = %d; `frac` credits the dominant kernel with "
+                              "the whole path's useful work, `frac_whole_step` = T_roof / t_measured of the whole step, "
+                              "`frac_executed_dfma` = executed DFMA of the dominant kernel (ncu)" % n,
                 "kernel_share_of_step": prof_top[0] / ms,
                 "timing": "dominant kernel: CUDA events on the ctx stream around its launches inside the timed region; "
                           "kernels_ms_per_step: a second pass of the same steps with every launch bracketed, %.3f ms/step "
                           "(the event records cost the difference to ms_per_step, so the headline loop does not carry them)" % (ms_bracketed / args.steps),
-                "hbm": {"min_bytes_per_event": min_bytes(n), "achieved_gbs": K_events * min_bytes(n) * args.steps / (ms * 1e-3) / 1e9},
+                "hbm": {"min_bytes_per_event": min_bytes(n), "achieved_gbs": K_events * min_bytes(n) * args.steps / (ms * 1e-3) / 1e9,
+                        "peak_gbs": hbm_gbs, "peak_source": hbm_src},
                 "kernels_ms_per_step": {k: v[0] / args.steps for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
-    # ---- CPU baseline: the oracle as it stands, bounded sample ----
+    # ---- CPU baseline: the oracle as it stands, bounded sample; discretisation and filter/smoother seconds apart
+    #      (BASELINE.md 3); batched workloads also on all host cores, one series per thread ----
     import oracle
     oracle.build()
     ns = oracle_sample_size(w, 12.0)
-    t_cpu = oracle_step(w, ns)
+    t_cpu, t_disc = oracle_step(w, ns, split=True)
     cpu = {"value": 2.0 * ns / t_cpu, "unit": "events/s", "cores": 1, "kind": "oracle",
+           "seconds": {"total": t_cpu, "discretisation": t_disc, "filter_smoother": t_cpu - t_disc},
            "sample": "first %d of %d exposures (%d events), oracle fp64 build, sequential filter + two-filter smoother, 1 thread, %.1f s" % (ns, N, 2 * ns, t_cpu)}
+    if batch > 1:
+        nser = min(batch, 4 * (os.cpu_count() or 1))
+        v_all, thr, t_all = oracle_all_cores(w, nser, min(ns, N))
+        cpu["all_cores"] = {"value": v_all, "unit": "events/s", "cores": thr,
+                            "sample": "%d series x first %d exposures, one series per thread, %.1f s" % (nser, min(ns, N), t_all)}
     line = {"metric": "events/sec for loglik+RTS smoother at N=1e5", "value": value, "unit": "events/s",
             "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfgname, "N": N, "events": 2 * N, "batch": batch, "state_dim": n,
                        "path": "a1 build_events + a2 discretise + a3 filter scan + a4 smoother + a5 loglik + a6 posterior",
-                       "l2": "flushed (512 MiB write) between timed iterations", "parallelism": "replicas x%d" % world},
+                       "l2": "flushed (512 MiB write) between timed iterations", "parallelism": "replicas x%d" % world,
+                       "plan": plan},
             "e2e": {"value": e2e_value, "unit": "events/s",
                     "h2d_bytes_per_step": int(hts.nbytes + hte.nbytes + hins.nbytes + hy.nbytes + hsg.nbytes + (0 if hamp is None else hamp.nbytes)),
                     "d2h_bytes_per_step": int(hout["mean"].nbytes + hout["var"].nbytes + hout["loglik"].nbytes),
                     "ms_per_step": ms_e2e / args.steps},
-            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+            "gpu_launches": int(launches), "specialised": "jit=1" in plan, "jit_log": jit_log,
+            "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
             "loglik": float(hout["loglik"][0])}
     print(json.dumps(line), flush=True)
     if world > 1:

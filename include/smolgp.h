@@ -33,7 +33,7 @@ extern "C" {
 
 typedef enum {
   SMOLGP_OK = 0,
-  SMOLGP_EINVAL = -1,       /* bad argument: N<=0, non-finite time, t_end<=t_start, instrument out of range, sigma<=0 */
+  SMOLGP_EINVAL = -1,       /* bad argument: N<=0, non-finite time, t_end<=t_start, instrument out of range, sigma<=0, amp<=0 */
   SMOLGP_EOVERLAP = -2,     /* an instrument overlaps itself (t_n^e > t_{n+1}^s) */
   SMOLGP_EUNSUPPORTED = -3, /* augmented dimension above SMOLGP_MAX_DIM, unknown family, too many instruments */
   SMOLGP_ENOMEM = -4,
@@ -89,14 +89,20 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);
 const char* smolgp_jit_log(smolgp_ctx* ctx);
+/* The scan plan of the last smolgp_loglik / smolgp_condition call of this ctx, as a ctx-owned string
+ * "n=21 batch=1 K=200000 chunk=136 chunks=1471 levels=10 fanin=2 lanes=8 cpl=3 jit=1 kernels=reg": which kernels
+ * ran (jit=1: the run-time specialised ones) and how the events were cut.  For bench.py and the tests. */
+const char* smolgp_plan_info(const smolgp_ctx* ctx);
 
 /* Step a1.  Turns N exposures [t_start[n], t_end[n]] of instrument
  * instrument[n] in [0, n_inst) into the time-sorted stream of K = 2N events (one reset event per
- * start, one observe event per end; at equal times ends come before starts so that back-to-back
- * exposures of one instrument, the Fig. 2 case P:543, are legal).  Device radix sort on the
- * order-preserving 64-bit image of the times; the reset/observe flags, the per-event set of idle
- * instruments and the validation that no instrument overlaps itself come from an
- * exclusive XOR scan of the instrument bits.  The three inputs are DEVICE pointers; the result
+ * start, one observe event per end).  ORDER OF THE STREAM: by (time, end before start, instrument,
+ * exposure index), whatever the order of the input arrays -- ends come before starts at equal times so
+ * that back-to-back exposures of one instrument, the Fig. 2 case P:543, are legal; simultaneous events
+ * of the same kind are ordered by instrument, then by exposure index (-0.0 and +0.0 are one time).  Device radix sort (stable, least significant digit
+ * first: (kind, instrument), then the bytes of the order-preserving 64-bit image of the times; digits on
+ * which all keys agree are skipped); the reset/observe flags, the per-event set of idle instruments and
+ * the validation that no instrument overlaps itself come from an XOR scan of the instrument bits.  The three inputs are DEVICE pointers; the result
  * is owned by the caller (smolgp_free_events; free it before destroying the ctx whose stream it was
  * allocated on) and can be reused across kernels and data.
  * Errors: EINVAL, EOVERLAP, EUNSUPPORTED (n_inst > SMOLGP_MAX_INST), ENOMEM, ECUDA. */
@@ -157,14 +163,10 @@ int64_t smolgp_launch_count(const smolgp_ctx* ctx);
  * smolgp_profile_read synchronises the stream, writes the summed milliseconds and launch counts per
  * kernel id (HOST arrays of SMOLGP_NKERNELS entries; names from smolgp_kernel_name) and clears the
  * window; smolgp_profile(ctx, 0) stops.  smolgp_kernel_name returns NULL outside [0, SMOLGP_NKERNELS). */
-#define SMOLGP_NKERNELS 17
+#define SMOLGP_NKERNELS 11
 int smolgp_profile(smolgp_ctx* ctx, int32_t enable);
 int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launches);
 const char* smolgp_kernel_name(int32_t id);
-
-/* FP64 FMA throughput probe (roofline denominator): runs a register-only
- * DFMA kernel on the ctx stream and returns the achieved TFLOP/s in *tflops. */
-int smolgp_probe_fp64(smolgp_ctx* ctx, double* tflops);
 
 #ifdef __cplusplus
 }

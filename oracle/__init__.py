@@ -157,4 +157,6 @@ def ssm(kern, ninst, ts, te, inst, y, sigma, flags=FLAG_TWO_FILTER, zprior=1.0, 
            ptr(var), ptr(mq), ptr(vq))
     if rc != 0:
         raise RuntimeError("oracle_ssm rc=%d" % rc)
-    return dict(loglik=ll.value, mean=mean, var=var, mq=mq, vq=vq)
+    g = _lib(prec).oracle_ssm_disc_seconds  # instrumentation: seconds of this call spent in the discretisation
+    g.restype = C.c_double
+    return dict(loglik=ll.value, mean=mean, var=var, mq=mq, vq=vq, disc_seconds=float(g()))

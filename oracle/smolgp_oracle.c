@@ -29,6 +29,7 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 
 #ifdef REAL_IS_LONG_DOUBLE
 typedef long double real;
@@ -693,6 +694,22 @@ int oracle_events(int N, const double *ts, const double *te, const int32_t *inst
 #define FLAG_IDLE_ZERO 1  /* also zero z_i at every event after which instrument i is idle (R6) */
 #define FLAG_TWO_FILTER 2 /* backward pass in two-filter (information) form instead of RTS (R7) */
 
+/* Instrumentation for bench.py's cpu_baseline split (discretisation and filter/smoother
+ * time reported separately); no arithmetic.  Seconds spent inside disc_model during the last
+ * oracle_ssm call made by the calling thread. */
+static __thread double g_disc_seconds;
+static double now_seconds(void) {
+  struct timespec ts;
+  clock_gettime(CLOCK_MONOTONIC, &ts);
+  return (double)ts.tv_sec + 1e-9 * (double)ts.tv_nsec;
+}
+static void disc_model_timed(const model *M, real dt, real *A, real *Q) {
+  double t0 = now_seconds();
+  disc_model(M, dt, A, Q);
+  g_disc_seconds += now_seconds() - t0;
+}
+double oracle_ssm_disc_seconds(void) { return g_disc_seconds; }
+
 /* zero entry j of a mean and row+column j of a covariance: the reset R_i of Eq. 3.18 */
 static void zero_state(int n, real *m, real *P, int j) {
   m[j] = 0;
@@ -709,6 +726,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
                int flags, double zprior, int M, const double *tq, int query_inst,
                double *loglik, double *mean, double *var, double *mq, double *vq) {
   model Md;
+  g_disc_seconds = 0;
   if (build_model(&Md, ncomp, comp, ninst)) return -1;
   const int n = Md.n, d = Md.d, nn = n * n, K = 2 * N;
   const int want_smooth = (mean || var || M > 0);
@@ -756,7 +774,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
   /* ------------------------------ forward: integrated Kalman filter ---------------------- */
   for (int k = 0; k < K; ++k) {
     real dt = k == 0 ? 0 : (real)ev[k].t - (real)ev[k - 1].t;
-    disc_model(&Md, dt, A, Q);
+    disc_model_timed(&Md, dt, A, Q);
     /* predict, Eq. 3.14 */
     mv(n, A, m, T1);
     memcpy(m, T1, sizeof(real) * n);
@@ -798,7 +816,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
     memcpy(MS(K - 1), MX(K - 1), sizeof(real) * per); /* last event is an end: P:231 */
     for (int k = K - 2; k >= 0; --k) {
       real dt = (real)ev[k + 1].t - (real)ev[k].t;
-      disc_model(&Md, dt, A, Q);
+      disc_model_timed(&Md, dt, A, Q);
       real Tm[MAXN * MAXN];
       memcpy(Tm, A, sizeof(real) * nn);
       for (int j = d; j < n; ++j) {
@@ -870,7 +888,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
         eta[zi] += (real)y[e] / (delta * r);
       }
       real dt = k == 0 ? 0 : (real)ev[k].t - (real)ev[k - 1].t;
-      disc_model(&Md, dt, A, Q);
+      disc_model_timed(&Md, dt, A, Q);
       real JA[MAXN * (MAXN + 1)], e2[MAXN];
       mm(n, J, Q, Tm);
       for (int i = 0; i < n; ++i) Tm[i * n + i] += 1;
@@ -905,7 +923,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
       real ms_[MAXN], Ps_[MAXN * MAXN], Gt[MAXN * MAXN], G[MAXN * MAXN], dm[MAXN], D[MAXN * MAXN];
       double t = tq[q];
       if (t < ev[0].t) { /* lines 3-9, on the x-block: m* = 0, P* = Pinf, P_1^- = Pinf */
-        disc_model(&Md, (real)ev[0].t - (real)t, A, Q);
+        disc_model_timed(&Md, (real)ev[0].t - (real)t, A, Q);
         real Ax[MAXN * MAXN] = {0}, Ppred[MAXN * MAXN];
         for (int i = 0; i < d; ++i)
           for (int j = 0; j < d; ++j) Ax[i * n + j] = A[i * n + j];
@@ -940,7 +958,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
         if (flags & FLAG_IDLE_ZERO)
           for (int qq = 0; qq < ninst; ++qq)
             if (!opst[(size_t)kp * ninst + qq]) zero_state(n, mc, Pc, d + qq);
-        disc_model(&Md, (real)t - (real)ev[kp].t, A, Q); /* lines 14-18 / 23-27 */
+        disc_model_timed(&Md, (real)t - (real)ev[kp].t, A, Q); /* lines 14-18 / 23-27 */
         mv(n, A, mc, mstar);
         mm(n, A, Pc, T1);
         mmt(n, T1, A, T2);
@@ -951,7 +969,7 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
         } else { /* interpolate: one smoothing step from the next state's (smoothed, predicted) */
           int kn = kp + 1;
           real Ppn[MAXN * MAXN], mpn[MAXN], Pm[MAXN * MAXN];
-          disc_model(&Md, (real)ev[kn].t - (real)t, A, Q);
+          disc_model_timed(&Md, (real)ev[kn].t - (real)t, A, Q);
           mv(n, A, mstar, mpn);
           mm(n, A, Pstar, T1);
           mmt(n, T1, A, T2);

@@ -5,6 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsmolgp_b200.so")
+PROBE_SO = os.path.join(HERE, "libsmolgp_probe.so")  # bench.py's FP64 throughput probe (not part of the product library)
 SOURCES = ["api.cu", "model.cu", "events.cu", "disc.cu", "scan.cu", "jit.cu"]
 JIT_PARTS = ["dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "dense_kernels.cuh"]  # run-time specialised source, in order
 DEPS = SOURCES + ["common.h", "dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "dense_kernels.cuh", "jit.h", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
@@ -61,6 +62,15 @@ def build(force=False, verbose=False):
             print(out.decode())
     subprocess.check_call([nvcc, "-shared", "-o", SO, *objs, "-lcudart", "-ldl"])
     return SO
+
+
+def build_probe(force=False):
+    """bench.py's measurement tool: a register-only FP64 FMA loop, its own shared object"""
+    src = os.path.join(CSRC, "probe_fp64.cu")
+    if force or not os.path.exists(PROBE_SO) or os.path.getmtime(PROBE_SO) < os.path.getmtime(src):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        subprocess.check_call([nvcc, *NVCC_FLAGS, "-shared", src, "-o", PROBE_SO, "-lcudart"])
+    return PROBE_SO
 
 
 if __name__ == "__main__":

@@ -14,8 +14,8 @@ STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
            "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
-           "smolgp_launch_count", "smolgp_probe_fp64", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log"]
-NKERNELS = 17
+           "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info"]
+NKERNELS = 11  # SMOLGP_NKERNELS
 
 
 class SmolgpError(RuntimeError):
@@ -61,13 +61,14 @@ def lib():
         L.smolgp_discretise_host.argtypes = [vp, C.POINTER(_Kernel), i32, C.c_double, dp, dp, C.POINTER(i32)]
         L.smolgp_launch_count.argtypes = [vp]
         L.smolgp_launch_count.restype = i64
-        L.smolgp_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
         L.smolgp_profile.argtypes = [vp, i32]
         L.smolgp_profile_read.argtypes = [vp, dp, dp]
         L.smolgp_kernel_name.argtypes = [i32]
         L.smolgp_kernel_name.restype = C.c_char_p
         L.smolgp_jit_log.argtypes = [vp]
         L.smolgp_jit_log.restype = C.c_char_p
+        L.smolgp_plan_info.argtypes = [vp]
+        L.smolgp_plan_info.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -80,16 +81,29 @@ def _kernel(kernel):
     return _Kernel(len(kernel), arr), arr
 
 
-def _dptr(t):
-    """device pointer of a contiguous torch CUDA tensor (None -> NULL)"""
+def _dptr(t, dtype="float64", numel=None, name="argument"):
+    """device pointer of a contiguous torch CUDA tensor (None -> NULL).  The C ABI sees plain pointers: dtype
+    and element count are checked here, where they are still known."""
     if t is None:
         return None
-    assert t.is_cuda and t.is_contiguous(), "expected a contiguous CUDA tensor"
+    if not (t.is_cuda and t.is_contiguous()):
+        raise TypeError("%s: expected a contiguous CUDA tensor" % name)
+    if str(t.dtype) != "torch." + dtype:
+        raise TypeError("%s: expected dtype %s, got %s" % (name, dtype, t.dtype))
+    if numel is not None and t.numel() != numel:
+        raise ValueError("%s: expected %d elements, got %d" % (name, numel, t.numel()))
     return t.data_ptr()
 
 
-def _hptr(a):
-    return None if a is None else a.ctypes.data
+def _hptr(a, numel=None, name="argument"):
+    """host pointer of a C-contiguous numpy array (None -> NULL); float64 / int32 arrays only"""
+    if a is None:
+        return None
+    if not a.flags["C_CONTIGUOUS"] or a.dtype not in (np.float64, np.int32, np.int64):
+        raise TypeError("%s: expected a C-contiguous float64 / int32 array" % name)
+    if numel is not None and a.size != numel:
+        raise ValueError("%s: expected %d elements, got %d" % (name, numel, a.size))
+    return a.ctypes.data
 
 
 class Events:
@@ -152,24 +166,24 @@ class Context:
     def jit_log(self):
         return lib().smolgp_jit_log(self.handle).decode()
 
-    def probe_fp64(self):
-        v = C.c_double()
-        self._check(lib().smolgp_probe_fp64(self.handle, C.byref(v)))
-        return v.value
+    def plan_info(self):
+        return lib().smolgp_plan_info(self.handle).decode()
 
     # ---- a1 ----
     def smolgp_build_events(self, t_start, t_end, instrument, n_inst):
         """device tensors: t_start, t_end float64 [N]; instrument int32 [N]"""
         N = t_start.numel()
         h = C.c_void_p()
-        self._check(lib().smolgp_build_events(self.handle, N, _dptr(t_start), _dptr(t_end), _dptr(instrument), int(n_inst), C.byref(h)))
+        self._check(lib().smolgp_build_events(self.handle, N, _dptr(t_start, name="t_start"), _dptr(t_end, numel=N, name="t_end"),
+                                              _dptr(instrument, "int32", N, "instrument"), int(n_inst), C.byref(h)))
         return Events(self, h, N, n_inst)
 
     def smolgp_build_events_host(self, t_start, t_end, instrument, n_inst):
         ts, te = np.ascontiguousarray(t_start, np.float64), np.ascontiguousarray(t_end, np.float64)
         ins = np.ascontiguousarray(instrument, np.int32)
         h = C.c_void_p()
-        self._check(lib().smolgp_build_events_host(self.handle, ts.size, _hptr(ts), _hptr(te), _hptr(ins), int(n_inst), C.byref(h)))
+        self._check(lib().smolgp_build_events_host(self.handle, ts.size, _hptr(ts), _hptr(te, ts.size, "t_end"), _hptr(ins, ts.size, "instrument"),
+                                                   int(n_inst), C.byref(h)))
         return Events(self, h, ts.size, n_inst)
 
     # ---- a2-a5 ----
@@ -179,7 +193,9 @@ class Context:
         if out is None:
             out = torch.empty(batch, dtype=torch.float64, device=y.device)
         k, keep = _kernel(kernel)
-        self._check(lib().smolgp_loglik(self.handle, ev.handle, C.byref(k), batch, _dptr(y), _dptr(noise_sigma), _dptr(amp), _dptr(out)))
+        self._check(lib().smolgp_loglik(self.handle, ev.handle, C.byref(k), batch, _dptr(y, numel=batch * ev.N, name="y"),
+                                        _dptr(noise_sigma, numel=ev.N, name="noise_sigma"), _dptr(amp, numel=batch, name="amp"),
+                                        _dptr(out, numel=batch, name="out")))
         return out
 
     def smolgp_loglik_host(self, ev, kernel, y, noise_sigma, amp=None):
@@ -189,7 +205,8 @@ class Context:
         am = None if amp is None else np.ascontiguousarray(amp, np.float64)
         out = np.empty(batch)
         k, keep = _kernel(kernel)
-        self._check(lib().smolgp_loglik_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y), _hptr(sg), _hptr(am), _hptr(out)))
+        self._check(lib().smolgp_loglik_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y, batch * ev.N, "y"), _hptr(sg, ev.N, "noise_sigma"),
+                                             _hptr(am, batch, "amp"), _hptr(out)))
         return out
 
     # ---- a2-a7 ----
@@ -207,9 +224,14 @@ class Context:
             out["mean_query"] = torch.empty((batch, M), dtype=torch.float64, device=y.device)
             out["var_query"] = torch.empty((batch, M), dtype=torch.float64, device=y.device)
         k, keep = _kernel(kernel)
-        self._check(lib().smolgp_condition(self.handle, ev.handle, C.byref(k), batch, _dptr(y), _dptr(noise_sigma), _dptr(amp),
-                                           M, _dptr(t_query), int(query_instrument), _dptr(out["mean"]), _dptr(out["var"]),
-                                           _dptr(out.get("mean_query")), _dptr(out.get("var_query")), _dptr(out["loglik"])))
+        bn, bm = batch * N, batch * M
+        self._check(lib().smolgp_condition(self.handle, ev.handle, C.byref(k), batch, _dptr(y, numel=bn, name="y"),
+                                           _dptr(noise_sigma, numel=N, name="noise_sigma"), _dptr(amp, numel=batch, name="amp"),
+                                           M, _dptr(t_query, name="t_query"), int(query_instrument),
+                                           _dptr(out["mean"], numel=bn, name="out[mean]"), _dptr(out["var"], numel=bn, name="out[var]"),
+                                           _dptr(out.get("mean_query"), numel=bm, name="out[mean_query]"),
+                                           _dptr(out.get("var_query"), numel=bm, name="out[var_query]"),
+                                           _dptr(out["loglik"], numel=batch, name="out[loglik]")))
         return out
 
     def smolgp_condition_host(self, ev, kernel, y, noise_sigma, amp=None, t_query=None, query_instrument=0, out=None):
@@ -225,9 +247,12 @@ class Context:
             if M:
                 out["mean_query"], out["var_query"] = np.empty((batch, M)), np.empty((batch, M))
         k, keep = _kernel(kernel)
-        self._check(lib().smolgp_condition_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y), _hptr(sg), _hptr(am), M,
-                                                _hptr(tq), int(query_instrument), _hptr(out["mean"]), _hptr(out["var"]),
-                                                _hptr(out.get("mean_query")), _hptr(out.get("var_query")), _hptr(out["loglik"])))
+        bn, bm = batch * N, batch * M
+        self._check(lib().smolgp_condition_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y, bn, "y"), _hptr(sg, N, "noise_sigma"),
+                                                _hptr(am, batch, "amp"), M, _hptr(tq), int(query_instrument),
+                                                _hptr(out["mean"], bn, "out[mean]"), _hptr(out["var"], bn, "out[var]"),
+                                                _hptr(out.get("mean_query"), bm, "out[mean_query]"),
+                                                _hptr(out.get("var_query"), bm, "out[var_query]"), _hptr(out["loglik"], batch, "out[loglik]")))
         return out
 
     def smolgp_discretise_host(self, kernel, n_inst, dt):

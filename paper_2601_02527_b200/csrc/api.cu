@@ -31,6 +31,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0; c->prof_cur = 0;
   c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
+  c->lb_status = nullptr; c->lb_words = 0; c->lb_epoch = 0;
   // pinned: the per-call model upload is a true asynchronous copy
   if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
   int v = 0;
@@ -59,6 +60,7 @@ extern "C" void smolgp_destroy(smolgp_ctx* ctx) {
   cudaFree(ctx->arena);
   cudaFree(ctx->pers);
   cudaFree(ctx->d_flags);
+  cudaFree(ctx->lb_status);
   for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto& e : ctx->evpool) cudaEventDestroy(e);
   cudaFreeHost(ctx->hmodel);
@@ -68,9 +70,9 @@ extern "C" void smolgp_destroy(smolgp_ctx* ctx) {
 extern "C" const char* smolgp_last_error(const smolgp_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 extern "C" int64_t smolgp_launch_count(const smolgp_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
-static const char* const KNAMES[KID_COUNT] = {"k_ev_init", "k_rs_hist", "k_rs_scan", "k_rs_scatter", "k_ev_gather",
-                                               "k_xs_reduce", "k_xs_tiles", "k_ev_final", "k_disc", "k_fold0", "k_foldD",
-                                               "k_downD", "k_down0", "k_ll_reduce", "k_probe_dfma", "k_query_locate", "k_query"};
+static const char* const KNAMES[KID_COUNT] = {"k_ev_init", "k_rs_pass", "k_ev_final", "k_disc", "k_fold0", "k_foldD",
+                                               "k_downD", "k_down0", "k_ll_reduce", "k_query_locate", "k_query"};
+static_assert(KID_COUNT == SMOLGP_NKERNELS, "smolgp.h: SMOLGP_NKERNELS out of step with the kernel ids");
 extern "C" const char* smolgp_kernel_name(int32_t id) { return (id >= 0 && id < KID_COUNT) ? KNAMES[id] : nullptr; }
 
 extern "C" int smolgp_profile(smolgp_ctx* ctx, int32_t enable) {
@@ -97,6 +99,7 @@ extern "C" int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launche
 }
 
 extern "C" const char* smolgp_jit_log(smolgp_ctx* ctx) { return ctx ? sg_jit_log(ctx) : ""; }
+extern "C" const char* smolgp_plan_info(const smolgp_ctx* ctx) { return ctx ? ctx->plan.c_str() : ""; }
 
 extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value) {
   if (!ctx || !name) return SMOLGP_EINVAL;
@@ -109,7 +112,7 @@ extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t valu
   return SMOLGP_OK;
 }
 
-// validation of sigma > 0 happens on the device inside the filter (S > 0 check) and here for amp
+// validation of sigma > 0 and amp > 0 happens on the device inside the filter (NUMF_SIGMA / NUMF_AMP flags)
 struct QuerySpec { int64_t M = 0; const double* tq = nullptr; int qinst = 0; double* mean = nullptr; double* var = nullptr; };
 
 static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
@@ -164,6 +167,7 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   if (qstore) cudaFreeAsync(qstore, ctx->stream);
   SG_CUDA(ctx, ce);
   if (flags & NUMF_SIGMA) { ctx->err = "noise_sigma must be finite and > 0 at every exposure"; return SMOLGP_EINVAL; }
+  if (flags & NUMF_AMP) { ctx->err = "amp must be finite and > 0 for every series"; return SMOLGP_EINVAL; }
   if (flags) { ctx->err = "non-finite value or non-positive innovation variance (check noise_sigma > 0, amp > 0, finite y)"; return SMOLGP_ENUMERIC; }
   return SMOLGP_OK;
 }
@@ -279,26 +283,9 @@ extern "C" int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kern
   std::vector<double> rec(hm.disc_stride);
   SG_CUDA(ctx, cudaMemcpyAsync(rec.data(), drec, hm.disc_stride * 8, cudaMemcpyDeviceToHost, ctx->stream));
   SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-  // block units -> raw units: x_i = s_i x''_i with s = sigma_b lambda^(derivative order); z = tau z' (tau = 1).
-  // sigma_b / T-scale come back out of cz: cz[q][b] = sigma_b T_b / tau_q for instruments in the mask, so
-  // recompute the scales from the kernel description instead (mask-independent).
-  std::vector<double> sc(n, 1.0), sigb(hm.nblk, 0.0);
-  {
-    int b = 0;
-    for (int c = 0; c < kernel->n_comp; ++c) {
-      const smolgp_component& k = kernel->comp[c];
-      if (k.family == SMOLGP_MATERN32_X_PERIODIC) {
-        const long double x = 1.0L / ((long double)k.p2 * k.p2);
-        for (int j = 0; j <= k.order; ++j) {
-          long double term = 1.0L;
-          for (int m = 1; m <= j; ++m) term *= (x / 2) / m;
-          long double sum = term;
-          for (int m = 1; m < 80; ++m) { term *= (x / 2) * (x / 2) / ((long double)m * (m + j)); sum += term; }
-          sigb[b++] = (double)(k.sigma * sqrtl((j == 0 ? 1.0L : 2.0L) * sum * expl(-x)));
-        }
-      } else sigb[b++] = k.sigma;
-    }
-  }
+  // block units -> raw units: x_i = s_i x''_i with s = sigma_b lambda^(derivative order); z = tau z' (tau = 1)
+  std::vector<double> sc(n, 1.0);
+  const double* sigb = hm.bsig; // sigma_b of every block (model.cu)
   for (int b = 0; b < hm.nblk; ++b) {
     const BlockConst& B = hm.blk[b];
     for (int i = 0; i < B.dim; ++i) {
@@ -331,46 +318,5 @@ extern "C" int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kern
     }
   }
   for (int q = 0; q < n_inst; ++q) A[(d + q) * n + d + q] = 1.0;
-  return SMOLGP_OK;
-}
-
-// ---- FP64 FMA probe --------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_probe_dfma(double* out, int iters) {
-  double a0 = threadIdx.x * 1e-3, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-  const double m = 0.999999, c = 1e-9;
-  for (int i = 0; i < iters; ++i) {
-    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-  }
-  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-  if (s == 123.456) out[0] = s;
-}
-
-extern "C" int smolgp_probe_fp64(smolgp_ctx* ctx, double* tflops) {
-  if (!ctx || !tflops) return SMOLGP_EINVAL;
-  SG_CUDA(ctx, cudaSetDevice(ctx->device));
-  void* ws;
-  int rc = sg_arena(ctx, 256, &ws);
-  if (rc) return rc;
-  const int iters = 1 << 15, blocks = ctx->sm_count * 8, threads = 256;
-  cudaEvent_t e0, e1;
-  SG_CUDA(ctx, cudaEventCreate(&e0));
-  SG_CUDA(ctx, cudaEventCreate(&e1));
-  k_probe_dfma<<<blocks, threads, 0, ctx->stream>>>((double*)ws, iters / 8);
-  float best = 1e30f;
-  for (int rep = 0; rep < 3; ++rep) {
-    cudaEventRecord(e0, ctx->stream);
-    k_probe_dfma<<<blocks, threads, 0, ctx->stream>>>((double*)ws, iters);
-    cudaEventRecord(e1, ctx->stream);
-    cudaEventSynchronize(e1);
-    float ms = 0;
-    cudaEventElapsedTime(&ms, e0, e1);
-    if (ms < best) best = ms;
-  }
-  ctx->launches += 4;
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  SG_CUDA(ctx, cudaGetLastError());
-  *tflops = 2.0 * 8.0 * (double)iters * blocks * threads / (best * 1e-3) / 1e12;
   return SMOLGP_OK;
 }

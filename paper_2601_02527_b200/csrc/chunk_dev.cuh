@@ -315,7 +315,8 @@ __device__ __forceinline__ void sandwich_Ft(const Grp<G>& g, const Tab& T, const
 }
 
 // X <- (X + X^T) / 2 on columns 0..n-1: lane j pairs with the n/2 columns after it (cyclically), so
-// every unordered pair is visited (twice for the antipodal pairs of an even n, with equal results)
+// every unordered pair is visited exactly once (the antipodal pairs of an even n by the lower lane only:
+// no two lanes ever touch the same cells)
 template <int G, int LD>
 __device__ __forceinline__ void symmetrise(const Grp<G>& g, const Tab& T, double* X) {
   constexpr int ld = LD;
@@ -323,7 +324,7 @@ __device__ __forceinline__ void symmetrise(const Grp<G>& g, const Tab& T, double
   if (j < n) {
 #pragma unroll
     for (int s = 1; s <= (LD - 1) / 2; ++s) {
-      if (s <= half) {
+      if (s <= half && !(((n & 1) == 0) && s == half && j >= half)) {
         int i = j + s;
         if (i >= n) i -= n;
         const double w = 0.5 * (X[i * ld + j] + X[j * ld + i]);

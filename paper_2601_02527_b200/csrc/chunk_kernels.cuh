@@ -209,6 +209,7 @@ __device__ __forceinline__ void down0_body(const ScanDev& P) {
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ampv = P.amp ? P.amp[series] : 1.0;
   const double ramp = 1.0 / ampv;
+  if (!(ampv > 0.0) || !isfinite(ampv)) atomicOr(P.flags, NUMF_AMP);
 
   RecStage rs;
   rs.init(g, recs, TSTRIDE);
@@ -427,6 +428,7 @@ __device__ __forceinline__ void query_body(const QueryDev& P) {
   const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
   const int64_t kp = P.kp[q];
   const double ampv = P.amp ? P.amp[series] : 1.0;
+  if (!(ampv > 0.0) || !isfinite(ampv)) atomicOr(P.flags, NUMF_AMP);
   RecStage rs;
   rs.init(g, recs, TSTRIDE);
   rs.issue(g, P.discq + q * (int64_t)TSTRIDE, 0);

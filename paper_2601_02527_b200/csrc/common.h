@@ -36,7 +36,6 @@ struct ModelDev {
   int n, d, n_inst, nblk;
   int disc_stride;                 // doubles per event in the discretisation array
   int disc_off[SG_MAXBLK];         // offset of block b inside one event's record
-  int row_lo[SG_NMAX], row_hi[SG_NMAX]; // x-row i of F only touches columns [row_lo, row_hi)
   double cz[SG_MAXINST][SG_MAXBLK]; // c_qb: coupling of block b's integral into z_q (equilibrated units), 0 if masked out
   double tau[SG_MAXINST];          // z_q is carried as z_q / tau_q
   double bsig[SG_MAXBLK];          // amplitude sigma_b of block b (H_b = sigma_b e_0 in block units)
@@ -65,14 +64,15 @@ struct smolgp_events {
 };
 
 // kernel ids for launch accounting / per-kernel timing (smolgp_profile_read)
-enum { KID_EV_INIT = 0, KID_RS_HIST, KID_RS_SCAN, KID_RS_SCATTER, KID_EV_GATHER, KID_XS_REDUCE, KID_XS_TILES,
-       KID_EV_FINAL, KID_DISC, KID_FOLD0, KID_FOLDD, KID_DOWND, KID_DOWN0, KID_LL_REDUCE, KID_PROBE, KID_QLOCATE, KID_QUERY, KID_COUNT };
+enum { KID_EV_INIT = 0, KID_RS_PASS, KID_EV_FINAL, KID_DISC, KID_FOLD0, KID_FOLDD, KID_DOWND, KID_DOWN0, KID_LL_REDUCE,
+       KID_QLOCATE, KID_QUERY, KID_COUNT };
 struct ProfRec { int id; cudaEvent_t a, b; };
 
 struct smolgp_ctx {
   int device;
   cudaStream_t stream;
   std::string err;
+  std::string plan; // smolgp_plan_info
   int64_t launches;
   int prof_on;   // 0 off, 1 every kernel, 2 + id: only kernel id (smolgp_profile)
   int prof_cur;  // the launch in flight is being timed
@@ -89,6 +89,10 @@ struct smolgp_ctx {
   ModelDev* hmodel; // host copy of the current model
   int sm_count;
   size_t smem_optin;
+  // decoupled look-back words of the event build (events.cu): persistent, told apart by epoch
+  unsigned long long* lb_status;
+  size_t lb_words;
+  uint32_t lb_epoch;
 };
 
 // bracket a kernel launch: counts it and, when profiling is on, times it with CUDA events on the ctx stream
@@ -124,9 +128,6 @@ int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const
 // disc.cu
 int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_model, const double* dt,
                    int64_t K, double* disc);
-// events.cu
-int sg_sort_pairs(smolgp_ctx* ctx, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
-                  int64_t n, uint32_t* hist, uint32_t* gcnt);
 // scan.cu
 struct ScanArgs {
   const ModelDev* d_model;

@@ -8,6 +8,7 @@
 #define SG_DENSE_NT 256 /* threads of the CTA that works on one dense combine */
 #define NUMF_BAD 1     /* numeric flag: non-finite value or non-positive innovation variance */
 #define NUMF_SIGMA 2   /* noise_sigma <= 0 or not finite at an exposure */
+#define NUMF_AMP 4     /* amp <= 0 or not finite for a series */
 
 // event meta word: bit 0 kind (1 = start/reset, 0 = end/observe), bits 1..5 instrument,
 // bits 8..23 zero-mask Z_k (instruments whose z is zeroed after event k: idle ones, and the

@@ -1,13 +1,26 @@
 // events.cu -- step a1: exposures -> time-sorted start/end event stream.
 //
 // 2N (key, payload) pairs: key = order-preserving 64-bit image of the event time, payload =
-// 2*exposure + kind.  The pairs are laid out [all ends | all starts] and sorted by a STABLE
-// least-significant-digit radix sort (8 passes of 8 bits), so equal times keep "end before start"
-// (reading R5: needed for back-to-back exposures, the Fig. 2 case P:543).  An inclusive XOR scan
-// of the instrument bits gives, for every event, the set of instruments that are exposing after
-// it; from it come the zero-mask Z_k (idle instruments and the event's own) and the check that
-// each instrument's events alternate start, end, start, ... (no self-overlap).
+// 2*exposure + kind.  Order of the stream (include/smolgp.h; SURVEY reading c5, DESIGN R5):
+//   (time, end before start, instrument, exposure index).
+// "End before start" makes back-to-back exposures of one instrument legal (the Fig. 2 case).
+// The pairs are laid out [all ends | all starts] in exposure order and sorted by a STABLE least-
+// significant-digit radix sort: digit 0 = (kind, instrument), digits 1..8 = the bytes of the time key.
+//   k_ev_init   builds the pairs, validates the input and accumulates the GLOBAL histograms of all
+//               nine digits in the same pass over the exposures;
+//   k_rs_pass   one launch per digit: per-tile stable ranking (warp match_any), the tile's global
+//               offsets by a decoupled look-back over the tiles' digit counts, scatter.  A digit on
+//               which all keys agree (the high bytes of the times of one data set; digit 0 when the
+//               exposures come grouped by instrument) is found from the global histogram on the
+//               device and its pass returns at once -- no host round trip decides it;
+//   k_ev_final  gather + inclusive XOR scan of the instrument bits (again one look-back word per
+//               tile) -> for every event the set of instruments exposing after it, hence the zero-mask
+//               Z_k (idle instruments and the event's own) and the check that each instrument's events
+//               alternate start, end, start, ... (no self-overlap); dt_k = t_k - t_{k-1}.
+// Eleven launches whatever N (round 1: 33), one small status read-back.
 #include <math.h>
+#include <stddef.h>
+#include <string.h>
 
 #include "common.h"
 
@@ -15,212 +28,320 @@
 #define EVF_BADINST 2
 #define EVF_OVERLAP 4
 
+#define RS_NT 256      /* threads per CTA of the sort and tail kernels */
+#define RS_DIGITS 9
+
+// device-resident control block of one build (zeroed by one memset per call)
+struct EvCtl {
+  uint32_t ghist[RS_DIGITS][256]; // global digit histograms
+  uint32_t ticket[RS_DIGITS + 1]; // tile tickets per pass (+ the tail kernel)
+  uint32_t ungrouped;             // some exposure has a smaller instrument index than its predecessor
+  int32_t flags;                  // EVF_*
+  unsigned long long maxdelta[SG_MAXINST]; // bits of the longest exposure per instrument
+  double tfirst, tlast;
+};
+
 __device__ __forceinline__ uint64_t time_key(double t) {
+  t = t + 0.0; // -0.0 -> +0.0: one key for one time
   uint64_t u = (uint64_t)__double_as_longlong(t);
   return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
 }
 
-__global__ void k_ev_init(int64_t N, const double* __restrict__ ts, const double* __restrict__ te,
-                          const int32_t* __restrict__ inst, int n_inst, uint64_t* __restrict__ keys,
-                          uint32_t* __restrict__ vals, int* __restrict__ flags,
-                          unsigned long long* __restrict__ maxdelta) {
+// warp-aggregated shared-memory histogram increment: one atomic when the whole warp agrees on the bin
+// (constant bytes of the keys would otherwise serialise 32-fold), plain atomics otherwise
+__device__ __forceinline__ void hist_add(uint32_t* h, int bin, bool live) {
+  const unsigned act = __ballot_sync(0xffffffffu, live);
+  if (!act) return;
+  const int lead = __ffs(act) - 1;
+  const int b0 = __shfl_sync(0xffffffffu, bin, lead);
+  const bool same = __all_sync(0xffffffffu, !live || bin == b0);
+  if (same) { if ((threadIdx.x & 31) == lead) atomicAdd(&h[b0], (uint32_t)__popc(act)); }
+  else if (live) atomicAdd(&h[bin], 1u);
+}
+
+__global__ void __launch_bounds__(RS_NT) k_ev_init(int64_t N, const double* __restrict__ ts, const double* __restrict__ te,
+                                                   const int32_t* __restrict__ inst, int n_inst, uint64_t* __restrict__ keys,
+                                                   uint32_t* __restrict__ vals, EvCtl* __restrict__ ctl) {
+  __shared__ uint32_t h[RS_DIGITS][256];
+  for (int e = threadIdx.x; e < RS_DIGITS * 256; e += RS_NT) (&h[0][0])[e] = 0u;
+  __syncthreads();
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   unsigned long long dbits = 0ull; // bits of this exposure's length (0 for dead / invalid lanes)
   int q = -1;
-  if (i < N) {
+  const bool live = i < N;
+  uint64_t ke = 0, ks = 0;
+  int qd = 0;
+  if (live) {
     const double s = ts[i], e = te[i];
     q = inst[i];
     int bad = 0;
     if (!isfinite(s) || !isfinite(e) || !(e > s)) bad |= EVF_BADTIME;
     if (q < 0 || q >= n_inst) bad |= EVF_BADINST;
-    if (bad) { atomicOr(flags, bad); q = -1; }
-    keys[i] = time_key(e);
+    qd = (q < 0 || q >= n_inst) ? 0 : q;
+    if (i > 0 && q < inst[i - 1]) atomicOr(&ctl->ungrouped, 1u);
+    if (bad) { atomicOr(&ctl->flags, bad); q = -1; }
+    ke = time_key(e); ks = time_key(s);
+    keys[i] = ke;
     vals[i] = (uint32_t)(2 * i);
-    keys[N + i] = time_key(s);
+    keys[N + i] = ks;
     vals[N + i] = (uint32_t)(2 * i + 1);
     if (!bad) dbits = (unsigned long long)__double_as_longlong(e - s); // positive doubles order like their bits
+  }
+  hist_add(h[0], qd, live);       // end event: kind 0
+  hist_add(h[0], 16 + qd, live);  // start event: kind 1
+#pragma unroll
+  for (int p = 0; p < 8; ++p) {
+    hist_add(h[1 + p], (int)((ke >> (8 * p)) & 255u), live);
+    hist_add(h[1 + p], (int)((ks >> (8 * p)) & 255u), live);
   }
   // longest exposure per instrument: one atomic per (warp, instrument) instead of one per exposure
   for (int r = 0; r < n_inst; ++r) {
     unsigned long long m = (q == r) ? dbits : 0ull;
     for (int o = 16; o; o >>= 1) { const unsigned long long x = __shfl_xor_sync(0xffffffffu, m, o); m = x > m ? x : m; }
-    if ((threadIdx.x & 31) == 0 && m) atomicMax(maxdelta + r, m);
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(&ctl->maxdelta[r], m);
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < RS_DIGITS * 256; e += RS_NT) {
+    const uint32_t c = (&h[0][0])[e];
+    if (c) atomicAdd(&ctl->ghist[0][0] + e, c);
   }
 }
 
-// ---- LSD radix sort, 8 bits per pass.  One warp per tile of RS_TILE keys, RS_WPB tiles per CTA. ----
-// hist: per-tile digit counts (digit-major) + global digit totals; scan: one CTA per digit turns its
-// row into global positions (base = total of the smaller digits); scatter: stable, warp-serial
-// ranking with match_any (equal keys keep their order: ends stay before starts, reading R5).
-#define RS_TILE 512
-#define RS_WPB 4
-__global__ void __launch_bounds__(32 * RS_WPB) k_rs_hist(const uint64_t* __restrict__ keys, int64_t n, int shift,
-                                                         uint32_t* __restrict__ hist, int ntiles, uint32_t* __restrict__ gcnt) {
-  __shared__ uint32_t cnt_all[RS_WPB][256];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int tile = blockIdx.x * RS_WPB + w;
-  uint32_t* cnt = cnt_all[w];
-  for (int b = lane; b < 256; b += 32) cnt[b] = 0;
-  __syncwarp();
-  if (tile < ntiles) {
-    const int64_t base = (int64_t)tile * RS_TILE;
-    for (int i = lane; i < RS_TILE; i += 32) {
-      const int64_t p = base + i;
-      if (p < n) atomicAdd(&cnt[(keys[p] >> shift) & 255u], 1u);
-    }
-    __syncwarp();
-    for (int b = lane; b < 256; b += 32) {
-      const uint32_t c = cnt[b];
-      hist[(int64_t)b * ntiles + tile] = c; // digit-major
-      if (c) atomicAdd(&gcnt[b], c);
-    }
-  }
-}
-// exclusive scan of the digit-major histogram: CTA d scans row d, starting at the total of digits < d
-__global__ void __launch_bounds__(256) k_rs_scan(uint32_t* __restrict__ hist, int ntiles, const uint32_t* __restrict__ gcnt) {
-  __shared__ uint32_t sm[256];
-  __shared__ uint32_t carry;
-  const int d = blockIdx.x, tid = threadIdx.x;
-  sm[tid] = (tid < d) ? gcnt[tid] : 0u;
+// ---- which passes move data: bit p set <=> pass p is skipped (all keys agree on digit p; digit 0: the
+// initial layout [ends | starts] is already in (kind, instrument, index) order).  Every CTA of every
+// pass recomputes it from the global histogram (9 x 256 words), so the ping-pong parity of the buffers
+// never needs the host.
+__device__ __forceinline__ unsigned skip_mask(const EvCtl* ctl, uint32_t n, unsigned* s_mask) {
+  if (threadIdx.x == 0) *s_mask = ctl->ungrouped ? 0u : 1u;
   __syncthreads();
-  for (int off = 128; off; off >>= 1) { if (tid < off) sm[tid] += sm[tid + off]; __syncthreads(); }
-  if (tid == 0) carry = sm[0];
+  unsigned m = 0;
+  for (int p = 1; p < RS_DIGITS; ++p)
+    if (ctl->ghist[p][threadIdx.x] == n) m |= 1u << p;
+  if (m) atomicOr(s_mask, m);
   __syncthreads();
-  uint32_t* row = hist + (int64_t)d * ntiles;
-  for (int t0 = 0; t0 < ntiles; t0 += 256) {
-    const int t = t0 + tid;
-    const uint32_t v = (t < ntiles) ? row[t] : 0u;
-    const uint32_t run0 = carry;
-    __syncthreads();
-    sm[tid] = v;
-    __syncthreads();
-    for (int off = 1; off < 256; off <<= 1) {
-      const uint32_t x = (tid >= off) ? sm[tid - off] : 0u;
-      __syncthreads();
-      sm[tid] += x;
-      __syncthreads();
-    }
-    if (t < ntiles) row[t] = run0 + sm[tid] - v;
-    if (tid == 255) carry = run0 + sm[255];
-    __syncthreads();
-  }
+  return *s_mask;
 }
-__global__ void __launch_bounds__(32 * RS_WPB) k_rs_scatter(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals,
-                                                            uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                                                            int64_t n, int shift, const uint32_t* __restrict__ hist, int ntiles) {
-  __shared__ uint32_t pos_all[RS_WPB][256];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int tile = blockIdx.x * RS_WPB + w;
-  if (tile >= ntiles) return;
-  uint32_t* pos = pos_all[w];
-  for (int b = lane; b < 256; b += 32) pos[b] = hist[(int64_t)b * ntiles + tile];
-  __syncwarp();
-  const int64_t base = (int64_t)tile * RS_TILE;
-  for (int i0 = 0; i0 < RS_TILE; i0 += 32) {
-    const int64_t p = base + i0 + lane;
+
+// look-back status word: [epoch:30 | flag:2 | count:32]; a word of another epoch reads as "not yet there"
+#define LB_AGG 1ull
+#define LB_INC 2ull
+__device__ __forceinline__ unsigned long long lb_pack(uint32_t epoch, unsigned long long flag, uint32_t v) {
+  return ((unsigned long long)epoch << 34) | (flag << 32) | v;
+}
+__device__ __forceinline__ unsigned long long lb_load(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void lb_store(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// One pass of the LSD radix sort.  Tile = RS_NT * ITEMS keys, warp w of the CTA ranks the contiguous run
+// [w * 32 * ITEMS, (w + 1) * 32 * ITEMS) of the tile in rounds of 32 (stable: run order, round order, lane
+// order).  status: [tiles][256] look-back words of this ctx (never cleared: the epoch tells the passes apart).
+template <int ITEMS>
+__global__ void __launch_bounds__(RS_NT) k_rs_pass(EvCtl* __restrict__ ctl, int pass, uint64_t* __restrict__ kA, uint32_t* __restrict__ vA,
+                                                   uint64_t* __restrict__ kB, uint32_t* __restrict__ vB, const int32_t* __restrict__ inst,
+                                                   int n_inst, uint32_t n, unsigned long long* __restrict__ status, uint32_t epoch) {
+  __shared__ uint32_t wcnt[RS_NT / 32][256];
+  __shared__ uint32_t base[256];
+  __shared__ uint32_t wsum[RS_NT / 32];
+  __shared__ unsigned s_mask;
+  __shared__ uint32_t s_tile;
+  const unsigned skip = skip_mask(ctl, n, &s_mask);
+  if ((skip >> pass) & 1u) return;
+  const int moved = __popc(~skip & ((1u << pass) - 1u)); // passes before this one that moved the data
+  const uint64_t* kin = (moved & 1) ? kB : kA;
+  const uint32_t* vin = (moved & 1) ? vB : vA;
+  uint64_t* kout = (moved & 1) ? kA : kB;
+  uint32_t* vout = (moved & 1) ? vA : vB;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  if (tid == 0) s_tile = atomicAdd(&ctl->ticket[pass], 1u); // tiles are taken in start order: a predecessor is always running
+  for (int e = tid; e < (RS_NT / 32) * 256; e += RS_NT) (&wcnt[0][0])[e] = 0u;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const uint32_t t0 = tile * (uint32_t)(RS_NT * ITEMS) + (uint32_t)w * (32 * ITEMS);
+  uint64_t k[ITEMS];
+  uint32_t v[ITEMS];
+  int dg[ITEMS];
+  uint32_t rk[ITEMS];
+#pragma unroll
+  for (int r = 0; r < ITEMS; ++r) {
+    const uint32_t p = t0 + r * 32 + lane;
     const bool live = p < n;
-    uint64_t k = 0;
-    uint32_t v = 0;
-    int dg = 256 + lane; // dead lanes get distinct pseudo-digits
-    if (live) { k = keys[p]; v = vals[p]; dg = (int)((k >> shift) & 255u); }
-    const unsigned peers = __match_any_sync(0xffffffffu, dg);
-    const int rank = __popc(peers & ((1u << lane) - 1u));
+    k[r] = 0; v[r] = 0; dg[r] = 256 + lane; // dead lanes get distinct pseudo-digits
+    if (live) {
+      k[r] = kin[p]; v[r] = vin[p];
+      if (pass == 0) {
+        int q = inst[v[r] >> 1];
+        if (q < 0 || q >= n_inst) q = 0;
+        dg[r] = (int)((v[r] & 1u) << 4) | q;
+      } else dg[r] = (int)((k[r] >> (8 * (pass - 1))) & 255u);
+    }
+    const unsigned peers = __match_any_sync(0xffffffffu, dg[r]);
     const int leader = __ffs(peers) - 1;
-    uint32_t basepos = 0;
-    if (live && lane == leader) { basepos = pos[dg]; pos[dg] = basepos + __popc(peers); }
-    basepos = __shfl_sync(0xffffffffu, basepos, leader);
-    if (live) { keys_out[basepos + rank] = k; vals_out[basepos + rank] = v; }
+    uint32_t old = 0;
+    if (live && lane == leader) { old = wcnt[w][dg[r]]; wcnt[w][dg[r]] = old + __popc(peers); }
+    old = __shfl_sync(0xffffffffu, old, leader);
+    rk[r] = old + __popc(peers & ((1u << lane) - 1u));
     __syncwarp();
   }
-}
-
-// gcnt: 8 x 256 counters (one slice per pass)
-int sg_sort_pairs(smolgp_ctx* ctx, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
-                  int64_t n, uint32_t* hist, uint32_t* gcnt) {
-  const int ntiles = (int)((n + RS_TILE - 1) / RS_TILE);
-  const unsigned blocks = (unsigned)((ntiles + RS_WPB - 1) / RS_WPB);
-  uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
-  cudaMemsetAsync(gcnt, 0, 8 * 256 * sizeof(uint32_t), ctx->stream);
-  for (int pass = 0; pass < 8; ++pass) {
-    const int shift = 8 * pass;
-    uint32_t* gc = gcnt + pass * 256;
-    sg_launch_begin(ctx, KID_RS_HIST);
-    k_rs_hist<<<blocks, 32 * RS_WPB, 0, ctx->stream>>>(kin, n, shift, hist, ntiles, gc);
-    sg_launch_end(ctx);
-    sg_launch_begin(ctx, KID_RS_SCAN);
-    k_rs_scan<<<256, 256, 0, ctx->stream>>>(hist, ntiles, gc);
-    sg_launch_end(ctx);
-    sg_launch_begin(ctx, KID_RS_SCATTER);
-    k_rs_scatter<<<blocks, 32 * RS_WPB, 0, ctx->stream>>>(kin, vin, kout, vout, n, shift, hist, ntiles);
-    sg_launch_end(ctx);
-    uint64_t* tk = kin; kin = kout; kout = tk;
-    uint32_t* tv = vin; vin = vout; vout = tv;
-  }
-  SG_CUDA(ctx, cudaGetLastError());
-  return SMOLGP_OK; // 8 passes: the result is back in (keys, vals)
-}
-
-// ---- after the sort --------------------------------------------------------------------------------
-__global__ void k_ev_gather(int64_t K, const uint32_t* __restrict__ vals, const double* __restrict__ ts,
-                            const double* __restrict__ te, const int32_t* __restrict__ inst, int n_inst,
-                            double* __restrict__ t, double* __restrict__ delta, int32_t* __restrict__ obs,
-                            uint32_t* __restrict__ bits) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= K) return;
-  const uint32_t v = vals[k];
-  const int64_t i = v >> 1;
-  const double s = ts[i], e = te[i];
-  int q = inst[i];
-  if (q < 0 || q >= n_inst) q = 0;
-  t[k] = (v & 1u) ? s : e;
-  delta[k] = e - s;
-  obs[k] = (int32_t)i;
-  bits[k] = 1u << q;
-}
-
-// inclusive XOR scan, three kernels (tile reduce, scan of tile sums, apply)
-#define XS_TILE 1024
-__global__ void __launch_bounds__(256) k_xs_reduce(const uint32_t* __restrict__ bits, int64_t K, uint32_t* __restrict__ tile) {
-  __shared__ uint32_t sm[8];
-  const int64_t base = (int64_t)blockIdx.x * XS_TILE;
-  uint32_t x = 0;
-  for (int i = threadIdx.x; i < XS_TILE; i += 256) if (base + i < K) x ^= bits[base + i];
-  for (int o = 16; o; o >>= 1) x ^= __shfl_xor_sync(0xffffffffu, x, o);
-  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = x;
   __syncthreads();
-  if (threadIdx.x == 0) { uint32_t r = 0; for (int w = 0; w < 8; ++w) r ^= sm[w]; tile[blockIdx.x] = r; }
-}
-__global__ void k_xs_tiles(uint32_t* __restrict__ tile, int ntiles) { // exclusive, serial: ntiles <= a few thousand
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
-    uint32_t run = 0;
-    for (int i = 0; i < ntiles; ++i) { uint32_t v = tile[i]; tile[i] = run; run ^= v; }
-  }
-}
-__global__ void __launch_bounds__(32) k_ev_final(int64_t K, const uint32_t* __restrict__ bits, const uint32_t* __restrict__ tile,
-                                                 const uint32_t* __restrict__ vals, const double* __restrict__ t,
-                                                 int n_inst, uint32_t* __restrict__ meta, double* __restrict__ dt,
-                                                 int* __restrict__ flags) {
-  const int lane = threadIdx.x;
-  const int64_t base = (int64_t)blockIdx.x * XS_TILE;
-  uint32_t run = tile[blockIdx.x];
-  const uint32_t all = (n_inst >= 32) ? 0xffffffffu : ((1u << n_inst) - 1u);
-  for (int i0 = 0; i0 < XS_TILE; i0 += 32) {
-    const int64_t k = base + i0 + lane;
-    const uint32_t b = (k < K) ? bits[k] : 0u;
-    uint32_t x = b;
-    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x ^= y; }
-    const uint32_t after = run ^ x, before = after ^ b;
-    if (k < K) {
-      const uint32_t kind = vals[k] & 1u;
-      const bool was_open = (before & b) != 0;
-      if ((kind == 1u) == was_open) atomicOr(flags, EVF_OVERLAP); // a start needs closed, an end needs open
-      const uint32_t zmask = ((~after) & all) | b;
-      const int q = __ffs(b) - 1;
-      meta[k] = kind | ((uint32_t)q << 1) | (zmask << 8);
-      dt[k] = (k == 0) ? 0.0 : t[k] - t[k - 1];
+  // thread d: exclusive scan over the warps of digit d's counts; tile count of digit d
+  uint32_t cnt = 0;
+#pragma unroll
+  for (int ww = 0; ww < RS_NT / 32; ++ww) { const uint32_t c = wcnt[ww][tid]; wcnt[ww][tid] = cnt; cnt += c; }
+  unsigned long long* st = status + (size_t)tile * 256 + tid;
+  lb_store(st, lb_pack(epoch, tile == 0 ? LB_INC : LB_AGG, cnt));
+  // exclusive scan over the digits of the global histogram (position of the first key of each digit)
+  const uint32_t g = ctl->ghist[pass][tid];
+  uint32_t x = g;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+  if (lane == 31) wsum[w] = x;
+  __syncthreads();
+  uint32_t wbase = 0;
+#pragma unroll
+  for (int ww = 0; ww < RS_NT / 32; ++ww) if (ww < w) wbase += wsum[ww];
+  uint32_t excl = 0;
+  if (tile > 0) {
+    int64_t t = (int64_t)tile - 1;
+    for (;;) {
+      const unsigned long long s = lb_load(status + (size_t)t * 256 + tid);
+      if ((uint32_t)(s >> 34) != epoch || ((s >> 32) & 3ull) == 0ull) continue; // not published yet
+      excl += (uint32_t)s;
+      if (((s >> 32) & 3ull) == LB_INC) break;
+      --t;
     }
-    run ^= __shfl_sync(0xffffffffu, x, 31);
+    lb_store(st, lb_pack(epoch, LB_INC, excl + cnt));
   }
+  base[tid] = wbase + x - g + excl;
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < ITEMS; ++r) {
+    const uint32_t p = t0 + r * 32 + lane;
+    if (p < n) {
+      const uint32_t pos = base[dg[r]] + wcnt[w][dg[r]] + rk[r];
+      kout[pos] = k[r];
+      vout[pos] = v[r];
+    }
+  }
+}
+
+// ---- after the sort: gather, inclusive XOR scan of the instrument bits, flags -----------------------
+#define EF_ITEMS 4
+__global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int64_t K, const uint32_t* __restrict__ vA,
+                                                    const uint32_t* __restrict__ vB, const double* __restrict__ ts,
+                                                    const double* __restrict__ te, const int32_t* __restrict__ inst, int n_inst,
+                                                    double* __restrict__ t, double* __restrict__ dt, double* __restrict__ delta,
+                                                    uint32_t* __restrict__ meta, int32_t* __restrict__ obs,
+                                                    unsigned long long* __restrict__ status, uint32_t epoch) {
+  __shared__ double st_t[RS_NT * EF_ITEMS + 1];
+  __shared__ uint32_t wx[RS_NT / 32];
+  __shared__ unsigned s_mask;
+  __shared__ uint32_t s_tile, s_run;
+  const unsigned skip = skip_mask(ctl, (uint32_t)K, &s_mask);
+  const int moved = __popc(~skip & ((1u << RS_DIGITS) - 1u));
+  const uint32_t* vals = (moved & 1) ? vB : vA;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  if (tid == 0) s_tile = atomicAdd(&ctl->ticket[RS_DIGITS], 1u);
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const int64_t k0 = (int64_t)tile * (RS_NT * EF_ITEMS) + tid * EF_ITEMS; // blocked: a thread holds EF_ITEMS consecutive events
+  uint32_t vv[EF_ITEMS], b[EF_ITEMS];
+  double tt[EF_ITEMS];
+  uint32_t x = 0;
+#pragma unroll
+  for (int r = 0; r < EF_ITEMS; ++r) {
+    const int64_t k = k0 + r;
+    vv[r] = 0; b[r] = 0; tt[r] = 0.0;
+    if (k < K) {
+      vv[r] = vals[k];
+      const int64_t i = vv[r] >> 1;
+      const double s = ts[i], e = te[i];
+      int q = inst[i];
+      if (q < 0 || q >= n_inst) q = 0;
+      tt[r] = ((vv[r] & 1u) ? s : e) + 0.0;
+      t[k] = tt[r];
+      delta[k] = e - s;
+      obs[k] = (int32_t)i;
+      b[r] = 1u << q;
+      if (k == 0) ctl->tfirst = tt[r];
+      if (k == K - 1) ctl->tlast = tt[r];
+    }
+    st_t[tid * EF_ITEMS + r + 1] = tt[r];
+    x ^= b[r];
+  }
+  if (tid == 0) { // time of the event before the tile
+    const int64_t kp = (int64_t)tile * (RS_NT * EF_ITEMS) - 1;
+    double tp = 0.0;
+    if (kp >= 0) { const uint32_t u = vals[kp]; tp = ((u & 1u) ? ts[u >> 1] : te[u >> 1]) + 0.0; }
+    st_t[0] = tp;
+  }
+  // inclusive XOR scan of the threads' partials over the CTA
+  uint32_t incl = x;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl ^= y; }
+  if (lane == 31) wx[w] = incl;
+  __syncthreads();
+  uint32_t pre = 0;
+#pragma unroll
+  for (int ww = 0; ww < RS_NT / 32; ++ww) if (ww < w) pre ^= wx[ww];
+  incl ^= pre;
+  if (tid == RS_NT - 1) { // tile aggregate -> look-back over the earlier tiles
+    unsigned long long* st = status + tile;
+    lb_store(st, lb_pack(epoch, tile == 0 ? LB_INC : LB_AGG, incl));
+    uint32_t run = 0;
+    if (tile > 0) {
+      int64_t tq = (int64_t)tile - 1;
+      for (;;) {
+        const unsigned long long s = lb_load(status + tq);
+        if ((uint32_t)(s >> 34) != epoch || ((s >> 32) & 3ull) == 0ull) continue;
+        run ^= (uint32_t)s;
+        if (((s >> 32) & 3ull) == LB_INC) break;
+        --tq;
+      }
+      lb_store(st, lb_pack(epoch, LB_INC, run ^ incl));
+    }
+    s_run = run;
+  }
+  __syncthreads();
+  uint32_t after = s_run ^ incl ^ x; // open set before this thread's first event
+  const uint32_t all = (n_inst >= 32) ? 0xffffffffu : ((1u << n_inst) - 1u);
+#pragma unroll
+  for (int r = 0; r < EF_ITEMS; ++r) {
+    const int64_t k = k0 + r;
+    const uint32_t before = after;
+    after ^= b[r];
+    if (k < K) {
+      const uint32_t kind = vv[r] & 1u;
+      const bool was_open = (before & b[r]) != 0;
+      if ((kind == 1u) == was_open) atomicOr(&ctl->flags, EVF_OVERLAP); // a start needs closed, an end needs open
+      const uint32_t zmask = ((~after) & all) | b[r];
+      const int q = __ffs(b[r]) - 1;
+      meta[k] = kind | ((uint32_t)q << 1) | (zmask << 8);
+      dt[k] = (k == 0) ? 0.0 : tt[r] - st_t[tid * EF_ITEMS + r];
+    }
+  }
+}
+
+// look-back words of this ctx (grown on demand, zeroed when allocated; epochs start at 1)
+static int lb_reserve(smolgp_ctx* ctx, size_t words) {
+  if (words <= ctx->lb_words) return SMOLGP_OK;
+  if (ctx->lb_status) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->lb_status); ctx->lb_status = nullptr; ctx->lb_words = 0; }
+  const size_t want = words + words / 4;
+  if (cudaMalloc(&ctx->lb_status, want * 8) != cudaSuccess) { cudaGetLastError(); ctx->lb_status = nullptr; ctx->err = "build_events: out of device memory (sort status)"; return SMOLGP_ENOMEM; }
+  cudaMemsetAsync(ctx->lb_status, 0, want * 8, ctx->stream);
+  ctx->lb_words = want;
+  return SMOLGP_OK;
+}
+static uint32_t lb_next_epoch(smolgp_ctx* ctx) {
+  if (++ctx->lb_epoch >= (1u << 30)) { // wrap: forget every old word first
+    cudaMemsetAsync(ctx->lb_status, 0, ctx->lb_words * 8, ctx->stream);
+    ctx->lb_epoch = 1;
+  }
+  return ctx->lb_epoch;
 }
 
 static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const double* te, const int32_t* inst,
@@ -244,63 +365,60 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
     ev->t = (double*)b; ev->dt = (double*)(b + k8); ev->delta = (double*)(b + 2 * k8);
     ev->meta = (uint32_t*)(b + 3 * k8); ev->obs = (int32_t*)(b + 3 * k8 + k4);
   }
-  // scratch: keys, keys_tmp (u64), vals, vals_tmp, bits (u32), hist, tiles, maxdelta
-  const int ntiles_rs = (int)((K + RS_TILE - 1) / RS_TILE), ntiles_xs = (int)((K + XS_TILE - 1) / XS_TILE);
-  size_t bytes = (size_t)K * (8 + 8 + 4 + 4 + 4) + (size_t)256 * ntiles_rs * 4 + (size_t)ntiles_xs * 4 + SG_MAXINST * 8 + 8 * 256 * 4 + 1024;
+  // tile size of the sort: 1024 keys up to 2^21 events (more CTAs than SMs already at 2e5), 4096 above
+  const int items = (K <= (1ll << 21)) ? 4 : 16;
+  const int64_t tile_rs = (int64_t)RS_NT * items, tile_ef = (int64_t)RS_NT * EF_ITEMS;
+  const int64_t ntiles_rs = (K + tile_rs - 1) / tile_rs, ntiles_ef = (K + tile_ef - 1) / tile_ef;
+  int rc = lb_reserve(ctx, (size_t)ntiles_rs * 256 > (size_t)ntiles_ef ? (size_t)ntiles_rs * 256 : (size_t)ntiles_ef);
+  if (rc) return fail(rc);
+  // scratch: control block, keys x2 (u64), vals x2 (u32)
+  const size_t ctl_b = (sizeof(EvCtl) + 255) / 256 * 256;
   void* scratch;
-  int rc = sg_arena(ctx, bytes, &scratch);
+  rc = sg_arena(ctx, ctl_b + 2 * k8 + 2 * k4, &scratch);
   if (rc) return fail(rc);
   char* p = (char*)scratch;
-  uint64_t* keys = (uint64_t*)p; p += K * 8;
-  uint64_t* keys_tmp = (uint64_t*)p; p += K * 8;
-  unsigned long long* maxdelta = (unsigned long long*)p; p += SG_MAXINST * 8;
-  uint32_t* vals = (uint32_t*)p; p += K * 4;
-  uint32_t* vals_tmp = (uint32_t*)p; p += K * 4;
-  uint32_t* bits = (uint32_t*)p; p += K * 4;
-  uint32_t* hist = (uint32_t*)p; p += (size_t)256 * ntiles_rs * 4;
-  uint32_t* gcnt = (uint32_t*)p; p += 8 * 256 * 4;
-  uint32_t* tiles = (uint32_t*)p;
+  EvCtl* ctl = (EvCtl*)p; p += ctl_b;
+  uint64_t* kA = (uint64_t*)p; p += k8;
+  uint64_t* kB = (uint64_t*)p; p += k8;
+  uint32_t* vA = (uint32_t*)p; p += k4;
+  uint32_t* vB = (uint32_t*)p;
   cudaStream_t st = ctx->stream;
-  cudaMemsetAsync(ctx->d_flags, 0, sizeof(int), st);
-  cudaMemsetAsync(maxdelta, 0, SG_MAXINST * 8, st);
+  cudaMemsetAsync(ctl, 0, sizeof(EvCtl), st);
   sg_launch_begin(ctx, KID_EV_INIT);
-  k_ev_init<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ts, te, inst, n_inst, keys, vals, ctx->d_flags, maxdelta);
+  k_ev_init<<<(unsigned)((N + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(N, ts, te, inst, n_inst, kA, vA, ctl);
   sg_launch_end(ctx);
-  rc = sg_sort_pairs(ctx, keys, vals, keys_tmp, vals_tmp, K, hist, gcnt);
-  if (rc) return fail(rc);
-  sg_launch_begin(ctx, KID_EV_GATHER);
-  k_ev_gather<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(K, vals, ts, te, inst, n_inst, ev->t, ev->delta, ev->obs, bits);
-  sg_launch_end(ctx);
-  sg_launch_begin(ctx, KID_XS_REDUCE);
-  k_xs_reduce<<<ntiles_xs, 256, 0, st>>>(bits, K, tiles);
-  sg_launch_end(ctx);
-  sg_launch_begin(ctx, KID_XS_TILES);
-  k_xs_tiles<<<1, 32, 0, st>>>(tiles, ntiles_xs);
-  sg_launch_end(ctx);
-  sg_launch_begin(ctx, KID_EV_FINAL);
-  k_ev_final<<<ntiles_xs, 32, 0, st>>>(K, bits, tiles, vals, ev->t, n_inst, ev->meta, ev->dt, ctx->d_flags);
-  sg_launch_end(ctx);
-  int flags = 0;
-  unsigned long long md[SG_MAXINST];
-  double tfl[2];
-  if (cudaMemcpyAsync(&flags, ctx->d_flags, sizeof(int), cudaMemcpyDeviceToHost, st) ||
-      cudaMemcpyAsync(md, maxdelta, sizeof(md), cudaMemcpyDeviceToHost, st) ||
-      cudaMemcpyAsync(&tfl[0], ev->t, 8, cudaMemcpyDeviceToHost, st) ||
-      cudaMemcpyAsync(&tfl[1], ev->t + (K - 1), 8, cudaMemcpyDeviceToHost, st) || cudaStreamSynchronize(st)) {
-    ctx->err = std::string("build_events: ") + cudaGetErrorString(cudaGetLastError());
-    return fail(SMOLGP_ECUDA);
+  for (int pass = 0; pass < RS_DIGITS; ++pass) {
+    const uint32_t epoch = lb_next_epoch(ctx);
+    sg_launch_begin(ctx, KID_RS_PASS);
+    if (items == 4) k_rs_pass<4><<<(unsigned)ntiles_rs, RS_NT, 0, st>>>(ctl, pass, kA, vA, kB, vB, inst, n_inst, (uint32_t)K, ctx->lb_status, epoch);
+    else k_rs_pass<16><<<(unsigned)ntiles_rs, RS_NT, 0, st>>>(ctl, pass, kA, vA, kB, vB, inst, n_inst, (uint32_t)K, ctx->lb_status, epoch);
+    sg_launch_end(ctx);
   }
+  {
+    const uint32_t epoch = lb_next_epoch(ctx);
+    sg_launch_begin(ctx, KID_EV_FINAL);
+    k_ev_final<<<(unsigned)ntiles_ef, RS_NT, 0, st>>>(ctl, K, vA, vB, ts, te, inst, n_inst, ev->t, ev->dt, ev->delta, ev->meta, ev->obs, ctx->lb_status, epoch);
+    sg_launch_end(ctx);
+  }
+  // ONE status read-back: validation flags, longest exposures, first / last event time
+  struct { int32_t pad; int32_t flags; unsigned long long md[SG_MAXINST]; double tfl[2]; } hs;
+  static_assert(offsetof(EvCtl, maxdelta) == offsetof(EvCtl, flags) + 4 && offsetof(EvCtl, tfirst) == offsetof(EvCtl, maxdelta) + 8 * SG_MAXINST &&
+                offsetof(EvCtl, tlast) == offsetof(EvCtl, tfirst) + 8, "EvCtl: flags | maxdelta | tfirst | tlast must be contiguous");
+  cudaError_t ce = cudaMemcpyAsync(&hs.flags, &ctl->flags, 4 + sizeof(hs.md) + sizeof(hs.tfl), cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+  if (ce != cudaSuccess) { ctx->err = std::string("build_events: ") + cudaGetErrorString(ce); cudaGetLastError(); return fail(SMOLGP_ECUDA); }
+  const int flags = hs.flags;
   if (flags & EVF_BADTIME) { ctx->err = "build_events: non-finite time or t_end <= t_start"; return fail(SMOLGP_EINVAL); }
   if (flags & EVF_BADINST) { ctx->err = "build_events: instrument index out of range"; return fail(SMOLGP_EINVAL); }
   if (flags & EVF_OVERLAP) { ctx->err = "build_events: an instrument overlaps itself (P:464)"; return fail(SMOLGP_EOVERLAP); }
   for (int q = 0; q < SG_MAXINST; ++q) {
     double dmax;
-    memcpy(&dmax, &md[q], 8);
+    memcpy(&dmax, &hs.md[q], 8);
     int e = 0;
     if (q < n_inst && dmax > 0) frexp(dmax, &e); // dmax = f 2^e, f in [0.5, 1)
     ev->tau[q] = (q < n_inst && dmax > 0) ? ldexp(1.0, e) : 1.0; // power of two >= the longest exposure
   }
-  ev->t_first = tfl[0]; ev->t_last = tfl[1];
+  ev->t_first = hs.tfl[0]; ev->t_last = hs.tfl[1];
   *out = ev;
   return SMOLGP_OK;
 }

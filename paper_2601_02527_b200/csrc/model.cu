@@ -167,15 +167,10 @@ int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const
   for (int b = 0; b < nb; ++b) { M->blk[b].off = d; d += M->blk[b].dim; M->disc_off[b] = off; off += disc_block_size(M->blk[b].dim); }
   if (d + n_inst > SMOLGP_MAX_DIM) { ctx->err = "augmented state dimension above SMOLGP_MAX_DIM"; return SMOLGP_EUNSUPPORTED; }
   M->n = d + n_inst; M->d = d; M->n_inst = n_inst; M->nblk = nb; M->disc_stride = off;
-  for (int b = 0; b < nb; ++b)
-    for (int i = 0; i < M->blk[b].dim; ++i) { M->row_lo[M->blk[b].off + i] = M->blk[b].off; M->row_hi[M->blk[b].off + i] = M->blk[b].off + M->blk[b].dim; }
   for (int q = 0; q < n_inst; ++q) {
-    M->row_lo[d + q] = 0; M->row_hi[d + q] = d; // z rows: the whole x range (plus their own diagonal)
     M->tau[q] = tau[q];
     for (int b = 0; b < nb; ++b)
-    {
       M->cz[q][b] = ((mask[b] >> q) & 1u) ? (double)(sig[b] / ((ld)M->blk[b].inv_T * (ld)tau[q])) : 0.0;
-    }
   }
   for (int b = 0; b < nb; ++b) { M->bsig[b] = (double)sig[b]; M->bmask[b] = mask[b]; }
   const int n = M->n;

@@ -20,7 +20,7 @@
 #include "dense_kernels.cuh"
 
 __global__ void k_ll_reduce(const double* __restrict__ llpart, int64_t c1, int64_t batch, int64_t N,
-                            const double* __restrict__ amp, double* __restrict__ loglik) {
+                            const double* __restrict__ amp, double* __restrict__ loglik, int* __restrict__ flags) {
   // one warp per series; fixed summation order (lane-strided partial sums, then a butterfly)
   const int64_t s = (int64_t)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
   if (s >= batch) return;
@@ -28,7 +28,11 @@ __global__ void k_ll_reduce(const double* __restrict__ llpart, int64_t c1, int64
   double acc = 0.0;
   for (int64_t c = lane; c < c1; c += 32) acc += llpart[s * c1 + c];
   for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if (lane == 0) loglik[s] = acc - (amp ? (double)N * log(amp[s]) : 0.0);
+  if (lane == 0) {
+    const double ll = acc - (amp ? (double)N * log(amp[s]) : 0.0);
+    if (!isfinite(ll)) atomicOr(flags, NUMF_BAD);
+    loglik[s] = ll;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------

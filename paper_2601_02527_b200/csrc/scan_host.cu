@@ -1,4 +1,5 @@
 #include <stddef.h>
+#include <stdio.h>
 
 #include "jit.h"
 // scan_host.cu -- host orchestration of the scan kernels (level plan, workspace carving, launches).
@@ -15,14 +16,12 @@ static int pick_lanes(const smolgp_ctx* ctx, int n) {
   return need;
 }
 
-static inline size_t tab_bytes() { return 0; } // the chunk kernels' tables travel in the kernel parameters
-
 // groups per CTA: the count that puts the most groups on one SM (228 KB of shared memory per SM,
 // 1 KB reserved per CTA, at most 128 threads per CTA); ties go to the smaller CTA
 static int groups_per_cta(size_t per_group, int G, int* groups_per_sm = nullptr) {
   int best = 1, best_sm = 0;
   for (int gpc = 1; gpc <= 128 / G; ++gpc) {
-    const size_t cta = tab_bytes() + per_group * gpc;
+    const size_t cta = per_group * gpc;
     if (cta > 227 * 1024) break;
     int ctas = (int)((228 * 1024) / (cta + 1024));
     if (ctas > 32) ctas = 32;
@@ -71,7 +70,7 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
   const int gd = fold ? fold0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G);
   const size_t per_group = (size_t)gd * 8;
   const int gpc = groups_per_cta(per_group, G);
-  const size_t smem = tab_bytes() + per_group * gpc;
+  const size_t smem = per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = P.batch * P.c1;
   const unsigned blocks = (unsigned)((groups + gpc - 1) / gpc);
@@ -264,10 +263,16 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   }
   rc = launch_level0_any(ctx, P, hm, false, G);
   if (rc) return rc;
+  {
+    char buf[256];
+    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=1 jit=%d kernels=%s", n,
+             (long long)batch, (long long)K, (long long)Lc, (long long)c1, pl.T, g, G, jk0 ? 1 : 0, "smem");
+    ctx->plan = buf;
+  }
   if (a.loglik) {
     const int wpb = 4;
     sg_launch_begin(ctx, KID_LL_REDUCE);
-    k_ll_reduce<<<(unsigned)((batch + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(P.llpart, c1, batch, N, a.amp, a.loglik);
+    k_ll_reduce<<<(unsigned)((batch + wpb - 1) / wpb), wpb * 32, 0, ctx->stream>>>(P.llpart, c1, batch, N, a.amp, a.loglik, ctx->d_flags);
     sg_launch_end(ctx);
     SG_CUDA(ctx, cudaGetLastError());
   }
@@ -278,7 +283,7 @@ template <int G, int LD>
 static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
   const size_t per_group = (size_t)query_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
   const int gpc = groups_per_cta(per_group, G);
-  const size_t smem = tab_bytes() + per_group * gpc;
+  const size_t smem = per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = Q.batch * Q.Mq;
   SG_CUDA(ctx, cudaFuncSetAttribute(k_query<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
