@@ -85,7 +85,9 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * "lanes": threads cooperating on one chunk (0 = automatic; 8, 16 or 32);
  * "jit": run-time specialisation of the chunk kernels for the kernel's structure with NVRTC
  * (0 = automatic: from 1e5 events per call, or after 32 calls with the same structure; 1 = always;
- * -1 = never).  A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
+ * -1 = never); "reg": -1 = the specialised chunk kernels in their shared-memory form instead of the register-resident
+ * one (default for n <= 24); "cpl": columns of the state per lane of the register-resident k_down0 (0 = automatic, 1-3).
+ * A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);
 const char* smolgp_jit_log(smolgp_ctx* ctx);

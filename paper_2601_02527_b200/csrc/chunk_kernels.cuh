@@ -26,6 +26,7 @@ struct ScanDev {
   double* E1;      // [batch*c1][elem]
   const double* PRE1; // [batch*c1][state] or NULL (prior)
   const double* SUF1; // [batch*c1][state] or NULL (zero)
+  const double* ADJ1; // [batch*c1][state] adjoint [lambda^ | Lambda^] at each chunk's last event (k_adjD; register kernels only) or NULL (zero)
   double* kbuf;    // [batch*N][2n+4] per end event: gain K, filtered z-column p, S, v, filtered z mean
   double* fstate;  // [batch*K][state] post-event filtered state of every event, or NULL (a7)
   double* binfo;   // [batch*K][state] information [eta | J] about the pre-update state of every event, or NULL (a7)
@@ -35,6 +36,15 @@ struct ScanDev {
   int* flags;
   int want_smooth;
 };
+
+// shared memory of one group of the register-resident kernels (chunk_reg.cuh): exchange buffer, two record
+// buffers + 2 mbarriers, three vector buffers.  Sizes in doubles; = 8 (mod 16) so that neighbouring groups of a
+// warp fall on complementary banks.
+__host__ __device__ inline int reg_ldt(int n) { return (n + 1) | 1; }
+__host__ __device__ inline int reg_tm(int n) { return ((n * reg_ldt(n) + 7) / 16) * 16 + 8; }
+__host__ __device__ inline int reg_vb(int n) { return 2 * (n + 2); }
+__host__ __device__ inline int reg_group_doubles(int n, int stride) { return ((reg_tm(n) + 2 * stride + 2 + 3 * reg_vb(n) + 7) / 16) * 16 + 8; }
+__host__ __device__ inline int reg_czs(int ni, int nb) { return (ni * nb + 1) & ~1; }
 
 // ---------------------------------------------------------------------------------------------------
 // k_fold0: chunk -> element.  Column-owned layout of chunk_dev.cuh.
@@ -497,8 +507,10 @@ __device__ __forceinline__ void query_body(const QueryDev& P) {
 // kernel entry points: templates for the static build, fixed C names for the specialised build
 // ---------------------------------------------------------------------------------------------------
 #ifdef SG_JIT
+#if !JT_REG /* otherwise chunk_reg.cuh provides the register-resident jit_fold0 / jit_down0 */
 extern "C" __global__ void __launch_bounds__(128) jit_fold0(const __grid_constant__ ScanDev P) { fold0_body<JT_G, JT_LD>(P); }
 extern "C" __global__ void __launch_bounds__(128) jit_down0(const __grid_constant__ ScanDev P) { down0_body<JT_G, JT_LD>(P); }
+#endif
 extern "C" __global__ void __launch_bounds__(128) jit_query(const __grid_constant__ QueryDev P) { query_body<JT_G, JT_LD>(P); }
 #else
 template <int G, int LD>

@@ -25,11 +25,10 @@
 
 #define RN JT_N
 #define RD JT_D
-#define RLDT ((JT_N + 1) | 1)                     /* odd row stride of the exchange buffer */
-#define RTM ((((JT_N * RLDT) + 7) / 16) * 16 + 8) /* its size, = 8 (mod 16): two groups of a warp fall on complementary banks */
-#define RVB (2 * (JT_N + 2))                      /* one vector buffer: (n + 1) pairs */
-
-__host__ __device__ inline int reg_group_doubles(int stride) { return (RTM + 2 * stride + 2 + 3 * RVB + 1) & ~1; }
+#define RLDT ((JT_N + 1) | 1)                     /* odd row stride of the exchange buffer: reg_ldt(n) */
+#define RTM ((((JT_N * RLDT) + 7) / 16) * 16 + 8) /* its size: reg_tm(n) */
+#define RVB (2 * (JT_N + 2))                      /* one vector buffer, (n + 1) pairs: reg_vb(n) */
+#define SG_REG_FENCE asm volatile("" ::: "memory")
 
 // ---- blocks of the transition on register columns -------------------------------------------------------
 // v[s][.] <- F v[s][.] for the slots S0 <= s < S1 of v (in place).  keep: bit s set => slot s keeps its old
@@ -58,6 +57,7 @@ __device__ __forceinline__ void rF_blocks(const double* __restrict__ rec, double
       for (int l = 0; l < DB; ++l) uu = fma(m[DB * DB + l], w[l], uu); // Phi-bar_b . v_b
       u[s][B] = uu;
     }
+    SG_REG_FENCE; // keeps the next block's record loads from being hoisted above this block (register pressure)
     rF_blocks<B + 1, NS, S0, S1>(rec, v, u, keep);
   }
 }
@@ -105,6 +105,7 @@ __device__ __forceinline__ void rFt_blocks(const Tab& T, const double* __restric
         v[s][OFF + l] = kp ? w[l] : acc;
       }
     }
+    SG_REG_FENCE;
     rFt_blocks<B + 1, NS>(T, rec, tz, v, keep);
   }
 }
@@ -307,8 +308,8 @@ __device__ __forceinline__ void reg_fold0_body(const ScanDev& P) {
   __syncthreads();
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  constexpr int CZS = (JT_NI * JT_NB + 1) & ~1;
-  RegSmem sm((double*)smem + CZS + (size_t)(threadIdx.x / G) * reg_group_doubles(JT_STRIDE));
+  constexpr int CZS = (JT_NI * JT_NB + 1) & ~1; // reg_czs
+  RegSmem sm((double*)smem + CZS + (size_t)(threadIdx.x / G) * reg_group_doubles(JT_N, JT_STRIDE));
   Cols<G, CPL> cl;
   cl.init(g.gl);
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
@@ -461,8 +462,8 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
   __syncthreads();
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  constexpr int CZS = (JT_NI * JT_NB + 1) & ~1;
-  RegSmem sm((double*)smem + CZS + (size_t)(threadIdx.x / G) * reg_group_doubles(JT_STRIDE));
+  constexpr int CZS = (JT_NI * JT_NB + 1) & ~1; // reg_czs
+  RegSmem sm((double*)smem + CZS + (size_t)(threadIdx.x / G) * reg_group_doubles(JT_N, JT_STRIDE));
   Cols<G, CPL> cl;
   cl.init(g.gl);
   const int ss = state_size(RN), ks = kbuf_stride(RN);

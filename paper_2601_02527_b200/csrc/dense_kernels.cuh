@@ -270,8 +270,65 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// k_adjD: the adjoint of the forward filter at each chunk's last event from the reverse scan's suffix
+// information (eta, J) about the state after the chunk and the state (m, P) there (= the prefix state of the
+// next chunk):  Lambda^ = (I + J P)^-1 J,  lambda^ = (I + J P)^-1 (J m - eta)   (I + J P has eigenvalues >= 1).
+// It starts the adjoint recursion of the register-resident k_down0, which therefore carries no solve workspace.
+// One CTA per chunk; the last chunk of a series has no later data: zero.  J P cancels like the products of the
+// dense combine: compensated (Dot2).
+// ---------------------------------------------------------------------------------------------------
+struct AdjArgs {
+  int n;
+  const double* PRE; // [batch*c1][state] prefix states [m | P]
+  const double* SUF; // [batch*c1][state] suffix information [eta | J]
+  double* ADJ;       // [batch*c1][state] out: [lambda^ | Lambda^]
+  int64_t c1, batch;
+};
+__host__ __device__ inline int adjD_group_doubles(int n) { return 2 * state_size(n) + n * (2 * n + 2) + n * (n + 1) + n; }
+
+template <int NT>
+__device__ __forceinline__ void adjD_body(const AdjArgs& P) {
+  extern __shared__ __align__(16) char smem[];
+#ifdef SG_JIT
+  const int n = JT_N;
+#else
+  const int n = P.n;
+#endif
+  const int n1 = n + 1, ss = state_size(n), ld = 2 * n + 1;
+  const Grp<NT> g;
+  const int64_t gid = blockIdx.x;
+  if (gid >= P.batch * P.c1) return;
+  const int64_t m = gid % P.c1;
+  double* out = P.ADJ + gid * (int64_t)ss;
+  if (m == P.c1 - 1) {
+    for (int e = g.gl; e < ss; e += NT) out[e] = 0.0;
+    return;
+  }
+  double* sJ = (double*)smem; double* sP = sJ + ss; double* Ws = sP + ss; double* Xs = Ws + n * (2 * n + 2); double* uv = Xs + n * n1;
+  const double* pj = P.SUF + gid * (int64_t)ss;
+  const double* pp = P.PRE + (gid + 1) * (int64_t)ss;
+  for (int e = g.gl; e < ss; e += NT) { sJ[e] = pj[e]; sP[e] = pp[e]; }
+  g.sync();
+  const double *eta = sJ, *J = sJ + n, *mv = sP, *Pm = sP + n;
+  mm(g, n, n, n, J, n, 1, Pm, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1); // J P
+  for (int i = NT - 1 - g.gl; i < n; i += NT) {
+    double acc = -eta[i], cmp = 0.0;
+    for (int l = 0; l < n; ++l) dot2_step(J[i * n + l], mv[l], acc, cmp);
+    uv[i] = acc + cmp;
+  }
+  g.sync();
+  for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n + j] = J[e]; }
+  for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + 2 * n] = uv[i]; }
+  g.sync();
+  gj_solve_np(g, n, 2 * n + 1, ld, Ws, Xs); // Xs = [Lambda^ | lambda^], row stride n + 1
+  for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; out[n + e] = 0.5 * (Xs[i * n1 + j] + Xs[j * n1 + i]); }
+  for (int i = g.gl; i < n; i += NT) out[i] = Xs[i * n1 + n];
+}
+
 
 #ifdef SG_JIT
+extern "C" __global__ void __launch_bounds__(SG_DENSE_NT) jit_adjD(const __grid_constant__ AdjArgs P) { adjD_body<SG_DENSE_NT>(P); }
 extern "C" __global__ void __launch_bounds__(SG_DENSE_NT) jit_foldD(const __grid_constant__ DenseArgs P) { foldD_body<SG_DENSE_NT>(P); }
 extern "C" __global__ void __launch_bounds__(SG_DENSE_NT) jit_downD(const __grid_constant__ DenseArgs P) { downD_body<SG_DENSE_NT>(P); }
 #else

@@ -123,6 +123,7 @@ __device__ __forceinline__ unsigned skip_mask(const EvCtl* ctl, uint32_t n, unsi
 }
 
 // look-back status word: [epoch:30 | flag:2 | count:32]; a word of another epoch reads as "not yet there"
+#define LB_WIN 8
 #define LB_AGG 1ull
 #define LB_INC 2ull
 __device__ __forceinline__ unsigned long long lb_pack(uint32_t epoch, unsigned long long flag, uint32_t v) {
@@ -206,13 +207,25 @@ __global__ void __launch_bounds__(RS_NT) k_rs_pass(EvCtl* __restrict__ ctl, int 
   for (int ww = 0; ww < RS_NT / 32; ++ww) if (ww < w) wbase += wsum[ww];
   uint32_t excl = 0;
   if (tile > 0) {
+    // look back LB_WIN tiles at a time (independent loads in flight: the walk costs one round trip per window, not per
+    // tile); entries are consumed nearest first, up to the first inclusive prefix or the first word not yet published
     int64_t t = (int64_t)tile - 1;
-    for (;;) {
-      const unsigned long long s = lb_load(status + (size_t)t * 256 + tid);
-      if ((uint32_t)(s >> 34) != epoch || ((s >> 32) & 3ull) == 0ull) continue; // not published yet
-      excl += (uint32_t)s;
-      if (((s >> 32) & 3ull) == LB_INC) break;
-      --t;
+    bool done = false;
+    while (!done) {
+      unsigned long long sw[LB_WIN];
+#pragma unroll
+      for (int i = 0; i < LB_WIN; ++i) sw[i] = (t - i >= 0) ? lb_load(status + (size_t)(t - i) * 256 + tid) : lb_pack(epoch, LB_INC, 0u);
+      int used = 0;
+#pragma unroll
+      for (int i = 0; i < LB_WIN; ++i) {
+        if (done || used != i) continue;
+        const unsigned long long s = sw[i];
+        if ((uint32_t)(s >> 34) != epoch || ((s >> 32) & 3ull) == 0ull) continue; // not published yet: retry from here
+        excl += (uint32_t)s;
+        used = i + 1;
+        if (((s >> 32) & 3ull) == LB_INC) done = true;
+      }
+      t -= used;
     }
     lb_store(st, lb_pack(epoch, LB_INC, excl + cnt));
   }

@@ -6,12 +6,13 @@
 // serves every likelihood evaluation of an optimisation over the same kernel structure.
 //
 // The source is the very text of the statically compiled kernels (csrc/jit_src.inc, written by
-// _build.py from dev_consts.h + grp_dev.cuh + chunk_dev.cuh + chunk_kernels.cuh + dense_kernels.cuh), compiled with NVRTC
+// _build.py from dev_consts.h + grp_dev.cuh + chunk_dev.cuh + chunk_kernels.cuh + chunk_reg.cuh + dense_kernels.cuh), compiled with NVRTC
 // for sm_100a and loaded through the runtime's library API.  NVRTC is opened with dlopen: when it is
 // not there, or a compilation fails, the generic kernels run instead (same arithmetic, same results).
 #include <dlfcn.h>
 #include <nvrtc.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "chunk_dev.cuh"
@@ -64,9 +65,9 @@ static bool open_nvrtc(NvrtcApi& a) {
   return true;
 }
 
-static std::string structure_key(const Tab& T, int G, int LD) {
-  char buf[64];
-  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, G, LD);
+static std::string structure_key(const Tab& T, const SgJitCfg& c) {
+  char buf[128];
+  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, c.G, c.LD, c.reg, c.rG, c.rCPL, c.fG, c.fCPL);
   std::string k = buf;
   for (int b = 0; b < T.nblk; ++b) { snprintf(buf, sizeof buf, "%d.%d.%d;", T.bdim[b], T.boff[b], T.roff[b]); k += buf; }
   k += "|";
@@ -83,7 +84,8 @@ static void int_table(std::string& s, const char* name, int cnt, const int* v) {
   s += "0}; return v[i]; }\n";
 }
 
-static std::string prelude(const Tab& T, int G, int LD) {
+static std::string prelude(const Tab& T, const SgJitCfg& c) {
+  const int G = c.G, LD = c.LD;
   std::string s = "#define SG_JIT 1\n"
                   "typedef long long int64_t;\ntypedef unsigned long long uint64_t;\n"
                   "typedef int int32_t;\ntypedef unsigned int uint32_t;\n";
@@ -93,6 +95,9 @@ static std::string prelude(const Tab& T, int G, int LD) {
   s += buf;
   snprintf(buf, sizeof buf, "#define JT_G %d\n#define JT_LD %d\n", G, LD);
   s += buf;
+  snprintf(buf, sizeof buf, "#define JT_REG %d\n#define JT_RG %d\n#define JT_RCPL %d\n#define JT_FG %d\n#define JT_FCPL %d\n", c.reg, c.rG, c.rCPL, c.fG, c.fCPL);
+  s += buf;
+  s += "#define JT_RTHREADS 32\n#define JT_FTHREADS 32\n";
   int v[SG_MAXINST * SG_MAXBLK];
   for (int b = 0; b < T.nblk; ++b) v[b] = T.bdim[b];
   int_table(s, "jt_bdim", T.nblk, v);
@@ -116,9 +121,9 @@ static JitState* state_of(smolgp_ctx* ctx) {
 // "hot": already compiled, or seen SG_JIT_HOT_CALLS times -- a hyper-parameter optimisation over a small
 // series then gets the specialised kernels after a few dozen evaluations, a one-off call never pays for them.
 #define SG_JIT_HOT_CALLS 32
-bool sg_jit_hot(smolgp_ctx* ctx, const Tab& T, int G, int LD, bool count) {
+bool sg_jit_hot(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg, bool count) {
   JitState* st = state_of(ctx);
-  const std::string key = structure_key(T, G, LD);
+  const std::string key = structure_key(T, cfg);
   for (auto& e : st->cache)
     if (e.key == key) return e.good;
   for (auto& c : st->calls)
@@ -141,9 +146,9 @@ const char* sg_jit_log(smolgp_ctx* ctx) { return ctx->jit ? ((JitState*)ctx->jit
 
 // returns the specialised kernels for (T's structure, G, LD), compiling them on first use; nullptr when
 // run-time compilation is unavailable or failed (the reason is kept in sg_jit_log)
-const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD) {
+const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg) {
   JitState* st = state_of(ctx);
-  const std::string key = structure_key(T, G, LD);
+  const std::string key = structure_key(T, cfg);
   for (auto& e : st->cache)
     if (e.key == key) return e.good ? &e.k : nullptr;
   if (!st->tried_open) { st->tried_open = true; if (!open_nvrtc(st->api)) st->log = "NVRTC not available (dlopen libnvrtc.so.12 failed)"; }
@@ -152,7 +157,10 @@ const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD) {
   ent.good = false;
   memset(&ent.k, 0, sizeof ent.k);
   if (st->api.ok) {
-    const std::string src = prelude(T, G, LD) + JIT_SRC;
+    const std::string src = prelude(T, cfg) + JIT_SRC;
+    if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the exact text handed to NVRTC
+      if (FILE* f = fopen(dump, "w")) { fwrite(src.data(), 1, src.size(), f); fclose(f); }
+    }
     nvrtcProgram prog = nullptr;
     const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo"};
     nvrtcResult r = st->api.create(&prog, src.c_str(), "smolgp_chunk_jit.cu", 0, nullptr, nullptr);
@@ -172,7 +180,15 @@ const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD) {
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.query, ent.k.lib, "jit_query");
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.foldD, ent.k.lib, "jit_foldD");
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.downD, ent.k.lib, "jit_downD");
-      if (e == cudaSuccess) ent.good = true;
+      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.adjD, ent.k.lib, "jit_adjD");
+      if (e == cudaSuccess) {
+        cudaFuncAttributes fa;
+        ent.k.regs_fold0 = (cudaFuncGetAttributes(&fa, (const void*)ent.k.fold0) == cudaSuccess) ? fa.numRegs : 255;
+        ent.k.regs_down0 = (cudaFuncGetAttributes(&fa, (const void*)ent.k.down0) == cudaSuccess) ? fa.numRegs : 255;
+        cudaGetLastError();
+        ent.k.cfg = cfg;
+        ent.good = true;
+      }
       else { st->log = std::string("loading the specialised kernels: ") + cudaGetErrorString(e); cudaGetLastError(); }
     }
     if (prog) st->api.destroy(&prog);

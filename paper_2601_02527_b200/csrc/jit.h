@@ -3,11 +3,20 @@
 #include "common.h"
 
 struct Tab;
+// what a specialised module is compiled for, beyond the model's structure
+struct SgJitCfg {
+  int G, LD;        // lanes per chunk and row stride of the shared-memory kernels (k_query; k_fold0 / k_down0 when !reg)
+  int reg;          // 1: k_fold0 / k_down0 are the register-resident kernels of chunk_reg.cuh
+  int rG, rCPL;     // k_down0 (register): lanes per chunk, columns per lane
+  int fG, fCPL;     // k_fold0 (register)
+};
 struct SgJitKernels {
   cudaLibrary_t lib;
-  cudaKernel_t fold0, down0, query, foldD, downD;
+  cudaKernel_t fold0, down0, query, foldD, downD, adjD;
+  SgJitCfg cfg;
+  int regs_fold0, regs_down0; // registers per thread of the compiled chunk kernels
 };
-const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, int G, int LD);
-bool sg_jit_hot(smolgp_ctx* ctx, const Tab& T, int G, int LD, bool count);
+const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg);
+bool sg_jit_hot(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg, bool count);
 void sg_jit_destroy(smolgp_ctx* ctx);
 const char* sg_jit_log(smolgp_ctx* ctx);

@@ -33,14 +33,63 @@ static int groups_per_cta(size_t per_group, int G, int* groups_per_sm = nullptr)
   return best;
 }
 
-// run-time specialised kernels (jit.cu): always when asked for; by default from 1e5 events per call, or
-// once the same structure has been evaluated a few dozen times (tiered: sg_jit_hot).  The one-off
-// compilation (~6 s per model structure) is cached in the ctx.
-static bool want_jit(smolgp_ctx* ctx, int64_t events, const Tab& T, int G, int ld, bool count) {
-  if (ctx->opt_jit != 0) return ctx->opt_jit > 0;
-  const bool hot = sg_jit_hot(ctx, T, G, ld, count); // counted once per API call (sg_run_scan)
-  return events >= 100000 || hot;
+// ---- which level-0 (chunk) kernels run ---------------------------------------------------------------
+// Run-time specialised kernels (jit.cu): always when asked for; by default from 1e5 events per call, or once the
+// same structure has been evaluated a few dozen times (tiered: sg_jit_hot).  The one-off compilation (a few
+// seconds per model structure) is cached in the ctx.  A specialised module holds the REGISTER-RESIDENT
+// k_fold0 / k_down0 (chunk_reg.cuh) when the state fits the register file (n <= SG_REG_NMAX), else the
+// shared-memory ones with n as a constant.
+#define SG_REG_NMAX 24
+struct L0Plan {
+  const SgJitKernels* jk; // nullptr: the statically compiled generic kernels
+  SgJitCfg cfg;
+};
+
+// lanes x columns-per-lane of the register-resident k_down0: G * CPL >= n + 1 with the least idle slots, at most
+// 63 state doubles per lane; ties go to fewer columns per lane (register pressure)
+static void pick_reg_shape(int n, int max_doubles, int mats, int* G, int* CPL) {
+  int bestG = 32, bestC = 1, bestW = 1 << 30;
+  for (int c = 1; c <= 3; ++c) {
+    if (c > 1 && mats * c * n > max_doubles) break;
+    for (int gsz = 4; gsz <= 32; gsz *= 2) {
+      if (gsz * c < n + 1) continue;
+      const int waste = gsz * c - (n + 1);
+      if (waste < bestW) { bestW = waste; bestG = gsz; bestC = c; }
+      break;
+    }
+  }
+  *G = bestG; *CPL = bestC;
 }
+
+static SgJitCfg make_cfg(smolgp_ctx* ctx, const Tab& T, int G) {
+  SgJitCfg c;
+  c.G = G; c.LD = (T.n + 1) | 1; // the specialised shared-memory kernels take the tightest odd stride
+  c.reg = (T.n <= SG_REG_NMAX && ctx->opt_reg >= 0) ? 1 : 0;
+  pick_reg_shape(T.n, 64, 1, &c.rG, &c.rCPL);
+  pick_reg_shape(T.n, 72, 3, &c.fG, &c.fCPL);
+  if (ctx->opt_rcpl >= 1 && ctx->opt_rcpl <= 3) { // tuning override: columns per lane of k_down0
+    c.rCPL = (int)ctx->opt_rcpl;
+    c.rG = 4;
+    while (c.rG * c.rCPL < T.n + 1) c.rG *= 2;
+  }
+  if (!c.reg) { c.rG = c.rCPL = c.fG = c.fCPL = 0; }
+  return c;
+}
+
+static L0Plan plan_l0(smolgp_ctx* ctx, const Tab& T, int G, int64_t events, bool count) {
+  L0Plan p;
+  p.cfg = make_cfg(ctx, T, G);
+  p.jk = nullptr;
+  bool want;
+  if (ctx->opt_jit != 0) want = ctx->opt_jit > 0;
+  else {
+    const bool hot = sg_jit_hot(ctx, T, p.cfg, count); // counted once per API call (sg_run_scan)
+    want = events >= 100000 || hot;
+  }
+  if (want) p.jk = sg_jit_get(ctx, T, p.cfg);
+  return p;
+}
+static int l0_ld(const L0Plan& p, int n) { return p.jk ? p.cfg.LD : chunk_ld(n); } // row stride of the shared-memory kernels in effect
 
 static int launch_jit(smolgp_ctx* ctx, cudaKernel_t k, int kid, unsigned blocks, unsigned threads, size_t smem, const void* params) {
   SG_CUDA(ctx, cudaFuncSetAttribute((const void*)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -52,16 +101,19 @@ static int launch_jit(smolgp_ctx* ctx, cudaKernel_t k, int kid, unsigned blocks,
   return SMOLGP_OK;
 }
 
-// row stride in effect: the specialised kernels take the tightest odd stride (n + 1) | 1 (less shared
-// memory per group => more groups per SM); the static variants are compiled for chunk_ld(n) only
-static int eff_ld(smolgp_ctx* ctx, const Tab& T, int G, int64_t events, const SgJitKernels** jk, bool count = false) {
-  *jk = nullptr;
-  const int ldj = (T.n + 1) | 1;
-  if (want_jit(ctx, events, T, G, ldj, count)) {
-    *jk = sg_jit_get(ctx, T, G, ldj);
-    if (*jk) return ldj;
-  }
-  return chunk_ld(T.n);
+// register-resident kernels: one warp per CTA, 32 / G chunks per warp
+static size_t reg_cta_smem(const ModelDev* hm, int G) {
+  return ((size_t)reg_czs(hm->n_inst, hm->nblk) + (size_t)(32 / G) * reg_group_doubles(hm->n, hm->disc_stride)) * 8;
+}
+// chunks resident per SM (shared memory, registers, 32 CTAs)
+static int reg_groups_per_sm(const ModelDev* hm, int G, int regs) {
+  const size_t cta = reg_cta_smem(hm, G);
+  int ctas = (int)((228 * 1024) / (cta + 1024));
+  if (ctas > 32) ctas = 32;
+  const int by_regs = 65536 / (((regs + 7) / 8 * 8) * 32);
+  if (ctas > by_regs) ctas = by_regs;
+  if (ctas < 1) ctas = 1;
+  return ctas * (32 / G);
 }
 
 template <int G, int LD>
@@ -108,9 +160,16 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
     else { ctx->err = "scan: unsupported (lanes, n) combination"; return SMOLGP_EUNSUPPORTED; } \
   } while (0)
 
-static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G) {
-  const SgJitKernels* jk;
-  const int LD = eff_ld(ctx, P.T, G, P.batch * P.K, &jk);
+static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G, const L0Plan& lp) {
+  const SgJitKernels* jk = lp.jk;
+  const int64_t groups = P.batch * P.c1;
+  if (jk && jk->cfg.reg) {
+    const int rg = fold ? jk->cfg.fG : jk->cfg.rG, gpc = 32 / rg;
+    const size_t smem = reg_cta_smem(hm, rg);
+    if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+    return launch_jit(ctx, fold ? jk->fold0 : jk->down0, fold ? KID_FOLD0 : KID_DOWN0, (unsigned)((groups + gpc - 1) / gpc), 32, smem, &P);
+  }
+  const int LD = l0_ld(lp, hm->n);
   if (jk) {
     const int n = hm->n;
     const int gd = fold ? fold0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) : down0_group_doubles(n, LD, hm->disc_stride, hm->nblk, G);
@@ -118,7 +177,6 @@ static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* 
     const int gpc = groups_per_cta(per_group, G);
     const size_t smem = per_group * gpc;
     if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
-    const int64_t groups = P.batch * P.c1;
     return launch_jit(ctx, fold ? jk->fold0 : jk->down0, fold ? KID_FOLD0 : KID_DOWN0, (unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, &P);
   }
 #define SG_CALL_L0(g_, ld_) return launch_level0<g_, ld_>(ctx, P, hm, fold)
@@ -164,8 +222,11 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   const int G = pick_lanes(ctx, n);
   Tab T0;
   tab_build(hm, &T0);
-  const SgJitKernels* jk0; // specialised kernels for this model's structure, or nullptr (generic kernels)
-  const int ld0 = eff_ld(ctx, T0, G, batch * K, &jk0, true);
+  const L0Plan lp = plan_l0(ctx, T0, G, batch * K, true); // specialised kernels for this model's structure, or the generic ones
+  const SgJitKernels* jk0 = lp.jk;
+  const bool reg = jk0 && jk0->cfg.reg;
+  const int ld0 = l0_ld(lp, n);
+  const int Gd = reg ? jk0->cfg.rG : G; // lanes per chunk of k_down0
   int g = (ctx->opt_group >= 2) ? (int)ctx->opt_group : 0; // 0: automatic, set once the chunk count is known
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
@@ -174,15 +235,19 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   if (Lc <= 0) {
     // one full wave: as many chunks as groups can be resident at once (equal work per chunk, no tail);
     // a batch that already fills the machine runs one chunk per series (the sequential filter, row a8)
-    int per_sm = 1;
-    groups_per_cta((size_t)down0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
-    int per_sm_f = 1;
-    groups_per_cta((size_t)fold0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
+    int per_sm = 1, per_sm_f = 1;
+    if (reg) {
+      per_sm = reg_groups_per_sm(hm, jk0->cfg.rG, jk0->regs_down0);
+      per_sm_f = reg_groups_per_sm(hm, jk0->cfg.fG, jk0->regs_fold0);
+    } else {
+      groups_per_cta((size_t)down0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
+      groups_per_cta((size_t)fold0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
+    }
     if (per_sm_f < per_sm) per_sm = per_sm_f;
     const int64_t resident = (int64_t)ctx->sm_count * per_sm;
     // measured on config 5 (profiles/r01_sweeps.md): once the batch alone gives every SM >= 4 warps, one
     // chunk per series wins, because chunking costs the extra fold pass (~ +70 % arithmetic)
-    if (batch >= resident || batch * G >= (int64_t)ctx->sm_count * 4 * 32) Lc = K;
+    if (batch >= resident || batch * Gd >= (int64_t)ctx->sm_count * 4 * 32) Lc = K;
     else {
       const int64_t per_series = (resident + batch - 1) / batch; // chunks per series
       Lc = (K + per_series - 1) / per_series;
@@ -222,6 +287,8 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     oSUF[l] = a.want_smooth ? add((size_t)batch * pl.cnt[l] * ss * 8) : 0;
   }
   const size_t oX = a.want_smooth ? add((size_t)batch * N * kbuf_stride(n) * 8) : 0;
+  const bool use_adj = reg && pl.T && a.want_smooth; // the register k_down0 takes the chunk-end adjoint from k_adjD
+  const size_t oADJ = use_adj ? add((size_t)batch * c1 * ss * 8) : 0;
   const size_t oLL = add((size_t)batch * c1 * 8);
   void* ws;
   int rc = sg_arena(ctx, bytes, &ws);
@@ -239,9 +306,10 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   P.llpart = (double*)(w + oLL);
   P.mean = a.mean; P.var = a.var; P.flags = ctx->d_flags; P.want_smooth = a.want_smooth;
   P.fstate = a.fstate; P.binfo = a.binfo;
+  P.ADJ1 = use_adj ? (const double*)(w + oADJ) : nullptr;
 
   if (pl.T) {
-    rc = launch_level0_any(ctx, P, hm, true, G);
+    rc = launch_level0_any(ctx, P, hm, true, G, lp);
     if (rc) return rc;
     for (int l = 1; l < pl.T; ++l) {
       DenseArgs D = {};
@@ -261,12 +329,24 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
       if (rc) return rc;
     }
   }
-  rc = launch_level0_any(ctx, P, hm, false, G);
+  if (use_adj) {
+    AdjArgs A;
+    A.n = n; A.PRE = P.PRE1; A.SUF = P.SUF1; A.ADJ = (double*)(w + oADJ); A.c1 = c1; A.batch = batch;
+    const size_t smem = (size_t)adjD_group_doubles(n) * 8;
+    SG_CUDA(ctx, cudaFuncSetAttribute((const void*)jk0->adjD, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    void* args[1] = {&A};
+    sg_launch_begin(ctx, KID_DOWND); // accounted with the dense down-sweep
+    cudaError_t e = cudaLaunchKernel((const void*)jk0->adjD, dim3((unsigned)(batch * c1)), dim3(SG_DENSE_NT), args, smem, ctx->stream);
+    sg_launch_end(ctx);
+    SG_CUDA(ctx, e);
+  }
+  rc = launch_level0_any(ctx, P, hm, false, G, lp);
   if (rc) return rc;
   {
     char buf[256];
-    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=1 jit=%d kernels=%s", n,
-             (long long)batch, (long long)K, (long long)Lc, (long long)c1, pl.T, g, G, jk0 ? 1 : 0, "smem");
+    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=%d fold_lanes=%d jit=%d kernels=%s regs=%d/%d", n,
+             (long long)batch, (long long)K, (long long)Lc, (long long)c1, pl.T, g, Gd, reg ? jk0->cfg.rCPL : 1, reg ? jk0->cfg.fG : G,
+             jk0 ? 1 : 0, reg ? "reg" : "smem", jk0 ? jk0->regs_fold0 : 0, jk0 ? jk0->regs_down0 : 0);
     ctx->plan = buf;
   }
   if (a.loglik) {
@@ -318,8 +398,9 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   Q.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
   Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
   const int G = pick_lanes(ctx, n);
-  const SgJitKernels* jk;
-  const int LD = eff_ld(ctx, Q.T, G, Q.batch * Q.K, &jk);
+  const L0Plan lp = plan_l0(ctx, Q.T, G, Q.batch * Q.K, false);
+  const SgJitKernels* jk = lp.jk;
+  const int LD = l0_ld(lp, n);
   if (jk) {
     const size_t per_group = (size_t)query_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) * 8;
     const int gpc = groups_per_cta(per_group, G);
