@@ -137,7 +137,7 @@ struct RecStage {
 // for even DB the rows come in as 128-bit shared-memory loads -- all lanes read the same address, so a
 // wider broadcast load halves the number of LSU wavefronts.
 template <int DB>
-__device__ __forceinline__ void load_block(const double* __restrict__ r, double (&m)[DB * DB + DB]) {
+__device__ __forceinline__ void load_block(const double* r, double (&m)[DB * DB + DB]) { // no __restrict__: a compiler fence between blocks must hold these loads back (chunk_reg.cuh)
   if constexpr (DB % 2 == 0) {
     const double2* r2 = reinterpret_cast<const double2*>(r);
 #pragma unroll

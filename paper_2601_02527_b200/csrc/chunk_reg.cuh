@@ -31,10 +31,9 @@
 #define SG_REG_FENCE asm volatile("" ::: "memory")
 
 // ---- blocks of the transition on register columns -------------------------------------------------------
-// v[s][.] <- F v[s][.] for the slots S0 <= s < S1 of v (in place).  keep: bit s set => slot s keeps its old
-// values (the companion column in the second product of a sandwich).
+// v[s][.] <- F v[s][.] for the slots S0 <= s < S1 of v (in place)
 template <int B, int NS, int S0, int S1>
-__device__ __forceinline__ void rF_blocks(const double* __restrict__ rec, double (&v)[NS][RN], double (&u)[NS][JT_NB], unsigned keep) {
+__device__ __forceinline__ void rF_blocks(const double* rec, double (&v)[NS][RN], double (&u)[NS][JT_NB]) {
   if constexpr (B < JT_NB) {
     constexpr int DB = jt_bdim(B), OFF = jt_boff(B), RO = jt_roff(B);
     double m[DB * DB + DB];
@@ -44,28 +43,27 @@ __device__ __forceinline__ void rF_blocks(const double* __restrict__ rec, double
       double w[DB];
 #pragma unroll
       for (int l = 0; l < DB; ++l) w[l] = v[s][OFF + l];
-      const bool kp = (keep >> s) & 1u;
 #pragma unroll
       for (int i = 0; i < DB; ++i) {
-        double acc = 0.0;
+        double acc = m[i * DB] * w[0];
 #pragma unroll
-        for (int l = 0; l < DB; ++l) acc = fma(m[i * DB + l], w[l], acc);
-        v[s][OFF + i] = kp ? w[i] : acc;
+        for (int l = 1; l < DB; ++l) acc = fma(m[i * DB + l], w[l], acc);
+        v[s][OFF + i] = acc;
       }
-      double uu = 0.0;
+      double uu = m[DB * DB] * w[0];
 #pragma unroll
-      for (int l = 0; l < DB; ++l) uu = fma(m[DB * DB + l], w[l], uu); // Phi-bar_b . v_b
+      for (int l = 1; l < DB; ++l) uu = fma(m[DB * DB + l], w[l], uu); // Phi-bar_b . v_b
       u[s][B] = uu;
     }
     SG_REG_FENCE; // keeps the next block's record loads from being hoisted above this block (register pressure)
-    rF_blocks<B + 1, NS, S0, S1>(rec, v, u, keep);
+    rF_blocks<B + 1, NS, S0, S1>(rec, v, u);
   }
 }
 
 template <int NS, int S0, int S1>
-__device__ __forceinline__ void r_apply_F(const Tab& T, const double* __restrict__ rec, unsigned tz, double (&v)[NS][RN], unsigned keep) {
+__device__ __forceinline__ void r_apply_F(const Tab& T, const double* rec, unsigned tz, double (&v)[NS][RN]) {
   double u[NS][JT_NB];
-  rF_blocks<0, NS, S0, S1>(rec, v, u, keep);
+  rF_blocks<0, NS, S0, S1>(rec, v, u);
 #pragma unroll
   for (int q = 0; q < JT_NI; ++q) {
     const bool zq = (tz >> q) & 1u;
@@ -75,14 +73,14 @@ __device__ __forceinline__ void r_apply_F(const Tab& T, const double* __restrict
 #pragma unroll
       for (int b = 0; b < JT_NB; ++b)
         if (jt_czmask(q * JT_NB + b)) acc = fma(T.cz[q * JT_NB + b], u[s][b], acc);
-      if (!((keep >> s) & 1u)) v[s][RD + q] = zq ? 0.0 : acc;
+      v[s][RD + q] = zq ? 0.0 : acc;
     }
   }
 }
 
 // v[s][.] <- F^T v[s][.]
 template <int B, int NS>
-__device__ __forceinline__ void rFt_blocks(const Tab& T, const double* __restrict__ rec, unsigned tz, double (&v)[NS][RN], unsigned keep) {
+__device__ __forceinline__ void rFt_blocks(const Tab& T, const double* rec, unsigned tz, double (&v)[NS][RN]) {
   if constexpr (B < JT_NB) {
     constexpr int DB = jt_bdim(B), OFF = jt_boff(B), RO = jt_roff(B);
     double m[DB * DB + DB];
@@ -96,35 +94,33 @@ __device__ __forceinline__ void rFt_blocks(const Tab& T, const double* __restric
       double w[DB];
 #pragma unroll
       for (int i = 0; i < DB; ++i) w[i] = v[s][OFF + i];
-      const bool kp = (keep >> s) & 1u;
 #pragma unroll
       for (int l = 0; l < DB; ++l) {
         double acc = m[DB * DB + l] * sz;
 #pragma unroll
         for (int i = 0; i < DB; ++i) acc = fma(m[i * DB + l], w[i], acc);
-        v[s][OFF + l] = kp ? w[l] : acc;
+        v[s][OFF + l] = acc;
       }
     }
     SG_REG_FENCE;
-    rFt_blocks<B + 1, NS>(T, rec, tz, v, keep);
+    rFt_blocks<B + 1, NS>(T, rec, tz, v);
   }
 }
 template <int NS>
-__device__ __forceinline__ void r_apply_Ft(const Tab& T, const double* __restrict__ rec, unsigned tz, double (&v)[NS][RN], unsigned keep) {
-  rFt_blocks<0, NS>(T, rec, tz, v, keep);
+__device__ __forceinline__ void r_apply_Ft(const Tab& T, const double* rec, unsigned tz, double (&v)[NS][RN]) {
+  rFt_blocks<0, NS>(T, rec, tz, v);
 #pragma unroll
   for (int q = 0; q < JT_NI; ++q)
 #pragma unroll
     for (int s = 0; s < NS; ++s)
-      if (!((keep >> s) & 1u) && ((tz >> q) & 1u)) v[s][RD + q] = 0.0;
+      if ((tz >> q) & 1u) v[s][RD + q] = 0.0;
 }
 
 // ---- what a lane knows about its columns (fixed for the whole kernel) -----------------------------------
 template <int G, int CPL>
 struct Cols {
   int jc[CPL];      // column index of slot c: gl + c G
-  int rbase[CPL];   // exchange read: row jc for a matrix column, column n for the companion (stride below)
-  int rstride[CPL];
+  int rbase[CPL];   // exchange read: row jc of the buffer for a matrix column (row 0, unused, otherwise)
   int myblk[CPL];   // block of an x column, -1 otherwise
   int qoff[CPL];    // record offset of column (jc - off_b) of the block's Q_xx; row stride qst
   int qst[CPL];
@@ -139,8 +135,7 @@ struct Cols {
       jc[c] = j;
       if (j == RN) comp |= 1u << c;
       if (j < RN) xcol |= 1u << c;
-      rbase[c] = (j < RN) ? j * RLDT : ((j == RN) ? RN : 0);
-      rstride[c] = (j == RN) ? RLDT : 1;
+      rbase[c] = (j < RN) ? j * RLDT : 0;
       int mb = -1, qo = 0, qs = 1, q12 = 0;
 #pragma unroll
       for (int b = 0; b < JT_NB; ++b) {
@@ -155,6 +150,8 @@ struct Cols {
 // can slot c hold a z column / the companion for SOME lane?  (compile-time: the code for it is only emitted there)
 template <int G>
 __host__ __device__ constexpr bool slot_has_z(int c) { return c * G < RN && c * G + G > RD; }
+template <int G>
+__host__ __device__ constexpr bool slot_has_comp(int c) { return c * G <= RN && c * G + G > RN; }
 
 // X[c][RD + q] with a run-time q (q < JT_NI): a select chain over compile-time register indices
 __device__ __forceinline__ double get_z(const double (&x)[RN], int q) {
@@ -172,8 +169,8 @@ __device__ __forceinline__ void add_z(double (&x)[RN], int q, double val) {
   for (int p = 0; p < JT_NI; ++p) x[RD + p] = (q == p) ? x[RD + p] + val : x[RD + p];
 }
 
-// exchange: the slots S0..S1-1 of v hold COLUMNS of a matrix T; on return they hold the ROWS of the same index
-// (the companion slot gets its own column back).  Two group barriers.
+// exchange: the slots S0..S1-1 of v hold COLUMNS of a matrix T; on return the matrix slots hold the ROWS of the same
+// index (the companion slot: see r_companion_back).  Two group barriers.
 template <int G, int CPL, int NS, int S0>
 __device__ __forceinline__ void r_exchange(const Grp<G>& g, const Cols<G, CPL>& cl, double* __restrict__ Tm, double (&v)[NS][RN]) {
 #pragma unroll
@@ -186,9 +183,21 @@ __device__ __forceinline__ void r_exchange(const Grp<G>& g, const Cols<G, CPL>& 
 #pragma unroll
   for (int c = 0; c < CPL; ++c) {
 #pragma unroll
-    for (int l = 0; l < RN; ++l) v[S0 + c][l] = Tm[cl.rbase[c] + l * cl.rstride[c]];
+    for (int l = 0; l < RN; ++l) v[S0 + c][l] = Tm[cl.rbase[c] + l];
   }
   g.sync();
+}
+
+// the companion column is not part of the second product of a sandwich: its slot gets back the column it wrote
+// into the exchange buffer (no barrier needed: a lane re-reads its own stores)
+template <int G, int CPL, int NS, int S0>
+__device__ __forceinline__ void r_companion_back(const Cols<G, CPL>& cl, const double* __restrict__ Tm, double (&v)[NS][RN]) {
+#pragma unroll
+  for (int c = 0; c < CPL; ++c)
+    if (slot_has_comp<G>(c) && ((cl.comp >> c) & 1u)) {
+#pragma unroll
+      for (int i = 0; i < RN; ++i) v[S0 + c][i] = Tm[i * RLDT + RN];
+    }
 }
 
 // X <- (X + X^T) / 2 on the matrix columns of the slots S0.. (periodic: the two triangles are rounded independently)
@@ -230,7 +239,7 @@ __device__ __forceinline__ void rQ_xrows(const Tab& T, unsigned tz, int myblk, c
   }
 }
 template <int B>
-__device__ __forceinline__ void rQ_zcol(const Tab& T, const double* __restrict__ rec, const double* __restrict__ czs, unsigned tz, int q0, double (&x)[RN]) {
+__device__ __forceinline__ void rQ_zcol(const Tab& T, const double* rec, const double* __restrict__ czs, unsigned tz, int q0, double (&x)[RN]) {
   if constexpr (B < JT_NB) {
     constexpr int DB = jt_bdim(B), OFF = jt_boff(B), RO = jt_roff(B);
     const double c0 = czs[q0 * JT_NB + B];
@@ -244,7 +253,7 @@ __device__ __forceinline__ void rQ_zcol(const Tab& T, const double* __restrict__
   }
 }
 template <int G, int CPL, int NS, int S0>
-__device__ __forceinline__ void r_add_Q(const Tab& T, const Cols<G, CPL>& cl, const double* __restrict__ rec, const double* __restrict__ czs, unsigned tz,
+__device__ __forceinline__ void r_add_Q(const Tab& T, const Cols<G, CPL>& cl, const double* rec, const double* __restrict__ czs, unsigned tz,
                                         double (&v)[NS][RN]) {
 #pragma unroll
   for (int c = 0; c < CPL; ++c) {
@@ -262,19 +271,21 @@ __device__ __forceinline__ void r_add_Q(const Tab& T, const Cols<G, CPL>& cl, co
 
 // X <- F X F^T (+ Q), x <- F x on the slots S0..S0+CPL-1
 template <int G, int CPL, int NS, int S0, bool ADDQ>
-__device__ __forceinline__ void r_sandwich_F(const Grp<G>& g, const Tab& T, const Cols<G, CPL>& cl, const double* __restrict__ rec,
+__device__ __forceinline__ void r_sandwich_F(const Grp<G>& g, const Tab& T, const Cols<G, CPL>& cl, const double* rec,
                                              const double* __restrict__ czs, unsigned tz, double* __restrict__ Tm, double (&v)[NS][RN]) {
-  r_apply_F<NS, S0, S0 + CPL>(T, rec, tz, v, 0u);
+  r_apply_F<NS, S0, S0 + CPL>(T, rec, tz, v);
   r_exchange<G, CPL, NS, S0>(g, cl, Tm, v);
-  r_apply_F<NS, S0, S0 + CPL>(T, rec, tz, v, cl.comp << S0);
+  r_apply_F<NS, S0, S0 + CPL>(T, rec, tz, v);
+  r_companion_back<G, CPL, NS, S0>(cl, Tm, v);
   if (ADDQ) r_add_Q<G, CPL, NS, S0>(T, cl, rec, czs, tz, v);
 }
 template <int G, int CPL>
-__device__ __forceinline__ void r_sandwich_Ft(const Grp<G>& g, const Tab& T, const Cols<G, CPL>& cl, const double* __restrict__ rec, unsigned tz,
+__device__ __forceinline__ void r_sandwich_Ft(const Grp<G>& g, const Tab& T, const Cols<G, CPL>& cl, const double* rec, unsigned tz,
                                               double* __restrict__ Tm, double (&v)[CPL][RN]) {
-  r_apply_Ft<CPL>(T, rec, tz, v, 0u);
+  r_apply_Ft<CPL>(T, rec, tz, v);
   r_exchange<G, CPL, CPL, 0>(g, cl, Tm, v);
-  r_apply_Ft<CPL>(T, rec, tz, v, cl.comp);
+  r_apply_Ft<CPL>(T, rec, tz, v);
+  r_companion_back<G, CPL, CPL, 0>(cl, Tm, v);
 }
 
 // carve one group's shared memory
@@ -344,9 +355,9 @@ __device__ __forceinline__ void reg_fold0_body(const ScanDev& P) {
     double dl_r = 1.0, sg_r = 0.0, y_r = 0.0;
     if (!kind) { dl_r = P.delta[k]; sg_r = P.sigma[ob]; y_r = P.y[series * P.N + ob]; }
     // [A | b] <- F [A | b] and T = F C with ONE pass over the record; then C <- F T^T + Q
-    r_apply_F<NS, 0, 2 * CPL>(T, rec, tz, S, 0u);
+    r_apply_F<NS, 0, 2 * CPL>(T, rec, tz, S);
     r_exchange<G, CPL, NS, CPL>(g, cl, sm.Tm, S);
-    r_apply_F<NS, CPL, 2 * CPL>(T, rec, tz, S, 0u);
+    r_apply_F<NS, CPL, 2 * CPL>(T, rec, tz, S);
     r_add_Q<G, CPL, NS, CPL>(T, cl, rec, czs, tz, S);
 #pragma unroll
     for (int c = 0; c < CPL; ++c) // column n of C is not part of the element: keep it zero
@@ -673,7 +684,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
   }
 }
 
-extern "C" __global__ void __launch_bounds__(JT_FTHREADS) jit_fold0(const __grid_constant__ ScanDev P) { reg_fold0_body<JT_FG, JT_FCPL>(P); }
-extern "C" __global__ void __launch_bounds__(JT_RTHREADS) jit_down0(const __grid_constant__ ScanDev P) { reg_down0_body<JT_RG, JT_RCPL>(P); }
+extern "C" __global__ void __launch_bounds__(JT_FTHREADS, JT_FMINB) jit_fold0(const __grid_constant__ ScanDev P) { reg_fold0_body<JT_FG, JT_FCPL>(P); }
+extern "C" __global__ void __launch_bounds__(JT_RTHREADS, JT_RMINB) jit_down0(const __grid_constant__ ScanDev P) { reg_down0_body<JT_RG, JT_RCPL>(P); }
 
 #endif // SG_JIT && JT_REG

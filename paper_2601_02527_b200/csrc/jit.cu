@@ -67,7 +67,8 @@ static bool open_nvrtc(NvrtcApi& a) {
 
 static std::string structure_key(const Tab& T, const SgJitCfg& c) {
   char buf[128];
-  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, c.G, c.LD, c.reg, c.rG, c.rCPL, c.fG, c.fCPL);
+  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, c.G, c.LD, c.reg, c.rG, c.rCPL, c.fG, c.fCPL,
+           c.rMinB, c.fMinB);
   std::string k = buf;
   for (int b = 0; b < T.nblk; ++b) { snprintf(buf, sizeof buf, "%d.%d.%d;", T.bdim[b], T.boff[b], T.roff[b]); k += buf; }
   k += "|";
@@ -97,7 +98,8 @@ static std::string prelude(const Tab& T, const SgJitCfg& c) {
   s += buf;
   snprintf(buf, sizeof buf, "#define JT_REG %d\n#define JT_RG %d\n#define JT_RCPL %d\n#define JT_FG %d\n#define JT_FCPL %d\n", c.reg, c.rG, c.rCPL, c.fG, c.fCPL);
   s += buf;
-  s += "#define JT_RTHREADS 32\n#define JT_FTHREADS 32\n";
+  snprintf(buf, sizeof buf, "#define JT_RTHREADS 32\n#define JT_FTHREADS 32\n#define JT_RMINB %d\n#define JT_FMINB %d\n", c.rMinB, c.fMinB);
+  s += buf;
   int v[SG_MAXINST * SG_MAXBLK];
   for (int b = 0; b < T.nblk; ++b) v[b] = T.bdim[b];
   int_table(s, "jt_bdim", T.nblk, v);
@@ -174,6 +176,9 @@ const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cf
       st->api.cubin_size(prog, &cs);
       std::vector<char> cubin(cs);
       st->api.cubin(prog, cubin.data());
+      if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the cubin beside the source (nvdisasm -g maps SASS to lines)
+        if (FILE* f = fopen((std::string(dump) + ".cubin").c_str(), "wb")) { fwrite(cubin.data(), 1, cubin.size(), f); fclose(f); }
+      }
       cudaError_t e = cudaLibraryLoadData(&ent.k.lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.fold0, ent.k.lib, "jit_fold0");
       if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.down0, ent.k.lib, "jit_down0");

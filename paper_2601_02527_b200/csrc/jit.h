@@ -9,6 +9,7 @@ struct SgJitCfg {
   int reg;          // 1: k_fold0 / k_down0 are the register-resident kernels of chunk_reg.cuh
   int rG, rCPL;     // k_down0 (register): lanes per chunk, columns per lane
   int fG, fCPL;     // k_fold0 (register)
+  int rMinB, fMinB; // __launch_bounds__ min CTAs per SM of the two register kernels (caps their registers)
 };
 struct SgJitKernels {
   cudaLibrary_t lib;

@@ -65,14 +65,19 @@ static SgJitCfg make_cfg(smolgp_ctx* ctx, const Tab& T, int G) {
   SgJitCfg c;
   c.G = G; c.LD = (T.n + 1) | 1; // the specialised shared-memory kernels take the tightest odd stride
   c.reg = (T.n <= SG_REG_NMAX && ctx->opt_reg >= 0) ? 1 : 0;
-  pick_reg_shape(T.n, 64, 1, &c.rG, &c.rCPL);
-  pick_reg_shape(T.n, 72, 3, &c.fG, &c.fCPL);
+  // one column per lane for both kernels: measured on config 3 (profiles/r02_sweeps.md), more columns per lane lose
+  // more to the smaller number of resident warps than they gain from the denser packing (the chunk count is bound
+  // by the dense levels, so it cannot grow with the packing); "cpl" overrides k_down0's shape for sweeps
+  pick_reg_shape(T.n, 0, 1, &c.rG, &c.rCPL);
+  pick_reg_shape(T.n, 0, 3, &c.fG, &c.fCPL);
   if (ctx->opt_rcpl >= 1 && ctx->opt_rcpl <= 3) { // tuning override: columns per lane of k_down0
     c.rCPL = (int)ctx->opt_rcpl;
     c.rG = 4;
     while (c.rG * c.rCPL < T.n + 1) c.rG *= 2;
   }
-  if (!c.reg) { c.rG = c.rCPL = c.fG = c.fCPL = 0; }
+  c.rMinB = (ctx->opt_rminb > 0) ? (int)ctx->opt_rminb : 8;
+  c.fMinB = (ctx->opt_fminb > 0) ? (int)ctx->opt_fminb : 8;
+  if (!c.reg) { c.rG = c.rCPL = c.fG = c.fCPL = c.rMinB = c.fMinB = 0; }
   return c;
 }
 
