@@ -86,7 +86,10 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * "jit": run-time specialisation of the chunk kernels for the kernel's structure with NVRTC
  * (0 = automatic: from 1e5 events per call, or after 32 calls with the same structure; 1 = always;
  * -1 = never); "reg": -1 = the specialised chunk kernels in their shared-memory form instead of the register-resident
- * one (default for n <= 24); "cpl": columns of the state per lane of the register-resident k_down0 (0 = automatic, 1-3).
+ * one (default for n <= 24); "cpl": columns of the state per lane of the register-resident k_down0 (0 = automatic, 1-3);
+ * "rminb" / "fminb": minimum resident CTAs per SM asked of the two register-resident kernels (caps their registers;
+ * 0 = 8); "dot2": which products of the dense levels are compensated (bit 0: those forming a solve's matrix,
+ * bit 1: the others; -1 = default 1) -- sweep knobs, see profiles/r02_sweeps.md.
  * A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);

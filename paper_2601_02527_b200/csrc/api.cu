@@ -30,7 +30,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0; c->prof_cur = 0;
-  c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->opt_reg = 0; c->opt_rcpl = 0; c->opt_rminb = 0; c->opt_fminb = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
+  c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->opt_reg = 0; c->opt_rcpl = 0; c->opt_rminb = 0; c->opt_fminb = 0; c->opt_dot2 = -1; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
   c->lb_status = nullptr; c->lb_words = 0; c->lb_epoch = 0;
   // pinned: the per-call model upload is a true asynchronous copy
   if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
@@ -111,6 +111,7 @@ extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t valu
   else if (!strcmp(name, "reg")) ctx->opt_reg = value;
   else if (!strcmp(name, "cpl")) ctx->opt_rcpl = value;
   else if (!strcmp(name, "rminb")) ctx->opt_rminb = value;
+  else if (!strcmp(name, "dot2")) ctx->opt_dot2 = value;
   else if (!strcmp(name, "fminb")) ctx->opt_fminb = value;
   else { ctx->err = std::string("unknown option ") + name; return SMOLGP_EINVAL; }
   return SMOLGP_OK;

@@ -79,6 +79,7 @@ struct smolgp_ctx {
   std::vector<ProfRec> prof;       // open records of the current profiling window
   std::vector<cudaEvent_t> evpool; // recycled events
   int64_t opt_chunk, opt_group, opt_lanes, opt_top, opt_jit; // opt_jit: 0 automatic, 1 always, -1 never
+  int64_t opt_dot2; // -1 default (3)
   int64_t opt_rminb, opt_fminb; // tuning: min CTAs per SM of the register kernels
   int64_t opt_reg, opt_rcpl; // opt_reg: -1 = specialised kernels in their shared-memory form; opt_rcpl: columns per lane of the register k_down0 (0 auto)
   void* jit;       // run-time specialised kernels (jit.cu)

@@ -11,12 +11,31 @@
 #define DN (P.n)
 #endif
 
+// Which dot products are accumulated with the compensated Dot2 scheme (grp_dev.cuh): class A = the products
+// that form the matrix of a solve, I + (covariance)(information), and its right-hand sides -- their terms cancel
+// by orders of magnitude; class B = every other product of a combine (sums of like-signed or
+// well-scaled terms).  Measured on config 3 at full size (profiles/r02_sweeps.md): compensating class A alone gives
+// the same accuracy as compensating everything (variance 7.6e-10 either way; 2.8e-8 with class B alone, 5.7e-8
+// with none), so class B is plain FMA.  Option "dot2" (bit 0 = A, bit 1 = B) overrides it in the specialised build.
+#if defined(SG_JIT) && defined(JT_DOT2)
+#define SG_DOT2_A ((JT_DOT2 & 1) != 0)
+#define SG_DOT2_B ((JT_DOT2 & 2) != 0)
+#else
+#define SG_DOT2_A true
+#define SG_DOT2_B false
+#endif
+template <bool COMP>
+__device__ __forceinline__ void dot_step(double a, double b, double& s, double& c) {
+  if constexpr (COMP) dot2_step(a, b, s, c);
+  else s = fma(a, b, s);
+}
+
 // general dense product  D[i,j] = (C ? C[i,j] : 0) + sum_l A[i,l] B[l,j],  strided operands.  A thread works on
 // two outputs at a time: the two compensated chains are independent, so their fixed-latency FP64 dependencies
 // overlap (the dense levels are latency-bound, profiles/r01_dense_level_ncu.md).  skew: number of work items the
 // group has already been dealt in this phase (the next item goes to lane skew % G), so that several products
 // between two barriers load the lanes evenly.
-template <int G>
+template <bool COMP, int G>
 __device__ __forceinline__ void mm(const Grp<G>& g, int nr, int nc, int nk, const double* A, int ar, int ac,
                                    const double* B, int br, int bc, const double* C, int cr, int cc, double* D, int dr, int dc,
                                    int skew = 0) {
@@ -32,8 +51,8 @@ __device__ __forceinline__ void mm(const Grp<G>& g, int nr, int nc, int nk, cons
     double acc = C ? C[i * cr + j * cc] : 0.0, accb = C ? C[ib * cr + jb * cc] : 0.0;
     double cmp = 0.0, cmpb = 0.0;
     for (int l = 0; l < nk; ++l) {
-      dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp);
-      dot2_step(A[ib * ar + l * ac], B[l * br + jb * bc], accb, cmpb);
+      dot_step<COMP>(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp);
+      dot_step<COMP>(A[ib * ar + l * ac], B[l * br + jb * bc], accb, cmpb);
     }
     D[i * dr + j * dc] = acc + cmp;
     if (eb != e) D[ib * dr + jb * dc] = accb + cmpb;
@@ -48,7 +67,7 @@ __device__ __forceinline__ void tri_index(int e, int& i, int& j) {
 }
 // symmetric result: D[i,j] = D[j,i] = C[i,j] + sum_l A[i,l] B[l,j] for i >= j (n x n; row strides cr, dr);
 // the n (n + 1) / 2 entries of the lower triangle are the work items, two at a time as in mm
-template <int G>
+template <bool COMP, int G>
 __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const double* A, int ar, int ac,
                                        const double* B, int br, int bc, const double* C, int cr, double* D, int dr, int skew = 0) {
   const int tot = n * (n + 1) / 2;
@@ -62,8 +81,8 @@ __device__ __forceinline__ void mm_sym(const Grp<G>& g, int n, int nk, const dou
     double acc = C[i * cr + j], accb = C[ib * cr + jb];
     double cmp = 0.0, cmpb = 0.0;
     for (int l = 0; l < nk; ++l) {
-      dot2_step(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp);
-      dot2_step(A[ib * ar + l * ac], B[l * br + jb * bc], accb, cmpb);
+      dot_step<COMP>(A[i * ar + l * ac], B[l * br + j * bc], acc, cmp);
+      dot_step<COMP>(A[ib * ar + l * ac], B[l * br + jb * bc], accb, cmpb);
     }
     acc += cmp;
     D[i * dr + j] = acc;
@@ -88,11 +107,11 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   const double *Aj = ej, *Cj = ej + n * n1, *Jj = Cj + n * n;
   double *Ao = eo, *Co = eo + n * n1, *Jo = Co + n * n;
   // phase 1 (everything that needs no solve): Tm = C_i [J_j | eta_j] (n x (n+1)); T2 = J_j A_i; u = eta_j - J_j b_i
-  mm(g, n, n1, n, Ci, n, 1, Jj, n1, 1, (const double*)nullptr, 0, 0, Tm, n1, 1);
-  mm(g, n, n, n, Jj, n1, 1, Ai, n1, 1, (const double*)nullptr, 0, 0, T2, n, 1, n * n1);
+  mm<SG_DOT2_A>(g, n, n1, n, Ci, n, 1, Jj, n1, 1, (const double*)nullptr, 0, 0, Tm, n1, 1);
+  mm<SG_DOT2_B>(g, n, n, n, Jj, n1, 1, Ai, n1, 1, (const double*)nullptr, 0, 0, T2, n, 1, n * n1);
   for (int i = G - 1 - g.gl; i < n; i += G) { // dealt from the last lane down: those have the fewest items above
     double acc = Jj[i * n1 + n];
-    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(-Jj[i * n1 + l], Ai[l * n1 + n], acc, cmp); acc += cmp; }
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot_step<SG_DOT2_B>(-Jj[i * n1 + l], Ai[l * n1 + n], acc, cmp); acc += cmp; }
     uv[i] = acc;
   }
   g.sync();
@@ -105,19 +124,19 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   }
   for (int i = g.gl; i < n; i += G) Ws[i * ld + 2 * n] = Ai[i * n1 + n] + Tm[i * n1 + n];
   g.sync();
-  gj_solve_np(g, n, 3 * n + 1, ld, Ws, Xs);
+  gj_solve_reg<G, SG_GJ_CPT>(g, n, 3 * n + 1, ld, Ws, Xs);
   const double* X1 = Xs;             // M A_i           (row stride lx)
   const double* X2 = Xs + n;         // M (b_i + C_i eta_j), then X3 = M C_i follows
   // phase 2: [A | b] = A_j [X1 | x2] (b_j is added in phase 3); Tm = A_j X3
-  mm(g, n, n1, n, Aj, n1, 1, X1, lx, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
-  mm(g, n, n, n, Aj, n1, 1, X2 + 1, lx, 1, (const double*)nullptr, 0, 0, Tm, n, 1, n * n1);
+  mm<SG_DOT2_B>(g, n, n1, n, Aj, n1, 1, X1, lx, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
+  mm<SG_DOT2_B>(g, n, n, n, Aj, n1, 1, X2 + 1, lx, 1, (const double*)nullptr, 0, 0, Tm, n, 1, n * n1);
   g.sync();
   // phase 3: C = Tm A_j^T + C_j;  J = X1^T T2 + J_i;  eta = X1^T u + eta_i;  b += b_j
-  mm_sym(g, n, n, Tm, n, 1, Aj, 1, n1, Cj, n, Co, n);
-  mm_sym(g, n, n, X1, 1, lx, T2, n, 1, Ji, n1, Jo, n1, ntri);
+  mm_sym<SG_DOT2_B>(g, n, n, Tm, n, 1, Aj, 1, n1, Cj, n, Co, n);
+  mm_sym<SG_DOT2_B>(g, n, n, X1, 1, lx, T2, n, 1, Ji, n1, Jo, n1, ntri);
   for (int i = G - 1 - g.gl; i < n; i += G) {
     double acc = Ji[i * n1 + n];
-    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X1[l * lx + i], uv[l], acc, cmp); acc += cmp; }
+    { double cmp = 0.0; for (int l = 0; l < n; ++l) dot_step<SG_DOT2_B>(X1[l * lx + i], uv[l], acc, cmp); acc += cmp; }
     Jo[i * n1 + n] = acc;
     Ao[i * n1 + n] += Aj[i * n1 + n];
   }
@@ -209,21 +228,21 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       g.sync();
       const double *mv = st, *Pm = st + n;
       // Ws = [I + P J | m + P eta | P]
-      mm(g, n, n1, n, Pm, n, 1, J, n1, 1, (const double*)nullptr, 0, 0, Ws, ld, 1); // cols 0..n: P [J | eta]
+      mm<SG_DOT2_A>(g, n, n1, n, Pm, n, 1, J, n1, 1, (const double*)nullptr, 0, 0, Ws, ld, 1); // cols 0..n: P [J | eta]
       g.sync();
       for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n1 + j] = Pm[e]; }
       for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + n] += mv[i]; }
       g.sync();
-      gj_solve_np(g, n, ld, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
+      gj_solve_reg<NT, SG_GJ_CPT>(g, n, ld, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
       // m' = A x + b ; Tm = A X ; P' = Tm A^T + C
       for (int i = g.gl; i < n; i += NT) {
         double acc = A[i * n1 + n];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(A[i * n1 + l], Xs[l * n1], acc, cmp); acc += cmp; }
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot_step<SG_DOT2_B>(A[i * n1 + l], Xs[l * n1], acc, cmp); acc += cmp; }
         st2[i] = acc;
       }
-      mm(g, n, n, n, A, n1, 1, Xs + 1, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
+      mm<SG_DOT2_B>(g, n, n, n, A, n1, 1, Xs + 1, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1);
       g.sync();
-      mm_sym(g, n, n, Tm, n, 1, A, 1, n1, C, n, st2 + n, n);
+      mm_sym<SG_DOT2_B>(g, n, n, Tm, n, 1, A, 1, n1, C, n, st2 + n, n);
       g.sync();
       double* t = st; st = st2; st2 = t;
     }
@@ -243,27 +262,27 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       const double *ev = st, *Je = st + n;
       const int ld2 = 2 * n + 1; // odd row stride, 2n columns in use
       // Ws = [I + C J_e | A]
-      mm(g, n, n, n, C, n, 1, Je, n, 1, (const double*)nullptr, 0, 0, Ws, ld2, 1);
+      mm<SG_DOT2_A>(g, n, n, n, C, n, 1, Je, n, 1, (const double*)nullptr, 0, 0, Ws, ld2, 1);
       g.sync();
       for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld2 + n + j] = A[i * n1 + j]; }
       for (int i = g.gl; i < n; i += NT) Ws[i * ld2 + i] += 1.0;
       // u = eta_e - J_e b
       for (int i = g.gl; i < n; i += NT) {
         double acc = ev[i];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(-Je[i * n + l], A[l * n1 + n], acc, cmp); acc += cmp; }
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot_step<SG_DOT2_B>(-Je[i * n + l], A[l * n1 + n], acc, cmp); acc += cmp; }
         uv[i] = acc;
       }
       g.sync();
-      gj_solve_np(g, n, 2 * n, ld2, Ws, Xs);
+      gj_solve_reg<NT, SG_GJ_CPT>(g, n, 2 * n, ld2, Ws, Xs);
       const double* X = Xs; // M A, row stride n
       for (int i = g.gl; i < n; i += NT) {
         double acc = J[i * n1 + n];
-        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot2_step(X[l * n + i], uv[l], acc, cmp); acc += cmp; }
+        { double cmp = 0.0; for (int l = 0; l < n; ++l) dot_step<SG_DOT2_B>(X[l * n + i], uv[l], acc, cmp); acc += cmp; }
         st2[i] = acc;
       }
-      mm(g, n, n, n, Je, n, 1, A, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1); // Tm = J_e A
+      mm<SG_DOT2_B>(g, n, n, n, Je, n, 1, A, n1, 1, (const double*)nullptr, 0, 0, Tm, n, 1); // Tm = J_e A
       g.sync();
-      mm_sym(g, n, n, X, 1, n, Tm, n, 1, J, n1, st2 + n, n); // J' = X^T (J_e A) + J
+      mm_sym<SG_DOT2_B>(g, n, n, X, 1, n, Tm, n, 1, J, n1, st2 + n, n); // J' = X^T (J_e A) + J
       g.sync();
       double* t = st; st = st2; st2 = t;
     }
@@ -311,17 +330,17 @@ __device__ __forceinline__ void adjD_body(const AdjArgs& P) {
   for (int e = g.gl; e < ss; e += NT) { sJ[e] = pj[e]; sP[e] = pp[e]; }
   g.sync();
   const double *eta = sJ, *J = sJ + n, *mv = sP, *Pm = sP + n;
-  mm(g, n, n, n, J, n, 1, Pm, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1); // J P
+  mm<SG_DOT2_A>(g, n, n, n, J, n, 1, Pm, n, 1, (const double*)nullptr, 0, 0, Ws, ld, 1); // J P
   for (int i = NT - 1 - g.gl; i < n; i += NT) {
     double acc = -eta[i], cmp = 0.0;
-    for (int l = 0; l < n; ++l) dot2_step(J[i * n + l], mv[l], acc, cmp);
+    for (int l = 0; l < n; ++l) dot_step<SG_DOT2_A>(J[i * n + l], mv[l], acc, cmp);
     uv[i] = acc + cmp;
   }
   g.sync();
   for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n + j] = J[e]; }
   for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + 2 * n] = uv[i]; }
   g.sync();
-  gj_solve_np(g, n, 2 * n + 1, ld, Ws, Xs); // Xs = [Lambda^ | lambda^], row stride n + 1
+  gj_solve_reg<NT, SG_GJ_CPT>(g, n, 2 * n + 1, ld, Ws, Xs); // Xs = [Lambda^ | lambda^], row stride n + 1
   for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; out[n + e] = 0.5 * (Xs[i * n1 + j] + Xs[j * n1 + i]); }
   for (int i = g.gl; i < n; i += NT) out[i] = Xs[i * n1 + n];
 }

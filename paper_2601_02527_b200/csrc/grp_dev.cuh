@@ -148,3 +148,85 @@ __device__ void gj_solve_np(const Grp<G>& g, int n, int nc_all, int ld, double* 
   }
   g.sync();
 }
+
+// Gauss-Jordan as gj_solve_np (partial pivoting, no row exchange, same pivots and the same arithmetic per entry), with
+// the augmented matrix held in REGISTERS during the elimination: thread t of the CTA owns row t / tpr and the
+// columns c, c + tpr, c + 2 tpr, ... (c = t % tpr, tpr = G / n threads per row), so a pivot step touches shared
+// memory only for what crosses threads -- the pivot column (n doubles, double-buffered) and the pivot row --
+// instead of re-reading and re-writing every entry (round 1: 21 k of a combine's 61 k cycles, profiles/r01_dense_level_ncu.md).
+// Two barriers per pivot.  W (n rows, nc_all columns, row stride ld) is read once; X (n x (nc_all - n), row
+// stride nc_all - n) receives M^-1 R.  CPT >= ceil(nc_all / tpr).
+#ifdef SG_JIT
+#define SG_GJ_CPT ((3 * JT_N + 1 + (SG_DENSE_NT / JT_N) - 1) / (SG_DENSE_NT / JT_N))
+#else
+#define SG_GJ_CPT 12 /* n = 31: 8 threads per row, 94 columns */
+#endif
+#define SG_GJ_MAXC 96
+template <int G, int CPT>
+__device__ void gj_solve_reg(const Grp<G>& g, int n, int nc_all, int ld, const double* W, double* X) {
+  __shared__ double colbuf[2][32];
+  __shared__ double rowbuf[SG_GJ_MAXC];
+  const int tpr = G / n;
+  const int i = g.gl / tpr, c = g.gl - i * tpr;
+  const bool act = i < n;
+  double w[CPT];
+#pragma unroll
+  for (int s = 0; s < CPT; ++s) {
+    const int j = c + s * tpr;
+    w[s] = (act && j < nc_all) ? W[i * ld + j] : 0.0;
+  }
+  const int lane = threadIdx.x & 31;
+  unsigned used = 0u;
+  int outrow = 0;
+  double rinv = 0.0;
+  if (act && c == 0) colbuf[0][i] = w[0];
+  g.sync();
+  for (int p = 0; p < n; ++p) {
+    const double* cb = colbuf[p & 1];
+    // arg-max of |W[., p]| over the rows not yet used as a pivot: as in gj_solve_np (every warp on its own)
+    const bool cand = lane < n && !((used >> lane) & 1u);
+    const unsigned long long key = cand ? (unsigned long long)__double_as_longlong(fabs(cb[lane])) + 1ull : 0ull;
+    const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+    const unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
+    const unsigned hit = __ballot_sync(0xffffffffu, hi == mhi && lo == mlo);
+    const int r = min(__ffs(hit) - 1, n - 1);
+    used |= 1u << r;
+    const double rpv = 1.0 / cb[r];
+    if (act && i == r) {
+#pragma unroll
+      for (int s = 0; s < CPT; ++s) {
+        const int j = c + s * tpr;
+        if (j > p && j < nc_all) rowbuf[j] = w[s];
+      }
+      outrow = p;
+      rinv = rpv;
+    }
+    g.sync();
+    if (act && i != r) {
+      const double f = -cb[i] * rpv;
+#pragma unroll
+      for (int s = 0; s < CPT; ++s) {
+        const int j = c + s * tpr;
+        if (j > p && j < nc_all) w[s] = fma(f, rowbuf[j], w[s]);
+      }
+    }
+    if (p + 1 < n) { // the owners of column p + 1 publish it for the next search
+      const int ps = (p + 1) / tpr, pc = (p + 1) - ps * tpr;
+      if (act && c == pc) {
+        double v = w[0];
+#pragma unroll
+        for (int s = 1; s < CPT; ++s) v = (s == ps) ? w[s] : v;
+        colbuf[(p + 1) & 1][i] = v;
+      }
+    }
+    g.sync();
+  }
+  const int m = nc_all - n;
+#pragma unroll
+  for (int s = 0; s < CPT; ++s) {
+    const int j = c + s * tpr;
+    if (act && j >= n && j < nc_all) X[outrow * m + (j - n)] = w[s] * rinv;
+  }
+  g.sync();
+}

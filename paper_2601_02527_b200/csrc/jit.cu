@@ -67,8 +67,8 @@ static bool open_nvrtc(NvrtcApi& a) {
 
 static std::string structure_key(const Tab& T, const SgJitCfg& c) {
   char buf[128];
-  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, c.G, c.LD, c.reg, c.rG, c.rCPL, c.fG, c.fCPL,
-           c.rMinB, c.fMinB);
+  snprintf(buf, sizeof buf, "%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d,%d|", T.n, T.d, T.ninst, T.nblk, T.stride, c.G, c.LD, c.reg, c.rG, c.rCPL, c.fG, c.fCPL,
+           c.rMinB, c.fMinB, c.dot2);
   std::string k = buf;
   for (int b = 0; b < T.nblk; ++b) { snprintf(buf, sizeof buf, "%d.%d.%d;", T.bdim[b], T.boff[b], T.roff[b]); k += buf; }
   k += "|";
@@ -98,7 +98,7 @@ static std::string prelude(const Tab& T, const SgJitCfg& c) {
   s += buf;
   snprintf(buf, sizeof buf, "#define JT_REG %d\n#define JT_RG %d\n#define JT_RCPL %d\n#define JT_FG %d\n#define JT_FCPL %d\n", c.reg, c.rG, c.rCPL, c.fG, c.fCPL);
   s += buf;
-  snprintf(buf, sizeof buf, "#define JT_RTHREADS 32\n#define JT_FTHREADS 32\n#define JT_RMINB %d\n#define JT_FMINB %d\n", c.rMinB, c.fMinB);
+  snprintf(buf, sizeof buf, "#define JT_RTHREADS 32\n#define JT_FTHREADS 32\n#define JT_RMINB %d\n#define JT_FMINB %d\n#define JT_DOT2 %d\n", c.rMinB, c.fMinB, c.dot2);
   s += buf;
   int v[SG_MAXINST * SG_MAXBLK];
   for (int b = 0; b < T.nblk; ++b) v[b] = T.bdim[b];

@@ -9,6 +9,7 @@ struct SgJitCfg {
   int reg;          // 1: k_fold0 / k_down0 are the register-resident kernels of chunk_reg.cuh
   int rG, rCPL;     // k_down0 (register): lanes per chunk, columns per lane
   int fG, fCPL;     // k_fold0 (register)
+  int dot2;         // bit 0: class-A products of the dense levels compensated, bit 1: class-B (dense_kernels.cuh)
   int rMinB, fMinB; // __launch_bounds__ min CTAs per SM of the two register kernels (caps their registers)
 };
 struct SgJitKernels {

@@ -75,6 +75,7 @@ static SgJitCfg make_cfg(smolgp_ctx* ctx, const Tab& T, int G) {
     c.rG = 4;
     while (c.rG * c.rCPL < T.n + 1) c.rG *= 2;
   }
+  c.dot2 = (ctx->opt_dot2 >= 0 && ctx->opt_dot2 <= 3) ? (int)ctx->opt_dot2 : 1;
   c.rMinB = (ctx->opt_rminb > 0) ? (int)ctx->opt_rminb : 8;
   c.fMinB = (ctx->opt_fminb > 0) ? (int)ctx->opt_fminb : 8;
   if (!c.reg) { c.rG = c.rCPL = c.fG = c.fCPL = c.rMinB = c.fMinB = 0; }
