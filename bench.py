@@ -395,6 +395,123 @@ def run_cuda(args, w, cfgname):
         dist.destroy_process_group()
 
 
+# ----------------------------------------------------------------------------------------------
+# prediction workload (the paper's third benchmark column): condition + predict at
+# M = mult x N query times
+# ----------------------------------------------------------------------------------------------
+def run_predict(args, w, cfgname):
+    import torch
+    from paper_2601_02527_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py --workload predict: single GPU only")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    ctx = B.Context(0)
+    N = w["t_start"].size
+    batch = w["batch"] or 1
+    n = model_dim(w)
+    M = int(args.predict_mult * N)
+    t0, t1 = float(w["t_start"].min()), float(w["t_end"].max())
+    tq_h = np.linspace(t0 - 0.001 * (t1 - t0), t1 + 0.001 * (t1 - t0), M)  # uniform grid over the data span (and a little beyond)
+    h2d = lambda a: torch.tensor(a, device=dev)
+    ts, te, ins, y, sg, tq = (h2d(a) for a in (w["t_start"], w["t_end"], w["instrument"], w["y"], w["sigma"], tq_h))
+    amp = None if w["amp"] is None else h2d(w["amp"])
+    out = dict(mean=torch.empty((batch, N), dtype=torch.float64, device=dev), var=torch.empty((batch, N), dtype=torch.float64, device=dev),
+               loglik=torch.empty(batch, dtype=torch.float64, device=dev),
+               mean_query=torch.empty((batch, M), dtype=torch.float64, device=dev), var_query=torch.empty((batch, M), dtype=torch.float64, device=dev))
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        ev = ctx.smolgp_build_events(ts, te, ins, w["n_inst"])
+        ctx.smolgp_condition(ev, w["kernel"], y, sg, amp=amp, t_query=tq, query_instrument=0, out=out)
+        ev.free()
+
+    sampler = ClockSampler(0)
+    sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    ctx.memory_info(reset_peak=True)
+    l0 = ctx.launch_count()
+    evs = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); step(); b.record()
+        evs.append((a, b))
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
+    launches = (ctx.launch_count() - l0) // args.steps
+    _, peak_bytes = ctx.memory_info()
+    ctx.profile(True)
+    step()
+    prof = ctx.profile_read()
+    ctx.profile(False)
+    # end to end from pinned host buffers (queries and their outputs cross PCIe every step)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    hts, hte, hins, hy, hsg, htq = (pin(a) for a in (w["t_start"], w["t_end"], w["instrument"], w["y"], w["sigma"], tq_h))
+    hamp = None if w["amp"] is None else pin(w["amp"])
+    hout = dict(mean=pin(np.empty((batch, N))), var=pin(np.empty((batch, N))), loglik=pin(np.empty(batch)),
+                mean_query=pin(np.empty((batch, M))), var_query=pin(np.empty((batch, M))))
+
+    def step_e2e():
+        ev = ctx.smolgp_build_events_host(hts, hte, hins, w["n_inst"])
+        ctx.smolgp_condition_host(ev, w["kernel"], hy, hsg, amp=hamp, t_query=htq, query_instrument=0, out=hout)
+        ev.free()
+
+    step_e2e()
+    torch.cuda.synchronize()
+    evs2 = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); step_e2e(); b.record()
+        evs2.append((a, b))
+    torch.cuda.synchronize()
+    ms_e2e = sum(a.elapsed_time(b) for a, b in evs2) / args.steps
+    clocks = sampler.stop()
+    hbm_gbs, hbm_src = hbm_peak_gbs()
+    # algorithmic bytes of the query kernel: per query the two stored states it combines (filtered state of the event
+    # before, adjoint of the event after: "all 2N states"), its two step records, 8 B in, 16 B out
+    stride_bytes = None
+    qbytes = 2 * 8 * (n + n * n) + 16 + 8
+    t_q = prof.get("k_query", (0.0, 1))[0]
+    roofline = {"bound": "hbm", "kernel": "k_query", "achieved": batch * M * qbytes / (t_q * 1e-3) / 1e9 if t_q else None,
+                "peak": hbm_gbs, "unit": "GB/s", "frac": (batch * M * qbytes / (t_q * 1e-3) / 1e9 / hbm_gbs) if t_q else None, "traffic": None,
+                "peak_source": hbm_src,
+                "work_model": "per query: two stored states of n + n^2 doubles + 24 B (neighbouring queries share the states through L2, so achieved can exceed the DRAM peak)",
+                "kernels_ms_per_step": {k: v[0] for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
+    # CPU baseline: the oracle's Algorithm 1 on a bounded sample (first ns exposures, mult x ns queries inside their span)
+    import oracle
+    oracle.build()
+    ns = min(N, 400)
+    sl = slice(0, ns)
+    yy = w["y"][0, sl] if w["y"].ndim == 2 else w["y"][sl]
+    kern = w["kernel"] if w.get("amp") is None else [dict(k, sigma=k["sigma"] * float(w["amp"][0])) for k in w["kernel"]]
+    tq_s = np.linspace(float(w["t_start"][sl].min()), float(w["t_end"][sl].max()), int(args.predict_mult * ns))
+    tc = time.perf_counter()
+    oracle.ssm(kern, w["n_inst"], w["t_start"][sl], w["t_end"][sl], w["instrument"][sl], yy, w["sigma"][sl],
+               flags=oracle.FLAG_TWO_FILTER, tq=tq_s, query_inst=0, prec="f64")
+    tc = time.perf_counter() - tc
+    line = {"metric": "queries/sec for condition + predict at M = %g N (P:561)" % args.predict_mult, "value": batch * M / (ms * 1e-3), "unit": "queries/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "predict: " + cfgname, "N": N, "events": 2 * N, "M": M, "batch": batch, "state_dim": n,
+                       "path": "a1-a6 + a7 (Algorithm 1 at M uniform query times)", "l2": "flushed (512 MiB write) between timed iterations",
+                       "plan": ctx.plan_info()},
+            "events_per_s": batch * 2 * N / (ms * 1e-3),
+            "peak_device_bytes": int(peak_bytes),
+            "e2e": {"value": batch * M / (ms_e2e * 1e-3), "unit": "queries/s", "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": int(hts.nbytes + hte.nbytes + hins.nbytes + hy.nbytes + hsg.nbytes + htq.nbytes + (0 if hamp is None else hamp.nbytes)),
+                    "d2h_bytes_per_step": int(sum(v.nbytes for v in hout.values()))},
+            "gpu_launches": int(launches), "specialised": "jit=1" in ctx.plan_info(), "jit_log": ctx.jit_log(), "clocks": clocks, "roofline": roofline,
+            "cpu_baseline": {"value": tq_s.size / tc, "unit": "queries/s", "cores": 1, "kind": "oracle",
+                             "sample": "first %d exposures, %d queries, oracle fp64 build (filter + two-filter smoother + Algorithm 1), 1 thread, %.1f s" % (ns, tq_s.size, tc)}}
+    print(json.dumps(line), flush=True)
+
+
 CFG_NAMES = {1: "cfg1 Matern-3/2 N=1e3", 2: "cfg2 SHO two instruments N=2e4",
              3: "cfg3 quasiperiodic Matern-3/2 x periodic(J=4), 3 overlapping instruments, n=21, N=1e5 (K=2e5 events)",
              4: "cfg4 joint multi-instrument n=17 N=1e6", 5: "cfg5 batched 4096 x N=2048, n=7"}
@@ -407,10 +524,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-5); 3 = the headline N=1e5")
+    ap.add_argument("--workload", default="condition", choices=["condition", "predict"],
+                    help="condition = the headline (rows a1-a6); predict = condition + prediction at --predict-mult x N query times (row a7)")
+    ap.add_argument("--predict-mult", type=float, default=100.0, help="queries per exposure of the predict workload (the paper uses M = 100 N, P:561)")
     args = ap.parse_args()
     w = W.make(args.config)
     if args.impl == "reference":
         run_reference(args, w, CFG_NAMES[args.config])
+    elif args.workload == "predict":
+        run_predict(args, w, CFG_NAMES[args.config])
     else:
         run_cuda(args, w, CFG_NAMES[args.config])
 

@@ -98,6 +98,12 @@ const char* smolgp_jit_log(smolgp_ctx* ctx);
  * "n=21 batch=1 K=200000 chunk=136 chunks=1471 levels=10 fanin=2 lanes=8 cpl=3 jit=1 kernels=reg": which kernels
  * ran (jit=1: the run-time specialised ones) and how the events were cut.  For bench.py and the tests. */
 const char* smolgp_plan_info(const smolgp_ctx* ctx);
+/* Device memory held by the ctx: bytes now, and the high-water mark since creation or the last reset (the
+ * workspace arena, the model + discretisation array, the event-build status words and, inside a call, the
+ * event stream it was given and the state store of query-time prediction: 2 batch K (n + n^2) doubles
+ * "all 2N states").  The per-query scratch of smolgp_condition is bounded (256 MB) whatever M is.  HOST outputs,
+ * either may be NULL. */
+int smolgp_memory_info(smolgp_ctx* ctx, int64_t* current_bytes, int64_t* peak_bytes, int32_t reset_peak);
 
 /* Step a1.  Turns N exposures [t_start[n], t_end[n]] of instrument
  * instrument[n] in [0, n_inst) into the time-sorted stream of K = 2N events (one reset event per

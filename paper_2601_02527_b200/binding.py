@@ -14,7 +14,7 @@ STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
            "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
-           "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info"]
+           "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info", "smolgp_memory_info"]
 NKERNELS = 11  # SMOLGP_NKERNELS
 
 
@@ -69,6 +69,7 @@ def lib():
         L.smolgp_jit_log.restype = C.c_char_p
         L.smolgp_plan_info.argtypes = [vp]
         L.smolgp_plan_info.restype = C.c_char_p
+        L.smolgp_memory_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), i32]
         _lib = L
     return _lib
 
@@ -165,6 +166,12 @@ class Context:
 
     def jit_log(self):
         return lib().smolgp_jit_log(self.handle).decode()
+
+    def memory_info(self, reset_peak=False):
+        """(bytes held now, high-water mark) of this ctx's device memory"""
+        cur, peak = C.c_int64(), C.c_int64()
+        self._check(lib().smolgp_memory_info(self.handle, C.byref(cur), C.byref(peak), int(bool(reset_peak))))
+        return cur.value, peak.value
 
     def plan_info(self):
         return lib().smolgp_plan_info(self.handle).decode()

@@ -18,6 +18,7 @@ int sg_arena(smolgp_ctx* ctx, size_t bytes, void** out) {
     }
     ctx->arena_bytes = want;
   }
+  sg_mem_mark(ctx);
   *out = ctx->arena;
   return SMOLGP_OK;
 }
@@ -31,7 +32,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0; c->prof_cur = 0;
   c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->opt_reg = 0; c->opt_rcpl = 0; c->opt_rminb = 0; c->opt_fminb = 0; c->opt_dot2 = -1; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
-  c->lb_status = nullptr; c->lb_words = 0; c->lb_epoch = 0;
+  c->lb_status = nullptr; c->lb_words = 0; c->lb_epoch = 0; c->mem_extra = 0; c->mem_peak = 0;
   // pinned: the per-call model upload is a true asynchronous copy
   if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
   int v = 0;
@@ -100,6 +101,13 @@ extern "C" int smolgp_profile_read(smolgp_ctx* ctx, double* ms, int64_t* launche
 
 extern "C" const char* smolgp_jit_log(smolgp_ctx* ctx) { return ctx ? sg_jit_log(ctx) : ""; }
 extern "C" const char* smolgp_plan_info(const smolgp_ctx* ctx) { return ctx ? ctx->plan.c_str() : ""; }
+extern "C" int smolgp_memory_info(smolgp_ctx* ctx, int64_t* current_bytes, int64_t* peak_bytes, int32_t reset_peak) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (current_bytes) *current_bytes = (int64_t)sg_mem_now(ctx);
+  if (peak_bytes) *peak_bytes = (int64_t)ctx->mem_peak;
+  if (reset_peak) ctx->mem_peak = sg_mem_now(ctx);
+  return SMOLGP_OK;
+}
 
 extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value) {
   if (!ctx || !name) return SMOLGP_EINVAL;
@@ -139,6 +147,8 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
     if (cudaMalloc(&ctx->pers, model_b + disc_b) != cudaSuccess) { cudaGetLastError(); ctx->pers = nullptr; ctx->err = "out of device memory (discretisation)"; return SMOLGP_ENOMEM; }
     ctx->pers_bytes = model_b + disc_b;
   }
+  const size_t ev_bytes = (size_t)ev->K * 28; // the caller's event stream: counted with the call that uses it
+  sg_mem_mark(ctx, ev_bytes);
   void* pers = ctx->pers;
   ModelDev* dm = (ModelDev*)pers;
   double* disc = (double*)((char*)pers + model_b);
@@ -157,6 +167,8 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
     const size_t one = (size_t)batch * ev->K * (hm.n + hm.n * hm.n) * 8;
     if (cudaMallocAsync(&qstore, 2 * one, ctx->stream) != cudaSuccess) { cudaGetLastError(); ctx->err = "out of device memory (states for query-time prediction)"; return SMOLGP_ENOMEM; }
     a.fstate = qstore; a.binfo = (double*)((char*)qstore + one);
+    ctx->mem_extra += 2 * one;
+    sg_mem_mark(ctx, ev_bytes);
   }
   rc = sg_run_scan(ctx, a);
   if (rc == SMOLGP_OK && qs.M > 0) {
@@ -165,6 +177,8 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
     q.fstate = a.fstate; q.binfo = a.binfo; q.mean = qs.mean; q.var = qs.var;
     rc = sg_run_query(ctx, q);
   }
+  sg_mem_mark(ctx, ev_bytes);
+  if (qstore) ctx->mem_extra -= 2 * (size_t)batch * ev->K * (hm.n + hm.n * hm.n) * 8;
   if (rc) { if (qstore) cudaFreeAsync(qstore, ctx->stream); return rc; }
   int flags = 0;
   cudaError_t ce = cudaMemcpyAsync(&flags, ctx->d_flags, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);

@@ -403,7 +403,8 @@ struct QueryDev {
   const double* fstate;
   const double* binfo;
   const double* amp;
-  int64_t K, Mq, batch;
+  int64_t K, Mq, batch; // Mq: queries of this slice
+  int64_t Mtot, q0;     // the outputs are [batch][Mtot]; the slice starts at query q0
   int qinst;
   double* mean; // [batch][M]
   double* var;
@@ -497,8 +498,8 @@ __device__ __forceinline__ void query_body(const QueryDev& P) {
   sv = group_sum(g, sv);
   if (g.gl == 0) {
     if (!isfinite(sv) || !isfinite(sm)) atomicOr(P.flags, NUMF_BAD);
-    P.mean[series * P.Mq + q] = ampv * sm;
-    P.var[series * P.Mq + q] = ampv * ampv * sv;
+    P.mean[series * P.Mtot + P.q0 + q] = ampv * sm;
+    P.var[series * P.Mtot + P.q0 + q] = ampv * ampv * sv;
   }
 }
 

@@ -92,6 +92,8 @@ struct smolgp_ctx {
   ModelDev* hmodel; // host copy of the current model
   int sm_count;
   size_t smem_optin;
+  size_t mem_extra;  // stream-ordered allocations alive inside the current call (query state store, host staging)
+  size_t mem_peak;   // high-water mark of the device memory this ctx holds (smolgp_memory_info)
   // decoupled look-back words of the event build (events.cu): persistent, told apart by epoch
   unsigned long long* lb_status;
   size_t lb_words;
@@ -165,3 +167,6 @@ struct QueryArgs {
 int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a);
 // arena helper
 int sg_arena(smolgp_ctx* ctx, size_t bytes, void** out);
+// device bytes held by the ctx right now (workspace arena, model + discretisation array, sort status, flags, in-call extras)
+static inline size_t sg_mem_now(const smolgp_ctx* ctx) { return ctx->arena_bytes + ctx->pers_bytes + ctx->lb_words * 8 + 64 + ctx->mem_extra; }
+static inline void sg_mem_mark(smolgp_ctx* ctx, size_t also = 0) { const size_t v = sg_mem_now(ctx) + also; if (v > ctx->mem_peak) ctx->mem_peak = v; }

@@ -389,6 +389,7 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   void* scratch;
   rc = sg_arena(ctx, ctl_b + 2 * k8 + 2 * k4, &scratch);
   if (rc) return fail(rc);
+  sg_mem_mark(ctx, 3 * k8 + 2 * k4);
   char* p = (char*)scratch;
   EvCtl* ctl = (EvCtl*)p; p += ctl_b;
   uint64_t* kA = (uint64_t*)p; p += k8;

@@ -380,41 +380,53 @@ static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) 
   return SMOLGP_OK;
 }
 
-// Row a7.  Scratch (kp, dtq, discq) comes from the arena: the scan's workspace is dead by now
-// (stream order), fstate/binfo live outside it.
+// Row a7.  Scratch (kp, dtq, discq) comes from the arena: the scan's workspace is dead by now (stream order),
+// fstate/binfo live outside it.  The queries are processed in slices so that the scratch (two discretisation
+// records per query) stays below SG_QUERY_SCRATCH bytes whatever M is (M = 100 N in the paper's third benchmark
+// column, would otherwise need 2 M records: 29 GB on config 3).
+#define SG_QUERY_SCRATCH ((size_t)256 << 20)
 int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   const ModelDev* hm = a.h_model;
   const int n = hm->n;
-  const int64_t M = a.M;
-  const size_t o_kp = 0, o_dt = ((size_t)M * 8 + 255) / 256 * 256, o_disc = o_dt + ((size_t)2 * M * 8 + 255) / 256 * 256;
+  const size_t per_query = (size_t)2 * hm->disc_stride * 8 + 24;
+  int64_t slice = (int64_t)(SG_QUERY_SCRATCH / per_query);
+  if (slice < 4096) slice = 4096;
+  if (slice > a.M) slice = a.M;
+  const size_t o_kp = 0, o_dt = ((size_t)slice * 8 + 255) / 256 * 256, o_disc = o_dt + ((size_t)2 * slice * 8 + 255) / 256 * 256;
   void* ws;
-  int rc = sg_arena(ctx, o_disc + (size_t)2 * M * hm->disc_stride * 8, &ws);
+  int rc = sg_arena(ctx, o_disc + (size_t)2 * slice * hm->disc_stride * 8, &ws);
   if (rc) return rc;
   int64_t* kp = (int64_t*)((char*)ws + o_kp);
   double* dtq = (double*)((char*)ws + o_dt);
   double* discq = (double*)((char*)ws + o_disc);
-  sg_launch_begin(ctx, KID_QLOCATE);
-  k_query_locate<<<(unsigned)((M + 127) / 128), 128, 0, ctx->stream>>>(M, a.tq, a.ev->K, a.ev->t, kp, dtq);
-  sg_launch_end(ctx);
-  SG_CUDA(ctx, cudaGetLastError());
-  rc = sg_launch_disc(ctx, a.d_model, hm, dtq, 2 * M, discq);
-  if (rc) return rc;
   QueryDev Q;
   tab_build(hm, &Q.T);
   Q.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
-  Q.K = a.ev->K; Q.Mq = M; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags;
+  Q.K = a.ev->K; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags; Q.Mtot = a.M;
   const int G = pick_lanes(ctx, n);
   const L0Plan lp = plan_l0(ctx, Q.T, G, Q.batch * Q.K, false);
   const SgJitKernels* jk = lp.jk;
   const int LD = l0_ld(lp, n);
-  if (jk) {
-    const size_t per_group = (size_t)query_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) * 8;
-    const int gpc = groups_per_cta(per_group, G);
-    const int64_t groups = Q.batch * Q.Mq;
-    return launch_jit(ctx, jk->query, KID_QUERY, (unsigned)((groups + gpc - 1) / gpc), gpc * G, per_group * gpc, &Q);
-  }
-#define SG_CALL_Q(g_, ld_) return launch_query<g_, ld_>(ctx, Q, hm)
-  SG_DISPATCH_GL(G, LD, SG_CALL_Q);
+  for (int64_t q0 = 0; q0 < a.M; q0 += slice) {
+    const int64_t M = (a.M - q0 < slice) ? a.M - q0 : slice;
+    Q.Mq = M; Q.q0 = q0;
+    sg_launch_begin(ctx, KID_QLOCATE);
+    k_query_locate<<<(unsigned)((M + 127) / 128), 128, 0, ctx->stream>>>(M, a.tq + q0, a.ev->K, a.ev->t, kp, dtq);
+    sg_launch_end(ctx);
+    SG_CUDA(ctx, cudaGetLastError());
+    rc = sg_launch_disc(ctx, a.d_model, hm, dtq, 2 * M, discq);
+    if (rc) return rc;
+    if (jk) {
+      const size_t per_group = (size_t)query_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) * 8;
+      const int gpc = groups_per_cta(per_group, G);
+      const int64_t groups = Q.batch * Q.Mq;
+      rc = launch_jit(ctx, jk->query, KID_QUERY, (unsigned)((groups + gpc - 1) / gpc), gpc * G, per_group * gpc, &Q);
+    } else {
+#define SG_CALL_Q(g_, ld_) rc = launch_query<g_, ld_>(ctx, Q, hm)
+      SG_DISPATCH_GL(G, LD, SG_CALL_Q);
 #undef SG_CALL_Q
-  return SMOLGP_EUNSUPPORTED;
+    }
+    if (rc) return rc;
+  }
+  return SMOLGP_OK;
 }
