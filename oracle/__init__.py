@@ -160,3 +160,36 @@ def ssm(kern, ninst, ts, te, inst, y, sigma, flags=FLAG_TWO_FILTER, zprior=1.0, 
     g = _lib(prec).oracle_ssm_disc_seconds  # instrumentation: seconds of this call spent in the discretisation
     g.restype = C.c_double
     return dict(loglik=ll.value, mean=mean, var=var, mq=mq, vq=vq, disc_seconds=float(g()))
+
+
+def _instant(fn, kern, ninst, t, inst, y, sigma, tq, query_inst, want_post, prec):
+    t, y, sigma = _d(t), _d(y), _d(sigma)
+    inst = np.ascontiguousarray(inst, dtype=np.int32)
+    N = t.size
+    M = 0 if tq is None else len(tq)
+    tq = _d(tq) if M else None
+    ll = C.c_double()
+    mean = np.empty(N) if want_post else None
+    var = np.empty(N) if want_post else None
+    mq = np.empty(M) if M else None
+    vq = np.empty(M) if M else None
+    f = getattr(_lib(prec), fn)
+    ptr = lambda a: None if a is None else a.ctypes.data
+    head = [len(kern), C.cast(_comps(kern), C.c_void_p)] + ([int(ninst)] if ninst is not None else [])
+    f.argtypes = [C.c_int, C.c_void_p] + ([C.c_int] if ninst is not None else []) + [C.c_int] + [C.c_void_p] * 4 + \
+                 [C.c_int, C.c_void_p, C.c_int] + [C.c_void_p] * 5
+    rc = f(*head, N, ptr(t), ptr(inst), ptr(y), ptr(sigma), M, ptr(tq), int(query_inst), C.addressof(ll), ptr(mean),
+           ptr(var), ptr(mq), ptr(vq))
+    if rc != 0:
+        raise RuntimeError("%s rc=%d" % (fn, rc))
+    return dict(loglik=ll.value, mean=mean, var=var, mq=mq, vq=vq)
+
+
+def dense_instant(kern, t, inst, y, sigma, tq=None, query_inst=0, want_post=True):
+    """The definition for instantaneous data (paper section 2): K_ij = k(|t_i - t_j|), Eq. 2.4 / 2.26."""
+    return _instant("oracle_dense_instant", kern, None, t, inst, y, sigma, tq, query_inst, want_post, "f80")
+
+
+def ssm_instant(kern, ninst, t, inst, y, sigma, tq=None, query_inst=0, want_post=True, prec="f80"):
+    """The paper's section-2 sequential algorithm (Kalman filter, RTS smoother, Algorithm 1) on instantaneous data."""
+    return _instant("oracle_ssm_instant", kern, ninst, t, inst, y, sigma, tq, query_inst, want_post, prec)

@@ -1001,3 +1001,221 @@ int oracle_ssm(int ncomp, const ocomp *comp, int ninst, int N, const double *ts,
   free(ev); free(opst); free(mx); free(mp); free(ms);
   return rc;
 }
+
+/* ==========================================================================================
+ * Part 6.  Instantaneous data (the paper's section 2: K = N states, no integral state).
+ *   oracle_dense_instant : the definition, Eq. 2.4 with K_ij = k(|t_i - t_j|) restricted to the
+ *                          components shared by the two samples' instruments; loglik as Eq. 2.26.
+ *   oracle_ssm_instant   : the sequential algorithm of section 2, step by step: Kalman filter Eq. 2.21-2.22
+ *                          (P:212-225), RTS smoother Eq. 2.23, log-likelihood Eq. 2.24-2.26
+ *                          (P:246-260), prediction at arbitrary times Algorithm 1 in its printed,
+ *                          non-augmented form.  State = the base state x (dimension d), H = the integrand row
+ *                          H_i of the sample's instrument.
+ * Pins (tests/test_oracle_instant_pins.py): dense_instant <- numpy on the pinned oracle_kernel; ssm_instant <-
+ * dense_instant on tiny N (Fig. 1's claim: SSM = GP on instantaneous data to machine precision); the
+ * exposure-integrated oracle with delta -> 0 converges to it with second order.
+ * ========================================================================================== */
+int oracle_dense_instant(int ncomp, const ocomp *comp, int N, const double *tt, const int32_t *inst,
+                         const double *y, const double *sigma, int M, const double *tq, int query_inst,
+                         double *loglik, double *mean, double *var, double *mq, double *vq) {
+  kterm t[64];
+  int nt = build_terms(ncomp, comp, t, 64);
+  if (nt < 0) return -1;
+  size_t NN = (size_t)N * N;
+  real *K = malloc(NN * sizeof(real)), *L = malloc(NN * sizeof(real));
+  real *a = malloc(N * sizeof(real)), *col = malloc(N * sizeof(real));
+  if (!K || !L || !a || !col) return -4;
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j <= i; ++j) {
+      real v = (real)kern_q(t, nt, inst[i], inst[j], (__float128)tt[i] - (__float128)tt[j]);
+      K[(size_t)i * N + j] = K[(size_t)j * N + i] = v;
+    }
+  memcpy(L, K, NN * sizeof(real));
+  for (int i = 0; i < N; ++i) L[(size_t)i * N + i] += (real)sigma[i] * (real)sigma[i];
+  if (chol_lower(L, N)) { free(K); free(L); free(a); free(col); return -2; }
+  for (int i = 0; i < N; ++i) a[i] = y[i];
+  fwd_sub(L, N, a);
+  real quad = 0, logdet = 0;
+  for (int i = 0; i < N; ++i) { quad += a[i] * a[i]; logdet += 2 * R_LOG(L[(size_t)i * N + i]); }
+  if (loglik) *loglik = (double)(-0.5L * (quad + logdet + N * R_LOG((real)(2 * PI_R))));
+  bwd_sub(L, N, a);
+  if (mean)
+    for (int i = 0; i < N; ++i) {
+      real s = 0;
+      for (int j = 0; j < N; ++j) s += K[(size_t)i * N + j] * a[j];
+      mean[i] = (double)s;
+    }
+  if (var)
+    for (int i = 0; i < N; ++i) {
+      for (int j = 0; j < N; ++j) col[j] = K[(size_t)j * N + i];
+      fwd_sub(L, N, col);
+      real s = 0;
+      for (int j = 0; j < N; ++j) s += col[j] * col[j];
+      var[i] = (double)(K[(size_t)i * N + i] - s);
+    }
+  for (int q = 0; q < M; ++q) {
+    for (int j = 0; j < N; ++j) col[j] = (real)kern_q(t, nt, query_inst, inst[j], (__float128)tq[q] - (__float128)tt[j]);
+    real s = 0;
+    for (int j = 0; j < N; ++j) s += col[j] * a[j];
+    if (mq) mq[q] = (double)s;
+    fwd_sub(L, N, col);
+    real v = (real)kern_q(t, nt, query_inst, query_inst, 0);
+    for (int j = 0; j < N; ++j) v -= col[j] * col[j];
+    if (vq) vq[q] = (double)v;
+  }
+  free(K); free(L); free(a); free(col);
+  return 0;
+}
+
+/* base transition Phi (d x d) and process noise Q (d x d) of one step: the x-block of the augmented pair */
+static void disc_base(const model *M, real dt, real *Phi, real *Q) {
+  real A[MAXN * MAXN], Qa[MAXN * MAXN];
+  disc_model(M, dt, A, Qa);
+  const int n = M->n, d = M->d;
+  for (int i = 0; i < d; ++i)
+    for (int j = 0; j < d; ++j) { Phi[i * d + j] = A[i * n + j]; Q[i * d + j] = Qa[i * n + j]; }
+}
+
+int oracle_ssm_instant(int ncomp, const ocomp *comp, int ninst, int N, const double *tt, const int32_t *inst,
+                       const double *y, const double *sigma, int M, const double *tq, int query_inst,
+                       double *loglik, double *mean, double *var, double *mq, double *vq) {
+  model Md;
+  if (build_model(&Md, ncomp, comp, ninst)) return -1;
+  const int d = Md.d, dd = d * d;
+  /* measurement rows: H_i = sum of the H_m of the components in instrument i's mask (Eq. 3.2's H_n; P:86 for one instrument) */
+  real H[32][MAXN] = {{0}};
+  for (int q = 0; q < 32; ++q)
+    for (int b = 0; b < Md.nblk; ++b)
+      if ((Md.blk[b].mask >> q) & 1u)
+        for (int j = 0; j < Md.blk[b].d; ++j) H[q][Md.off[b] + j] = Md.blk[b].H[j];
+  event *ev = malloc(sizeof(event) * (size_t)N);
+  if (!ev) return -4;
+  for (int i = 0; i < N; ++i) {
+    if (inst[i] < 0 || inst[i] >= ninst || !(sigma[i] > 0)) { free(ev); return -1; }
+    ev[i] = (event){tt[i], 0, inst[i], i};
+  }
+  qsort(ev, (size_t)N, sizeof(event), ev_cmp);
+  const int want_smooth = (mean || var || M > 0);
+  size_t per = (size_t)d + dd;
+  real *pr = malloc(sizeof(real) * per * N), *fi = malloc(sizeof(real) * per * N), *sm = want_smooth ? malloc(sizeof(real) * per * N) : NULL;
+  if (!pr || !fi || (want_smooth && !sm)) { free(ev); free(pr); free(fi); free(sm); return -4; }
+#define IM(a, k) ((a) + per * (size_t)(k))
+#define IP(a, k) ((a) + per * (size_t)(k) + d)
+  real m[MAXN] = {0}, P[MAXN * MAXN] = {0}, Phi[MAXN * MAXN], Q[MAXN * MAXN], T1[MAXN * MAXN], T2[MAXN * MAXN], Pinf[MAXN * MAXN] = {0};
+  for (int b = 0; b < Md.nblk; ++b)
+    for (int i = 0; i < Md.blk[b].d; ++i)
+      for (int j = 0; j < Md.blk[b].d; ++j) Pinf[(Md.off[b] + i) * d + Md.off[b] + j] = Md.blk[b].P[i * Md.blk[b].d + j];
+  memcpy(P, Pinf, sizeof(real) * dd); /* m0 = 0, P0 = Pinf */
+  real ll = 0;
+  int rc = 0;
+  for (int k = 0; k < N; ++k) {
+    real dt = k == 0 ? 0 : (real)ev[k].t - (real)ev[k - 1].t;
+    disc_base(&Md, dt, Phi, Q);
+    mv(d, Phi, m, T1); /* predict, Eq. 2.21 */
+    memcpy(m, T1, sizeof(real) * d);
+    mm(d, Phi, P, T1);
+    mmt(d, T1, Phi, T2);
+    for (int i = 0; i < dd; ++i) P[i] = T2[i] + Q[i];
+    symmetrise(d, P);
+    memcpy(IM(pr, k), m, sizeof(real) * d); memcpy(IP(pr, k), P, sizeof(real) * dd);
+    const real *h = H[ev[k].inst]; /* update, Eq. 2.22 */
+    int e = ev[k].idx;
+    real v = (real)y[e], S = (real)sigma[e] * (real)sigma[e], Ph[MAXN];
+    for (int i = 0; i < d; ++i) v -= h[i] * m[i];
+    for (int i = 0; i < d; ++i) { real s = 0; for (int j = 0; j < d; ++j) s += P[i * d + j] * h[j]; Ph[i] = s; }
+    for (int i = 0; i < d; ++i) S += h[i] * Ph[i];
+    for (int i = 0; i < d; ++i) m[i] += Ph[i] / S * v;
+    for (int i = 0; i < d; ++i)
+      for (int j = 0; j < d; ++j) P[i * d + j] -= Ph[i] * Ph[j] / S;
+    symmetrise(d, P);
+    ll += -(R_LOG(2 * (real)PI_R * S) + v * v / S) / 2; /* Eq. 2.26 */
+    memcpy(IM(fi, k), m, sizeof(real) * d); memcpy(IP(fi, k), P, sizeof(real) * dd);
+  }
+  if (loglik) *loglik = (double)ll;
+  if (want_smooth) { /* RTS, Eq. 2.23 */
+    memcpy(IM(sm, N - 1), IM(fi, N - 1), sizeof(real) * per);
+    for (int k = N - 2; k >= 0 && rc == 0; --k) {
+      real dt = (real)ev[k + 1].t - (real)ev[k].t;
+      disc_base(&Md, dt, Phi, Q);
+      real Pm[MAXN * MAXN], Gt[MAXN * MAXN], G[MAXN * MAXN], D[MAXN * MAXN], dm[MAXN];
+      memcpy(Pm, IP(pr, k + 1), sizeof(real) * dd);
+      mm(d, Phi, IP(fi, k), Gt); /* G^T = (P-_{k+1})^-1 Phi P_k */
+      if (lu_solve(d, Pm, Gt, d)) { rc = -3; break; }
+      for (int i = 0; i < d; ++i)
+        for (int j = 0; j < d; ++j) G[i * d + j] = Gt[j * d + i];
+      for (int i = 0; i < d; ++i) dm[i] = IM(sm, k + 1)[i] - IM(pr, k + 1)[i];
+      for (int i = 0; i < dd; ++i) D[i] = IP(sm, k + 1)[i] - IP(pr, k + 1)[i];
+      mv(d, G, dm, T1);
+      for (int i = 0; i < d; ++i) IM(sm, k)[i] = IM(fi, k)[i] + T1[i];
+      mm(d, G, D, T1);
+      mmt(d, T1, G, T2);
+      for (int i = 0; i < dd; ++i) IP(sm, k)[i] = IP(fi, k)[i] + T2[i];
+      symmetrise(d, IP(sm, k));
+    }
+    for (int k = 0; k < N && rc == 0; ++k) {
+      const real *h = H[ev[k].inst];
+      real mu = 0, vv = 0;
+      for (int i = 0; i < d; ++i) { mu += h[i] * IM(sm, k)[i]; for (int j = 0; j < d; ++j) vv += h[i] * IP(sm, k)[i * d + j] * h[j]; }
+      if (mean) mean[ev[k].idx] = (double)mu;
+      if (var) var[ev[k].idx] = (double)vv;
+    }
+  }
+  /* Algorithm 1 as printed, with the missing G^T of lines 9/20 restored (reading c7) */
+  for (int q = 0; q < M && rc == 0; ++q) {
+    const real *h = H[query_inst];
+    real ms_[MAXN], Ps_[MAXN * MAXN], Gt[MAXN * MAXN], G[MAXN * MAXN], dm[MAXN], D[MAXN * MAXN], Pm[MAXN * MAXN];
+    double t = tq[q];
+    if (t < ev[0].t) { /* retrodict: m* = m0 = 0, P* = Pinf; next = state 1 predicted from t* */
+      disc_base(&Md, (real)ev[0].t - (real)t, Phi, Q);
+      mm(d, Phi, Pinf, T1);
+      mmt(d, T1, Phi, T2);
+      for (int i = 0; i < dd; ++i) Pm[i] = T2[i] + Q[i]; /* P-_1 seen from t* (= Pinf: the prior is stationary) */
+      mm(d, Phi, Pinf, Gt);
+      if (lu_solve(d, Pm, Gt, d)) { rc = -3; break; }
+      for (int i = 0; i < d; ++i)
+        for (int j = 0; j < d; ++j) G[i * d + j] = Gt[j * d + i];
+      mm(d, Phi, Pinf, T1); mmt(d, T1, Phi, T2);
+      for (int i = 0; i < d; ++i) dm[i] = IM(sm, 0)[i];
+      for (int i = 0; i < dd; ++i) D[i] = IP(sm, 0)[i] - (T2[i] + Q[i]);
+      mv(d, G, dm, ms_);
+      mm(d, G, D, T1); mmt(d, T1, G, T2);
+      for (int i = 0; i < dd; ++i) Ps_[i] = Pinf[i] + T2[i];
+    } else {
+      int kp;
+      if (t >= ev[N - 1].t) kp = N - 1;
+      else { int lo = 0, hi = N - 1; while (hi - lo > 1) { int mid = (lo + hi) / 2; if (ev[mid].t <= t) lo = mid; else hi = mid; } kp = lo; }
+      real mstar[MAXN], Pstar[MAXN * MAXN];
+      disc_base(&Md, (real)t - (real)ev[kp].t, Phi, Q);
+      mv(d, Phi, IM(fi, kp), mstar);
+      mm(d, Phi, IP(fi, kp), T1); mmt(d, T1, Phi, T2);
+      for (int i = 0; i < dd; ++i) Pstar[i] = T2[i] + Q[i];
+      if (kp == N - 1) { memcpy(ms_, mstar, sizeof(real) * d); memcpy(Ps_, Pstar, sizeof(real) * dd); }
+      else {
+        int kn = kp + 1;
+        real mpn[MAXN];
+        disc_base(&Md, (real)ev[kn].t - (real)t, Phi, Q);
+        mv(d, Phi, mstar, mpn);
+        mm(d, Phi, Pstar, T1); mmt(d, T1, Phi, T2);
+        for (int i = 0; i < dd; ++i) Pm[i] = T2[i] + Q[i];
+        real Ppn[MAXN * MAXN];
+        memcpy(Ppn, Pm, sizeof(real) * dd);
+        mm(d, Phi, Pstar, Gt);
+        if (lu_solve(d, Pm, Gt, d)) { rc = -3; break; }
+        for (int i = 0; i < d; ++i)
+          for (int j = 0; j < d; ++j) G[i * d + j] = Gt[j * d + i];
+        for (int i = 0; i < d; ++i) dm[i] = IM(sm, kn)[i] - mpn[i];
+        for (int i = 0; i < dd; ++i) D[i] = IP(sm, kn)[i] - Ppn[i];
+        mv(d, G, dm, T1);
+        for (int i = 0; i < d; ++i) ms_[i] = mstar[i] + T1[i];
+        mm(d, G, D, T1); mmt(d, T1, G, T2);
+        for (int i = 0; i < dd; ++i) Ps_[i] = Pstar[i] + T2[i];
+      }
+    }
+    real mu = 0, vv = 0;
+    for (int i = 0; i < d; ++i) { mu += h[i] * ms_[i]; for (int j = 0; j < d; ++j) vv += h[i] * Ps_[i * d + j] * h[j]; }
+    if (mq) mq[q] = (double)mu;
+    if (vq) vq[q] = (double)vv;
+  }
+  free(ev); free(pr); free(fi); free(sm);
+  return rc;
+}
