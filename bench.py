@@ -152,6 +152,11 @@ def oracle_step(w, n_sample, series=0, split=False):
     kern = w["kernel"]
     if w.get("amp") is not None:
         kern = [dict(k, sigma=k["sigma"] * float(w["amp"][series])) for k in kern]
+    if w.get("instant"):
+        t0 = time.perf_counter()
+        oracle.ssm_instant(kern, w["n_inst"], w["t_start"][sl], w["instrument"][sl], y, w["sigma"][sl], prec="f64")
+        dt = time.perf_counter() - t0
+        return (dt, float("nan")) if split else dt
     t0 = time.perf_counter()
     r = oracle.ssm(kern, w["n_inst"], w["t_start"][sl], w["t_end"][sl], w["instrument"][sl], y, w["sigma"][sl],
                    flags=oracle.FLAG_IDLE_ZERO | oracle.FLAG_TWO_FILTER, prec="f64")
@@ -190,8 +195,10 @@ def run_reference(args, w, cfgname):
         oracle_step(w, min(ns, 2000))
     ts = [oracle_step(w, ns) for _ in range(args.steps)]
     tot = sum(ts)
-    val = 2.0 * ns * args.steps / tot
-    sample = "first %d of %d exposures (%d events) per step, oracle fp64 build, sequential filter + two-filter smoother, 1 thread" % (ns, w["t_start"].size, 2 * ns)
+    epe = 1 if w.get("instant") else 2
+    val = float(epe) * ns * args.steps / tot
+    sample = "first %d of %d exposures (%d events) per step, oracle fp64 build, sequential filter + %s, 1 thread" % (
+        ns, w["t_start"].size, epe * ns, "RTS smoother (section 2)" if w.get("instant") else "two-filter smoother")
     line = {"impl": "reference", "metric": "events/sec for loglik+RTS smoother at N=1e5", "value": val, "unit": "events/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -251,8 +258,12 @@ def run_cuda(args, w, cfgname):
                loglik=torch.empty(batch, dtype=torch.float64, device=dev))
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)  # > the 126 MB L2
 
+    instant = bool(w.get("instant"))
+    ev_per_exp = 1 if instant else 2
+    K_events = ev_per_exp * N * batch
+
     def step():
-        ev = ctx.smolgp_build_events(ts, te, ins, w["n_inst"])                       # a1
+        ev = ctx.smolgp_build_events_instant(ts, ins, w["n_inst"]) if instant else ctx.smolgp_build_events(ts, te, ins, w["n_inst"])  # a1
         ctx.smolgp_condition(ev, w["kernel"], y, sg, amp=amp, out=out)               # a2-a6
         ev.free()
 
@@ -307,7 +318,7 @@ def run_cuda(args, w, cfgname):
     hout = dict(mean=pin(np.empty((batch, N))), var=pin(np.empty((batch, N))), loglik=pin(np.empty(batch)))
 
     def step_e2e():
-        ev = ctx.smolgp_build_events_host(hts, hte, hins, w["n_inst"])
+        ev = ctx.smolgp_build_events_instant_host(hts, hins, w["n_inst"]) if instant else ctx.smolgp_build_events_host(hts, hte, hins, w["n_inst"])
         ctx.smolgp_condition_host(ev, w["kernel"], hy, hsg, amp=hamp, out=hout)
         ev.free()
 
@@ -368,9 +379,9 @@ def run_cuda(args, w, cfgname):
     oracle.build()
     ns = oracle_sample_size(w, 12.0)
     t_cpu, t_disc = oracle_step(w, ns, split=True)
-    cpu = {"value": 2.0 * ns / t_cpu, "unit": "events/s", "cores": 1, "kind": "oracle",
+    cpu = {"value": ev_per_exp * ns / t_cpu, "unit": "events/s", "cores": 1, "kind": "oracle",
            "seconds": {"total": t_cpu, "discretisation": t_disc, "filter_smoother": t_cpu - t_disc},
-           "sample": "first %d of %d exposures (%d events), oracle fp64 build, sequential filter + two-filter smoother, 1 thread, %.1f s" % (ns, N, 2 * ns, t_cpu)}
+           "sample": "first %d of %d exposures (%d events), oracle fp64 build, sequential filter + %s, 1 thread, %.1f s" % (ns, N, ev_per_exp * ns, "RTS smoother (section 2)" if instant else "two-filter smoother", t_cpu)}
     if batch > 1:
         nser = min(batch, 4 * (os.cpu_count() or 1))
         v_all, thr, t_all = oracle_all_cores(w, nser, min(ns, N))
@@ -379,7 +390,7 @@ def run_cuda(args, w, cfgname):
     line = {"metric": "events/sec for loglik+RTS smoother at N=1e5", "value": value, "unit": "events/s",
             "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfgname, "N": N, "events": 2 * N, "batch": batch, "state_dim": n,
+            "config": {"workload": cfgname, "N": N, "events": ev_per_exp * N, "batch": batch, "state_dim": n,
                        "path": "a1 build_events + a2 discretise + a3 filter scan + a4 smoother + a5 loglik + a6 posterior",
                        "l2": "flushed (512 MiB write) between timed iterations", "parallelism": "replicas x%d" % world,
                        "plan": plan},
@@ -512,7 +523,8 @@ def run_predict(args, w, cfgname):
     print(json.dumps(line), flush=True)
 
 
-CFG_NAMES = {1: "cfg1 Matern-3/2 N=1e3", 2: "cfg2 SHO two instruments N=2e4",
+CFG_NAMES = {"instant": "instantaneous samples (paper section 2), SHO + Matern-5/2 (Fig. 1 kernel), N=1e5 (K=1e5 events)",
+             1: "cfg1 Matern-3/2 N=1e3", 2: "cfg2 SHO two instruments N=2e4",
              3: "cfg3 quasiperiodic Matern-3/2 x periodic(J=4), 3 overlapping instruments, n=21, N=1e5 (K=2e5 events)",
              4: "cfg4 joint multi-instrument n=17 N=1e6", 5: "cfg5 batched 4096 x N=2048, n=7"}
 
@@ -523,11 +535,12 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-5); 3 = the headline N=1e5")
+    ap.add_argument("--config", default="3", help="BASELINE.json config (1-5; 3 = the headline N=1e5) or `instant` (section-2 instantaneous data, SURVEY 8(f) item 3)")
     ap.add_argument("--workload", default="condition", choices=["condition", "predict"],
                     help="condition = the headline (rows a1-a6); predict = condition + prediction at --predict-mult x N query times (row a7)")
     ap.add_argument("--predict-mult", type=float, default=100.0, help="queries per exposure of the predict workload (the paper uses M = 100 N, P:561)")
     args = ap.parse_args()
+    args.config = args.config if args.config == "instant" else int(args.config)
     w = W.make(args.config)
     if args.impl == "reference":
         run_reference(args, w, CFG_NAMES[args.config])

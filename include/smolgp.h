@@ -123,7 +123,20 @@ int smolgp_build_events_host(smolgp_ctx* ctx, int64_t N, const double* t_start, 
                              const int32_t* instrument, int32_t n_inst, smolgp_events** out);
 void smolgp_free_events(smolgp_events* ev);
 
-/* Read back the event stream (HOST output arrays of length 2N, any may be NULL): event time,
+/* Instantaneous data -- the paper's section 2 (Fig. 1, Fig. 4 workloads P:561): y_n is a noisy
+ * sample of the latent of instrument instrument[n] AT time t[n], not an exposure average.  The stream has K = N
+ * observe events ordered by (time, instrument, sample index); simultaneous samples are legal.  Every other call
+ * (smolgp_loglik, smolgp_condition incl. query times) takes the result unchanged: mean_obs / var_obs are then the
+ * posterior of the noise-free latent H_i x at the sample times.  Internally the per-instrument state z_i carries
+ * H_i x at the instrument's samples instead of an integral, so the kernels are the
+ * same.  A data set is either exposure-integrated or instantaneous: the two kinds cannot be mixed in one stream.
+ * Errors: EINVAL (N <= 0, non-finite time, instrument out of range), EUNSUPPORTED, ENOMEM, ECUDA. */
+int smolgp_build_events_instant(smolgp_ctx* ctx, int64_t N, const double* t, const int32_t* instrument,
+                                int32_t n_inst, smolgp_events** out);
+int smolgp_build_events_instant_host(smolgp_ctx* ctx, int64_t N, const double* t, const int32_t* instrument,
+                                     int32_t n_inst, smolgp_events** out);
+
+/* Read back the event stream (HOST output arrays of length K = 2N, or N for instantaneous data; any may be NULL): event time,
  * kind (1 = start/reset, 0 = end/observe), instrument, exposure index.  For tests. */
 int smolgp_events_export(smolgp_ctx* ctx, const smolgp_events* ev, double* t, int32_t* kind,
                          int32_t* instrument, int32_t* exposure);

@@ -12,7 +12,7 @@ from . import _build
 MATERN32, MATERN52, SHO, MATERN32_X_PERIODIC = 0, 1, 2, 3
 STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM", -5: "ECUDA", -6: "ENUMERIC"}
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
-           "smolgp_build_events_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
+           "smolgp_build_events_host", "smolgp_build_events_instant", "smolgp_build_events_instant_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
            "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info", "smolgp_memory_info"]
 NKERNELS = 11  # SMOLGP_NKERNELS
@@ -51,6 +51,8 @@ def lib():
         L.smolgp_set_option.argtypes = [vp, C.c_char_p, i64]
         for f in (L.smolgp_build_events, L.smolgp_build_events_host):
             f.argtypes = [vp, i64, dp, dp, dp, i32, C.POINTER(vp)]
+        for f in (L.smolgp_build_events_instant, L.smolgp_build_events_instant_host):
+            f.argtypes = [vp, i64, dp, dp, i32, C.POINTER(vp)]
         L.smolgp_free_events.argtypes = [vp]
         L.smolgp_free_events.restype = None
         L.smolgp_events_export.argtypes = [vp, vp, dp, dp, dp, dp]
@@ -108,11 +110,12 @@ def _hptr(a, numel=None, name="argument"):
 
 
 class Events:
-    def __init__(self, ctx, handle, N, n_inst):
-        self.ctx, self.handle, self.N, self.n_inst = ctx, handle, N, n_inst
+    def __init__(self, ctx, handle, N, n_inst, instant=False):
+        self.ctx, self.handle, self.N, self.n_inst, self.instant = ctx, handle, N, n_inst, instant
+        self.K = N if instant else 2 * N
 
     def export(self):
-        K = 2 * self.N
+        K = self.K
         t = np.empty(K)
         kind, inst, idx = (np.empty(K, dtype=np.int32) for _ in range(3))
         self.ctx._check(lib().smolgp_events_export(self.ctx.handle, self.handle, _hptr(t), _hptr(kind), _hptr(inst), _hptr(idx)))
@@ -192,6 +195,22 @@ class Context:
         self._check(lib().smolgp_build_events_host(self.handle, ts.size, _hptr(ts), _hptr(te, ts.size, "t_end"), _hptr(ins, ts.size, "instrument"),
                                                    int(n_inst), C.byref(h)))
         return Events(self, h, ts.size, n_inst)
+
+    # ---- instantaneous data (paper section 2) ----
+    def smolgp_build_events_instant(self, t, instrument, n_inst):
+        """device tensors: t float64 [N], instrument int32 [N]"""
+        N = t.numel()
+        h = C.c_void_p()
+        self._check(lib().smolgp_build_events_instant(self.handle, N, _dptr(t, name="t"), _dptr(instrument, "int32", N, "instrument"),
+                                                      int(n_inst), C.byref(h)))
+        return Events(self, h, N, n_inst, instant=True)
+
+    def smolgp_build_events_instant_host(self, t, instrument, n_inst):
+        tt = np.ascontiguousarray(t, np.float64)
+        ins = np.ascontiguousarray(instrument, np.int32)
+        h = C.c_void_p()
+        self._check(lib().smolgp_build_events_instant_host(self.handle, tt.size, _hptr(tt), _hptr(ins, tt.size, "instrument"), int(n_inst), C.byref(h)))
+        return Events(self, h, tt.size, n_inst, instant=True)
 
     # ---- a2-a5 ----
     def smolgp_loglik(self, ev, kernel, y, noise_sigma, amp=None, out=None):

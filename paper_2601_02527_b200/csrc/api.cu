@@ -138,7 +138,7 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   if (ev->device != ctx->device) { ctx->err = "events belong to another device"; return SMOLGP_EINVAL; }
   SG_CUDA(ctx, cudaSetDevice(ctx->device));
   ModelDev& hm = *ctx->hmodel;
-  int rc = sg_build_model(ctx, kernel, ev->n_inst, ev->tau, &hm);
+  int rc = sg_build_model(ctx, kernel, ev->n_inst, ev->tau, ev->instant, &hm);
   if (rc) return rc;
   const size_t model_b = (sizeof(ModelDev) + 255) / 256 * 256;
   const size_t disc_b = ((size_t)ev->K * hm.disc_stride * 8 + 255) / 256 * 256;
@@ -284,7 +284,7 @@ extern "C" int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kern
   ModelDev& hm = *ctx->hmodel;
   double tau[SG_MAXINST];
   for (int q = 0; q < SG_MAXINST; ++q) tau[q] = 1.0;
-  int rc = sg_build_model(ctx, kernel, n_inst, tau, &hm);
+  int rc = sg_build_model(ctx, kernel, n_inst, tau, 0, &hm);
   if (rc) return rc;
   const int n = hm.n, d = hm.d;
   if (n_out) *n_out = n;

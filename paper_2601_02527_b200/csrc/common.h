@@ -34,6 +34,7 @@ struct BlockConst {
 // Whole model, device resident (built on the host by model.cu for each call's kernel).
 struct ModelDev {
   int n, d, n_inst, nblk;
+  int instant;                     // 1: instantaneous-data mode: the "integral" rows of a record hold H Phi, Q H^T, H Q H^T (disc.cu)
   int disc_stride;                 // doubles per event in the discretisation array
   int disc_off[SG_MAXBLK];         // offset of block b inside one event's record
   double cz[SG_MAXINST][SG_MAXBLK]; // c_qb: coupling of block b's integral into z_q (equilibrated units), 0 if masked out
@@ -52,6 +53,7 @@ struct smolgp_events {
   int device;
   int64_t N, K;
   int n_inst;
+  int instant;     // 1: instantaneous samples (paper section 2): K = N observe events, z_i carries H_i x at its sample
   double* t;       // [K] event time
   double* dt;      // [K] t_k - t_{k-1}, dt_0 = 0
   double* delta;   // [K] exposure length of the event's exposure
@@ -129,7 +131,7 @@ static inline void sg_launch_end(smolgp_ctx* ctx) {
   } while (0)
 
 // model.cu
-int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const double* tau, ModelDev* out);
+int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const double* tau, int instant, ModelDev* out);
 // disc.cu
 int sg_launch_disc(smolgp_ctx* ctx, const ModelDev* d_model, const ModelDev* h_model, const double* dt,
                    int64_t K, double* disc);

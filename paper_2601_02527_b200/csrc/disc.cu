@@ -67,7 +67,7 @@ __device__ __forceinline__ void phi_closed<4>(const BlockConst& B, double h, dou
 }
 
 template <int DB>
-__device__ void disc_block(const BlockConst& B, double dts, double* __restrict__ out) {
+__device__ void disc_block(const BlockConst& B, double dts, int instant, double* __restrict__ out) {
   constexpr int M = DB + 1;
   double h = dts;
   int s = 0;
@@ -155,6 +155,16 @@ __device__ void disc_block(const BlockConst& B, double dts, double* __restrict__
   for (int i = 0; i < DB; ++i)
 #pragma unroll
     for (int j = 0; j < DB; ++j) { out[i * DB + j] = A[i][j]; out[DB * DB + DB + i * DB + j] = Q[i][j]; }
+  if (instant) {
+    // instantaneous data (paper section 2): the extra state of the block is not its integral but its
+    // latent after the step, H'' x'' = x''_0: row 0 of Phi, Cov(x'', x''_0) = column 0 of Q, Var(x''_0) = Q_00.  The
+    // chunk kernels then carry z_q = H_q x at each sample with their unchanged arithmetic (z_q is idle, i.e.
+    // zero, before its sample, so the "+ z_q" of the integral row adds nothing).
+#pragma unroll
+    for (int j = 0; j < DB; ++j) { out[DB * DB + j] = A[0][j]; out[2 * DB * DB + DB + j] = Q[j][0]; }
+    out[2 * DB * DB + 2 * DB] = Q[0][0];
+    return;
+  }
 #pragma unroll
   for (int j = 0; j < DB; ++j) { out[DB * DB + j] = A[DB][j]; out[2 * DB * DB + DB + j] = Q[DB][j]; }
   out[2 * DB * DB + 2 * DB] = Q[DB][DB];
@@ -173,9 +183,9 @@ __global__ void __launch_bounds__(128) k_disc(const ModelDev* __restrict__ Mp, c
     const double dts = dt[k] * B.inv_T;
     double* out = stage + threadIdx.x * bs;
     switch (B.dim) {
-      case 2: disc_block<2>(B, dts, out); break;
-      case 3: disc_block<3>(B, dts, out); break;
-      default: disc_block<4>(B, dts, out); break;
+      case 2: disc_block<2>(B, dts, Mp->instant, out); break;
+      case 3: disc_block<3>(B, dts, Mp->instant, out); break;
+      default: disc_block<4>(B, dts, Mp->instant, out); break;
     }
   }
   __syncthreads();

@@ -71,11 +71,12 @@ __global__ void __launch_bounds__(RS_NT) k_ev_init(int64_t N, const double* __re
   const bool live = i < N;
   uint64_t ke = 0, ks = 0;
   int qd = 0;
+  const bool instant = (te == nullptr); // instantaneous samples (paper section 2): one observe event per sample
   if (live) {
-    const double s = ts[i], e = te[i];
+    const double s = ts[i], e = instant ? s : te[i];
     q = inst[i];
     int bad = 0;
-    if (!isfinite(s) || !isfinite(e) || !(e > s)) bad |= EVF_BADTIME;
+    if (!isfinite(s) || !isfinite(e) || (!instant && !(e > s))) bad |= EVF_BADTIME;
     if (q < 0 || q >= n_inst) bad |= EVF_BADINST;
     qd = (q < 0 || q >= n_inst) ? 0 : q;
     if (i > 0 && q < inst[i - 1]) atomicOr(&ctl->ungrouped, 1u);
@@ -83,16 +84,18 @@ __global__ void __launch_bounds__(RS_NT) k_ev_init(int64_t N, const double* __re
     ke = time_key(e); ks = time_key(s);
     keys[i] = ke;
     vals[i] = (uint32_t)(2 * i);
-    keys[N + i] = ks;
-    vals[N + i] = (uint32_t)(2 * i + 1);
-    if (!bad) dbits = (unsigned long long)__double_as_longlong(e - s); // positive doubles order like their bits
+    if (!instant) {
+      keys[N + i] = ks;
+      vals[N + i] = (uint32_t)(2 * i + 1);
+    }
+    if (!bad && !instant) dbits = (unsigned long long)__double_as_longlong(e - s); // positive doubles order like their bits
   }
-  hist_add(h[0], qd, live);       // end event: kind 0
-  hist_add(h[0], 16 + qd, live);  // start event: kind 1
+  hist_add(h[0], qd, live);                    // end event: kind 0
+  hist_add(h[0], 16 + qd, live && !instant);   // start event: kind 1
 #pragma unroll
   for (int p = 0; p < 8; ++p) {
     hist_add(h[1 + p], (int)((ke >> (8 * p)) & 255u), live);
-    hist_add(h[1 + p], (int)((ks >> (8 * p)) & 255u), live);
+    hist_add(h[1 + p], (int)((ks >> (8 * p)) & 255u), live && !instant);
   }
   // longest exposure per instrument: one atomic per (warp, instrument) instead of one per exposure
   for (int r = 0; r < n_inst; ++r) {
@@ -254,6 +257,7 @@ __global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int
   __shared__ uint32_t wx[RS_NT / 32];
   __shared__ unsigned s_mask;
   __shared__ uint32_t s_tile, s_run;
+  const bool instant = (te == nullptr);
   const unsigned skip = skip_mask(ctl, (uint32_t)K, &s_mask);
   const int moved = __popc(~skip & ((1u << RS_DIGITS) - 1u));
   const uint32_t* vals = (moved & 1) ? vB : vA;
@@ -272,24 +276,24 @@ __global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int
     if (k < K) {
       vv[r] = vals[k];
       const int64_t i = vv[r] >> 1;
-      const double s = ts[i], e = te[i];
+      const double s = ts[i], e = instant ? s : te[i];
       int q = inst[i];
       if (q < 0 || q >= n_inst) q = 0;
       tt[r] = ((vv[r] & 1u) ? s : e) + 0.0;
       t[k] = tt[r];
-      delta[k] = e - s;
+      delta[k] = instant ? 1.0 : e - s; // an instantaneous sample observes H x itself: h = hs e_z with hs = tau / delta = 1
       obs[k] = (int32_t)i;
       b[r] = 1u << q;
       if (k == 0) ctl->tfirst = tt[r];
       if (k == K - 1) ctl->tlast = tt[r];
     }
     st_t[tid * EF_ITEMS + r + 1] = tt[r];
-    x ^= b[r];
+    x ^= instant ? 0u : b[r]; // instantaneous samples open nothing
   }
   if (tid == 0) { // time of the event before the tile
     const int64_t kp = (int64_t)tile * (RS_NT * EF_ITEMS) - 1;
     double tp = 0.0;
-    if (kp >= 0) { const uint32_t u = vals[kp]; tp = ((u & 1u) ? ts[u >> 1] : te[u >> 1]) + 0.0; }
+    if (kp >= 0) { const uint32_t u = vals[kp]; tp = ((u & 1u) || instant ? ts[u >> 1] : te[u >> 1]) + 0.0; }
     st_t[0] = tp;
   }
   // inclusive XOR scan of the threads' partials over the CTA
@@ -326,11 +330,11 @@ __global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int
   for (int r = 0; r < EF_ITEMS; ++r) {
     const int64_t k = k0 + r;
     const uint32_t before = after;
-    after ^= b[r];
+    after ^= instant ? 0u : b[r];
     if (k < K) {
       const uint32_t kind = vv[r] & 1u;
       const bool was_open = (before & b[r]) != 0;
-      if ((kind == 1u) == was_open) atomicOr(&ctl->flags, EVF_OVERLAP); // a start needs closed, an end needs open
+      if (!instant && (kind == 1u) == was_open) atomicOr(&ctl->flags, EVF_OVERLAP); // a start needs closed, an end needs open
       const uint32_t zmask = ((~after) & all) | b[r];
       const int q = __ffs(b[r]) - 1;
       meta[k] = kind | ((uint32_t)q << 1) | (zmask << 8);
@@ -360,14 +364,15 @@ static uint32_t lb_next_epoch(smolgp_ctx* ctx) {
 static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const double* te, const int32_t* inst,
                              int32_t n_inst, smolgp_events** out) {
   if (!ctx) return SMOLGP_EINVAL;
-  if (!out || !ts || !te || !inst) { ctx->err = "build_events: null argument"; return SMOLGP_EINVAL; }
+  if (!out || !ts || !inst) { ctx->err = "build_events: null argument"; return SMOLGP_EINVAL; }
   *out = nullptr;
   if (N <= 0 || N > (1ll << 30)) { ctx->err = "build_events: N must be in [1, 2^30]"; return SMOLGP_EINVAL; }
   if (n_inst < 1 || n_inst > SG_MAXINST) { ctx->err = "build_events: n_inst out of range"; return SMOLGP_EUNSUPPORTED; }
   SG_CUDA(ctx, cudaSetDevice(ctx->device));
-  const int64_t K = 2 * N;
+  const bool instant = (te == nullptr); // instantaneous samples: K = N observe events (paper section 2)
+  const int64_t K = instant ? N : 2 * N;
   smolgp_events* ev = new smolgp_events();
-  ev->device = ctx->device; ev->N = N; ev->K = K; ev->n_inst = n_inst;
+  ev->device = ctx->device; ev->N = N; ev->K = K; ev->n_inst = n_inst; ev->instant = instant ? 1 : 0;
   ev->t = ev->dt = ev->delta = nullptr; ev->meta = nullptr; ev->obs = nullptr; ev->base = nullptr; ev->stream = ctx->stream;
   auto fail = [&](int rc) { smolgp_free_events(ev); return rc; };
   // stream-ordered allocation (cudaMallocAsync): no device-wide synchronisation on alloc or free
@@ -439,13 +444,37 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
 
 extern "C" int smolgp_build_events(smolgp_ctx* ctx, int64_t N, const double* t_start, const double* t_end,
                                    const int32_t* instrument, int32_t n_inst, smolgp_events** out) {
+  if (ctx && !t_end) { ctx->err = "build_events: null argument"; return SMOLGP_EINVAL; }
   return build_events_impl(ctx, N, t_start, t_end, instrument, n_inst, out);
+}
+
+extern "C" int smolgp_build_events_instant(smolgp_ctx* ctx, int64_t N, const double* t, const int32_t* instrument, int32_t n_inst,
+                                           smolgp_events** out) {
+  return build_events_impl(ctx, N, t, nullptr, instrument, n_inst, out);
+}
+
+extern "C" int smolgp_build_events_instant_host(smolgp_ctx* ctx, int64_t N, const double* t, const int32_t* instrument,
+                                                int32_t n_inst, smolgp_events** out) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (N <= 0 || !t || !instrument) { ctx->err = "build_events_instant_host: bad argument"; return SMOLGP_EINVAL; }
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  char* stage = nullptr;
+  const size_t n8 = ((size_t)N * 8 + 255) / 256 * 256;
+  if (cudaMallocAsync(&stage, n8 + (size_t)N * 4, ctx->stream) != cudaSuccess) {
+    cudaGetLastError(); ctx->err = "build_events_instant_host: out of device memory"; return SMOLGP_ENOMEM;
+  }
+  cudaMemcpyAsync(stage, t, N * 8, cudaMemcpyHostToDevice, ctx->stream);
+  cudaMemcpyAsync(stage + n8, instrument, N * 4, cudaMemcpyHostToDevice, ctx->stream);
+  int rc = build_events_impl(ctx, N, (const double*)stage, nullptr, (const int32_t*)(stage + n8), n_inst, out);
+  cudaFreeAsync(stage, ctx->stream);
+  return rc;
 }
 
 extern "C" int smolgp_build_events_host(smolgp_ctx* ctx, int64_t N, const double* t_start, const double* t_end,
                                         const int32_t* instrument, int32_t n_inst, smolgp_events** out) {
   if (!ctx) return SMOLGP_EINVAL;
   if (N <= 0 || !t_start || !t_end || !instrument) { ctx->err = "build_events_host: bad argument"; return SMOLGP_EINVAL; }
+  // (instantaneous samples have their own entry point: smolgp_build_events_instant_host)
   SG_CUDA(ctx, cudaSetDevice(ctx->device));
   double *ds = nullptr, *de = nullptr; int32_t* di = nullptr;
   char* stage = nullptr;

@@ -131,7 +131,7 @@ static void make_m32rot(BlockConst& B, ld lambda, ld omega) {
   B.sho_case = 0;
 }
 
-int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const double* tau, ModelDev* M) {
+int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const double* tau, int instant, ModelDev* M) {
   if (!kern || kern->n_comp <= 0 || !kern->comp) { ctx->err = "kernel: no components"; return SMOLGP_EINVAL; }
   if (n_inst < 1 || n_inst > SG_MAXINST) { ctx->err = "n_inst out of range"; return SMOLGP_EUNSUPPORTED; }
   memset(M, 0, sizeof(*M));
@@ -166,11 +166,14 @@ int sg_build_model(smolgp_ctx* ctx, const smolgp_kernel* kern, int n_inst, const
   int off = 0;
   for (int b = 0; b < nb; ++b) { M->blk[b].off = d; d += M->blk[b].dim; M->disc_off[b] = off; off += disc_block_size(M->blk[b].dim); }
   if (d + n_inst > SMOLGP_MAX_DIM) { ctx->err = "augmented state dimension above SMOLGP_MAX_DIM"; return SMOLGP_EUNSUPPORTED; }
-  M->n = d + n_inst; M->d = d; M->n_inst = n_inst; M->nblk = nb; M->disc_stride = off;
+  M->n = d + n_inst; M->d = d; M->n_inst = n_inst; M->nblk = nb; M->disc_stride = off; M->instant = instant;
   for (int q = 0; q < n_inst; ++q) {
     M->tau[q] = tau[q];
     for (int b = 0; b < nb; ++b)
-      M->cz[q][b] = ((mask[b] >> q) & 1u) ? (double)(sig[b] / ((ld)M->blk[b].inv_T * (ld)tau[q])) : 0.0;
+      // integrated data: z_q/tau_q gathers sigma_b T_b I''_b (I'' = int x''_0 dt'').  Instantaneous data (section 2): z_q is
+      // SET to H_q x = sum_b sigma_b x''_{b,0} at its sample, through the same coupling with the record's integral
+      // rows replaced by H Phi (disc.cu), so the coupling is sigma_b / tau_q
+      M->cz[q][b] = ((mask[b] >> q) & 1u) ? (double)(instant ? sig[b] / (ld)tau[q] : sig[b] / ((ld)M->blk[b].inv_T * (ld)tau[q])) : 0.0;
   }
   for (int b = 0; b < nb; ++b) { M->bsig[b] = (double)sig[b]; M->bmask[b] = mask[b]; }
   const int n = M->n;

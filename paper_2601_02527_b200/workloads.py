@@ -129,14 +129,14 @@ def synth_y(rng, kernel, ts, te, inst, sigma, batch=None, amp=None, n_features=2
 # ------------------------------------------------------------------------------------------
 # the five BASELINE.json configs, plus the paper's Fig. 2 / Fig. 3 shapes
 # ------------------------------------------------------------------------------------------
-FULL_N = {1: 1000, 2: 20000, 3: 100000, 4: 1000000, 5: 2048, "fig2": 400, "fig3": 600}
+FULL_N = {1: 1000, 2: 20000, 3: 100000, 4: 1000000, 5: 2048, "fig2": 400, "fig3": 600, "instant": 100000}
 FULL_BATCH = {5: 4096}
 
 
 def make(cfg, N=None, batch=None, seed=None, n_features=None):
     """Returns dict(name, kernel, n_inst, t_start, t_end, instrument, y, sigma, amp, batch)."""
     N = FULL_N[cfg] if N is None else int(N)
-    default_seed = {1: 0, 2: 1, 3: 2, 4: 3, 5: 4, "fig2": 12, "fig3": 13}[cfg]
+    default_seed = {1: 0, 2: 1, 3: 2, 4: 3, 5: 4, "fig2": 12, "fig3": 13, "instant": 14}[cfg]
     rng = np.random.default_rng(default_seed if seed is None else seed)
     U = rng.uniform
     amp = None
@@ -200,6 +200,13 @@ def make(cfg, N=None, batch=None, seed=None, n_features=None):
         ts, te = np.concatenate([tsA, tsB]), np.concatenate([teA, teB])
         inst = np.concatenate([np.zeros(NA, np.int32), np.ones(NB, np.int32)])
         noise = np.array([0.3, 0.3])
+    elif cfg == "instant":
+        name = "instantaneous samples (paper section 2; Fig. 1 kernel P:334: SHO + Matern-5/2), one instrument, gaps U[5,60] s"
+        kernel = [comp(SHO, 1.0, 2 * np.pi / 300.0, 2.0), comp(MATERN52, 0.7, 900.0)]
+        ts = np.cumsum(U(5.0, 60.0, N))
+        te = ts + 1e-9   # only used by the spectral synthesis of y (sinc(w 1e-9 / 2) = 1): the samples are instantaneous
+        inst = np.zeros(N, dtype=np.int32)
+        noise = np.array([0.3])
     else:
         raise ValueError(cfg)
     n_inst = int(noise.size)
@@ -219,4 +226,4 @@ def make(cfg, N=None, batch=None, seed=None, n_features=None):
     else:
         y = synth_y(rng, kernel, ts, te, inst, sigma, batch=batch, amp=amp, n_features=J)
     return dict(name=name, cfg=cfg, kernel=kernel, n_inst=n_inst, t_start=ts, t_end=te, instrument=inst,
-                y=y, sigma=sigma, amp=amp, batch=batch)
+                y=y, sigma=sigma, amp=amp, batch=batch, instant=(cfg == "instant"))

@@ -558,3 +558,109 @@ def test_profile_modes(ctx):
     finally:
         ctx.profile(False)
         _reset(ctx)
+
+
+# ---------------------------------------------------------------------------------------------
+# instantaneous data (the paper's section 2, K = N events) against the oracle's section-2
+# sequential algorithm and the dense definition
+# ---------------------------------------------------------------------------------------------
+INSTANT_KERNELS = {
+    "fig1": ([W.comp(W.SHO, 1.0, 2 * np.pi / 300.0, 2.0), W.comp(W.MATERN52, 0.7, 900.0)], 1),   # Fig. 1: SHO + Matern-5/2
+    "masked": ([W.comp(W.SHO, 1.0, 2 * np.pi / 330.0, 10.0), W.comp(W.MATERN32, 0.5, 900.0, inst_mask=2)], 2),
+    "qp": ([W.comp(W.MATERN32_X_PERIODIC, 1.0, 4000.0, 9000.0, 1.0, order=2)], 1),
+}
+
+
+def _instant_data(rng, kern, N, ninst, span, ties=False):
+    t = np.sort(rng.uniform(0, span, N))
+    if ties:
+        t[1::9] = t[0::9][: t[1::9].size]
+    inst = rng.integers(0, ninst, N).astype(np.int32)
+    sigma = rng.uniform(0.1, 0.4, N)
+    y = W.synth_y(rng, kern, t, t + 1e-9, inst, sigma)
+    return t, inst, y, sigma
+
+
+@pytest.mark.parametrize("opt", ["auto", "deep", "ragged", "jit", "sequential"])
+@pytest.mark.parametrize("name", sorted(INSTANT_KERNELS))
+def test_instantaneous_data_matches_oracle(ctx, oracle, name, opt):
+    kern, ninst = INSTANT_KERNELS[name]
+    rng = np.random.default_rng(31)
+    t, inst, y, sigma = _instant_data(rng, kern, 1500, ninst, 1500 * 40.0, ties=(name == "masked"))
+    p = rng.permutation(t.size)   # samples in arbitrary order
+    t, inst, y, sigma = t[p], inst[p], y[p], sigma[p]
+    tq = np.concatenate([rng.uniform(t.min() - 300, t.max() + 300, 50), t[:3]])
+    for k, v in SCAN_OPTS[opt]:
+        ctx.set_option(k, v)
+    try:
+        ev = ctx.smolgp_build_events_instant_host(t, inst, ninst)
+        et, kind, ei, ex = ev.export()
+        out = ctx.smolgp_condition_host(ev, kern, y, sigma, t_query=tq, query_instrument=ninst - 1)
+        ll = ctx.smolgp_loglik_host(ev, kern, y, sigma)
+    finally:
+        _reset(ctx)
+    # the stream: K = N observe events by (time, instrument, index)
+    order = np.lexsort((np.arange(t.size), inst, t))
+    assert et.size == t.size and np.array_equal(et, t[order]) and np.array_equal(ex, order) and np.all(kind == 0) and np.array_equal(ei, inst[order])
+    ref = oracle.ssm_instant(kern, ninst, t, inst, y, sigma, tq=tq, query_inst=ninst - 1)
+    assert abs(out["loglik"][0] - ref["loglik"]) <= PU.LL_RTOL * abs(ref["loglik"])
+    assert abs(ll[0] - ref["loglik"]) <= PU.LL_RTOL * abs(ref["loglik"])
+    psd = np.sqrt(np.array([oracle.kernel(kern, int(q), int(q), np.zeros(1))[0] for q in inst]))   # prior sd of the sampled latent
+    assert np.max(np.abs(out["mean"][0] - ref["mean"]) / (np.abs(ref["mean"]) + psd)) <= PU.POST_RTOL
+    assert np.max(np.abs(out["var"][0] - ref["var"]) / ref["var"]) <= PU.POST_RTOL
+    k0 = float(oracle.kernel(kern, ninst - 1, ninst - 1, np.zeros(1))[0])
+    assert np.max(np.abs(out["mean_query"][0] - ref["mq"])) <= 1e-8 * (np.sqrt(k0) + np.max(np.abs(ref["mq"])))
+    assert np.max(np.abs(out["var_query"][0] - ref["vq"]) / ref["vq"]) <= 1e-8
+
+
+def test_instantaneous_data_matches_dense_definition(ctx, oracle):
+    rng = np.random.default_rng(32)
+    for name in sorted(INSTANT_KERNELS):
+        kern, ninst = INSTANT_KERNELS[name]
+        t, inst, y, sigma = _instant_data(rng, kern, 160, ninst, 160 * 60.0, ties=True)
+        tq = rng.uniform(t.min() - 200, t.max() + 200, 30)
+        ev = ctx.smolgp_build_events_instant_host(t, inst, ninst)
+        out = ctx.smolgp_condition_host(ev, kern, y, sigma, t_query=tq, query_instrument=0)
+        ref = oracle.dense_instant(kern, t, inst, y, sigma, tq=tq, query_inst=0)
+        assert abs(out["loglik"][0] - ref["loglik"]) <= 1e-9 * abs(ref["loglik"])
+        k0 = float(oracle.kernel(kern, 0, 0, np.zeros(1))[0])
+        assert np.max(np.abs(out["mean"][0] - ref["mean"])) <= 1e-8 * (np.sqrt(k0) + np.max(np.abs(ref["mean"])))
+        assert np.max(np.abs(out["var"][0] - ref["var"])) <= 1e-8 * k0
+        assert np.max(np.abs(out["mean_query"][0] - ref["mq"])) <= 1e-8 * (np.sqrt(k0) + np.max(np.abs(ref["mq"])))
+        assert np.max(np.abs(out["var_query"][0] - ref["vq"])) <= 1e-8 * k0
+
+
+def test_instantaneous_data_full_size_fig1_kernel(ctx, oracle):
+    """N = 1e5 samples, SHO + Matern-5/2 (the Fig. 1 kernel): device-pointer entry point, automatic plan; loglik
+    against the long-double section-2 oracle, posterior on the whole series"""
+    import torch
+    kern, ninst = INSTANT_KERNELS["fig1"]
+    rng = np.random.default_rng(33)
+    N = 100000
+    t = np.cumsum(rng.uniform(5.0, 60.0, N))
+    inst = np.zeros(N, np.int32)
+    sigma = np.full(N, 0.3)
+    sub = np.random.default_rng(34)
+    y = np.concatenate([W.synth_y(np.random.default_rng(35), kern, t[a:a + 20000], t[a:a + 20000] + 1e-9, inst[a:a + 20000], np.zeros(min(20000, N - a)))
+                        for a in range(0, N, 20000)]) + sigma * sub.standard_normal(N)
+    dev = torch.device("cuda:0")
+    ev = ctx.smolgp_build_events_instant(torch.tensor(t, device=dev), torch.tensor(inst, device=dev), 1)
+    out = ctx.smolgp_condition(ev, kern, torch.tensor(y, device=dev), torch.tensor(sigma, device=dev))
+    torch.cuda.synchronize()
+    ref = oracle.ssm_instant(kern, 1, t, inst, y, sigma)
+    assert abs(float(out["loglik"][0]) - ref["loglik"]) <= PU.LL_RTOL * abs(ref["loglik"])
+    k0 = float(oracle.kernel(kern, 0, 0, np.zeros(1))[0])
+    assert np.max(np.abs(out["mean"][0].cpu().numpy() - ref["mean"]) / (np.abs(ref["mean"]) + np.sqrt(k0))) <= PU.POST_RTOL
+    assert np.max(np.abs(out["var"][0].cpu().numpy() - ref["var"]) / ref["var"]) <= PU.POST_RTOL
+
+
+def test_instantaneous_events_validation(ctx):
+    from paper_2601_02527_b200.binding import SmolgpError
+    t, ins = np.array([3.0, 1.0, 2.0]), np.zeros(3, np.int32)
+    ctx.smolgp_build_events_instant_host(t, ins, 1).free()
+    with pytest.raises(SmolgpError) as e:
+        ctx.smolgp_build_events_instant_host(np.array([3.0, np.nan, 2.0]), ins, 1)
+    assert e.value.rc == -1
+    with pytest.raises(SmolgpError) as e:
+        ctx.smolgp_build_events_instant_host(t, np.array([0, 1, 0], np.int32), 1)
+    assert e.value.rc == -1
