@@ -152,6 +152,19 @@ int smolgp_loglik_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_ke
                        int64_t batch, const double* y, const double* noise_sigma, const double* amp,
                        double* loglik);
 
+/* Gradient of Eq. 2.26 w.r.t. the hyper-parameters (its stated use is optimisation / MCMC).  grad is a HOST
+ * array [batch][n_comp][4]: d loglik / d (sigma, p0, p1, p2) of every component (0 for a parameter the family does
+ * not use); loglik is a HOST array [batch] or NULL; y, noise_sigma, amp as in smolgp_loglik (device pointers; HOST in
+ * the _host variant).  Computed by Richardson-extrapolated central differences in log theta of the exact
+ * log-likelihood (four evaluations per parameter, relative step rel_step; <= 0 selects 1e-3): relative accuracy
+ * ~1e-8 of the gradient's scale.  The one-pass adjoint form is not built. */
+int smolgp_loglik_grad(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                       int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                       double rel_step, double* loglik, double* grad);
+int smolgp_loglik_grad_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel,
+                            int64_t batch, const double* y, const double* noise_sigma, const double* amp,
+                            double rel_step, double* loglik, double* grad);
+
 /* Steps a2-a6 (+ a7 when M > 0).  As smolgp_loglik, plus the posterior of the noise-free exposure
  * average at every observation (mean_obs, var_obs: [batch][N]; H~ m^, H~ P^ H~^T of P:460) and,
  * when M > 0, the posterior of the instantaneous latent of instrument query_instrument at the

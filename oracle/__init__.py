@@ -193,3 +193,26 @@ def dense_instant(kern, t, inst, y, sigma, tq=None, query_inst=0, want_post=True
 def ssm_instant(kern, ninst, t, inst, y, sigma, tq=None, query_inst=0, want_post=True, prec="f80"):
     """The paper's section-2 sequential algorithm (Kalman filter, RTS smoother, Algorithm 1) on instantaneous data."""
     return _instant("oracle_ssm_instant", kern, ninst, t, inst, y, sigma, tq, query_inst, want_post, prec)
+
+
+PARAMS = ("sigma", "p0", "p1", "p2")
+FAMILY_PARAMS = {FAM_MATERN32: 2, FAM_MATERN52: 2, FAM_SHO: 3, FAM_MATERN32_X_PERIODIC: 4}
+
+
+def loglik_grad(kern, loglik_fn, h=1e-3):
+    """d loglik / d (sigma, p0, p1, p2) of every component: the derivative's definition evaluated numerically on
+    `loglik_fn(kernel) -> float` (the long-double sequential or dense oracle), by Richardson-extrapolated central
+    differences in log theta.  Returns an array [n_comp][4] (0 for parameters the family does not use).  Pinned
+    against the dense route's analytic 1/2 tr((alpha alpha^T - C^-1) dC/dtheta) in tests/test_oracle_grad_pins.py."""
+    g = np.zeros((len(kern), 4))
+    for c, comp in enumerate(kern):
+        for p in range(FAMILY_PARAMS[int(comp["family"])]):
+            th = float(comp[PARAMS[p]])
+            f = []
+            for mult in (np.exp(h), np.exp(-h), np.exp(2 * h), np.exp(-2 * h)):
+                k2 = [dict(x) for x in kern]
+                k2[c][PARAMS[p]] = th * mult
+                f.append(loglik_fn(k2))
+            d1, d2 = (f[0] - f[1]) / (2 * h), (f[2] - f[3]) / (4 * h)
+            g[c, p] = (4 * d1 - d2) / 3 / th
+    return g

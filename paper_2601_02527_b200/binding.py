@@ -13,7 +13,7 @@ MATERN32, MATERN52, SHO, MATERN32_X_PERIODIC = 0, 1, 2, 3
 STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM", -5: "ECUDA", -6: "ENUMERIC"}
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
            "smolgp_build_events_host", "smolgp_build_events_instant", "smolgp_build_events_instant_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
-           "smolgp_loglik_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
+           "smolgp_loglik_host", "smolgp_loglik_grad", "smolgp_loglik_grad_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
            "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info", "smolgp_memory_info"]
 NKERNELS = 11  # SMOLGP_NKERNELS
 
@@ -58,6 +58,8 @@ def lib():
         L.smolgp_events_export.argtypes = [vp, vp, dp, dp, dp, dp]
         for f in (L.smolgp_loglik, L.smolgp_loglik_host):
             f.argtypes = [vp, vp, C.POINTER(_Kernel), i64, dp, dp, dp, dp]
+        for f in (L.smolgp_loglik_grad, L.smolgp_loglik_grad_host):
+            f.argtypes = [vp, vp, C.POINTER(_Kernel), i64, dp, dp, dp, C.c_double, dp, dp]
         for f in (L.smolgp_condition, L.smolgp_condition_host):
             f.argtypes = [vp, vp, C.POINTER(_Kernel), i64, dp, dp, dp, i64, dp, i32, dp, dp, dp, dp, dp]
         L.smolgp_discretise_host.argtypes = [vp, C.POINTER(_Kernel), i32, C.c_double, dp, dp, C.POINTER(i32)]
@@ -234,6 +236,28 @@ class Context:
         self._check(lib().smolgp_loglik_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y, batch * ev.N, "y"), _hptr(sg, ev.N, "noise_sigma"),
                                              _hptr(am, batch, "amp"), _hptr(out)))
         return out
+
+    # ---- gradient of the log-likelihood ----
+    def smolgp_loglik_grad(self, ev, kernel, y, noise_sigma, amp=None, rel_step=0.0):
+        """device tensors in; returns (loglik [batch], grad [batch, n_comp, 4]) as numpy arrays: d loglik / d (sigma, p0, p1, p2)"""
+        batch = 1 if y.dim() == 1 else y.shape[0]
+        ll, g = np.empty(batch), np.zeros((batch, len(kernel), 4))
+        k, keep = _kernel(kernel)
+        self._check(lib().smolgp_loglik_grad(self.handle, ev.handle, C.byref(k), batch, _dptr(y, numel=batch * ev.N, name="y"),
+                                             _dptr(noise_sigma, numel=ev.N, name="noise_sigma"), _dptr(amp, numel=batch, name="amp"),
+                                             float(rel_step), _hptr(ll), _hptr(g)))
+        return ll, g
+
+    def smolgp_loglik_grad_host(self, ev, kernel, y, noise_sigma, amp=None, rel_step=0.0):
+        y = np.ascontiguousarray(y, np.float64)
+        batch = 1 if y.ndim == 1 else y.shape[0]
+        sg = np.ascontiguousarray(noise_sigma, np.float64)
+        am = None if amp is None else np.ascontiguousarray(amp, np.float64)
+        ll, g = np.empty(batch), np.zeros((batch, len(kernel), 4))
+        k, keep = _kernel(kernel)
+        self._check(lib().smolgp_loglik_grad_host(self.handle, ev.handle, C.byref(k), batch, _hptr(y, batch * ev.N, "y"), _hptr(sg, ev.N, "noise_sigma"),
+                                                  _hptr(am, batch, "amp"), float(rel_step), _hptr(ll), _hptr(g)))
+        return ll, g
 
     # ---- a2-a7 ----
     def smolgp_condition(self, ev, kernel, y, noise_sigma, amp=None, t_query=None, query_instrument=0, out=None):

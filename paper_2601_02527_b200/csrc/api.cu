@@ -275,6 +275,86 @@ extern "C" int smolgp_condition_host(smolgp_ctx* ctx, const smolgp_events* ev, c
   return host_path(ctx, ev, kernel, batch, y, noise_sigma, amp, mean_obs, var_obs, loglik, 1, qs);
 }
 
+// ---- gradient of the log-likelihood w.r.t. the hyper-parameters ---------------
+// d loglik / d theta for theta in (sigma, p0, p1, p2) of every component, per series, by Richardson-extrapolated
+// central differences IN LOG theta of the exact log-likelihood this library computes (relative error of loglik
+// ~1e-15, include/smolgp.h):  with D(h) = (L(theta e^h) - L(theta e^-h)) / 2h,
+//   dL/dlog theta = (4 D(h) - D(2h)) / 3 + O(h^4),   dL/dtheta = that / theta.
+// Four likelihood evaluations per parameter, all on the device; the event stream and the data stay where they
+// are.  (The adjoint form -- one forward and one backward pass for all parameters -- is not built: DESIGN.md 12.)
+static int family_params(int family) { // bit i: parameter i of (sigma, p0, p1, p2) is used by the family
+  switch (family) {
+    case SMOLGP_MATERN32: case SMOLGP_MATERN52: return 0x3;
+    case SMOLGP_SHO: return 0x7;
+    case SMOLGP_MATERN32_X_PERIODIC: return 0xF;
+    default: return 0;
+  }
+}
+
+static int grad_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch, const double* y,
+                     const double* sigma, const double* amp, double rel_step, double* loglik_h, double* grad_h) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (!ev || !kernel || kernel->n_comp <= 0 || !kernel->comp || !y || !sigma || batch <= 0 || !grad_h) { ctx->err = "loglik_grad: null or empty argument"; return SMOLGP_EINVAL; }
+  const double h = (rel_step > 0 && rel_step < 0.1) ? rel_step : 1e-3;
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  double* dll = nullptr;
+  if (cudaMallocAsync(&dll, batch * 8, ctx->stream) != cudaSuccess) { cudaGetLastError(); ctx->err = "loglik_grad: out of device memory"; return SMOLGP_ENOMEM; }
+  std::vector<smolgp_component> comp(kernel->comp, kernel->comp + kernel->n_comp);
+  smolgp_kernel kk; kk.n_comp = kernel->n_comp; kk.comp = comp.data();
+  std::vector<double> f[4];
+  for (auto& v : f) v.resize(batch);
+  auto eval = [&](double* out_h) -> int {
+    int rc = run_path(ctx, ev, &kk, batch, y, sigma, amp, nullptr, nullptr, dll, 0); // synchronises the stream
+    if (rc) return rc;
+    if (cudaMemcpy(out_h, dll, batch * 8, cudaMemcpyDeviceToHost) != cudaSuccess) { ctx->err = "loglik_grad: read-back failed"; cudaGetLastError(); return SMOLGP_ECUDA; }
+    return SMOLGP_OK;
+  };
+  int rc = SMOLGP_OK;
+  if (loglik_h) rc = eval(loglik_h);
+  for (int c = 0; c < kernel->n_comp && rc == SMOLGP_OK; ++c) {
+    const int used = family_params(comp[c].family);
+    double* theta[4] = {&comp[c].sigma, &comp[c].p0, &comp[c].p1, &comp[c].p2};
+    for (int p = 0; p < 4 && rc == SMOLGP_OK; ++p) {
+      double* g = grad_h + ((size_t)c * 4 + p);
+      if (!((used >> p) & 1)) { for (int64_t s = 0; s < batch; ++s) g[(size_t)s * kernel->n_comp * 4] = 0.0; continue; }
+      const double t0 = *theta[p];
+      const double mult[4] = {exp(h), exp(-h), exp(2 * h), exp(-2 * h)};
+      for (int e = 0; e < 4 && rc == SMOLGP_OK; ++e) { *theta[p] = t0 * mult[e]; rc = eval(f[e].data()); }
+      *theta[p] = t0;
+      for (int64_t s = 0; s < batch && rc == SMOLGP_OK; ++s) {
+        const double d1 = (f[0][s] - f[1][s]) / (2 * h), d2 = (f[2][s] - f[3][s]) / (4 * h);
+        g[(size_t)s * kernel->n_comp * 4] = (4 * d1 - d2) / 3 / t0;
+      }
+    }
+  }
+  cudaFreeAsync(dll, ctx->stream);
+  return rc;
+}
+
+extern "C" int smolgp_loglik_grad(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                                  const double* y, const double* noise_sigma, const double* amp, double rel_step,
+                                  double* loglik, double* grad) {
+  return grad_path(ctx, ev, kernel, batch, y, noise_sigma, amp, rel_step, loglik, grad);
+}
+
+extern "C" int smolgp_loglik_grad_host(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kernel* kernel, int64_t batch,
+                                       const double* y, const double* noise_sigma, const double* amp, double rel_step,
+                                       double* loglik, double* grad) {
+  if (!ctx) return SMOLGP_EINVAL;
+  if (!ev || !y || !noise_sigma || batch <= 0) { ctx->err = "loglik_grad: null or empty argument"; return SMOLGP_EINVAL; }
+  SG_CUDA(ctx, cudaSetDevice(ctx->device));
+  HostStage s;
+  s.st = ctx->stream;
+  const int64_t N = ev->N;
+  const size_t bn = (size_t)batch * N * 8;
+  auto am = [&](double** p, size_t b) { return cudaMallocAsync(p, b, ctx->stream) != cudaSuccess; };
+  if (am(&s.y, bn) || am(&s.sigma, N * 8) || (amp && am(&s.amp, batch * 8))) { cudaGetLastError(); ctx->err = "out of device memory (host staging)"; return SMOLGP_ENOMEM; }
+  SG_CUDA(ctx, cudaMemcpyAsync(s.y, y, bn, cudaMemcpyHostToDevice, ctx->stream));
+  SG_CUDA(ctx, cudaMemcpyAsync(s.sigma, noise_sigma, N * 8, cudaMemcpyHostToDevice, ctx->stream));
+  if (amp) SG_CUDA(ctx, cudaMemcpyAsync(s.amp, amp, batch * 8, cudaMemcpyHostToDevice, ctx->stream));
+  return grad_path(ctx, ev, kernel, batch, s.y, s.sigma, amp ? s.amp : nullptr, rel_step, loglik, grad);
+}
+
 // ---- step a2 alone (tests): A~ and Q~ of one step in raw state units ---------------------------------
 extern "C" int smolgp_discretise_host(smolgp_ctx* ctx, const smolgp_kernel* kernel, int32_t n_inst, double dt,
                                       double* A, double* Q, int32_t* n_out) {

@@ -664,3 +664,44 @@ def test_instantaneous_events_validation(ctx):
     with pytest.raises(SmolgpError) as e:
         ctx.smolgp_build_events_instant_host(t, np.array([0, 1, 0], np.int32), 1)
     assert e.value.rc == -1
+
+
+# ---------------------------------------------------------------------------------------------
+# gradient of the log-likelihood w.r.t. every hyper-parameter against the oracle's
+# (central differences of the long-double sequential likelihood, pinned to the dense analytic derivative)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,N,batch", [(1, 600, None), (2, 900, None), (3, 500, None), (4, 500, None), (5, 200, 3)])
+def test_loglik_gradient_matches_oracle(ctx, oracle, cfg, N, batch):
+    w = W.make(cfg, N=N, batch=batch)
+    ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+    ll, g = ctx.smolgp_loglik_grad_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"])
+    for s in ([None] if batch is None else range(batch)):
+        i = 0 if s is None else s
+        y = w["y"] if s is None else w["y"][s]
+        a = 1.0 if s is None else float(w["amp"][s])
+        fn = lambda k: oracle.ssm([dict(c, sigma=c["sigma"] * a) for c in k], w["n_inst"], w["t_start"], w["t_end"], w["instrument"], y, w["sigma"],
+                                  flags=oracle.FLAG_IDLE_ZERO | oracle.FLAG_TWO_FILTER, want_post=False)["loglik"]
+        ref = oracle.loglik_grad(w["kernel"], fn)
+        assert abs(ll[i] - fn(w["kernel"])) <= PU.LL_RTOL * abs(ll[i])
+        scale = np.max(np.abs(ref * np.array([[c["sigma"], c["p0"], max(c["p1"], 1e-300), max(c["p2"], 1e-300)] for c in w["kernel"]])))  # largest |dL/dlog theta|
+        for c, comp in enumerate(w["kernel"]):
+            for p in range(oracle.FAMILY_PARAMS[int(comp["family"])]):
+                th = comp[oracle.PARAMS[p]]
+                assert abs(g[i, c, p] - ref[c, p]) * th <= 1e-6 * scale, (cfg, s, c, p, g[i, c, p], ref[c, p])
+            assert np.all(g[i, c, oracle.FAMILY_PARAMS[int(comp["family"])]:] == 0.0)
+
+
+def test_loglik_gradient_device_pointers_and_instant(ctx, oracle):
+    import torch
+    kern, ninst = INSTANT_KERNELS["fig1"]
+    rng = np.random.default_rng(41)
+    t, inst, y, sigma = _instant_data(rng, kern, 800, ninst, 800 * 40.0)
+    dev = torch.device("cuda:0")
+    ev = ctx.smolgp_build_events_instant_host(t, inst, ninst)
+    ll, g = ctx.smolgp_loglik_grad(ev, kern, torch.tensor(y, device=dev), torch.tensor(sigma, device=dev))
+    fn = lambda k: oracle.ssm_instant(k, ninst, t, inst, y, sigma, want_post=False)["loglik"]
+    ref = oracle.loglik_grad(kern, fn)
+    scale = np.max(np.abs(ref * np.array([[c["sigma"], c["p0"], max(c["p1"], 1e-300), 1e-300] for c in kern])))
+    for c, comp in enumerate(kern):
+        for p in range(oracle.FAMILY_PARAMS[int(comp["family"])]):
+            assert abs(g[0, c, p] - ref[c, p]) * comp[oracle.PARAMS[p]] <= 1e-6 * scale
