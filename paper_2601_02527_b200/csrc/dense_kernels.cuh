@@ -106,6 +106,13 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   const double *Ai = ei, *Ci = ei + n * n1, *Ji = Ci + n * n;
   const double *Aj = ej, *Cj = ej + n * n1, *Jj = Cj + n * n;
   double *Ao = eo, *Co = eo + n * n1, *Jo = Co + n * n;
+#ifdef SG_DENSE_CLK
+  long long ck[8]; int ci = 0;
+#define SG_CK() do { ck[ci++] = clock64(); } while (0)
+#else
+#define SG_CK() do {} while (0)
+#endif
+  SG_CK();
   // phase 1 (everything that needs no solve): Tm = C_i [J_j | eta_j] (n x (n+1)); T2 = J_j A_i; u = eta_j - J_j b_i
   mm<SG_DOT2_A>(g, n, n1, n, Ci, n, 1, Jj, n1, 1, (const double*)nullptr, 0, 0, Tm, n1, 1);
   mm<SG_DOT2_B>(g, n, n, n, Jj, n1, 1, Ai, n1, 1, (const double*)nullptr, 0, 0, T2, n, 1, n * n1);
@@ -115,6 +122,7 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
     uv[i] = acc;
   }
   g.sync();
+  SG_CK();
   // Ws = [I + C_i J_j | A_i | b_i + C_i eta_j | C_i]
   for (int e = g.gl; e < n * n; e += G) {
     const int i = e / n, j = e - i * n;
@@ -124,13 +132,16 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
   }
   for (int i = g.gl; i < n; i += G) Ws[i * ld + 2 * n] = Ai[i * n1 + n] + Tm[i * n1 + n];
   g.sync();
-  gj_solve_reg<G, SG_GJ_CPT>(g, n, 3 * n + 1, ld, Ws, Xs);
+  SG_CK();
+  gj_solve_wcol<G, SG_GJ_WCPT>(g, n, 3 * n + 1, ld, Ws, Xs);
+  SG_CK();
   const double* X1 = Xs;             // M A_i           (row stride lx)
   const double* X2 = Xs + n;         // M (b_i + C_i eta_j), then X3 = M C_i follows
   // phase 2: [A | b] = A_j [X1 | x2] (b_j is added in phase 3); Tm = A_j X3
   mm<SG_DOT2_B>(g, n, n1, n, Aj, n1, 1, X1, lx, 1, (const double*)nullptr, 0, 0, Ao, n1, 1);
   mm<SG_DOT2_B>(g, n, n, n, Aj, n1, 1, X2 + 1, lx, 1, (const double*)nullptr, 0, 0, Tm, n, 1, n * n1);
   g.sync();
+  SG_CK();
   // phase 3: C = Tm A_j^T + C_j;  J = X1^T T2 + J_i;  eta = X1^T u + eta_i;  b += b_j
   mm_sym<SG_DOT2_B>(g, n, n, Tm, n, 1, Aj, 1, n1, Cj, n, Co, n);
   mm_sym<SG_DOT2_B>(g, n, n, X1, 1, lx, T2, n, 1, Ji, n1, Jo, n1, ntri);
@@ -141,6 +152,10 @@ __device__ void dense_combine(const Grp<G>& g, int n, const double* ei, const do
     Ao[i * n1 + n] += Aj[i * n1 + n];
   }
   g.sync();
+  SG_CK();
+#ifdef SG_DENSE_CLK
+  if (threadIdx.x == 0 && blockIdx.x == 0) printf("combine cycles: phase1 %lld assemble %lld gj %lld phase2 %lld phase3 %lld\n", ck[1] - ck[0], ck[2] - ck[1], ck[3] - ck[2], ck[4] - ck[3], ck[5] - ck[4]);
+#endif
 }
 
 __host__ __device__ inline int foldD_group_doubles(int n) { return 3 * elem_size(n) + n * (3 * n + 2) + n * (n + 1) + n + n * (2 * n + 1) + n * n; }
@@ -176,8 +191,14 @@ __device__ __forceinline__ void foldD_body(const DenseArgs& P) {
   const double* src = P.Ein + (series * P.cin + m0) * (int64_t)es;
   // the first two elements of the group are consecutive in memory (e0, e1 too): one pass of loads for both
   const int first = (m0 + 1 < m1) ? 2 * es : es;
+#ifdef SG_DENSE_CLK
+  const long long c_ld0 = clock64();
+#endif
   for (int e = g.gl; e < first; e += NT) e0[e] = src[e];
   g.sync();
+#ifdef SG_DENSE_CLK
+  if (threadIdx.x == 0 && blockIdx.x == 0) printf("foldD load cycles %lld (grid %d)\n", clock64() - c_ld0, gridDim.x);
+#endif
   double* acc = e0; double* nxt = e1; double* out = e2;
   for (int64_t m = m0 + 1; m < m1; ++m) {
     src += es;
@@ -233,7 +254,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
       for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n1 + j] = Pm[e]; }
       for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + n] += mv[i]; }
       g.sync();
-      gj_solve_reg<NT, SG_GJ_CPT>(g, n, ld, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
+      gj_solve_wcol<NT, SG_GJ_WCPT>(g, n, ld, ld, Ws, Xs); // Xs = M^-1 [m + P eta | P], row stride n + 1
       // m' = A x + b ; Tm = A X ; P' = Tm A^T + C
       for (int i = g.gl; i < n; i += NT) {
         double acc = A[i * n1 + n];
@@ -273,7 +294,7 @@ __device__ __forceinline__ void downD_body(const DenseArgs& P) {
         uv[i] = acc;
       }
       g.sync();
-      gj_solve_reg<NT, SG_GJ_CPT>(g, n, 2 * n, ld2, Ws, Xs);
+      gj_solve_wcol<NT, SG_GJ_WCPT>(g, n, 2 * n, ld2, Ws, Xs);
       const double* X = Xs; // M A, row stride n
       for (int i = g.gl; i < n; i += NT) {
         double acc = J[i * n1 + n];
@@ -340,7 +361,7 @@ __device__ __forceinline__ void adjD_body(const AdjArgs& P) {
   for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; Ws[i * ld + n + j] = J[e]; }
   for (int i = g.gl; i < n; i += NT) { Ws[i * ld + i] += 1.0; Ws[i * ld + 2 * n] = uv[i]; }
   g.sync();
-  gj_solve_reg<NT, SG_GJ_CPT>(g, n, 2 * n + 1, ld, Ws, Xs); // Xs = [Lambda^ | lambda^], row stride n + 1
+  gj_solve_wcol<NT, SG_GJ_WCPT>(g, n, 2 * n + 1, ld, Ws, Xs); // Xs = [Lambda^ | lambda^], row stride n + 1
   for (int e = g.gl; e < n * n; e += NT) { const int i = e / n, j = e - i * n; out[n + e] = 0.5 * (Xs[i * n1 + j] + Xs[j * n1 + i]); }
   for (int i = g.gl; i < n; i += NT) out[i] = Xs[i * n1 + n];
 }

@@ -98,135 +98,82 @@ __device__ void gj_solve(const Grp<G>& g, int n, int ld, double* W) {
   g.sync();
 }
 
-// Gauss-Jordan with partial pivoting and NO row exchange, for a group that is a whole CTA (G > 32, n <= 32):
-// the dense levels run one solve per combine on the latency-critical path, so the barriers per pivot count.
-// The pivot of column p is the largest entry among the rows not yet used as a pivot; it is found by every
-// warp on its own (lane l holds row l, warp-reduction arg-max, ties to the lower row, so all warps agree without
-// a barrier), the row stays where it is and only its index is recorded.  Elimination p writes columns > p of
-// the other rows and reads column p and row r only, so ONE barrier per pivot (before the next search) is
-// enough, against three in gj_solve.  Same pivots, hence the same arithmetic per entry, as gj_solve.
-// W = [M | R] (n rows, nc_all = n + m columns, row stride ld >= nc_all: an odd ld keeps the column reads of the
-// pivot search and the row pairs of a warp off the same banks) is destroyed; X (n x m, row stride m) receives M^-1 R.
-template <int G>
-__device__ void gj_solve_np(const Grp<G>& g, int n, int nc_all, int ld, double* W, double* X) {
-  __shared__ int rowof[32];
-  const int lane = threadIdx.x & 31;
-  unsigned used = 0u;
-  for (int p = 0; p < n; ++p) {
-    // arg-max of |W[., p]| over the unused rows: the bit pattern of a non-negative double orders like the value,
-    // so the maximum is two 32-bit warp reductions (high word, then low word among the lanes that hold the
-    // maximal high word) and a ballot; ties go to the lowest row
-    const bool cand = lane < n && !((used >> lane) & 1u);
-    const unsigned long long key = cand ? (unsigned long long)__double_as_longlong(fabs(W[lane * ld + p])) + 1ull : 0ull;
-    const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
-    const unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
-    const unsigned hit = __ballot_sync(0xffffffffu, hi == mhi && lo == mlo);
-    int r = min(__ffs(hit) - 1, n - 1); // non-finite input: still one in-range row for the whole CTA
-    used |= 1u << r;
-    if (g.gl == 0) rowof[p] = r;
-    const double rpv = 1.0 / W[r * ld + p];
-    const int nc = nc_all - p - 1;
-    const float rnc = 1.0f / (float)nc;
-    const int tot = (n - 1) * nc;
-    for (int e = g.gl; e < tot; e += G) {
-      int i, j;
-      divmod_small(e, nc, rnc, i, j);
-      if (i >= r) ++i;
-      j += p + 1;
-      W[i * ld + j] = fma(-W[i * ld + p] * rpv, W[r * ld + j], W[i * ld + j]);
-    }
-    g.sync();
-  }
-  const int m = nc_all - n;
-  const float rm = 1.0f / (float)m;
-  for (int e = g.gl; e < n * m; e += G) {
-    int i, j;
-    divmod_small(e, m, rm, i, j);
-    const int r = rowof[i];
-    X[e] = W[r * ld + n + j] / W[r * ld + i];
-  }
-  g.sync();
-}
-
-// Gauss-Jordan as gj_solve_np (partial pivoting, no row exchange, same pivots and the same arithmetic per entry), with
-// the augmented matrix held in REGISTERS during the elimination: thread t of the CTA owns row t / tpr and the
-// columns c, c + tpr, c + 2 tpr, ... (c = t % tpr, tpr = G / n threads per row), so a pivot step touches shared
-// memory only for what crosses threads -- the pivot column (n doubles, double-buffered) and the pivot row --
-// instead of re-reading and re-writing every entry (round 1: 21 k of a combine's 61 k cycles, profiles/r01_dense_level_ncu.md).
-// Two barriers per pivot.  W (n rows, nc_all columns, row stride ld) is read once; X (n x (nc_all - n), row
-// stride nc_all - n) receives M^-1 R.  CPT >= ceil(nc_all / tpr).
-#ifdef SG_JIT
-#define SG_GJ_CPT ((3 * JT_N + 1 + (SG_DENSE_NT / JT_N) - 1) / (SG_DENSE_NT / JT_N))
-#else
-#define SG_GJ_CPT 12 /* n = 31: 8 threads per row, 94 columns */
-#endif
 #define SG_GJ_MAXC 96
+#ifdef SG_JIT
+#define SG_GJ_WCPT ((3 * JT_N + 1 + (SG_DENSE_NT / 32) - 1) / (SG_DENSE_NT / 32))
+#else
+#define SG_GJ_WCPT 12 /* 94 columns on 8 warps */
+#endif
+
+// Gauss-Jordan with partial pivoting and no row exchange, register-resident, COLUMNS PER WARP: warp w of the CTA owns
+// the columns w, w + NW, w + 2 NW, ... of the augmented matrix and lane l holds row l of each of them.  A pivot
+// step is then: the warp that owns column p finds the pivot row r by a warp reduction on its own registers,
+// forms the multipliers f_i = W[i][p] / W[r][p] (each lane its own reciprocal candidate, so the division runs
+// beside the reductions) and publishes them with r (n + 2 doubles, double-buffered): ONE barrier; every warp
+// then eliminates its own columns with the pivot row's entries taken by a warp shuffle from lane r -- no shared-memory
+// traffic for the matrix beyond that.  The pivot of column p is the largest entry among the rows not yet used as a
+// pivot (arg-max by two 32-bit warp reductions on the bit pattern of |x|, which orders like the value, and a
+// ballot; ties to the lower row); the row stays where it is and only its index is recorded, so no rows move.
+// M = I + (PSD)(PSD) in every use (eigenvalues >= 1): a zero pivot cannot occur for finite input.
+// W = [M | R] (n rows, nc_all columns, row stride ld: odd keeps the loads of a lane's row off one bank) is read
+// once; X (n x (nc_all - n), row stride nc_all - n) receives M^-1 R.  Measured: profiles/r02_dense_level.md.
 template <int G, int CPT>
-__device__ void gj_solve_reg(const Grp<G>& g, int n, int nc_all, int ld, const double* W, double* X) {
-  __shared__ double colbuf[2][32];
-  __shared__ double rowbuf[SG_GJ_MAXC];
-  const int tpr = G / n;
-  const int i = g.gl / tpr, c = g.gl - i * tpr;
-  const bool act = i < n;
-  double w[CPT];
+__device__ void gj_solve_wcol(const Grp<G>& g, int n, int nc_all, int ld, const double* W, double* X) {
+  __shared__ double fbuf[2][34];
+  __shared__ __align__(16) double rowb[G / 32][CPT + (CPT & 1)];
+  constexpr int NW = G / 32;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const bool act = lane < n;
+  double v[CPT];
 #pragma unroll
   for (int s = 0; s < CPT; ++s) {
-    const int j = c + s * tpr;
-    w[s] = (act && j < nc_all) ? W[i * ld + j] : 0.0;
+    const int j = w + s * NW;
+    v[s] = (act && j < nc_all) ? W[lane * ld + j] : 0.0;
   }
-  const int lane = threadIdx.x & 31;
   unsigned used = 0u;
   int outrow = 0;
   double rinv = 0.0;
-  if (act && c == 0) colbuf[0][i] = w[0];
-  g.sync();
   for (int p = 0; p < n; ++p) {
-    const double* cb = colbuf[p & 1];
-    // arg-max of |W[., p]| over the rows not yet used as a pivot: as in gj_solve_np (every warp on its own)
-    const bool cand = lane < n && !((used >> lane) & 1u);
-    const unsigned long long key = cand ? (unsigned long long)__double_as_longlong(fabs(cb[lane])) + 1ull : 0ull;
-    const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
-    const unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
-    const unsigned hit = __ballot_sync(0xffffffffu, hi == mhi && lo == mlo);
-    const int r = min(__ffs(hit) - 1, n - 1);
+    const int os = p / NW, ow = p - os * NW;
+    double* fb = fbuf[p & 1];
+    if (w == ow) {
+      double a = v[0];
+#pragma unroll
+      for (int s = 1; s < CPT; ++s) a = (s == os) ? v[s] : a;
+      const bool cand = act && !((used >> lane) & 1u);
+      const unsigned long long key = cand ? (unsigned long long)__double_as_longlong(fabs(a)) + 1ull : 0ull;
+      const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+      const double rc = 1.0 / a; // every lane its own candidate reciprocal: independent of the search below
+      const unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
+      const unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
+      const unsigned hit = __ballot_sync(0xffffffffu, hi == mhi && lo == mlo);
+      const int r = min(__ffs(hit) - 1, n - 1);
+      const double rpv = __shfl_sync(0xffffffffu, rc, r);
+      fb[lane] = (lane == r) ? 0.0 : a * rpv; // multiplier of row `lane` (none for the pivot row itself)
+      if (lane == 0) { fb[32] = rpv; fb[33] = (double)r; }
+    }
+    g.sync();
+    const int r = (int)fb[33];
+    const double rpv = fb[32], f = -fb[lane];
     used |= 1u << r;
-    const double rpv = 1.0 / cb[r];
-    if (act && i == r) {
+    if (lane == r) { outrow = p; rinv = rpv; }
+    // the pivot row's entries of this warp's columns: lane r stores them, everyone reads them back as broadcasts
+    // (shuffles from lane r measured the same).  Every slot, unconditionally: the columns <= p are dead (never read again; the pivot entries
+    // live on in rinv), the slots beyond nc_all hold zeros.
+    double* rb = rowb[w];
+    if (lane == r) {
 #pragma unroll
-      for (int s = 0; s < CPT; ++s) {
-        const int j = c + s * tpr;
-        if (j > p && j < nc_all) rowbuf[j] = w[s];
-      }
-      outrow = p;
-      rinv = rpv;
+      for (int s = 0; s < CPT; ++s) rb[s] = v[s];
     }
-    g.sync();
-    if (act && i != r) {
-      const double f = -cb[i] * rpv;
+    __syncwarp();
 #pragma unroll
-      for (int s = 0; s < CPT; ++s) {
-        const int j = c + s * tpr;
-        if (j > p && j < nc_all) w[s] = fma(f, rowbuf[j], w[s]);
-      }
-    }
-    if (p + 1 < n) { // the owners of column p + 1 publish it for the next search
-      const int ps = (p + 1) / tpr, pc = (p + 1) - ps * tpr;
-      if (act && c == pc) {
-        double v = w[0];
-#pragma unroll
-        for (int s = 1; s < CPT; ++s) v = (s == ps) ? w[s] : v;
-        colbuf[(p + 1) & 1][i] = v;
-      }
-    }
-    g.sync();
+    for (int s = 0; s < CPT; ++s) v[s] = fma(f, rb[s], v[s]);
   }
   const int m = nc_all - n;
 #pragma unroll
   for (int s = 0; s < CPT; ++s) {
-    const int j = c + s * tpr;
-    if (act && j >= n && j < nc_all) X[outrow * m + (j - n)] = w[s] * rinv;
+    const int j = w + s * NW;
+    if (act && j >= n && j < nc_all) X[outrow * m + (j - n)] = v[s] * rinv;
   }
   g.sync();
 }

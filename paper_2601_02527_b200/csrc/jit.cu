@@ -159,7 +159,9 @@ const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cf
   ent.good = false;
   memset(&ent.k, 0, sizeof ent.k);
   if (st->api.ok) {
-    const std::string src = prelude(T, cfg) + JIT_SRC;
+    std::string src = prelude(T, cfg);
+    if (const char* defs = getenv("SMOLGP_JIT_DEFS")) { src += defs; src += "\n"; } // debugging aid: extra #defines for the specialised build
+    src += JIT_SRC;
     if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the exact text handed to NVRTC
       if (FILE* f = fopen(dump, "w")) { fwrite(src.data(), 1, src.size(), f); fclose(f); }
     }
