@@ -40,11 +40,11 @@ struct ScanDev {
 // shared memory of one group of the register-resident kernels (chunk_reg.cuh): exchange buffer, two record
 // buffers + 2 mbarriers, three vector buffers.  Sizes in doubles; = 8 (mod 16) so that neighbouring groups of a
 // warp fall on complementary banks.
-__host__ __device__ inline int reg_ldt(int n) { return (n + 1) | 1; }
+__host__ __device__ inline int reg_ldt(int n) { return (n + 2) | 1; }
 __host__ __device__ inline int reg_tm(int n) { return ((n * reg_ldt(n) + 7) / 16) * 16 + 8; }
 __host__ __device__ inline int reg_vb(int n) { return 2 * (n + 2); }
 __host__ __device__ inline int reg_group_doubles(int n, int stride) { return ((reg_tm(n) + 2 * stride + 2 + 3 * reg_vb(n) + 7) / 16) * 16 + 8; }
-__host__ __device__ inline int reg_czs(int ni, int nb) { return (ni * nb + 1) & ~1; }
+__host__ __device__ inline int reg_czs(int ni, int nb) { return ((ni + 1) * nb + 1) & ~1; }
 
 // ---------------------------------------------------------------------------------------------------
 // k_fold0: chunk -> element.  Column-owned layout of chunk_dev.cuh.

@@ -25,7 +25,7 @@
 
 #define RN JT_N
 #define RD JT_D
-#define RLDT ((JT_N + 1) | 1)                     /* odd row stride of the exchange buffer: reg_ldt(n) */
+#define RLDT ((JT_N + 2) | 1)                     /* odd row stride of the exchange buffer, >= n + 2 columns (one spare): reg_ldt(n) */
 #define RTM ((((JT_N * RLDT) + 7) / 16) * 16 + 8) /* its size: reg_tm(n) */
 #define RVB (2 * (JT_N + 2))                      /* one vector buffer, (n + 1) pairs: reg_vb(n) */
 #define SG_REG_FENCE asm volatile("" ::: "memory")
@@ -125,9 +125,14 @@ struct Cols {
   int qoff[CPL];    // record offset of column (jc - off_b) of the block's Q_xx; row stride qst
   int qst[CPL];
   int q12off[CPL];  // record offset of q12[jc - off_b]
+  int wcol[CPL];    // exchange write: column jc of the buffer (the spare column n + 1 for a lane without a column)
+  int vidx[CPL];    // entry of this column in an end event's vector buffers (the spare entry n + 1 without a column)
+  int c0base[CPL];  // row of the shared coupling table for a z column (jc = d + q: q NB), the all-zero row otherwise
+  int zq[CPL];      // q of a z column, 0 otherwise
+  double czown[CPL][JT_NI]; // c_qb of the column's own block b for every instrument q (0 for a column that is not an x column)
   unsigned comp;    // bit c: slot c is the companion column n
   unsigned xcol;    // bit c: jc < n (a matrix column)
-  __device__ __forceinline__ void init(int gl) {
+  __device__ __forceinline__ void init(int gl, const double* czs) {
     comp = 0u; xcol = 0u;
 #pragma unroll
     for (int c = 0; c < CPL; ++c) {
@@ -136,6 +141,11 @@ struct Cols {
       if (j == RN) comp |= 1u << c;
       if (j < RN) xcol |= 1u << c;
       rbase[c] = (j < RN) ? j * RLDT : 0;
+      wcol[c] = (j <= RN) ? j : RN + 1;
+      vidx[c] = (j <= RN) ? j : RN + 1;
+      const bool isz = j >= RD && j < RN;
+      zq[c] = isz ? j - RD : 0;
+      c0base[c] = isz ? (j - RD) * JT_NB : JT_NI * JT_NB;
       int mb = -1, qo = 0, qs = 1, q12 = 0;
 #pragma unroll
       for (int b = 0; b < JT_NB; ++b) {
@@ -143,6 +153,8 @@ struct Cols {
         if (jj >= 0 && jj < db) { mb = b; qo = ro + db * db + db + jj; qs = db; q12 = ro + 2 * db * db + db + jj; }
       }
       myblk[c] = mb; qoff[c] = qo; qst[c] = qs; q12off[c] = q12;
+#pragma unroll
+      for (int q = 0; q < JT_NI; ++q) czown[c][q] = (mb >= 0) ? czs[q * JT_NB + mb] : 0.0;
     }
   }
 };
@@ -173,12 +185,13 @@ __device__ __forceinline__ void add_z(double (&x)[RN], int q, double val) {
 // index (the companion slot: see r_companion_back).  Two group barriers.
 template <int G, int CPL, int NS, int S0>
 __device__ __forceinline__ void r_exchange(const Grp<G>& g, const Cols<G, CPL>& cl, double* __restrict__ Tm, double (&v)[NS][RN]) {
+  // no lane-dependent branch anywhere (a divergent branch serialises the warp behind a reconvergence barrier:
+  // measured 4x on these few lines): a lane without a column writes the buffer's spare column
 #pragma unroll
-  for (int c = 0; c < CPL; ++c)
-    if (cl.jc[c] <= RN) {
+  for (int c = 0; c < CPL; ++c) {
 #pragma unroll
-      for (int i = 0; i < RN; ++i) Tm[i * RLDT + cl.jc[c]] = v[S0 + c][i];
-    }
+    for (int i = 0; i < RN; ++i) Tm[i * RLDT + cl.wcol[c]] = v[S0 + c][i];
+  }
   g.sync();
 #pragma unroll
   for (int c = 0; c < CPL; ++c) {
@@ -194,9 +207,13 @@ template <int G, int CPL, int NS, int S0>
 __device__ __forceinline__ void r_companion_back(const Cols<G, CPL>& cl, const double* __restrict__ Tm, double (&v)[NS][RN]) {
 #pragma unroll
   for (int c = 0; c < CPL; ++c)
-    if (slot_has_comp<G>(c) && ((cl.comp >> c) & 1u)) {
+    if (slot_has_comp<G>(c)) { // compile-time
+      const bool isc = (cl.comp >> c) & 1u;
 #pragma unroll
-      for (int i = 0; i < RN; ++i) v[S0 + c][i] = Tm[i * RLDT + RN];
+      for (int i = 0; i < RN; ++i) {
+        const double r = Tm[i * RLDT + RN]; // one address for the whole group: a broadcast
+        v[S0 + c][i] = isc ? r : v[S0 + c][i];
+      }
     }
 }
 
@@ -204,16 +221,15 @@ __device__ __forceinline__ void r_companion_back(const Cols<G, CPL>& cl, const d
 template <int G, int CPL, int NS, int S0>
 __device__ __forceinline__ void r_symmetrise(const Grp<G>& g, const Cols<G, CPL>& cl, double* __restrict__ Tm, double (&v)[NS][RN]) {
 #pragma unroll
-  for (int c = 0; c < CPL; ++c)
-    if ((cl.xcol >> c) & 1u) {
+  for (int c = 0; c < CPL; ++c) {
 #pragma unroll
-      for (int i = 0; i < RN; ++i) Tm[i * RLDT + cl.jc[c]] = v[S0 + c][i];
-    }
+    for (int i = 0; i < RN; ++i) Tm[i * RLDT + cl.wcol[c]] = v[S0 + c][i]; // (the companion's column n is never read back)
+  }
   g.sync();
 #pragma unroll
   for (int c = 0; c < CPL; ++c) {
     const bool isx = (cl.xcol >> c) & 1u;
-    const int rb = isx ? cl.jc[c] * RLDT : 0;
+    const int rb = cl.rbase[c];
 #pragma unroll
     for (int l = 0; l < RN; ++l) {
       const double r = Tm[rb + l];
@@ -223,33 +239,31 @@ __device__ __forceinline__ void r_symmetrise(const Grp<G>& g, const Cols<G, CPL>
   g.sync();
 }
 
-// column jc of X += column jc of Q = R Q~ R^T (Eq. 3.10 P:403-405 per block; z rows / columns through c_qb)
-template <int B, int NS>
-__device__ __forceinline__ void rQ_xrows(const Tab& T, unsigned tz, int myblk, const double (&qv)[SG_MAXBD], double q12, double (&x)[RN]) {
+// column jc of X += column jc of Q = R Q~ R^T (Eq. 3.10 P:403-405 per block; z rows / columns through c_qb).  Branch-free:
+// what depends on the lane's column (its block, whether it is a z column) enters as 0 / 1 factors and per-lane
+// table rows, never as a divergent branch.
+template <int B>
+__device__ __forceinline__ void rQ_xrows(int myblk, const double (&qv)[SG_MAXBD], double (&x)[RN]) {
   if constexpr (B < JT_NB) {
     constexpr int DB = jt_bdim(B), OFF = jt_boff(B);
-    if (myblk == B) {
+    const double ind = (myblk == B) ? 1.0 : 0.0;
 #pragma unroll
-      for (int i = 0; i < DB; ++i) x[OFF + i] += qv[i];
-#pragma unroll
-      for (int q = 0; q < JT_NI; ++q)
-        if (jt_czmask(q * JT_NB + B)) x[RD + q] = fma(((tz >> q) & 1u) ? 0.0 : T.cz[q * JT_NB + B], q12, x[RD + q]);
-    }
-    rQ_xrows<B + 1, NS>(T, tz, myblk, qv, q12, x);
+    for (int i = 0; i < DB; ++i) x[OFF + i] = fma(qv[i], ind, x[OFF + i]);
+    rQ_xrows<B + 1>(myblk, qv, x);
   }
 }
 template <int B>
-__device__ __forceinline__ void rQ_zcol(const Tab& T, const double* rec, const double* __restrict__ czs, unsigned tz, int q0, double (&x)[RN]) {
+__device__ __forceinline__ void rQ_zcol(const Tab& T, const double* rec, const double* __restrict__ c0row, double keep, unsigned tz, double (&x)[RN]) {
   if constexpr (B < JT_NB) {
     constexpr int DB = jt_bdim(B), OFF = jt_boff(B), RO = jt_roff(B);
-    const double c0 = czs[q0 * JT_NB + B];
+    const double c0 = c0row[B] * keep; // c_{q0 b} for the lane's z column q0 (0 for any other column, or when q0 is zeroed)
 #pragma unroll
     for (int l = 0; l < DB; ++l) x[OFF + l] = fma(c0, rec[RO + 2 * DB * DB + DB + l], x[OFF + l]);
     const double q22 = rec[RO + 2 * DB * DB + 2 * DB];
 #pragma unroll
     for (int p = 0; p < JT_NI; ++p)
       if (jt_czmask(p * JT_NB + B)) x[RD + p] = fma(((tz >> p) & 1u) ? 0.0 : c0 * T.cz[p * JT_NB + B], q22, x[RD + p]);
-    rQ_zcol<B + 1>(T, rec, czs, tz, q0, x);
+    rQ_zcol<B + 1>(T, rec, c0row, keep, tz, x);
   }
 }
 template <int G, int CPL, int NS, int S0>
@@ -261,23 +275,38 @@ __device__ __forceinline__ void r_add_Q(const Tab& T, const Cols<G, CPL>& cl, co
 #pragma unroll
     for (int i = 0; i < SG_MAXBD; ++i) qv[i] = rec[cl.qoff[c] + i * cl.qst[c]];
     const double q12 = rec[cl.q12off[c]];
-    rQ_xrows<0, NS>(T, tz, cl.myblk[c], qv, q12, v[S0 + c]);
-    if (slot_has_z<G>(c)) {
-      const int q0 = cl.jc[c] - RD;
-      if (q0 >= 0 && q0 < JT_NI && !((tz >> q0) & 1u)) rQ_zcol<0>(T, rec, czs, tz, q0, v[S0 + c]);
+    rQ_xrows<0>(cl.myblk[c], qv, v[S0 + c]);
+#pragma unroll
+    for (int q = 0; q < JT_NI; ++q) v[S0 + c][RD + q] = fma(((tz >> q) & 1u) ? 0.0 : cl.czown[c][q], q12, v[S0 + c][RD + q]);
+    if (slot_has_z<G>(c)) { // compile-time: only the slots that hold a z column on some lane
+      const double keep = ((tz >> cl.zq[c]) & 1u) ? 0.0 : 1.0;
+      rQ_zcol<0>(T, rec, czs + cl.c0base[c], keep, tz, v[S0 + c]);
     }
   }
 }
 
 // X <- F X F^T (+ Q), x <- F x on the slots S0..S0+CPL-1
+#ifdef SG_CHUNK_CLK /* debugging aid (SMOLGP_JIT_DEFS): cycles per phase of the forward sandwich, accumulated per chunk */
+#define SG_CCK(i) do { const long long t_ = clock64(); sg_cck[i] += t_ - sg_ct; sg_ct = t_; } while (0)
+#define SG_CCK_ARGS , long long (&sg_cck)[12], long long& sg_ct
+#define SG_CCK_PASS , sg_cck, sg_ct
+#else
+#define SG_CCK(i) do {} while (0)
+#define SG_CCK_ARGS
+#define SG_CCK_PASS
+#endif
 template <int G, int CPL, int NS, int S0, bool ADDQ>
 __device__ __forceinline__ void r_sandwich_F(const Grp<G>& g, const Tab& T, const Cols<G, CPL>& cl, const double* rec,
-                                             const double* __restrict__ czs, unsigned tz, double* __restrict__ Tm, double (&v)[NS][RN]) {
+                                             const double* __restrict__ czs, unsigned tz, double* __restrict__ Tm, double (&v)[NS][RN] SG_CCK_ARGS) {
   r_apply_F<NS, S0, S0 + CPL>(T, rec, tz, v);
+  SG_CCK(1);
   r_exchange<G, CPL, NS, S0>(g, cl, Tm, v);
+  SG_CCK(2);
   r_apply_F<NS, S0, S0 + CPL>(T, rec, tz, v);
+  SG_CCK(3);
   r_companion_back<G, CPL, NS, S0>(cl, Tm, v);
   if (ADDQ) r_add_Q<G, CPL, NS, S0>(T, cl, rec, czs, tz, v);
+  SG_CCK(4);
 }
 template <int G, int CPL>
 __device__ __forceinline__ void r_sandwich_Ft(const Grp<G>& g, const Tab& T, const Cols<G, CPL>& cl, const double* rec, unsigned tz,
@@ -314,15 +343,15 @@ __device__ __forceinline__ void reg_fold0_body(const ScanDev& P) {
   const Tab& T = P.T;
   const Grp<G> g;
   const int gpc = blockDim.x / G;
-  double* czs = (double*)smem; // [NI x NB] couplings, read with lane-dependent indices
-  for (int e = threadIdx.x; e < JT_NI * JT_NB; e += blockDim.x) czs[e] = T.cz[e];
+  double* czs = (double*)smem; // [(NI + 1) x NB] couplings, read with lane-dependent indices; the last row is zero
+  for (int e = threadIdx.x; e < (JT_NI + 1) * JT_NB; e += blockDim.x) czs[e] = (e < JT_NI * JT_NB) ? T.cz[e] : 0.0;
   __syncthreads();
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  constexpr int CZS = (JT_NI * JT_NB + 1) & ~1; // reg_czs
+  constexpr int CZS = ((JT_NI + 1) * JT_NB + 1) & ~1; // reg_czs
   RegSmem sm((double*)smem + CZS + (size_t)(threadIdx.x / G) * reg_group_doubles(JT_N, JT_STRIDE));
   Cols<G, CPL> cl;
-  cl.init(g.gl);
+  cl.init(g.gl, czs);
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
@@ -377,7 +406,7 @@ __device__ __forceinline__ void reg_fold0_body(const ScanDev& P) {
       for (int c = 0; c < CPL; ++c) {
         av_o[c] = hs * get_z(S[c], q);
         cv_o[c] = hs * get_z(S[CPL + c], q);
-        if (cl.jc[c] <= RN) avcv[cl.jc[c]] = make_double2(av_o[c], cv_o[c]);
+        avcv[cl.vidx[c]] = make_double2(av_o[c], cv_o[c]);
       }
       g.sync();
       const double Sv = hs * avcv[zi].y + sg * sg;
@@ -407,9 +436,10 @@ __device__ __forceinline__ void reg_fold0_body(const ScanDev& P) {
       for (int c = 0; c < CPL; ++c) {
         set_z(S[c], q, 0.0);
         set_z(S[CPL + c], q, 0.0);
-        if (slot_has_z<G>(c) && cl.jc[c] == zi) {
+        if (slot_has_z<G>(c)) {
+          const bool kz = cl.jc[c] == zi;
 #pragma unroll
-          for (int i = 0; i < RN; ++i) S[CPL + c][i] = 0.0;
+          for (int i = 0; i < RN; ++i) S[CPL + c][i] = kz ? 0.0 : S[CPL + c][i];
         }
       }
       g.sync();
@@ -469,14 +499,14 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
   const Grp<G> g;
   const int gpc = blockDim.x / G;
   double* czs = (double*)smem;
-  for (int e = threadIdx.x; e < JT_NI * JT_NB; e += blockDim.x) czs[e] = T.cz[e];
+  for (int e = threadIdx.x; e < (JT_NI + 1) * JT_NB; e += blockDim.x) czs[e] = (e < JT_NI * JT_NB) ? T.cz[e] : 0.0;
   __syncthreads();
   const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
   if (gid >= P.batch * P.c1) return;
-  constexpr int CZS = (JT_NI * JT_NB + 1) & ~1; // reg_czs
+  constexpr int CZS = ((JT_NI + 1) * JT_NB + 1) & ~1; // reg_czs
   RegSmem sm((double*)smem + CZS + (size_t)(threadIdx.x / G) * reg_group_doubles(JT_N, JT_STRIDE));
   Cols<G, CPL> cl;
-  cl.init(g.gl);
+  cl.init(g.gl, czs);
   const int ss = state_size(RN), ks = kbuf_stride(RN);
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
@@ -496,6 +526,10 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
   rs.init(g, sm.recs, JT_STRIDE);
   rs.issue(g, P.disc + k0 * (int64_t)JT_STRIDE, 0);
   double ll = 0.0;
+#ifdef SG_CHUNK_CLK
+  long long sg_cck[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  long long sg_ct = clock64();
+#endif
   // ---- forward ----
   uint32_t meta_nx = P.meta[k0];
   int32_t ob_nx = P.obs[k0];
@@ -503,6 +537,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
     const int it = (int)(k - k0);
     const double* rec = rs.wait(it & 1);
     g.sync();
+    SG_CCK(0);
     if (k + 1 < k1) rs.issue(g, P.disc + (k + 1) * (int64_t)JT_STRIDE, (it + 1) & 1);
     const uint32_t meta = meta_nx;
     const int32_t ob = ob_nx;
@@ -512,7 +547,8 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
     double dl_r = 1.0, sg_r = 0.0, y_r = 0.0;
     if (!kind) { dl_r = P.delta[k]; sg_r = P.sigma[ob]; y_r = P.y[series * P.N + ob]; }
-    r_sandwich_F<G, CPL, CPL, 0, true>(g, T, cl, rec, czs, tz, sm.Tm, X);
+    SG_CCK(5);
+    r_sandwich_F<G, CPL, CPL, 0, true>(g, T, cl, rec, czs, tz, sm.Tm, X SG_CCK_PASS);
     if (!kind) {
       const int zi = RD + q;
       const double hs = T.tau[q] / dl_r;
@@ -522,7 +558,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
 #pragma unroll
       for (int c = 0; c < CPL; ++c) {
         xz[c] = hs * get_z(X[c], q); // hs P[z, j] = hs P[j, z];  companion: hs m_z
-        if (cl.jc[c] <= RN) cvb[cl.jc[c]] = xz[c];
+        cvb[cl.vidx[c]] = xz[c];
       }
       g.sync();
       const double Sv = hs * cvb[zi] + sg * sg;
@@ -554,18 +590,28 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
 #pragma unroll
       for (int c = 0; c < CPL; ++c) {
         set_z(X[c], q, 0.0);
-        if (slot_has_z<G>(c) && cl.jc[c] == zi) {
+        if (slot_has_z<G>(c)) {
+          const bool kz = cl.jc[c] == zi;
 #pragma unroll
-          for (int i = 0; i < RN; ++i) X[c][i] = 0.0;
+          for (int i = 0; i < RN; ++i) X[c][i] = kz ? 0.0 : X[c][i];
         }
       }
       g.sync();
     }
+    SG_CCK(6);
     // the two triangles of F P F^T are rounded independently: re-symmetrised every 8th event
     if ((it & 7) == 7) r_symmetrise<G, CPL, CPL, 0>(g, cl, sm.Tm, X);
+    SG_CCK(7);
     if (P.fstate) reg_store_state<G, CPL>(cl, X, P.fstate + (series * P.K + k) * (int64_t)ss); // row a7
   }
   if (g.gl == 0) P.llpart[gid] = ll;
+#ifdef SG_CHUNK_CLK
+  if (gid == 5 && g.gl == 0) {
+    const long long ne = k1 - k0;
+    printf("down0 fwd cycles/event: wait+sync %lld | meta etc %lld | F1 %lld | exchange %lld | F2 %lld | comp+Q %lld | end-event %lld | sym %lld\n", sg_cck[0] / ne,
+           sg_cck[5] / ne, sg_cck[1] / ne, sg_cck[2] / ne, sg_cck[3] / ne, sg_cck[4] / ne, sg_cck[6] / ne, sg_cck[7] / ne);
+  }
+#endif
   if (!P.want_smooth) return;
 
   // ---- adjoint at the chunk's last event (k_adjD: Lambda^ = (I + J P)^-1 J, lambda^ = (I + J P)^-1 (J m - eta)) ----
@@ -611,9 +657,10 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
 #pragma unroll
         for (int c = 0; c < CPL; ++c) {
           X[c][RD + r] = 0.0;
-          if (slot_has_z<G>(c) && cl.jc[c] == RD + r) {
+          if (slot_has_z<G>(c)) {
+            const bool kz = cl.jc[c] == RD + r;
 #pragma unroll
-            for (int i = 0; i < RN; ++i) X[c][i] = 0.0;
+            for (int i = 0; i < RN; ++i) X[c][i] = kz ? 0.0 : X[c][i];
           }
         }
       }
@@ -624,8 +671,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
       double2* kp = reinterpret_cast<double2*>(sm.vb1); // (K_i, p_i) pairs
       double* gvb = sm.vb2;
 #pragma unroll
-      for (int c = 0; c < CPL; ++c)
-        if (cl.jc[c] < RN) kp[cl.jc[c]] = make_double2(kv_c[c], pv_c[c]);
+      for (int c = 0; c < CPL; ++c) kp[cl.vidx[c]] = make_double2(kv_c[c], pv_c[c]); // (entries n, n + 1: never read)
       g.sync();
       double a[CPL], b[CPL];
 #pragma unroll
@@ -643,7 +689,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
         quad += isx ? pv_c[c] * a[c] : 0.0;
         kap += isx ? kv_c[c] * b[c] : 0.0;
         an += isc ? a[c] : 0.0;
-        if (isx) gvb[cl.jc[c]] = b[c];
+        gvb[cl.vidx[c]] = b[c];
       }
       quad = group_sum(g, quad);
       kap = group_sum(g, kap);
@@ -661,10 +707,11 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
         const bool isx = (cl.xcol >> c) & 1u, isc = (cl.comp >> c) & 1u;
         const double dz = isx ? -hs * b[c] : (isc ? -hs * (b[c] + v * rS) : 0.0);
         add_z(X[c], q, dz); // row z of the lane's columns
-        if (slot_has_z<G>(c) && cl.jc[c] == zi) { // column z
+        if (slot_has_z<G>(c)) { // column z: the lane that owns it, by a 0 / 1 factor
+          const double hz = (cl.jc[c] == zi) ? hs : 0.0;
 #pragma unroll
-          for (int j = 0; j < RN; ++j) X[c][j] -= hs * gvb[j];
-          add_z(X[c], q, hs * hs * (kap + rS));
+          for (int j = 0; j < RN; ++j) X[c][j] = fma(-hz, gvb[j], X[c][j]);
+          add_z(X[c], q, hz * hs * (kap + rS));
         }
       }
       g.sync();
