@@ -143,7 +143,9 @@ __device__ void gj_solve_wcol(const Grp<G>& g, int n, int nc_all, int ld, const 
       const bool cand = act && !((used >> lane) & 1u);
       const unsigned long long key = cand ? (unsigned long long)__double_as_longlong(fabs(a)) + 1ull : 0ull;
       const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
-      const double rc = 1.0 / a; // every lane its own candidate reciprocal: independent of the search below
+      // every lane its own candidate reciprocal, independent of the search below.  Lanes beyond the last row hold
+      // zeros: 1 / 0 would send the whole warp through the division's slow path at every pivot (measured)
+      const double rc = 1.0 / (act ? a : 1.0);
       const unsigned mhi = __reduce_max_sync(0xffffffffu, hi);
       const unsigned mlo = __reduce_max_sync(0xffffffffu, hi == mhi ? lo : 0u);
       const unsigned hit = __ballot_sync(0xffffffffu, hi == mhi && lo == mlo);
