@@ -84,20 +84,39 @@ __device__ void disc_block(const BlockConst& B, double dts, int instant, double*
     double rel = 1.0;
     while (rel > 3.5e-18 && kt < SG_KT) { ++kt; rel *= x / (double)kt; }
   }
+  // Horner only for what has no cheap closed form: the integral row Phi-bar (row DB of Phi~) and the lower triangle of
+  // the symmetric Q~ (DB + M (M + 1) / 2 series instead of 2 M^2); Phi(h) itself is the family's closed form, the last
+  // column of Phi~ is (0, ..., 0, 1)
   double A[M][M], Q[M][M];
+  {
+    double P[DB][DB];
+    phi_closed<DB>(B, h, P);
+#pragma unroll
+    for (int i = 0; i < DB; ++i) {
+#pragma unroll
+      for (int j = 0; j < DB; ++j) A[i][j] = P[i][j];
+      A[i][DB] = 0.0;
+    }
+    A[DB][DB] = 1.0;
+  }
+#pragma unroll
+  for (int j = 0; j < DB; ++j) A[DB][j] = B.tayA[kt][DB * SG_BE + j];
 #pragma unroll
   for (int i = 0; i < M; ++i)
 #pragma unroll
-    for (int j = 0; j < M; ++j) { A[i][j] = B.tayA[kt][i * SG_BE + j]; Q[i][j] = B.tayQ[kt][i * SG_BE + j]; }
+    for (int j = 0; j <= i; ++j) Q[i][j] = B.tayQ[kt][i * SG_BE + j];
   for (int k = kt - 1; k >= 0; --k) {
+#pragma unroll
+    for (int j = 0; j < DB; ++j) A[DB][j] = fma(A[DB][j], h, B.tayA[k][DB * SG_BE + j]);
 #pragma unroll
     for (int i = 0; i < M; ++i)
 #pragma unroll
-      for (int j = 0; j < M; ++j) {
-        A[i][j] = fma(A[i][j], h, B.tayA[k][i * SG_BE + j]);
-        Q[i][j] = fma(Q[i][j], h, B.tayQ[k][i * SG_BE + j]);
-      }
+      for (int j = 0; j <= i; ++j) Q[i][j] = fma(Q[i][j], h, B.tayQ[k][i * SG_BE + j]);
   }
+#pragma unroll
+  for (int i = 0; i < M; ++i)
+#pragma unroll
+    for (int j = i + 1; j < M; ++j) Q[i][j] = Q[j][i];
   for (int lev = 0; lev < s; ++lev) {
     if (lev > 0) {
       double P[DB][DB];
