@@ -22,6 +22,15 @@ static const char* const JIT_SRC =
 #include "jit_src.inc"
     ;
 
+// ahead-of-time copies of the specialised module for the structures of the shipped workloads (_build.py: PREBUILT):
+// binary blobs linked into this library, looked up by the same structure key as the run-time cache
+struct SgPrebuilt { const char* key; const unsigned char* begin; const unsigned char* end; };
+#define SG_INCBIN(sym, file)                                                                                              \
+  asm(".section .rodata\n.balign 16\n.global " #sym "\n" #sym ":\n.incbin \"" file "\"\n.global " #sym "_end\n" #sym "_end:\n.byte 0\n.previous\n"); \
+  extern "C" const unsigned char sym[];                                                                                   \
+  extern "C" const unsigned char sym##_end[];
+#include "prebuilt.inc"
+
 struct NvrtcApi {
   void* h = nullptr;
   nvrtcResult (*create)(nvrtcProgram*, const char*, const char*, int, const char* const*, const char* const*) = nullptr;
@@ -146,6 +155,33 @@ void sg_jit_destroy(smolgp_ctx* ctx) {
 
 const char* sg_jit_log(smolgp_ctx* ctx) { return ctx->jit ? ((JitState*)ctx->jit)->log.c_str() : ""; }
 
+static bool load_module(JitState* st, JitEntry& ent, const void* cubin, const SgJitCfg& cfg) {
+  cudaError_t e = cudaLibraryLoadData(&ent.k.lib, cubin, nullptr, nullptr, 0, nullptr, nullptr, 0);
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.fold0, ent.k.lib, "jit_fold0");
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.down0, ent.k.lib, "jit_down0");
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.query, ent.k.lib, "jit_query");
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.foldD, ent.k.lib, "jit_foldD");
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.downD, ent.k.lib, "jit_downD");
+  if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.adjD, ent.k.lib, "jit_adjD");
+  if (e != cudaSuccess) { st->log = std::string("loading the specialised kernels: ") + cudaGetErrorString(e); cudaGetLastError(); return false; }
+  cudaFuncAttributes fa;
+  ent.k.regs_fold0 = (cudaFuncGetAttributes(&fa, (const void*)ent.k.fold0) == cudaSuccess) ? fa.numRegs : 255;
+  ent.k.regs_down0 = (cudaFuncGetAttributes(&fa, (const void*)ent.k.down0) == cudaSuccess) ? fa.numRegs : 255;
+  cudaGetLastError();
+  ent.k.cfg = cfg;
+  return true;
+}
+
+static const SgPrebuilt* find_prebuilt(const std::string& key) {
+  if (getenv("SMOLGP_NO_PREBUILT") || getenv("SMOLGP_JIT_DEFS") || getenv("SMOLGP_JIT_DUMP")) return nullptr; // debugging aids: force the NVRTC path
+  for (const SgPrebuilt& p : SG_PREBUILT)
+    if (key == p.key) return &p;
+  return nullptr;
+}
+
+// is there an ahead-of-time module for this structure?  (then it is used from the first call)
+bool sg_jit_prebuilt(smolgp_ctx*, const Tab& T, const SgJitCfg& cfg) { return find_prebuilt(structure_key(T, cfg)) != nullptr; }
+
 // returns the specialised kernels for (T's structure, G, LD), compiling them on first use; nullptr when
 // run-time compilation is unavailable or failed (the reason is kept in sg_jit_log)
 const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg) {
@@ -153,52 +189,44 @@ const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cf
   const std::string key = structure_key(T, cfg);
   for (auto& e : st->cache)
     if (e.key == key) return e.good ? &e.k : nullptr;
-  if (!st->tried_open) { st->tried_open = true; if (!open_nvrtc(st->api)) st->log = "NVRTC not available (dlopen libnvrtc.so.12 failed)"; }
   JitEntry ent;
   ent.key = key;
   ent.good = false;
   memset(&ent.k, 0, sizeof ent.k);
-  if (st->api.ok) {
-    std::string src = prelude(T, cfg);
-    if (const char* defs = getenv("SMOLGP_JIT_DEFS")) { src += defs; src += "\n"; } // debugging aid: extra #defines for the specialised build
-    src += JIT_SRC;
-    if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the exact text handed to NVRTC
-      if (FILE* f = fopen(dump, "w")) { fwrite(src.data(), 1, src.size(), f); fclose(f); }
-    }
-    nvrtcProgram prog = nullptr;
-    const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo"};
-    nvrtcResult r = st->api.create(&prog, src.c_str(), "smolgp_chunk_jit.cu", 0, nullptr, nullptr);
-    if (r == NVRTC_SUCCESS) r = st->api.compile(prog, 3, opts);
-    if (r != NVRTC_SUCCESS) {
-      size_t ls = 0;
-      if (prog && st->api.log_size(prog, &ls) == NVRTC_SUCCESS && ls > 1) { st->log.resize(ls); st->api.log(prog, &st->log[0]); }
-      else st->log = "nvrtc: compilation failed";
-    } else {
-      size_t cs = 0;
-      st->api.cubin_size(prog, &cs);
-      std::vector<char> cubin(cs);
-      st->api.cubin(prog, cubin.data());
-      if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the cubin beside the source (nvdisasm -g maps SASS to lines)
-        if (FILE* f = fopen((std::string(dump) + ".cubin").c_str(), "wb")) { fwrite(cubin.data(), 1, cubin.size(), f); fclose(f); }
+  ent.k.prebuilt = 0;
+  if (const SgPrebuilt* pb = find_prebuilt(key)) {
+    ent.good = load_module(st, ent, pb->begin, cfg);
+    ent.k.prebuilt = ent.good ? 1 : 0;
+  }
+  if (!ent.good) {
+    if (!st->tried_open) { st->tried_open = true; if (!open_nvrtc(st->api)) st->log = "NVRTC not available (dlopen libnvrtc.so.12 failed)"; }
+    if (st->api.ok) {
+      std::string src = prelude(T, cfg);
+      if (const char* defs = getenv("SMOLGP_JIT_DEFS")) { src += defs; src += "\n"; } // debugging aid: extra #defines for the specialised build
+      src += JIT_SRC;
+      if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the exact text handed to NVRTC
+        if (FILE* f = fopen(dump, "w")) { fwrite(src.data(), 1, src.size(), f); fclose(f); }
       }
-      cudaError_t e = cudaLibraryLoadData(&ent.k.lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.fold0, ent.k.lib, "jit_fold0");
-      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.down0, ent.k.lib, "jit_down0");
-      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.query, ent.k.lib, "jit_query");
-      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.foldD, ent.k.lib, "jit_foldD");
-      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.downD, ent.k.lib, "jit_downD");
-      if (e == cudaSuccess) e = cudaLibraryGetKernel(&ent.k.adjD, ent.k.lib, "jit_adjD");
-      if (e == cudaSuccess) {
-        cudaFuncAttributes fa;
-        ent.k.regs_fold0 = (cudaFuncGetAttributes(&fa, (const void*)ent.k.fold0) == cudaSuccess) ? fa.numRegs : 255;
-        ent.k.regs_down0 = (cudaFuncGetAttributes(&fa, (const void*)ent.k.down0) == cudaSuccess) ? fa.numRegs : 255;
-        cudaGetLastError();
-        ent.k.cfg = cfg;
-        ent.good = true;
+      nvrtcProgram prog = nullptr;
+      const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo"};
+      nvrtcResult r = st->api.create(&prog, src.c_str(), "smolgp_chunk_jit.cu", 0, nullptr, nullptr);
+      if (r == NVRTC_SUCCESS) r = st->api.compile(prog, 3, opts);
+      if (r != NVRTC_SUCCESS) {
+        size_t ls = 0;
+        if (prog && st->api.log_size(prog, &ls) == NVRTC_SUCCESS && ls > 1) { st->log.resize(ls); st->api.log(prog, &st->log[0]); }
+        else st->log = "nvrtc: compilation failed";
+      } else {
+        size_t cs = 0;
+        st->api.cubin_size(prog, &cs);
+        std::vector<char> cubin(cs);
+        st->api.cubin(prog, cubin.data());
+        if (const char* dump = getenv("SMOLGP_JIT_DUMP")) { // debugging aid: the cubin beside the source (nvdisasm -g maps SASS to lines)
+          if (FILE* f = fopen((std::string(dump) + ".cubin").c_str(), "wb")) { fwrite(cubin.data(), 1, cubin.size(), f); fclose(f); }
+        }
+        ent.good = load_module(st, ent, cubin.data(), cfg);
       }
-      else { st->log = std::string("loading the specialised kernels: ") + cudaGetErrorString(e); cudaGetLastError(); }
+      if (prog) st->api.destroy(&prog);
     }
-    if (prog) st->api.destroy(&prog);
   }
   st->cache.push_back(ent);
   return st->cache.back().good ? &st->cache.back().k : nullptr;

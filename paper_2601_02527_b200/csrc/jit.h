@@ -17,8 +17,10 @@ struct SgJitKernels {
   cudaKernel_t fold0, down0, query, foldD, downD, adjD;
   SgJitCfg cfg;
   int regs_fold0, regs_down0; // registers per thread of the compiled chunk kernels
+  int prebuilt;               // 1: the module is the ahead-of-time copy linked into the library (no NVRTC involved)
 };
 const SgJitKernels* sg_jit_get(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg);
+bool sg_jit_prebuilt(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg);
 bool sg_jit_hot(smolgp_ctx* ctx, const Tab& T, const SgJitCfg& cfg, bool count);
 void sg_jit_destroy(smolgp_ctx* ctx);
 const char* sg_jit_log(smolgp_ctx* ctx);

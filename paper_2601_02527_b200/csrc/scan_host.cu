@@ -90,7 +90,7 @@ static L0Plan plan_l0(smolgp_ctx* ctx, const Tab& T, int G, int64_t events, bool
   if (ctx->opt_jit != 0) want = ctx->opt_jit > 0;
   else {
     const bool hot = sg_jit_hot(ctx, T, p.cfg, count); // counted once per API call (sg_run_scan)
-    want = events >= 100000 || hot;
+    want = events >= 100000 || hot || sg_jit_prebuilt(ctx, T, p.cfg); // an ahead-of-time module costs nothing to use
   }
   if (want) p.jk = sg_jit_get(ctx, T, p.cfg);
   return p;
@@ -350,9 +350,9 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   if (rc) return rc;
   {
     char buf[256];
-    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=%d fold_lanes=%d jit=%d kernels=%s regs=%d/%d", n,
+    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=%d fold_lanes=%d jit=%d kernels=%s regs=%d/%d prebuilt=%d", n,
              (long long)batch, (long long)K, (long long)Lc, (long long)c1, pl.T, g, Gd, reg ? jk0->cfg.rCPL : 1, reg ? jk0->cfg.fG : G,
-             jk0 ? 1 : 0, reg ? "reg" : "smem", jk0 ? jk0->regs_fold0 : 0, jk0 ? jk0->regs_down0 : 0);
+             jk0 ? 1 : 0, reg ? "reg" : "smem", jk0 ? jk0->regs_fold0 : 0, jk0 ? jk0->regs_down0 : 0, jk0 ? jk0->prebuilt : 0);
     ctx->plan = buf;
   }
   if (a.loglik) {

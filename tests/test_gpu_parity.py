@@ -35,7 +35,8 @@ SCAN_OPTS = {
     "deep": (("chunk", 16), ("group", 2), ("top", 2)),         # many dense levels, tree up to the root
     "walk": (("chunk", 16), ("group", 2), ("top", 13)),        # long sequential walk at the top level
     "ragged": (("chunk", 37), ("group", 3), ("lanes", 32)),    # chunk/group sizes dividing nothing
-    "jit": (("chunk", 29), ("jit", 1)),                        # run-time specialised chunk kernels (NVRTC)
+    "jit": (("chunk", 29), ("jit", 1)),                        # specialised chunk kernels (ahead-of-time module or NVRTC)
+    "generic": (("chunk", 23), ("jit", -1)),                   # the statically compiled shared-memory kernels
 }
 
 
@@ -705,3 +706,24 @@ def test_loglik_gradient_device_pointers_and_instant(ctx, oracle):
     for c, comp in enumerate(kern):
         for p in range(oracle.FAMILY_PARAMS[int(comp["family"])]):
             assert abs(g[0, c, p] - ref[c, p]) * comp[oracle.PARAMS[p]] <= 1e-6 * scale
+
+
+def test_shipped_structures_use_the_ahead_of_time_modules(ctx):
+    """the structures of BASELINE.json's configs (and fig2 / fig3 / the instantaneous Fig. 1 kernel) are compiled when the
+    library is built (_build.py: PREBUILT) and used from the first call, without NVRTC"""
+    from paper_2601_02527_b200 import binding as B
+    c2 = B.Context(0)   # a fresh ctx: nothing is "hot" yet
+    try:
+        for cfg, N, batch in [(1, 200, None), (2, 300, None), (3, 300, None), (4, 300, None), (5, 100, 2), ("fig2", 100, None), ("fig3", 150, None)]:
+            w = W.make(cfg, N=N, batch=batch, n_features=4)
+            ev = c2.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
+            c2.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"])
+            assert "prebuilt=1" in c2.plan_info() and "kernels=reg" in c2.plan_info(), (cfg, c2.plan_info())
+            ev.free()
+        w = W.make("instant", N=300, n_features=4)
+        ev = c2.smolgp_build_events_instant_host(w["t_start"], w["instrument"], 1)
+        c2.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"])
+        assert "prebuilt=1" in c2.plan_info(), c2.plan_info()
+        assert c2.jit_log() == ""
+    finally:
+        c2.close()
