@@ -29,6 +29,39 @@
 #define RTM ((((JT_N * RLDT) + 7) / 16) * 16 + 8) /* its size: reg_tm(n) */
 #define RVB (2 * (JT_N + 2))                      /* one vector buffer, (n + 1) pairs: reg_vb(n) */
 #define SG_REG_FENCE asm volatile("" ::: "memory")
+#ifndef SG_SYM_MASK
+#define SG_SYM_MASK 31 /* the state is re-symmetrised every SG_SYM_MASK + 1 events (measured: 8, 32, 128 or never give the same accuracy on configs 3 and 4) */
+#endif
+
+// ---- record staging for these kernels: every lane of the group copies 16-byte pieces with cp.async (LDGSTS) ------------
+// The TMA bulk copy of chunk_dev.cuh (RecStage) is issued by one elected lane through the uniform datapath and waited
+// for on an mbarrier: per event that cost ~600 cycles of this latency-bound stream (clock64: "wait + sync" 263, issue
+// and prefetch 339); a record is only 1.5 KB, so three cp.async per lane do the same with less ceremony.
+#ifndef SG_REC_CP
+#define SG_REC_CP 1
+#endif
+struct RecCp {
+  double* buf;
+  template <int G>
+  __device__ __forceinline__ void init(const Grp<G>&, double* recs, int) { buf = recs; }
+  template <int G>
+  __device__ __forceinline__ void issue(const Grp<G>& g, const double* __restrict__ src, int b) {
+    double* dst = buf + b * JT_STRIDE;
+#pragma unroll
+    for (int o = 2 * g.gl; o < JT_STRIDE; o += 2 * G)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(dst + o)), "l"(src + o) : "memory");
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+  }
+  __device__ __forceinline__ const double* wait(int b) {
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+    return buf + b * JT_STRIDE; // the caller's group barrier makes the other lanes' pieces visible
+  }
+};
+#if SG_REC_CP
+typedef RecCp RegRecStage;
+#else
+typedef RecStage RegRecStage;
+#endif
 
 // ---- blocks of the transition on register columns -------------------------------------------------------
 // v[s][.] <- F v[s][.] for the slots S0 <= s < S1 of v (in place)
@@ -366,7 +399,7 @@ __device__ __forceinline__ void reg_fold0_body(const ScanDev& P) {
 #pragma unroll
     for (int i = 0; i < RN; ++i) S[c][i] = (cl.jc[c] == i) ? 1.0 : 0.0;
 
-  RecStage rs;
+  RegRecStage rs;
   rs.init(g, sm.recs, JT_STRIDE);
   rs.issue(g, P.disc + k0 * (int64_t)JT_STRIDE, 0);
   uint32_t meta_nx = P.meta[k0];
@@ -522,7 +555,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
 #pragma unroll
       for (int i = 0; i < RN; ++i) X[c][i] = (cl.jc[c] < RN) ? P.p0[cl.jc[c] * RN + i] : 0.0;
   }
-  RecStage rs;
+  RegRecStage rs;
   rs.init(g, sm.recs, JT_STRIDE);
   rs.issue(g, P.disc + k0 * (int64_t)JT_STRIDE, 0);
   double ll = 0.0;
@@ -600,7 +633,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
     }
     SG_CCK(6);
     // the two triangles of F P F^T are rounded independently: re-symmetrised every 8th event
-    if ((it & 7) == 7) r_symmetrise<G, CPL, CPL, 0>(g, cl, sm.Tm, X);
+    if ((it & SG_SYM_MASK) == SG_SYM_MASK) r_symmetrise<G, CPL, CPL, 0>(g, cl, sm.Tm, X);
     SG_CCK(7);
     if (P.fstate) reg_store_state<G, CPL>(cl, X, P.fstate + (series * P.K + k) * (int64_t)ss); // row a7
   }
@@ -716,7 +749,7 @@ __device__ __forceinline__ void reg_down0_body(const ScanDev& P) {
       }
       g.sync();
     }
-    if ((it & 7) == 7) r_symmetrise<G, CPL, CPL, 0>(g, cl, sm.Tm, X);
+    if ((it & SG_SYM_MASK) == SG_SYM_MASK) r_symmetrise<G, CPL, CPL, 0>(g, cl, sm.Tm, X);
     if (P.binfo) reg_store_state<G, CPL>(cl, X, P.binfo + (series * P.K + k) * (int64_t)ss);
     if (k == k0) break;
     if (!META_KIND(meta_nx)) { // request event k-1's record now: it arrives during the step below
