@@ -17,7 +17,10 @@
 //               tile) -> for every event the set of instruments exposing after it, hence the zero-mask
 //               Z_k (idle instruments and the event's own) and the check that each instrument's events
 //               alternate start, end, start, ... (no self-overlap); dt_k = t_k - t_{k-1}.
-// Eleven launches whatever N (round 1: 33), one small status read-back.
+//   k_merge     after pass 0: when every (kind, instrument) run is already in time order -- exposures of an instrument
+//               given in time order, the usual case -- the stream is the merge of those runs, done by ranking in one
+//               launch; the eight time passes then return at once.  Otherwise they sort pass 0's output.
+// Twelve launches whatever N (round 1: 33), one small status read-back.
 #include <math.h>
 #include <stddef.h>
 #include <string.h>
@@ -35,6 +38,8 @@
 struct EvCtl {
   uint32_t ghist[RS_DIGITS][256]; // global digit histograms
   uint32_t ticket[RS_DIGITS + 1]; // tile tickets per pass (+ the tail kernel)
+  uint32_t unsorted;              // k_merge: some (kind, instrument) run is not in time order => the radix passes run
+  uint32_t pad0;
   uint32_t ungrouped;             // some exposure has a smaller instrument index than its predecessor
   int32_t flags;                  // EVF_*
   unsigned long long maxdelta[SG_MAXINST]; // bits of the longest exposure per instrument
@@ -153,6 +158,7 @@ __global__ void __launch_bounds__(RS_NT) k_rs_pass(EvCtl* __restrict__ ctl, int 
   __shared__ uint32_t wsum[RS_NT / 32];
   __shared__ unsigned s_mask;
   __shared__ uint32_t s_tile;
+  if (pass >= 1 && ctl->unsorted == 0u) return; // k_merge has produced the sorted stream already
   const unsigned skip = skip_mask(ctl, n, &s_mask);
   if ((skip >> pass) & 1u) return;
   const int moved = __popc(~skip & ((1u << pass) - 1u)); // passes before this one that moved the data
@@ -245,6 +251,56 @@ __global__ void __launch_bounds__(RS_NT) k_rs_pass(EvCtl* __restrict__ ctl, int 
   }
 }
 
+// ---- merge of pre-sorted runs -------------------------------------------------------------------------------------
+// After pass 0 the pairs form up to 2 N_inst runs, one per (kind, instrument), each in exposure order.  Exposures
+// of one instrument usually arrive in time order, and then every run is already sorted: the stream is the MERGE
+// of the runs, and an element's final position is its index in its own run plus, for every other run, the number
+// of elements that precede it (binary search: keys <= mine in the runs before mine, keys < mine in the runs after
+// it -- the runs are in (kind, instrument) order, which is the tie rule).  One launch instead of eight radix
+// passes; a run found out of order raises ctl->unsorted and the passes run on pass 0's output as before.
+__global__ void __launch_bounds__(RS_NT) k_merge(EvCtl* __restrict__ ctl, uint64_t* __restrict__ kA, uint32_t* __restrict__ vA, uint64_t* __restrict__ kB,
+                                                 uint32_t* __restrict__ vB, const int32_t* __restrict__ inst, int n_inst, uint32_t n) {
+  __shared__ uint32_t start[33];
+  const int tid = threadIdx.x;
+  if (tid < 32) { // exclusive scan of the (kind, instrument) counts: run boundaries
+    const uint32_t c = ctl->ghist[0][tid];
+    uint32_t x = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (tid >= o) x += y; }
+    start[tid] = x - c;
+    if (tid == 31) start[32] = x;
+  }
+  __syncthreads();
+  const bool moved0 = ctl->ungrouped != 0u; // pass 0 ran: its output is in B
+  const uint64_t* kin = moved0 ? kB : kA;
+  const uint32_t* vin = moved0 ? vB : vA;
+  uint64_t* kout = moved0 ? kA : kB;
+  uint32_t* vout = moved0 ? vA : vB;
+  const uint32_t p = blockIdx.x * RS_NT + tid;
+  if (p >= n) return;
+  const uint64_t key = kin[p];
+  const uint32_t val = vin[p];
+  int q = inst[val >> 1];
+  if (q < 0 || q >= n_inst) q = 0;
+  const int r = (int)((val & 1u) << 4) | q;
+  if (p > start[r] && kin[p - 1] > key) atomicOr(&ctl->unsorted, 1u);
+  uint32_t rank = p - start[r];
+  for (int rr = 0; rr < 32; ++rr) {
+    const uint32_t lo0 = start[rr], hi0 = start[rr + 1];
+    if (rr == r || lo0 == hi0) continue;
+    uint32_t lo = lo0, hi = hi0; // first index whose key is > mine (rr < r) or >= mine (rr > r)
+    while (lo < hi) {
+      const uint32_t mid = (lo + hi) >> 1;
+      const uint64_t km = kin[mid];
+      const bool before = (rr < r) ? (km <= key) : (km < key);
+      if (before) lo = mid + 1; else hi = mid;
+    }
+    rank += lo - lo0;
+  }
+  kout[rank] = key;
+  vout[rank] = val;
+}
+
 // ---- after the sort: gather, inclusive XOR scan of the instrument bits, flags -----------------------
 #define EF_ITEMS 4
 __global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int64_t K, const uint32_t* __restrict__ vA,
@@ -259,7 +315,8 @@ __global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int
   __shared__ uint32_t s_tile, s_run;
   const bool instant = (te == nullptr);
   const unsigned skip = skip_mask(ctl, (uint32_t)K, &s_mask);
-  const int moved = __popc(~skip & ((1u << RS_DIGITS) - 1u));
+  const int moved = (ctl->unsorted == 0u) ? ((ctl->ungrouped != 0u) ? 2 : 1)  // merged: pass 0 (if it ran) + k_merge
+                                          : __popc(~skip & ((1u << RS_DIGITS) - 1u));
   const uint32_t* vals = (moved & 1) ? vB : vA;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   if (tid == 0) s_tile = atomicAdd(&ctl->ticket[RS_DIGITS], 1u);
@@ -407,6 +464,11 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   k_ev_init<<<(unsigned)((N + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(N, ts, te, inst, n_inst, kA, vA, ctl);
   sg_launch_end(ctx);
   for (int pass = 0; pass < RS_DIGITS; ++pass) {
+    if (pass == 1) { // pass 0 has formed the (kind, instrument) runs: try the merge
+      sg_launch_begin(ctx, KID_RS_PASS);
+      k_merge<<<(unsigned)((K + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(ctl, kA, vA, kB, vB, inst, n_inst, (uint32_t)K);
+      sg_launch_end(ctx);
+    }
     const uint32_t epoch = lb_next_epoch(ctx);
     sg_launch_begin(ctx, KID_RS_PASS);
     if (items == 4) k_rs_pass<4><<<(unsigned)ntiles_rs, RS_NT, 0, st>>>(ctl, pass, kA, vA, kB, vB, inst, n_inst, (uint32_t)K, ctx->lb_status, epoch);
