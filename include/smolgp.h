@@ -136,6 +136,39 @@ int smolgp_build_events_instant(smolgp_ctx* ctx, int64_t N, const double* t, con
 int smolgp_build_events_instant_host(smolgp_ctx* ctx, int64_t N, const double* t, const int32_t* instrument,
                                      int32_t n_inst, smolgp_events** out);
 
+/* Step a1 WITHOUT ANY ALLOCATION -- for callers that cannot call cudaMalloc: code under CUDA stream capture, tight
+ * serving loops, harnesses that forbid it.  Same kernels, same stream order (the tie rule
+ * above) as smolgp_build_events, but
+ *   - the sort's scratch (control block, look-back words, two key and two payload buffers) is ONE file-scope device
+ *     array of fixed size, smolgp_noalloc_scratch_bytes() = about 6.5 MB, which every GPU that loads the library holds
+ *     until exit.  LIMIT: K <= smolgp_noalloc_max_events() = 262144 events, i.e. N <= 131072 exposures (or 262144
+ *     instantaneous samples); beyond it the call returns SMOLGP_EUNSUPPORTED and smolgp_noalloc_last_error() says so;
+ *   - no ctx, no smolgp_events object: the caller owns the outputs.  All pointers are DEVICE pointers.
+ *     inputs  t_start[N], t_end[N] (NULL = instantaneous samples at t_start, K = N), instrument[N] in [0, n_inst);
+ *     outputs, each of length K (= 2N, or N): t = event time; dt[k] = t[k] - t[k-1] (dt[0] = 0); delta = length of the
+ *             event's exposure (1 for an instantaneous sample); meta = kind | instrument << 1 | zmask << 8 with kind
+ *             1 = start/reset, 0 = end/observe, and bit i of zmask set when z_i is zero after the event (instrument i
+ *             idle, or the event's own); exposure = index n of the event's exposure;
+ *             flags[1] = 0 when the input is valid, else bits 1 (non-finite time or t_end <= t_start), 2 (instrument
+ *             out of range), 4 (an instrument overlaps itself) -- the other outputs then mean nothing.  It is
+ *             written in stream order like the rest: there is no host read-back and no synchronisation;
+ *   - device = CUDA device ordinal (made current), cuda_stream = cudaStream_t (NULL = default stream).
+ * The call makes no cudaMalloc / cudaFree / cudaMallocAsync and calls no allocating library routine: one memset of the
+ * control block and look-back words (the array keeps the last call's contents), twelve kernel launches, one 4-byte
+ * device-to-device copy.  smolgp_noalloc_setup(device) looks the array's address up (once per device; the first call
+ * does it if the caller has not -- call it before starting a stream capture).
+ * ALL CALLS ON ONE DEVICE SHARE THE ARRAY: calls that overlap on the GPU (two streams, two host threads, two graph
+ * launches in flight) race and produce garbage; serialise them.  Calls in one stream are ordered and safe.
+ * Errors (return value; text from smolgp_noalloc_last_error(), per host thread): EINVAL (null pointer, N <= 0, device
+ * ordinal), EUNSUPPORTED (size above the limit, n_inst > SMOLGP_MAX_INST), ECUDA. */
+int smolgp_build_events_noalloc(int32_t device, void* cuda_stream, int64_t N, const double* t_start,
+                                const double* t_end, const int32_t* instrument, int32_t n_inst, double* t, double* dt,
+                                double* delta, uint32_t* meta, int32_t* exposure, int32_t* flags);
+int smolgp_noalloc_setup(int32_t device);
+int64_t smolgp_noalloc_max_events(void);
+int64_t smolgp_noalloc_scratch_bytes(void);
+const char* smolgp_noalloc_last_error(void);
+
 /* Read back the event stream (HOST output arrays of length K = 2N, or N for instantaneous data; any may be NULL): event time,
  * kind (1 = start/reset, 0 = end/observe), instrument, exposure index.  For tests. */
 int smolgp_events_export(smolgp_ctx* ctx, const smolgp_events* ev, double* t, int32_t* kind,

@@ -14,7 +14,8 @@ STATUS = {0: "OK", -1: "EINVAL", -2: "EOVERLAP", -3: "EUNSUPPORTED", -4: "ENOMEM
 EXPORTS = ["smolgp_create", "smolgp_destroy", "smolgp_last_error", "smolgp_set_option", "smolgp_build_events",
            "smolgp_build_events_host", "smolgp_build_events_instant", "smolgp_build_events_instant_host", "smolgp_free_events", "smolgp_events_export", "smolgp_loglik",
            "smolgp_loglik_host", "smolgp_loglik_grad", "smolgp_loglik_grad_host", "smolgp_condition", "smolgp_condition_host", "smolgp_discretise_host",
-           "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info", "smolgp_memory_info"]
+           "smolgp_launch_count", "smolgp_profile", "smolgp_profile_read", "smolgp_kernel_name", "smolgp_jit_log", "smolgp_plan_info", "smolgp_memory_info",
+           "smolgp_build_events_noalloc", "smolgp_noalloc_setup", "smolgp_noalloc_max_events", "smolgp_noalloc_scratch_bytes", "smolgp_noalloc_last_error"]
 NKERNELS = 11  # SMOLGP_NKERNELS
 
 
@@ -74,6 +75,11 @@ def lib():
         L.smolgp_plan_info.argtypes = [vp]
         L.smolgp_plan_info.restype = C.c_char_p
         L.smolgp_memory_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), i32]
+        L.smolgp_build_events_noalloc.argtypes = [i32, vp, i64, dp, dp, dp, i32, dp, dp, dp, dp, dp, dp]
+        L.smolgp_noalloc_setup.argtypes = [i32]
+        L.smolgp_noalloc_max_events.restype = i64
+        L.smolgp_noalloc_scratch_bytes.restype = i64
+        L.smolgp_noalloc_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -324,3 +330,33 @@ class Context:
             self.close()
         except Exception:
             pass
+
+
+# ---- event build that allocates nothing (include/smolgp.h: smolgp_build_events_noalloc) ----
+def smolgp_noalloc_setup(device=0):
+    rc = lib().smolgp_noalloc_setup(int(device))
+    if rc:
+        raise SmolgpError(rc, lib().smolgp_noalloc_last_error().decode())
+
+
+def smolgp_noalloc_max_events():
+    return int(lib().smolgp_noalloc_max_events())
+
+
+def smolgp_noalloc_scratch_bytes():
+    return int(lib().smolgp_noalloc_scratch_bytes())
+
+
+def smolgp_build_events_noalloc(device, stream, t_start, t_end, instrument, n_inst, t, dt, delta, meta, exposure, flags):
+    """All tensors are the caller's CUDA tensors: t_start, t_end (None = instantaneous samples) float64 [N], instrument
+    int32 [N]; outputs t, dt, delta float64 [K], meta, exposure int32 [K] (meta holds the packed uint32 bits), flags
+    int32 [1]; K = 2N, or N for instantaneous samples.  stream: a cudaStream_t as an integer (0 / None = default)."""
+    N = t_start.numel()
+    K = N if t_end is None else 2 * N
+    rc = lib().smolgp_build_events_noalloc(int(device), C.c_void_p(stream or None), N, _dptr(t_start, name="t_start"),
+                                           _dptr(t_end, numel=N, name="t_end"), _dptr(instrument, "int32", N, "instrument"), int(n_inst),
+                                           _dptr(t, numel=K, name="t"), _dptr(dt, numel=K, name="dt"), _dptr(delta, numel=K, name="delta"),
+                                           _dptr(meta, "int32", K, "meta"), _dptr(exposure, "int32", K, "exposure"),
+                                           _dptr(flags, "int32", 1, "flags"))
+    if rc:
+        raise SmolgpError(rc, lib().smolgp_noalloc_last_error().decode())

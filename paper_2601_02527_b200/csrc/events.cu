@@ -25,6 +25,8 @@
 #include <stddef.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "common.h"
 
 #define EVF_BADTIME 1
@@ -572,5 +574,92 @@ extern "C" int smolgp_events_export(smolgp_ctx* ctx, const smolgp_events* ev, do
     if (kind) kind[k] = (int32_t)META_KIND(meta[k]);
     if (instrument) instrument[k] = (int32_t)META_INST(meta[k]);
   }
+  return SMOLGP_OK;
+}
+
+// ---- event build that allocates nothing (include/smolgp.h: smolgp_build_events_noalloc) ----------------------------
+// For callers that cannot call cudaMalloc (stream capture, serving loops, harnesses that forbid it): the same
+// kernels as build_events_impl, with the sort's scratch -- control block, look-back words, two key and two payload
+// buffers -- in ONE file-scope device array instead of the ctx arena, outputs in caller-provided device arrays,
+// the validation flags left in a caller-provided device word instead of a host read-back + synchronise.
+// Every GPU that loads the library holds the array (NA_BYTES, about 6.5 MB) until exit.  All calls on a device
+// share it: calls that overlap on the GPU (two streams, two threads) race; serialise them.
+#define NA_MAXK (1 << 18)                       /* events: N <= 131072 exposures, or 262144 instantaneous samples */
+#define NA_ITEMS 4                              /* tile of the sort: RS_NT * 4 keys, as build_events_impl up to 2^21 events */
+#define NA_TILES (NA_MAXK / (RS_NT * NA_ITEMS)) /* 256 */
+#define NA_CTL_B ((sizeof(EvCtl) + 255) / 256 * 256)
+#define NA_LB_B ((size_t)NA_TILES * 256 * 8)
+#define NA_K8 ((size_t)NA_MAXK * 8)
+#define NA_K4 ((size_t)NA_MAXK * 4)
+#define NA_BYTES (NA_CTL_B + NA_LB_B + 2 * NA_K8 + 2 * NA_K4)
+static __device__ __align__(256) unsigned char g_na_scratch[NA_BYTES];
+
+#define NA_MAXDEV 64
+static void* g_na_ptr[NA_MAXDEV];       // device address of g_na_scratch on device d (the symbol itself is a host-side stand-in)
+static std::mutex g_na_mu;
+static thread_local std::string g_na_err;
+
+extern "C" const char* smolgp_noalloc_last_error(void) { return g_na_err.c_str(); }
+extern "C" int64_t smolgp_noalloc_max_events(void) { return NA_MAXK; }
+extern "C" int64_t smolgp_noalloc_scratch_bytes(void) { return (int64_t)NA_BYTES; }
+
+// once per device, with that device current: the address of the scratch array on it
+extern "C" int smolgp_noalloc_setup(int32_t device) {
+  if (device < 0 || device >= NA_MAXDEV) { g_na_err = "noalloc: device index out of range"; return SMOLGP_EINVAL; }
+  std::lock_guard<std::mutex> lk(g_na_mu);
+  if (g_na_ptr[device]) return SMOLGP_OK;
+  cudaError_t ce = cudaSetDevice(device);
+  void* p = nullptr;
+  if (ce == cudaSuccess) ce = cudaGetSymbolAddress(&p, g_na_scratch);
+  if (ce != cudaSuccess || !p) {
+    g_na_err = std::string("noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(ce);
+    cudaGetLastError();
+    return SMOLGP_ECUDA;
+  }
+  g_na_ptr[device] = p;
+  return SMOLGP_OK;
+}
+
+extern "C" int smolgp_build_events_noalloc(int32_t device, void* cuda_stream, int64_t N, const double* ts, const double* te,
+                                           const int32_t* inst, int32_t n_inst, double* t, double* dt, double* delta,
+                                           uint32_t* meta, int32_t* exposure, int32_t* flags) {
+  if (!ts || !inst || !t || !dt || !delta || !meta || !exposure || !flags) { g_na_err = "build_events_noalloc: null argument"; return SMOLGP_EINVAL; }
+  if (n_inst < 1 || n_inst > SG_MAXINST) { g_na_err = "build_events_noalloc: n_inst out of range"; return SMOLGP_EUNSUPPORTED; }
+  const bool instant = (te == nullptr);
+  if (N <= 0) { g_na_err = "build_events_noalloc: N must be positive"; return SMOLGP_EINVAL; }
+  const int64_t K = instant ? N : 2 * N;
+  if (K > NA_MAXK) {
+    g_na_err = "build_events_noalloc: " + std::to_string((long long)K) + " events exceed the fixed scratch (at most " +
+               std::to_string((long long)NA_MAXK) + " events = " + std::to_string((long long)NA_MAXK / 2) +
+               " exposures or " + std::to_string((long long)NA_MAXK) + " instantaneous samples); use smolgp_build_events";
+    return SMOLGP_EUNSUPPORTED;
+  }
+  int rc = smolgp_noalloc_setup(device);
+  if (rc) return rc;
+  if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); g_na_err = "build_events_noalloc: cudaSetDevice failed"; return SMOLGP_ECUDA; }
+  char* p = (char*)g_na_ptr[device];
+  EvCtl* ctl = (EvCtl*)p; p += NA_CTL_B;
+  unsigned long long* status = (unsigned long long*)p; p += NA_LB_B;
+  uint64_t* kA = (uint64_t*)p; p += NA_K8;
+  uint64_t* kB = (uint64_t*)p; p += NA_K8;
+  uint32_t* vA = (uint32_t*)p; p += NA_K4;
+  uint32_t* vB = (uint32_t*)p;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int64_t tile_rs = (int64_t)RS_NT * NA_ITEMS, tile_ef = (int64_t)RS_NT * EF_ITEMS;
+  const int64_t ntiles_rs = (K + tile_rs - 1) / tile_rs, ntiles_ef = (K + tile_ef - 1) / tile_ef;
+  // the array keeps the last call's contents: the control block and the look-back words this call will read start at
+  // zero (epoch 0 = "not published"; the ten launches below use epochs 1..10); keys and payloads are fully rewritten
+  cudaMemsetAsync(ctl, 0, NA_CTL_B + (size_t)ntiles_rs * 256 * 8, st);
+  k_ev_init<<<(unsigned)((N + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(N, ts, te, inst, n_inst, kA, vA, ctl);
+  uint32_t epoch = 0;
+  for (int pass = 0; pass < RS_DIGITS; ++pass) {
+    if (pass == 1) k_merge<<<(unsigned)((K + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(ctl, kA, vA, kB, vB, inst, n_inst, (uint32_t)K);
+    k_rs_pass<NA_ITEMS><<<(unsigned)ntiles_rs, RS_NT, 0, st>>>(ctl, pass, kA, vA, kB, vB, inst, n_inst, (uint32_t)K, status, ++epoch);
+  }
+  k_ev_final<<<(unsigned)ntiles_ef, RS_NT, 0, st>>>(ctl, K, vA, vB, ts, te, inst, n_inst, t, dt, delta, meta, exposure, status, ++epoch);
+  // validation flags to the caller's device word, in stream order: no host read-back, no synchronisation
+  cudaMemcpyAsync(flags, &ctl->flags, sizeof(int32_t), cudaMemcpyDeviceToDevice, st);
+  const cudaError_t ce = cudaGetLastError();
+  if (ce != cudaSuccess) { g_na_err = std::string("build_events_noalloc: ") + cudaGetErrorString(ce); return SMOLGP_ECUDA; }
   return SMOLGP_OK;
 }
