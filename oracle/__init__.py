@@ -162,6 +162,25 @@ def ssm(kern, ninst, ts, te, inst, y, sigma, flags=FLAG_TWO_FILTER, zprior=1.0, 
     return dict(loglik=ll.value, mean=mean, var=var, mq=mq, vq=vq, disc_seconds=float(g()))
 
 
+def ssm_sqrt(kern, ninst, ts, te, inst, y, sigma, zprior=1.0, want_post=True, prec="f80"):
+    """The sequential passes in square-root (Cholesky-factor) array form (oracle_ssm_sqrt): same
+    posterior as ssm(flags=IDLE_ZERO | TWO_FILTER).  Returns dict(loglik, mean, var)."""
+    ts, te, y, sigma = _d(ts), _d(te), _d(y), _d(sigma)
+    inst = np.ascontiguousarray(inst, dtype=np.int32)
+    N = ts.size
+    ll = C.c_double()
+    mean = np.empty(N) if want_post else None
+    var = np.empty(N) if want_post else None
+    f = _lib(prec).oracle_ssm_sqrt
+    f.argtypes = [C.c_int, C.c_void_p, C.c_int, C.c_int] + [C.c_void_p] * 5 + [C.c_double] + [C.c_void_p] * 3
+    ptr = lambda a: None if a is None else a.ctypes.data
+    rc = f(len(kern), C.cast(_comps(kern), C.c_void_p), ninst, N, ptr(ts), ptr(te), ptr(inst), ptr(y), ptr(sigma),
+           float(zprior), C.addressof(ll), ptr(mean), ptr(var))
+    if rc != 0:
+        raise RuntimeError("oracle_ssm_sqrt rc=%d" % rc)
+    return dict(loglik=ll.value, mean=mean, var=var)
+
+
 def _instant(fn, kern, ninst, t, inst, y, sigma, tq, query_inst, want_post, prec):
     t, y, sigma = _d(t), _d(y), _d(sigma)
     inst = np.ascontiguousarray(inst, dtype=np.int32)

@@ -19,6 +19,9 @@
  *      A second backward pass (two-filter / backward information form) is provided
  *      because the textbook RTS gain inverts a nearly singular P^-_{k+1} right after a
  *      reset; it is the parity reference for stiff cases (R7).
+ *  (3) oracle_ssm_sqrt (Part 7): the same passes in square-root (Cholesky-factor) array form,
+ *      the paper's named remedy for the conditioning of (2); pinned to (1) and (2)
+ *      in tests/test_oracle_sqrt_pins.py.
  *
  * Compile twice: -DREAL_IS_LONG_DOUBLE (parity reference, x87 80-bit) and plain
  * double (the timed CPU baseline).  Pins: tests/test_oracle_*.py (-m "not gpu").
@@ -1218,4 +1221,306 @@ int oracle_ssm_instant(int ncomp, const ocomp *comp, int ninst, int N, const dou
   }
   free(ev); free(pr); free(fi); free(sm);
   return rc;
+}
+
+/* ==========================================================================================
+ * Part 7.  Square-root (Cholesky-factor) form of the sequential passes.
+ *
+ * The paper names it as the remedy for the conditioning of the covariance recursions ("numerical
+ * instabilities ... square-root"; Yaghoobi et al. 2025) and prints no algorithm:
+ * what it must compute is the SAME posterior as Part 5 (and as the dense definition of Part 2), so
+ * Parts 2 and 5 are its pins (tests/test_oracle_sqrt_pins.py).  Written here in the textbook ARRAY
+ * form (Kailath, Sayed & Hassibi, "Linear Estimation", ch. 12): every covariance P is carried as a
+ * factor S with P = S S^T, every information matrix J as Z with J = Z Z^T, and every step is
+ * "stack the factors side by side, re-triangularise":  tria(M) = the lower-triangular L with
+ * L L^T = M M^T.  No covariance is ever formed, nothing is subtracted, nothing ill-conditioned is
+ * inverted.
+ *   predict (Eq. 3.14)     S^- = tria([A S | G]),  G G^T = Q~  (G from the blocks' own
+ *                                Cholesky factors -- Q~ itself is singular)
+ *   reset (Eq. 3.15 / 3.18)      zero row z_i of S and m_zi
+ *   update (Eq. 2.22)      tria([[sqrt r, h^T S^-], [0, S^-]]) = [[sqrt s, 0], [K sqrt s, S^+]]
+ *   backward, two-filter form of Part 5 (reading R7) with J = Z Z^T:
+ *     smoothed   P^ = S (I + S^T J S)^-1 S^T,  m^ = m + S (I + S^T J S)^-1 S^T (eta - J m)
+ *     end event  Z <- tria([Z | h / sqrt r]),  eta += h y / r
+ *     step       (J^-1 + Q)^-1 = Z (I + Z^T Q Z)^-1 Z^T:  T = tria([I | Z^T G]),  Z <- A^T Z T^-T,
+ *                eta <- A^T (eta - Z (T T^T)^-1 Z^T Q eta)
+ * ========================================================================================== */
+#define MAXQ (MAXN + MAXBLK) /* columns of G: d + nblk */
+
+/* L (n x n, lower, row-major) with L L^T = M M^T, M n x m row-major (destroyed): Householder reflections
+ * applied from the right, one per row */
+static void tria(int n, int m, real *M, real *L) {
+  for (int j = 0; j < n; ++j) {
+    real *rj = M + (size_t)j * m;
+    real ss = 0;
+    for (int c = j; c < m; ++c) ss += rj[c] * rj[c];
+    real sig = R_SQRT(ss);
+    if (sig > 0 && j < m) {
+      /* reflector v = u - alpha e_j with alpha = -sign(u_j) |u|, used in the scale-free form v / |u| so that
+       * rows of any magnitude (the information factors span hundreds of orders) neither overflow nor vanish */
+      real alpha = rj[j] > 0 ? -sig : sig;
+      real v0 = (rj[j] - alpha) / sig;
+      real beta = 1 / (1 + R_FABS(rj[j]) / sig);
+      for (int c = j + 1; c < m; ++c) rj[c] /= sig;
+      for (int i = j + 1; i < n; ++i) {
+        real *ri = M + (size_t)i * m;
+        real dsum = ri[j] * v0;
+        for (int c = j + 1; c < m; ++c) dsum += ri[c] * rj[c];
+        real w = beta * dsum;
+        ri[j] -= w * v0;
+        for (int c = j + 1; c < m; ++c) ri[c] -= w * rj[c];
+      }
+      rj[j] = alpha;
+      for (int c = j + 1; c < m; ++c) rj[c] = 0;
+    }
+  }
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) L[i * n + j] = (j <= i && j < m) ? M[(size_t)i * m + j] : 0;
+}
+
+/* lower Cholesky factor of a positive SEMI-definite m x m matrix (row-major): a pivot that rounding
+ * has driven to <= 0 (or below 2^-44 of its diagonal entry) gives a zero column */
+static void chol_psd(int m, const real *A, real *L) {
+  memset(L, 0, sizeof(real) * m * m);
+  for (int j = 0; j < m; ++j) {
+    real p = A[j * m + j];
+    for (int k = 0; k < j; ++k) p -= L[j * m + k] * L[j * m + k];
+    if (!(p > A[j * m + j] * (real)5.7e-14)) continue;
+    real r = R_SQRT(p);
+    L[j * m + j] = r;
+    for (int i = j + 1; i < m; ++i) {
+      real a = A[i * m + j];
+      for (int k = 0; k < j; ++k) a -= L[i * m + k] * L[j * m + k];
+      L[i * m + j] = a / r;
+    }
+  }
+}
+
+/* A~ (n x n) as disc_model, and G (n x nq, nq = d + nblk) with G G^T = Q~ of Eq. 3.17: block b's
+ * augmented Q_b = [Qxx q12; q12^T q22] is factored on its own, L_b L_b^T = Q_b, and placed like Q_b itself:
+ * x rows of the block in its own columns, the integral row into z_i for every instrument i that integrates it */
+static void disc_model_factor(const model *M, real dt, real *A, real *G, int *nq_out) {
+  int n = M->n, d = M->d, nq = d + M->nblk;
+  memset(A, 0, sizeof(real) * n * n);
+  memset(G, 0, sizeof(real) * n * nq);
+  for (int q = 0; q < M->ninst; ++q) A[(d + q) * n + d + q] = 1;
+  for (int b = 0; b < M->nblk; ++b) {
+    const block *B = &M->blk[b];
+    int db = B->d, m = db + 1, o = M->off[b], c0 = o + b; /* first column of block b in G */
+    real Ph[MB * MB], Qb[MB * MB], Lb[MB * MB];
+    disc_block(B, dt, Ph, Qb);
+    chol_psd(m, Qb, Lb);
+    for (int i = 0; i < db; ++i) {
+      for (int j = 0; j < db; ++j) A[(o + i) * n + o + j] = Ph[i * m + j];
+      for (int j = 0; j < m; ++j) G[(o + i) * nq + c0 + j] = Lb[i * m + j];
+    }
+    for (int q = 0; q < M->ninst; ++q) {
+      if (!((B->mask >> q) & 1u)) continue;
+      for (int j = 0; j < db; ++j) A[(d + q) * n + o + j] = Ph[db * m + j];
+      for (int j = 0; j < m; ++j) G[(d + q) * nq + c0 + j] = Lb[db * m + j];
+    }
+  }
+  *nq_out = nq;
+}
+
+/* solve L x = b in place (L lower n x n, zero pivots give x_i = 0: the direction carries nothing) */
+static void lsolve(int n, const real *L, real *b) {
+  for (int i = 0; i < n; ++i) {
+    real a = b[i];
+    for (int k = 0; k < i; ++k) a -= L[i * n + k] * b[k];
+    b[i] = (L[i * n + i] != 0) ? a / L[i * n + i] : 0;
+  }
+}
+static void ltsolve(int n, const real *L, real *b) { /* L^T x = b */
+  for (int i = n - 1; i >= 0; --i) {
+    real a = b[i];
+    for (int k = i + 1; k < n; ++k) a -= L[k * n + i] * b[k];
+    b[i] = (L[i * n + i] != 0) ? a / L[i * n + i] : 0;
+  }
+}
+
+/* Same contract as oracle_ssm with flags = IDLE_ZERO | TWO_FILTER (readings R6, R7), no query times.
+ * Returns 0; -1 bad input; -2 same-instrument overlap; -4 out of memory. */
+int oracle_ssm_sqrt(int ncomp, const ocomp *comp, int ninst, int N, const double *ts, const double *te,
+                    const int32_t *inst, const double *y, const double *sigma, double zprior,
+                    double *loglik, double *mean, double *var) {
+  model Md;
+  if (build_model(&Md, ncomp, comp, ninst)) return -1;
+  const int n = Md.n, d = Md.d, nn = n * n, K = 2 * N;
+  const int want_smooth = (mean || var);
+  event *ev = malloc(sizeof(event) * (size_t)K);
+  unsigned char *opst = malloc((size_t)K * ninst);
+  if (!ev || !opst) { free(ev); free(opst); return -4; }
+  for (int i = 0; i < N; ++i) {
+    if (!(te[i] > ts[i]) || inst[i] < 0 || inst[i] >= ninst || !(sigma[i] > 0)) { free(ev); free(opst); return -1; }
+    ev[2 * i] = (event){ts[i], 1, inst[i], i};
+    ev[2 * i + 1] = (event){te[i], 0, inst[i], i};
+  }
+  qsort(ev, (size_t)K, sizeof(event), ev_cmp);
+  {
+    int open[MAXINST] = {0};
+    for (int k = 0; k < K; ++k) {
+      int i = ev[k].inst;
+      if (ev[k].kind == open[i]) { free(ev); free(opst); return -2; }
+      open[i] = ev[k].kind;
+      for (int q = 0; q < ninst; ++q) opst[(size_t)k * ninst + q] = (unsigned char)open[q];
+    }
+  }
+  /* stored per END event (exposure index): the filtered factor and mean the smoother refines */
+  size_t per = (size_t)n + nn;
+  real *sx = want_smooth ? malloc(sizeof(real) * per * (size_t)N) : NULL;
+  if (want_smooth && !sx) { free(ev); free(opst); return -4; }
+  real m[MAXN] = {0}, S[MAXN * MAXN] = {0}, A[MAXN * MAXN], G[MAXN * MAXQ];
+  static __thread real W[(MAXN + 1) * (2 * MAXN + MAXQ + 1)];
+  for (int b = 0; b < Md.nblk; ++b) { /* S0 = blkdiag(chol Pinf_b, sqrt(zprior) I) */
+    int db = Md.blk[b].d, o = Md.off[b];
+    real Lb[MAXBD * MAXBD];
+    chol_psd(db, Md.blk[b].P, Lb);
+    for (int i = 0; i < db; ++i)
+      for (int j = 0; j < db; ++j) S[(o + i) * n + o + j] = Lb[i * db + j];
+  }
+  for (int q = 0; q < ninst; ++q) S[(d + q) * n + d + q] = R_SQRT((real)zprior);
+  real ll = 0;
+  int nq = 0;
+  for (int k = 0; k < K; ++k) {
+    real dt = k == 0 ? 0 : (real)ev[k].t - (real)ev[k - 1].t;
+    disc_model_factor(&Md, dt, A, G, &nq);
+    { /* predict: m <- A m, S <- tria([A S | G]) */
+      real t1[MAXN];
+      mv(n, A, m, t1);
+      memcpy(m, t1, sizeof(real) * n);
+      int mc = n + nq;
+      for (int i = 0; i < n; ++i) {
+        for (int j = 0; j < n; ++j) {
+          real a = 0;
+          for (int l = 0; l < n; ++l) a += A[i * n + l] * S[l * n + j];
+          W[i * mc + j] = a;
+        }
+        for (int j = 0; j < nq; ++j) W[i * mc + n + j] = G[i * nq + j];
+      }
+      tria(n, mc, W, S);
+    }
+    int zi = d + ev[k].inst;
+    if (ev[k].kind == 1) { /* start: reset, Eq. 3.15 */
+      m[zi] = 0;
+      for (int j = 0; j < n; ++j) S[zi * n + j] = 0;
+    } else { /* end: array update with h = e_z / delta */
+      int e = ev[k].idx;
+      real delta = (real)te[e] - (real)ts[e], sg = (real)sigma[e];
+      int mc = n + 1;
+      real Lw[(MAXN + 1) * (MAXN + 1)];
+      memset(W, 0, sizeof(real) * (size_t)(n + 1) * mc);
+      W[0] = sg;
+      for (int j = 0; j < n; ++j) W[1 + j] = S[zi * n + j] / delta; /* h^T S */
+      for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j) W[(size_t)(i + 1) * mc + 1 + j] = S[i * n + j];
+      /* tria of the (n+1) x (n+1) pre-array, written into an (n+1)-square L */
+      {
+        real Mw[(MAXN + 1) * (MAXN + 1)];
+        memcpy(Mw, W, sizeof(real) * (size_t)(n + 1) * mc);
+        int n1 = n + 1;
+        /* tria() is written for leading dimension = column count: here both are n + 1 */
+        tria(n1, n1, Mw, Lw);
+      }
+      int n1 = n + 1;
+      real rs = Lw[0]; /* +- sqrt(s) */
+      real s = rs * rs;
+      real v = (real)y[e] - m[zi] / delta;
+      for (int i = 0; i < n; ++i) m[i] += Lw[(i + 1) * n1] / rs * v; /* K = Kbar / sqrt(s) */
+      for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j) S[i * n + j] = Lw[(i + 1) * n1 + 1 + j];
+      ll += -(R_LOG(2 * (real)PI_R * s) + v * v / s) / 2;
+      if (sx) { memcpy(sx + per * (size_t)e, m, sizeof(real) * n); memcpy(sx + per * (size_t)e + n, S, sizeof(real) * nn); }
+    }
+    for (int q = 0; q < ninst; ++q)
+      if (!opst[(size_t)k * ninst + q]) { m[d + q] = 0; for (int j = 0; j < n; ++j) S[(d + q) * n + j] = 0; }
+  }
+  if (loglik) *loglik = (double)ll;
+  if (want_smooth) {
+    real Z[MAXN * MAXN] = {0}, eta[MAXN] = {0};
+    for (int k = K - 1; k >= 0; --k) {
+      int zi = d + ev[k].inst;
+      if (ev[k].kind == 1) { eta[zi] = 0; for (int j = 0; j < n; ++j) Z[zi * n + j] = 0; }
+      for (int q = 0; q < ninst; ++q)
+        if (!opst[(size_t)k * ninst + q]) { eta[d + q] = 0; for (int j = 0; j < n; ++j) Z[(d + q) * n + j] = 0; }
+      if (ev[k].kind == 0) {
+        int e = ev[k].idx;
+        const real *mf = sx + per * (size_t)e, *Sf = mf + n;
+        real delta = (real)te[e] - (real)ts[e], r = (real)sigma[e] * (real)sigma[e];
+        /* U U^T = I + V V^T, V = S^T Z */
+        real U[MAXN * MAXN];
+        int mc = 2 * n;
+        for (int i = 0; i < n; ++i)
+          for (int j = 0; j < n; ++j) {
+            real a = 0;
+            for (int l = 0; l < n; ++l) a += Sf[l * n + i] * Z[l * n + j];
+            W[i * mc + j] = (i == j) ? 1 : 0;
+            W[i * mc + n + j] = a;
+          }
+        tria(n, mc, W, U);
+        real w[MAXN], gvec[MAXN], zt[MAXN], u[MAXN];
+        for (int j = 0; j < n; ++j) w[j] = Sf[zi * n + j]; /* S^T e_z */
+        lsolve(n, U, w);
+        mtv(n, Z, mf, zt); /* Z^T m */
+        mv(n, Z, zt, gvec);
+        for (int i = 0; i < n; ++i) gvec[i] = eta[i] - gvec[i]; /* eta - J m */
+        mtv(n, Sf, gvec, u);
+        lsolve(n, U, u);
+        real vv = 0, mu = mf[zi];
+        for (int j = 0; j < n; ++j) { vv += w[j] * w[j]; mu += w[j] * u[j]; }
+        if (mean) mean[e] = (double)(mu / delta);
+        if (var) var[e] = (double)(vv / (delta * delta));
+        /* the exposure's own information: Z <- tria([Z | h / sqrt r]), eta += h y / r */
+        mc = n + 1;
+        for (int i = 0; i < n; ++i) {
+          for (int j = 0; j < n; ++j) W[i * mc + j] = Z[i * n + j];
+          W[i * mc + n] = (i == zi) ? 1 / (delta * R_SQRT(r)) : 0;
+        }
+        tria(n, mc, W, Z);
+        eta[zi] += (real)y[e] / (delta * r);
+      }
+      real dt = k == 0 ? 0 : (real)ev[k].t - (real)ev[k - 1].t;
+      disc_model_factor(&Md, dt, A, G, &nq);
+      { /* T T^T = I + Y Y^T, Y = Z^T G;  Z <- A^T Z T^-T;  eta <- A^T (eta - Z (T T^T)^-1 Y G^T eta) */
+        real T[MAXN * MAXN], Y[MAXN * MAXQ], ge[MAXQ], ye[MAXN], Zp[MAXN * MAXN];
+        int mc = n + nq;
+        for (int i = 0; i < n; ++i) {
+          for (int j = 0; j < nq; ++j) {
+            real a = 0;
+            for (int l = 0; l < n; ++l) a += Z[l * n + i] * G[l * nq + j];
+            Y[i * nq + j] = a;
+          }
+          for (int j = 0; j < n; ++j) W[i * mc + j] = (i == j) ? 1 : 0;
+          for (int j = 0; j < nq; ++j) W[i * mc + n + j] = Y[i * nq + j];
+        }
+        tria(n, mc, W, T);
+        for (int j = 0; j < nq; ++j) {
+          real a = 0;
+          for (int l = 0; l < n; ++l) a += G[l * nq + j] * eta[l];
+          ge[j] = a;
+        }
+        for (int i = 0; i < n; ++i) {
+          real a = 0;
+          for (int j = 0; j < nq; ++j) a += Y[i * nq + j] * ge[j];
+          ye[i] = a;
+        }
+        lsolve(n, T, ye);
+        ltsolve(n, T, ye);
+        real e2[MAXN];
+        mv(n, Z, ye, e2);
+        for (int i = 0; i < n; ++i) e2[i] = eta[i] - e2[i];
+        /* rows of Z T^-T: for each row z of Z solve T x = z^T */
+        for (int i = 0; i < n; ++i) {
+          real x[MAXN];
+          for (int j = 0; j < n; ++j) x[j] = Z[i * n + j];
+          lsolve(n, T, x);
+          for (int j = 0; j < n; ++j) Zp[i * n + j] = x[j];
+        }
+        mtm(n, A, Zp, Z);
+        mtv(n, A, e2, eta);
+      }
+    }
+  }
+  free(ev); free(opst); free(sx);
+  return 0;
 }
