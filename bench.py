@@ -246,6 +246,8 @@ def run_cuda(args, w, cfgname):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     ctx = B.Context(local)  # NULL stream = the legacy default stream = torch's current stream here
+    if args.form == "sqrt":
+        ctx.set_option("form", 1)  # square-root form of the chunk recursions: one chunk per series
     N = w["t_start"].size
     batch = w["batch"] or 1
     n = model_dim(w)
@@ -357,7 +359,7 @@ def run_cuda(args, w, cfgname):
     hbm_gbs, hbm_src = hbm_peak_gbs()
     t_step = ms / args.steps * 1e-3
     t_roof = max(K_events * w_useful_flops(n) / (peak * 1e12), K_events * min_bytes(n) / (hbm_gbs * 1e9))
-    traffic, dfma_frac, cap_src = ncu_capture(top, args.config)
+    traffic, dfma_frac, cap_src = ncu_capture(top, args.config) if args.form == "cov" else (None, None, "the capture is of the covariance form")
     roofline = {"bound": "alu", "kernel": top, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": traffic,
                 "frac_whole_step": t_roof / t_step, "frac_executed_dfma": dfma_frac, "capture": cap_src,
@@ -398,7 +400,7 @@ def run_cuda(args, w, cfgname):
             "config": {"workload": cfgname, "N": N, "events": ev_per_exp * N, "batch": batch, "state_dim": n,
                        "path": "a1 build_events + a2 discretise + a3 filter scan + a4 smoother + a5 loglik + a6 posterior",
                        "l2": "flushed (512 MiB write) between timed iterations", "parallelism": "replicas x%d" % world,
-                       "plan": plan},
+                       "plan": plan, "form": args.form},
             "e2e": {"value": e2e_value, "unit": "events/s",
                     "h2d_bytes_per_step": int(hts.nbytes + hte.nbytes + hins.nbytes + hy.nbytes + hsg.nbytes + (0 if hamp is None else hamp.nbytes)),
                     "d2h_bytes_per_step": int(hout["mean"].nbytes + hout["var"].nbytes + hout["loglik"].nbytes),
@@ -543,6 +545,9 @@ def main():
     ap.add_argument("--config", default="3", help="BASELINE.json config (1-5; 3 = the headline N=1e5) or `instant` (section-2 instantaneous data, SURVEY 8(f) item 3)")
     ap.add_argument("--workload", default="condition", choices=["condition", "predict"],
                     help="condition = the headline (rows a1-a6); predict = condition + prediction at --predict-mult x N query times (row a7)")
+    ap.add_argument("--form", default="cov", choices=["cov", "sqrt"],
+                    help="cov = covariance form (default, the headline); sqrt = square-root (Cholesky-factor) form of the chunk recursions, one chunk per series "
+                         "(SURVEY 8(f) item 1; meant for the batched config 5)")
     ap.add_argument("--predict-mult", type=float, default=100.0, help="queries per exposure of the predict workload (the paper uses M = 100 N, P:561)")
     args = ap.parse_args()
     args.config = args.config if args.config == "instant" else int(args.config)

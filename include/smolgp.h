@@ -89,7 +89,13 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * one (default for n <= 24); "cpl": columns of the state per lane of the register-resident k_down0 (0 = automatic, 1-3);
  * "rminb" / "fminb": minimum resident CTAs per SM asked of the two register-resident kernels (caps their registers;
  * 0 = 8); "dot2": which products of the dense levels are compensated (bit 0: those forming a solve's matrix,
- * bit 1: the others; -1 = default 1) -- sweep knobs, see profiles/r02_sweeps.md.
+ * bit 1: the others; -1 = default 1) -- sweep knobs, see profiles/r02_sweeps.md;
+ * "form": 0 = covariance form (default); 1 = SQUARE-ROOT (Cholesky-factor) form of the filter and smoother recursions, the
+ * paper's remedy for their conditioning: covariances and adjoint matrices are carried as factors and
+ * re-triangularised, nothing is subtracted or compensated (csrc/chunk_sqrt.cuh).  Same inputs, outputs and
+ * tolerances; each series is then ONE sequential pass by one group of lanes (no chunked scan: made for batches of
+ * series, row a8; a single long series takes seconds), "chunk" / "jit" / "reg" are ignored, and query times
+ * (M > 0) return SMOLGP_EUNSUPPORTED.
  * A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);

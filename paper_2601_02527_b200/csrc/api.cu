@@ -31,7 +31,7 @@ extern "C" int smolgp_create(smolgp_ctx** out, int device, void* cuda_stream) {
   if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SMOLGP_ECUDA; }
   smolgp_ctx* c = new smolgp_ctx();
   c->device = device; c->stream = (cudaStream_t)cuda_stream; c->launches = 0; c->prof_on = 0; c->prof_cur = 0;
-  c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->opt_reg = 0; c->opt_rcpl = 0; c->opt_rminb = 0; c->opt_fminb = 0; c->opt_dot2 = -1; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
+  c->opt_chunk = 0; c->opt_group = 0; c->opt_top = 0; c->opt_jit = 0; c->opt_reg = 0; c->opt_rcpl = 0; c->opt_rminb = 0; c->opt_fminb = 0; c->opt_dot2 = -1; c->opt_form = 0; c->jit = nullptr; c->opt_lanes = 0; c->arena = nullptr; c->arena_bytes = 0; c->d_flags = nullptr; c->pers = nullptr; c->pers_bytes = 0; c->hmodel = nullptr;
   c->lb_status = nullptr; c->lb_words = 0; c->lb_epoch = 0; c->mem_extra = 0; c->mem_peak = 0;
   // pinned: the per-call model upload is a true asynchronous copy
   if (cudaMallocHost((void**)&c->hmodel, sizeof(ModelDev)) != cudaSuccess) { cudaGetLastError(); delete c; return SMOLGP_ENOMEM; }
@@ -121,6 +121,10 @@ extern "C" int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t valu
   else if (!strcmp(name, "rminb")) ctx->opt_rminb = value;
   else if (!strcmp(name, "dot2")) ctx->opt_dot2 = value;
   else if (!strcmp(name, "fminb")) ctx->opt_fminb = value;
+  else if (!strcmp(name, "form")) {
+    if (value != 0 && value != 1) { ctx->err = "option form: 0 (covariance) or 1 (square-root)"; return SMOLGP_EINVAL; }
+    ctx->opt_form = value;
+  }
   else { ctx->err = std::string("unknown option ") + name; return SMOLGP_EINVAL; }
   return SMOLGP_OK;
 }
@@ -140,6 +144,8 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   ModelDev& hm = *ctx->hmodel;
   int rc = sg_build_model(ctx, kernel, ev->n_inst, ev->tau, ev->instant, &hm);
   if (rc) return rc;
+  hm.sqrt_form = (ctx->opt_form == 1) ? 1 : 0;
+  if (hm.sqrt_form && qs.M > 0) { ctx->err = "condition: query times are not available in square-root form (option form = 1)"; return SMOLGP_EUNSUPPORTED; }
   const size_t model_b = (sizeof(ModelDev) + 255) / 256 * 256;
   const size_t disc_b = ((size_t)ev->K * hm.disc_stride * 8 + 255) / 256 * 256;
   if (ctx->pers_bytes < model_b + disc_b) {

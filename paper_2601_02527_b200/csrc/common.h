@@ -35,6 +35,7 @@ struct BlockConst {
 struct ModelDev {
   int n, d, n_inst, nblk;
   int instant;                     // 1: instantaneous-data mode: the "integral" rows of a record hold H Phi, Q H^T, H Q H^T (disc.cu)
+  int sqrt_form;                   // 1: square-root form: a record's (Qxx, q12, q22) slots hold the block's Cholesky factor (Lxx, Lzx, Lzz) (disc.cu, chunk_sqrt.cuh)
   int disc_stride;                 // doubles per event in the discretisation array
   int disc_off[SG_MAXBLK];         // offset of block b inside one event's record
   double cz[SG_MAXINST][SG_MAXBLK]; // c_qb: coupling of block b's integral into z_q (equilibrated units), 0 if masked out
@@ -83,6 +84,7 @@ struct smolgp_ctx {
   int64_t opt_chunk, opt_group, opt_lanes, opt_top, opt_jit; // opt_jit: 0 automatic, 1 always, -1 never
   int64_t opt_dot2; // -1 default (3)
   int64_t opt_rminb, opt_fminb; // tuning: min CTAs per SM of the register kernels
+  int64_t opt_form; // 0 covariance form, 1 square-root (Cholesky-factor) form of the chunk recursions (chunk_sqrt.cuh)
   int64_t opt_reg, opt_rcpl; // opt_reg: -1 = specialised kernels in their shared-memory form; opt_rcpl: columns per lane of the register k_down0 (0 auto)
   void* jit;       // run-time specialised kernels (jit.cu)
   // workspace arena (grown on demand, reused across calls)

@@ -67,7 +67,7 @@ __device__ __forceinline__ void phi_closed<4>(const BlockConst& B, double h, dou
 }
 
 template <int DB>
-__device__ void disc_block(const BlockConst& B, double dts, int instant, double* __restrict__ out) {
+__device__ void disc_block(const BlockConst& B, double dts, int instant, int sqrt_form, double* __restrict__ out) {
   constexpr int M = DB + 1;
   double h = dts;
   int s = 0;
@@ -169,7 +169,33 @@ __device__ void disc_block(const BlockConst& B, double dts, int instant, double*
 #pragma unroll
       for (int j = 0; j < DB; ++j) A[i][j] = P[i][j];
   }
-  // record: Phi | phibar | Qxx | q12 | q22
+  if (sqrt_form) {
+    // square-root form (chunk_sqrt.cuh): the record carries L with L L^T = Q~ instead of Q~.  Lower Cholesky factor
+    // of a positive SEMI-definite matrix: a pivot that rounding has driven to <= 2^-44 of its diagonal entry gives a
+    // zero column (Q~ = 0 at a zero step; for instantaneous data the extra state is a copy of x_0, so only the
+    // DB x DB part is factored and the extra row of the factor is row 0 of L_xx)
+    const int mm = instant ? DB : M;
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      if (j >= mm) break;
+      double p = Q[j][j];
+#pragma unroll
+      for (int k = 0; k < j; ++k) p = fma(-Q[j][k], Q[j][k], p);
+      const bool ok = p > Q[j][j] * 5.7e-14;
+      const double r = ok ? sqrt(p) : 0.0, rr = ok ? 1.0 / r : 0.0;
+#pragma unroll
+      for (int i = j + 1; i < M; ++i) {
+        double a = Q[i][j];
+#pragma unroll
+        for (int k = 0; k < j; ++k) a = fma(-Q[i][k], Q[j][k], a);
+        Q[i][j] = (i < mm) ? a * rr : Q[i][j];
+      }
+      Q[j][j] = r;
+#pragma unroll
+      for (int i = 0; i < j; ++i) Q[i][j] = 0.0;
+    }
+  }
+  // record: Phi | phibar | Qxx | q12 | q22   (square-root form: Phi | phibar | Lxx | Lzx | Lzz)
 #pragma unroll
   for (int i = 0; i < DB; ++i)
 #pragma unroll
@@ -180,8 +206,8 @@ __device__ void disc_block(const BlockConst& B, double dts, int instant, double*
     // chunk kernels then carry z_q = H_q x at each sample with their unchanged arithmetic (z_q is idle, i.e.
     // zero, before its sample, so the "+ z_q" of the integral row adds nothing).
 #pragma unroll
-    for (int j = 0; j < DB; ++j) { out[DB * DB + j] = A[0][j]; out[2 * DB * DB + DB + j] = Q[j][0]; }
-    out[2 * DB * DB + 2 * DB] = Q[0][0];
+    for (int j = 0; j < DB; ++j) { out[DB * DB + j] = A[0][j]; out[2 * DB * DB + DB + j] = sqrt_form ? Q[0][j] : Q[j][0]; }
+    out[2 * DB * DB + 2 * DB] = sqrt_form ? 0.0 : Q[0][0];
     return;
   }
 #pragma unroll
@@ -202,9 +228,9 @@ __global__ void __launch_bounds__(128) k_disc(const ModelDev* __restrict__ Mp, c
     const double dts = dt[k] * B.inv_T;
     double* out = stage + threadIdx.x * bs;
     switch (B.dim) {
-      case 2: disc_block<2>(B, dts, Mp->instant, out); break;
-      case 3: disc_block<3>(B, dts, Mp->instant, out); break;
-      default: disc_block<4>(B, dts, Mp->instant, out); break;
+      case 2: disc_block<2>(B, dts, Mp->instant, Mp->sqrt_form, out); break;
+      case 3: disc_block<3>(B, dts, Mp->instant, Mp->sqrt_form, out); break;
+      default: disc_block<4>(B, dts, Mp->instant, Mp->sqrt_form, out); break;
     }
   }
   __syncthreads();

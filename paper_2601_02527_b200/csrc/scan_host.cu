@@ -166,6 +166,23 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
     else { ctx->err = "scan: unsupported (lanes, n) combination"; return SMOLGP_EUNSUPPORTED; } \
   } while (0)
 
+// square-root form (chunk_sqrt.cuh): the generic kernel, one group per series
+template <int G, int LD>
+static int launch_sqrt(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm) {
+  const size_t per_group = (size_t)sqrt_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
+  const int gpc = groups_per_cta(per_group, G);
+  const size_t smem = per_group * gpc;
+  if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+  if (hm->n + hm->d + hm->nblk > sqrt_ldm(LD)) { ctx->err = "scan: model too wide for the square-root kernel"; return SMOLGP_EUNSUPPORTED; }
+  const int64_t groups = P.batch * P.c1;
+  SG_CUDA(ctx, cudaFuncSetAttribute(k_down0_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  sg_launch_begin(ctx, KID_DOWN0);
+  k_down0_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(P);
+  sg_launch_end(ctx);
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
+}
+
 static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G, const L0Plan& lp) {
   const SgJitKernels* jk = lp.jk;
   const int64_t groups = P.batch * P.c1;
@@ -228,7 +245,10 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   const int G = pick_lanes(ctx, n);
   Tab T0;
   tab_build(hm, &T0);
-  const L0Plan lp = plan_l0(ctx, T0, G, batch * K, true); // specialised kernels for this model's structure, or the generic ones
+  const bool sq = hm->sqrt_form != 0; // square-root form: generic kernel, one chunk per series (the dense levels have no factor form)
+  L0Plan lp;
+  if (sq) { lp.jk = nullptr; lp.cfg = make_cfg(ctx, T0, G); }
+  else lp = plan_l0(ctx, T0, G, batch * K, true); // specialised kernels for this model's structure, or the generic ones
   const SgJitKernels* jk0 = lp.jk;
   const bool reg = jk0 && jk0->cfg.reg;
   const int ld0 = l0_ld(lp, n);
@@ -237,7 +257,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
   // already fills it runs one chunk per series (the sequential filter, row a8)
-  int64_t Lc = ctx->opt_chunk;
+  int64_t Lc = sq ? K : ctx->opt_chunk;
   if (Lc <= 0) {
     // one full wave: as many chunks as groups can be resident at once (equal work per chunk, no tail);
     // a batch that already fills the machine runs one chunk per series (the sequential filter, row a8)
@@ -346,13 +366,17 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     sg_launch_end(ctx);
     SG_CUDA(ctx, e);
   }
-  rc = launch_level0_any(ctx, P, hm, false, G, lp);
+  if (sq) {
+#define SG_CALL_SQ(g_, ld_) rc = launch_sqrt<g_, ld_>(ctx, P, hm)
+    SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_SQ);
+#undef SG_CALL_SQ
+  } else rc = launch_level0_any(ctx, P, hm, false, G, lp);
   if (rc) return rc;
   {
     char buf[256];
-    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=%d fold_lanes=%d jit=%d kernels=%s regs=%d/%d prebuilt=%d", n,
+    snprintf(buf, sizeof buf, "n=%d batch=%lld K=%lld chunk=%lld chunks=%lld levels=%d fanin=%d lanes=%d cpl=%d fold_lanes=%d jit=%d kernels=%s regs=%d/%d prebuilt=%d form=%s", n,
              (long long)batch, (long long)K, (long long)Lc, (long long)c1, pl.T, g, Gd, reg ? jk0->cfg.rCPL : 1, reg ? jk0->cfg.fG : G,
-             jk0 ? 1 : 0, reg ? "reg" : "smem", jk0 ? jk0->regs_fold0 : 0, jk0 ? jk0->regs_down0 : 0, jk0 ? jk0->prebuilt : 0);
+             jk0 ? 1 : 0, reg ? "reg" : "smem", jk0 ? jk0->regs_fold0 : 0, jk0 ? jk0->regs_down0 : 0, jk0 ? jk0->prebuilt : 0, sq ? "sqrt" : "cov");
     ctx->plan = buf;
   }
   if (a.loglik) {
