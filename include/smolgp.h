@@ -90,12 +90,13 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * "rminb" / "fminb": minimum resident CTAs per SM asked of the two register-resident kernels (caps their registers;
  * 0 = 8); "dot2": which products of the dense levels are compensated (bit 0: those forming a solve's matrix,
  * bit 1: the others; -1 = default 1) -- sweep knobs, see profiles/r02_sweeps.md;
- * "form": 0 = covariance form (default); 1 = SQUARE-ROOT (Cholesky-factor) form of the filter and smoother recursions, the
- * paper's remedy for their conditioning: covariances and adjoint matrices are carried as factors and
- * re-triangularised, nothing is subtracted or compensated (csrc/chunk_sqrt.cuh).  Same inputs, outputs and
- * tolerances; each series is then ONE sequential pass by one group of lanes (no chunked scan: made for batches of
- * series, row a8; a single long series takes seconds), "chunk" / "jit" / "reg" are ignored, and query times
- * (M > 0) return SMOLGP_EUNSUPPORTED.
+ * "form": 0 = covariance form (default); 1 = SQUARE-ROOT (Cholesky-factor) form of the whole scan, the paper's remedy for
+ * the conditioning of the covariance recursions: covariances, informations and adjoint matrices are carried
+ * as factors (P = S S^T, J = Z Z^T) and re-triangularised, in the chunk recursions and in the dense combines alike; nothing
+ * is subtracted from a covariance, no I + C J is formed or inverted, no product is compensated (csrc/chunk_sqrt.cuh,
+ * csrc/dense_sqrt.cuh).  Same inputs, outputs, tolerances and scan plans ("chunk", "group", "top", "lanes"
+ * apply); the kernels are the generic shared-memory ones ("jit" / "reg" are ignored), about ten times slower than the
+ * covariance form and one to three orders more accurate; query times (M > 0) return SMOLGP_EUNSUPPORTED.
  * A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);

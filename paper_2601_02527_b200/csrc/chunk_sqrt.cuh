@@ -14,15 +14,75 @@
 // tria(M) = lower-triangular L with L L^T = M M^T: Householder reflections from the right, LANE i OWNS ROW i of M
 // (odd row stride: conflict-free), the reflector's row is read as a broadcast, so a reflection needs no cross-lane
 // reduction; reflectors are applied in the scale-free form v / |u| (information factors span hundreds of orders).
-// Generic (statically compiled) kernel, matrices in shared memory; one group of lanes per chunk.
-// Plan: one chunk per series (the sequential filter, row a8) -- the dense levels have no factor form yet.
+// Generic (statically compiled) kernels, matrices in shared memory; one group of lanes per chunk.
+// Chunked scan: k_fold0_sqrt folds a chunk into ONE element (A, b, U, eta, Z) with C = U U^T, J = Z Z^T (the recursion of
+// fold0_body with C -> U by tria / Potter and J += a a^T / s as Z <- tria([Z | a / sqrt s])); the dense levels combine
+// such elements in factor form (dense_sqrt.cuh); k_down0_sqrt starts from the chunk's prefix state [m | S] and from the
+// chunk-end adjoint  W = Z T'^-T,  T' T'^T = I + (S^T Z)^T (S^T Z),  of the suffix information [eta | Z].
 #pragma once
 #include "chunk_kernels.cuh"
 
 // row stride of the stacked matrix [S | G] (n + d + nblk <= 2.5 n columns) and [W | extra] (n + 1 columns): odd
 __host__ __device__ constexpr int sqrt_ldm(int ld) { return ((5 * ld) / 2) | 1; }
 __host__ __device__ inline int sqrt_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  return ((ld - 1) * sqrt_ldm(ld) + 2 * stride + 2 + nblk * G + 6 * ld + 1) & ~1;
+  return (2 * (ld - 1) * sqrt_ldm(ld) + 2 * stride + 2 + nblk * G + 6 * ld + 1) & ~1;
+}
+__host__ __device__ inline int fold0s_group_doubles(int n, int ld, int stride, int nblk, int G) {
+  return ((ld - 1) * sqrt_ldm(ld) + 2 * (ld - 1) * ld + 2 * stride + 2 + nblk * G + 5 * ld + 1) & ~1;
+}
+
+// One reflection of tria, columns c0..m-1 of the reflector's row rj and of the lane's own row ri.  The loops are
+// unrolled by hand with the loads ahead of the arithmetic: the trip count is a run-time value and ri / rj may alias as
+// far as the compiler knows, so a plain loop runs one shared-memory round trip per column (measured: 3x slower).
+__device__ __forceinline__ void hh_dots(const double* rj, const double* ri, int c0, int m, bool act, double& ss, double& dd) {
+  double s0 = 0.0, s1 = 0.0, d0 = 0.0, d1 = 0.0;
+  int c = c0;
+  for (; c + 3 < m; c += 4) {
+    const double u0 = rj[c], u1 = rj[c + 1], u2 = rj[c + 2], u3 = rj[c + 3];
+    double x0 = 0.0, x1 = 0.0, x2 = 0.0, x3 = 0.0;
+    if (act) { x0 = ri[c]; x1 = ri[c + 1]; x2 = ri[c + 2]; x3 = ri[c + 3]; }
+    s0 = fma(u0, u0, s0); s1 = fma(u1, u1, s1); s0 = fma(u2, u2, s0); s1 = fma(u3, u3, s1);
+    d0 = fma(x0, u0, d0); d1 = fma(x1, u1, d1); d0 = fma(x2, u2, d0); d1 = fma(x3, u3, d1);
+  }
+  for (; c < m; ++c) {
+    const double u0 = rj[c];
+    s0 = fma(u0, u0, s0);
+    if (act) d0 = fma(ri[c], u0, d0);
+  }
+  ss += s0 + s1;
+  dd = d0 + d1;
+}
+__device__ __forceinline__ void hh_axpy(const double* rj, double* ri, int c0, int m, double ws) {
+  int c = c0;
+  for (; c + 3 < m; c += 4) {
+    const double u0 = rj[c], u1 = rj[c + 1], u2 = rj[c + 2], u3 = rj[c + 3];
+    const double x0 = ri[c], x1 = ri[c + 1], x2 = ri[c + 2], x3 = ri[c + 3];
+    ri[c] = fma(-ws, u0, x0); ri[c + 1] = fma(-ws, u1, x1); ri[c + 2] = fma(-ws, u2, x2); ri[c + 3] = fma(-ws, u3, x3);
+  }
+  for (; c < m; ++c) ri[c] = fma(-ws, rj[c], ri[c]);
+}
+
+// column sums  a = sum_r col[r * st] p[r],  b = sum_r col[r * st] k[r]  (same hand unrolling)
+__device__ __forceinline__ void col_dots2(const double* col, int st, const double* p, const double* k, int n, double& a, double& b) {
+  double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+  int r = 0;
+  for (; r + 3 < n; r += 4) {
+    const double x0 = col[r * st], x1 = col[(r + 1) * st], x2 = col[(r + 2) * st], x3 = col[(r + 3) * st];
+    a0 = fma(x0, p[r], a0); a1 = fma(x1, p[r + 1], a1); a0 = fma(x2, p[r + 2], a0); a1 = fma(x3, p[r + 3], a1);
+    b0 = fma(x0, k[r], b0); b1 = fma(x1, k[r + 1], b1); b0 = fma(x2, k[r + 2], b0); b1 = fma(x3, k[r + 3], b1);
+  }
+  for (; r < n; ++r) { const double x = col[r * st]; a0 = fma(x, p[r], a0); b0 = fma(x, k[r], b0); }
+  a = a0 + a1; b = b0 + b1;
+}
+// col[r * st] += f v[r]
+__device__ __forceinline__ void col_axpy(double* col, int st, const double* v, int n, double f) {
+  int r = 0;
+  for (; r + 3 < n; r += 4) {
+    const double x0 = col[r * st], x1 = col[(r + 1) * st], x2 = col[(r + 2) * st], x3 = col[(r + 3) * st];
+    const double v0 = v[r], v1 = v[r + 1], v2 = v[r + 2], v3 = v[r + 3];
+    col[r * st] = fma(v0, f, x0); col[(r + 1) * st] = fma(v1, f, x1); col[(r + 2) * st] = fma(v2, f, x2); col[(r + 3) * st] = fma(v3, f, x3);
+  }
+  for (; r < n; ++r) col[r * st] = fma(v[r], f, col[r * st]);
 }
 
 // L L^T = M M^T in place: M = n rows x m columns at row stride LDM; on return the lower triangle of the first n
@@ -36,22 +96,18 @@ __device__ __forceinline__ void tria_rows(const Grp<G>& g, int n, int m, double*
     const bool act = (i > j) && (i < n);
     const double u0 = rj[j];
     double ss = u0 * u0, dd = 0.0;
-    for (int c = j + 1; c < m; ++c) {
-      const double uj = rj[c];
-      ss = fma(uj, uj, ss);
-      if (act) dd = fma(ri[c], uj, dd);
-    }
+    hh_dots(rj, ri, j + 1, m, act, ss, dd);
     const double sig = sqrt(ss);
     double alpha = 0.0;
     if (sig > 0.0) { // the same for every lane
       alpha = u0 > 0.0 ? -sig : sig;
-      const double v0 = (u0 - alpha) / sig;            // reflector v = (u - alpha e_j) / |u|
-      const double beta = 1.0 / (1.0 + fabs(u0) / sig); // H = I - beta v v^T
+      const double rsig = 1.0 / sig;                    // (sig > 0 in fp64 after a sum of squares: >= 1e-162, no overflow)
+      const double v0 = (u0 - alpha) * rsig;            // reflector v = (u - alpha e_j) / |u|
+      const double beta = 1.0 / (1.0 + fabs(u0) * rsig); // H = I - beta v v^T
       if (act) {
-        const double w = beta * fma(ri[j], v0, dd / sig);
+        const double w = beta * fma(ri[j], v0, dd * rsig);
         ri[j] = fma(-w, v0, ri[j]);
-        const double ws = w / sig;
-        for (int c = j + 1; c < m; ++c) ri[c] = fma(-ws, rj[c], ri[c]);
+        hh_axpy(rj, ri, j + 1, m, w * rsig);
       }
     }
     g.sync();
@@ -101,7 +157,8 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
   if (gid >= P.batch * P.c1) return;
   double* base = (double*)smem + (size_t)(threadIdx.x / G) * sqrt_group_doubles(n, LD, TSTRIDE, TNB, G);
   double* Mx = base;                       // [S | G], later [W | extra column]
-  double* recs = Mx + NR * LDM;            // 2 x stride + 2 mbarriers
+  double* Bx = Mx + NR * LDM;              // second stacked matrix: the chunk-end adjoint is built here
+  double* recs = Bx + NR * LDM;            // 2 x stride + 2 mbarriers
   double* U = recs + 2 * TSTRIDE + 2 + g.gl;
   double* mv = recs + 2 * TSTRIDE + 2 + TNB * G; // filtered mean, later lambda
   double* pv = mv + LD;
@@ -123,7 +180,12 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
   zero_fill(g, Mx, NR * LDM);
   zero_fill(g, mv, 5 * LD);
   g.sync();
-  chol_psd_rows<G, LDM>(g, n, P.p0, n, Mx); // S0 S0^T = blkdiag(Pinf, 0)  (Eq. 3.19, reading R6)
+  if (P.PRE1) { // the chunk's prefix state [m | S] from the dense levels
+    const double* sp = P.PRE1 + gid * (int64_t)state_size(n);
+    for (int c = i; c <= n; c += G)
+      for (int r = 0; r < n; ++r) { if (c < n) Mx[r * LDM + c] = sp[n + r * n + c]; else mv[r] = sp[r]; }
+    g.sync();
+  } else chol_psd_rows<G, LDM>(g, n, P.p0, n, Mx); // S0 S0^T = blkdiag(Pinf, 0)  (Eq. 3.19, reading R6)
   double ll = 0.0;
   // ---- forward: square-root Kalman filter ----
   uint32_t meta_nx = P.meta[k0];
@@ -168,7 +230,7 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
       if (i < n) pv[i] = hs * Mx[zi * LDM + i]; // phi = S^T h
       g.sync();
       double ss = 0.0, a = 0.0;
-      for (int c = 0; c < n; ++c) { const double f = pv[c]; ss = fma(f, f, ss); if (i < n) a = fma(ri[c], f, a); } // a = (S phi)_i = (P h)_i
+      hh_dots(pv, ri, 0, n, i < n, ss, a); // ss = |phi|^2, a = (S phi)_i = (P h)_i
       const double S = ss + sg * sg;
       const double v = yy - hs * mv[zi];
       if (!(sg_r > 0.0) || !isfinite(sg_r)) atomicOr(P.flags, NUMF_SIGMA);
@@ -178,8 +240,7 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
       const double gam = 1.0 / (S + sqrt(sg * sg * S));
       g.sync(); // every lane has read m_z
       if (i < n) {
-        const double ga = gam * a;
-        for (int c = 0; c < n; ++c) ri[c] = fma(-ga, pv[c], ri[c]);
+        hh_axpy(pv, ri, 0, n, gam * a);
         mv[i] = fma(a * rS, v, mv[i]);
         kv[i] = a * rS;
       }
@@ -189,8 +250,8 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
         g.sync();
         double* kb = P.kbuf + (series * P.N + ob) * (int64_t)ks;
         if (i < n) {
-          double p = 0.0;
-          for (int c = 0; c < n; ++c) p = fma(ri[c], bv[c], p); // P_f e_z
+          double p = 0.0, dummy = 0.0;
+          hh_dots(bv, ri, 0, n, true, dummy, p); // P_f e_z
           kb[i] = kv[i];
           kb[n + i] = p;
         }
@@ -207,9 +268,47 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
 
   // ---- backward: adjoint recursion with Lambda = W W^T (zero after the last event of the series) ----
   rs.issue(g, P.disc + (k1 - 1) * (int64_t)TSTRIDE, 0);
-  zero_fill(g, Mx, NR * LDM);
-  zero_fill(g, mv, LD);
-  g.sync();
+  if (P.SUF1 && chunk + 1 < P.c1) {
+    // adjoint at the chunk's last event from the suffix information [eta | Z] about the state after the chunk and
+    // the filtered state (m, S) there:  Lambda^ = (I + J P)^-1 J = W W^T with W = Z T'^-T, T' T'^T = I + V^T V,
+    // V = S^T Z;  lambda^ = (I + J P)^-1 (J m - eta) = u - W W^T P u,  u = Z Z^T m - eta
+    const double* sj = P.SUF1 + gid * (int64_t)state_size(n);
+    for (int c = i; c <= n; c += G)
+      for (int r = 0; r < n; ++r) { if (c < n) Bx[r * LDM + c] = sj[n + r * n + c]; else pv[r] = sj[r]; }
+    g.sync();
+    if (i < n) { double a = 0.0; for (int r = 0; r < n; ++r) a = fma(Bx[r * LDM + i], mv[r], a); kv[i] = a; }            // Z^T m
+    g.sync();
+    double* bi = Bx + (i < n ? i : 0) * LDM;
+    if (i < n) { double a = -pv[i]; for (int c = 0; c < n; ++c) a = fma(bi[c], kv[c], a); bv[i] = a; }                     // u
+    g.sync();
+    if (i < n) { double a = 0.0; for (int r = 0; r < n; ++r) a = fma(Mx[r * LDM + i], bv[r], a); kv[i] = a; }            // S^T u
+    g.sync();
+    if (i < n) { double a = 0.0; for (int c = 0; c < n; ++c) a = fma(ri[c], kv[c], a); av[i] = a; }                        // P u
+    if (i < n)                                                                                                             // column i of V^T = Z^T S
+      for (int r2 = 0; r2 < n; ++r2) { double a = 0.0; for (int r = 0; r < n; ++r) a = fma(Bx[r * LDM + r2], Mx[r * LDM + i], a); Bx[r2 * LDM + n + i] = a; }
+    g.sync();
+    if (i < n)
+      for (int c = 0; c < n; ++c) { ri[c] = (c == i) ? 1.0 : 0.0; ri[n + c] = bi[n + c]; }                                 // Mx = [I | V^T]
+    g.sync();
+    tria_rows<G, LDM>(g, n, 2 * n, Mx);                                                                                    // T'
+    if (i < n)
+      for (int c = 0; c < n; ++c) { double a = bi[c]; for (int k2 = 0; k2 < c; ++k2) a = fma(-Mx[c * LDM + k2], bi[k2], a); bi[c] = a / Mx[c * LDM + c]; } // row i of W
+    g.sync();
+    if (i < n) { double a = 0.0; for (int r = 0; r < n; ++r) a = fma(Bx[r * LDM + i], av[r], a); kv[i] = a; }            // W^T P u
+    g.sync();
+    if (i < n) {
+      double a = bv[i];
+      for (int c = 0; c < n; ++c) a = fma(-bi[c], kv[c], a);
+      mv[i] = a;                                                                                                           // lambda^
+      for (int c = 0; c < n; ++c) ri[c] = bi[c];
+      ri[n] = 0.0;
+    }
+    g.sync();
+  } else {
+    zero_fill(g, Mx, NR * LDM);
+    zero_fill(g, mv, LD);
+    g.sync();
+  }
   uint32_t meta_b = P.meta[k1 - 1];
   int32_t ob_b = P.obs[k1 - 1];
   for (int64_t k = k1 - 1; k >= k0; --k) {
@@ -234,7 +333,7 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
       g.sync();
       double a = 0.0, b = 0.0, lp = 0.0, lk = 0.0;
       if (i < n) {
-        for (int r = 0; r < n; ++r) { const double x = Mx[r * LDM + i]; a = fma(x, pv[r], a); b = fma(x, kv[r], b); } // (W^T p)_i, (W^T K)_i
+        col_dots2(Mx + i, LDM, pv, kv, n, a, b); // (W^T p)_i, (W^T K)_i
         lp = mv[i] * pv[i];
         lk = mv[i] * kv[i];
       }
@@ -265,5 +364,119 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
   }
 }
 
+// chunk -> one element in factor form
+template <int G, int LD>
+__device__ __forceinline__ void fold0_sqrt_body(const ScanDev& P) {
+  extern __shared__ __align__(16) char smem[];
+  const Tab& T = P.T;
+  constexpr int LDM = sqrt_ldm(LD);
+  constexpr int NR = LD - 1, ld = LD;
+  const int n = TN, d = TD, nblk = TNB, nq = TD + TNB;
+  const Grp<G> g;
+  const int gpc = blockDim.x / G;
+  const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
+  if (gid >= P.batch * P.c1) return;
+  double* base = (double*)smem + (size_t)(threadIdx.x / G) * fold0s_group_doubles(n, LD, TSTRIDE, TNB, G);
+  double* Mx = base;                       // [U | G]
+  double* AB = Mx + NR * LDM;              // [A | b], column-owned, row stride LD
+  double* Bx = AB + NR * ld;               // [Z | extra column], row stride LD
+  double* recs = Bx + NR * ld;
+  double* U = recs + 2 * TSTRIDE + 2 + g.gl;
+  double* ev = recs + 2 * TSTRIDE + 2 + TNB * G; // eta
+  double* pv = ev + LD;
+  double* cv = pv + LD;
+  double* av = cv + LD;                    // n + 1
+  const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
+  const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
+  const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
+  const int i = g.gl;
+  double* ri = Mx + (i < n ? i : 0) * LDM;
+
+  RecStage rs;
+  rs.init(g, recs, TSTRIDE);
+  rs.issue(g, P.disc + k0 * (int64_t)TSTRIDE, 0);
+  zero_fill(g, Mx, NR * LDM + 2 * NR * ld);
+  zero_fill(g, ev, 4 * LD);
+  g.sync();
+  for (int r = i; r < n; r += G) AB[r * ld + r] = 1.0;
+  g.sync();
+  uint32_t meta_nx = P.meta[k0];
+  int32_t ob_nx = P.obs[k0];
+  for (int64_t k = k0; k < k1; ++k) {
+    const double* rec = rs.wait((int)((k - k0) & 1));
+    g.sync();
+    if (k + 1 < k1) rs.issue(g, P.disc + (k + 1) * (int64_t)TSTRIDE, (int)((k + 1 - k0) & 1));
+    const uint32_t meta = meta_nx;
+    const int32_t ob = ob_nx;
+    if (k + 1 < k1) { meta_nx = P.meta[k + 1]; ob_nx = P.obs[k + 1]; }
+    const int kind = META_KIND(meta), q = META_INST(meta);
+    const unsigned zm = META_ZMASK(meta);
+    const unsigned tz = kind ? zm : (zm & ~(1u << q));
+    double dl_r = 1.0, sg_r = 0.0, y_r = 0.0;
+    if (!kind) { dl_r = P.delta[k]; sg_r = P.sigma[ob]; y_r = P.y[series * P.N + ob]; }
+    // [A | b] <- F [A | b];  U <- tria([F U | G])
+    if (i <= n) apply_F<G, LD, LD>(T, rec, tz, AB + i, AB + i, U);
+    if (i < n) apply_F<G, LDM, LDM>(T, rec, tz, Mx + i, Mx + i, U);
+    for (int cg = i; cg < nq; cg += G) {
+      double* col = Mx + n + cg;
+      for (int r = 0; r < n; ++r) col[r * LDM] = 0.0;
+      for (int b = 0; b < nblk; ++b) {
+        const int db = TBDIM(b), off = TBOFF(b), l = cg - off - b;
+        if (l < 0 || l > db) continue;
+        const double* r = rec + TROFF(b);
+        if (l < db)
+          for (int r2 = l; r2 < db; ++r2) col[(off + r2) * LDM] = r[db * db + db + r2 * db + l];
+        const double lz = r[2 * db * db + db + l];
+        for (int p = 0; p < TNI; ++p)
+          if (!((tz >> p) & 1u)) col[(d + p) * LDM] = TCZ(p * nblk + b) * lz;
+      }
+    }
+    g.sync();
+    tria_rows<G, LDM>(g, n, n + nq, Mx);
+    if (!kind) {
+      // fold the end event's primitive element onto the aggregate (SG21 Eq. 10, rank-one J_j: fold0_body), in factors
+      const int zi = d + q;
+      const double hs = TTAU(q) / dl_r;
+      const double sg = sg_r * ramp;
+      const double yy = y_r * ramp;
+      if (i < n) pv[i] = hs * Mx[zi * LDM + i];       // phi = U^T h
+      if (i <= n) av[i] = hs * AB[zi * ld + i];       // a = A^T h (entry n: h . b)
+      g.sync();
+      double ss = 0.0, a = 0.0;
+      hh_dots(pv, ri, 0, n, i < n, ss, a);
+      const double S = ss + sg * sg;
+      if (!(S > 0.0) || !isfinite(S)) atomicOr(P.flags, NUMF_BAD);
+      const double rS = 1.0 / S, resid = yy - av[n];
+      const double gam = 1.0 / (S + sqrt(sg * sg * S));
+      if (i < n) {
+        cv[i] = a;                                    // c = C h
+        hh_axpy(pv, ri, 0, n, gam * a);                // Potter: C -= c c^T / s
+        ev[i] = fma(av[i], resid * rS, ev[i]);        // eta += a resid / s
+        Bx[i * ld + n] = av[i] * sqrt(rS);            // J += a a^T / s
+      }
+      g.sync();
+      if (i <= n) { // column i of A -= c a_i / s;  b += c resid / s
+        const double f = (i < n) ? -av[i] * rS : resid * rS;
+        col_axpy(AB + i, ld, cv, n, f);
+      }
+      tria_rows<G, LD>(g, n, n + 1, Bx);
+      // the instrument is idle after its end: zero z_q (reading R6)
+      if (i <= n) AB[zi * ld + i] = 0.0;
+      if (i == zi) for (int c = 0; c < n; ++c) ri[c] = 0.0;
+      g.sync();
+    }
+  }
+  double* out = P.E1 + gid * (int64_t)elem_size(n);
+  const int n1 = n + 1;
+  for (int j = i; j <= n; j += G)
+    for (int r = 0; r < n; ++r) {
+      out[r * n1 + j] = AB[r * ld + j];
+      out[n * n1 + n * n + r * n1 + j] = (j < n) ? Bx[r * ld + j] : ev[r];
+      if (j < n) out[n * n1 + r * n + j] = Mx[r * LDM + j];
+    }
+}
+
+template <int G, int LD>
+__global__ void __launch_bounds__(128) k_fold0_sqrt(const __grid_constant__ ScanDev P) { fold0_sqrt_body<G, LD>(P); }
 template <int G, int LD>
 __global__ void __launch_bounds__(128) k_down0_sqrt(const __grid_constant__ ScanDev P) { down0_sqrt_body<G, LD>(P); }

@@ -166,18 +166,24 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
     else { ctx->err = "scan: unsupported (lanes, n) combination"; return SMOLGP_EUNSUPPORTED; } \
   } while (0)
 
-// square-root form (chunk_sqrt.cuh): the generic kernel, one group per series
+// square-root form (chunk_sqrt.cuh, dense_sqrt.cuh): generic kernels
 template <int G, int LD>
-static int launch_sqrt(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm) {
-  const size_t per_group = (size_t)sqrt_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
+static int launch_sqrt(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold) {
+  const size_t per_group = (size_t)(fold ? fold0s_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) : sqrt_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G)) * 8;
   const int gpc = groups_per_cta(per_group, G);
   const size_t smem = per_group * gpc;
   if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
   if (hm->n + hm->d + hm->nblk > sqrt_ldm(LD)) { ctx->err = "scan: model too wide for the square-root kernel"; return SMOLGP_EUNSUPPORTED; }
   const int64_t groups = P.batch * P.c1;
-  SG_CUDA(ctx, cudaFuncSetAttribute(k_down0_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  sg_launch_begin(ctx, KID_DOWN0);
-  k_down0_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(P);
+  if (fold) {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_FOLD0);
+    k_fold0_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(P);
+  } else {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_down0_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_DOWN0);
+    k_down0_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(P);
+  }
   sg_launch_end(ctx);
   SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
@@ -206,6 +212,24 @@ static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* 
   SG_DISPATCH_GL(G, LD, SG_CALL_L0);
 #undef SG_CALL_L0
   return SMOLGP_EUNSUPPORTED;
+}
+
+static int launch_dense_sqrt(smolgp_ctx* ctx, const DenseArgs& D, int n, bool fold) {
+  const size_t smem = (size_t)(fold ? foldDs_group_doubles(n) : downDs_group_doubles(n)) * 8;
+  if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+  dim3 grid((unsigned)(D.batch * D.cout), fold ? 1 : (D.want_suffix ? 2 : 1));
+  if (fold) {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD_sqrt<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_FOLDD);
+    k_foldD_sqrt<SG_DENSE_NT><<<grid, SG_DENSE_NT, smem, ctx->stream>>>(D);
+  } else {
+    SG_CUDA(ctx, cudaFuncSetAttribute(k_downD_sqrt<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    sg_launch_begin(ctx, KID_DOWND);
+    k_downD_sqrt<SG_DENSE_NT><<<grid, SG_DENSE_NT, smem, ctx->stream>>>(D);
+  }
+  sg_launch_end(ctx);
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
 }
 
 static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, const SgJitKernels* jk, bool fold) {
@@ -245,7 +269,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   const int G = pick_lanes(ctx, n);
   Tab T0;
   tab_build(hm, &T0);
-  const bool sq = hm->sqrt_form != 0; // square-root form: generic kernel, one chunk per series (the dense levels have no factor form)
+  const bool sq = hm->sqrt_form != 0; // square-root form: the generic factor-form kernels (chunk_sqrt.cuh, dense_sqrt.cuh)
   L0Plan lp;
   if (sq) { lp.jk = nullptr; lp.cfg = make_cfg(ctx, T0, G); }
   else lp = plan_l0(ctx, T0, G, batch * K, true); // specialised kernels for this model's structure, or the generic ones
@@ -257,7 +281,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
 
   // chunk length: enough chunks to fill the machine about twice, within [16, 512]; a batch that
   // already fills it runs one chunk per series (the sequential filter, row a8)
-  int64_t Lc = sq ? K : ctx->opt_chunk;
+  int64_t Lc = ctx->opt_chunk;
   if (Lc <= 0) {
     // one full wave: as many chunks as groups can be resident at once (equal work per chunk, no tail);
     // a batch that already fills the machine runs one chunk per series (the sequential filter, row a8)
@@ -265,6 +289,9 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     if (reg) {
       per_sm = reg_groups_per_sm(hm, jk0->cfg.rG, jk0->regs_down0);
       per_sm_f = reg_groups_per_sm(hm, jk0->cfg.fG, jk0->regs_fold0);
+    } else if (sq) {
+      groups_per_cta((size_t)sqrt_group_doubles(n, chunk_ld(n), hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
+      groups_per_cta((size_t)fold0s_group_doubles(n, chunk_ld(n), hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
     } else {
       groups_per_cta((size_t)down0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm);
       groups_per_cta((size_t)fold0_group_doubles(n, ld0, hm->disc_stride, hm->nblk, G) * 8, G, &per_sm_f);
@@ -335,13 +362,17 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   P.ADJ1 = use_adj ? (const double*)(w + oADJ) : nullptr;
 
   if (pl.T) {
-    rc = launch_level0_any(ctx, P, hm, true, G, lp);
+    if (sq) {
+#define SG_CALL_SQF(g_, ld_) rc = launch_sqrt<g_, ld_>(ctx, P, hm, true)
+      SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_SQF);
+#undef SG_CALL_SQF
+    } else rc = launch_level0_any(ctx, P, hm, true, G, lp);
     if (rc) return rc;
     for (int l = 1; l < pl.T; ++l) {
       DenseArgs D = {};
       D.n = n; D.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); D.Ein = (const double*)(w + oE[l]); D.Eout = (double*)(w + oE[l + 1]);
       D.cin = pl.cnt[l]; D.cout = pl.cnt[l + 1]; D.batch = batch; D.g = g;
-      rc = launch_dense(ctx, D, n, jk0, true);
+      rc = sq ? launch_dense_sqrt(ctx, D, n, true) : launch_dense(ctx, D, n, jk0, true);
       if (rc) return rc;
     }
     for (int l = pl.T; l >= 1; --l) {
@@ -351,7 +382,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
       if (l == pl.T) { D.cout = 1; D.g = (int)pl.cnt[l]; D.PREup = nullptr; D.SUFup = nullptr; }
       else { D.cout = pl.cnt[l + 1]; D.g = g; D.PREup = (const double*)(w + oPRE[l + 1]); D.SUFup = a.want_smooth ? (const double*)(w + oSUF[l + 1]) : nullptr; }
       D.PRE = (double*)(w + oPRE[l]); D.SUF = a.want_smooth ? (double*)(w + oSUF[l]) : nullptr;
-      rc = launch_dense(ctx, D, n, jk0, false);
+      rc = sq ? launch_dense_sqrt(ctx, D, n, false) : launch_dense(ctx, D, n, jk0, false);
       if (rc) return rc;
     }
   }
@@ -367,7 +398,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     SG_CUDA(ctx, e);
   }
   if (sq) {
-#define SG_CALL_SQ(g_, ld_) rc = launch_sqrt<g_, ld_>(ctx, P, hm)
+#define SG_CALL_SQ(g_, ld_) rc = launch_sqrt<g_, ld_>(ctx, P, hm, false)
     SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_SQ);
 #undef SG_CALL_SQ
   } else rc = launch_level0_any(ctx, P, hm, false, G, lp);

@@ -1,7 +1,7 @@
-"""GPU parity of the square-root (Cholesky-factor) form of the chunk recursions (option "form" = 1; SURVEY 8(f) item 1,
-P:535; csrc/chunk_sqrt.cuh) against the long-double oracle: same bars as the covariance form (loglik 1e-9,
-posterior 1e-8), on every model structure; plus what the form is for -- fewer digits lost, with no compensated product
-anywhere on its path."""
+"""GPU parity of the square-root (Cholesky-factor) form of the whole scan (option "form" = 1; SURVEY 8(f) item 1, P:535,
+P:557; csrc/chunk_sqrt.cuh, csrc/dense_sqrt.cuh) against the long-double oracle: same bars as the covariance form
+(loglik 1e-9, posterior 1e-8), on every model structure and every scan plan (chunk lengths, fan-ins, the sequential
+plan); plus what the form is for -- fewer digits lost, with no compensated product anywhere on its path."""
 import numpy as np
 import pytest
 
@@ -29,26 +29,39 @@ def _golden(cfg):
         np.array([float(r[2]) for r in rows[1:]])
 
 
-def _run(ctx, w, form, **kw):
+SCAN_OPTS = {
+    "auto": (),
+    "sequential": (("chunk", 1 << 40),),                       # one chunk per series (row a8): no dense level on the path
+    "deep": (("chunk", 16), ("group", 2), ("top", 2)),         # many dense levels, tree up to the root
+    "walk": (("chunk", 16), ("group", 2), ("top", 13)),        # long sequential walk at the top level
+    "ragged": (("chunk", 37), ("group", 3), ("lanes", 32)),    # chunk / group sizes dividing nothing
+}
+
+
+def _run(ctx, w, form, opts=(), **kw):
     ctx.set_option("form", form)
+    for k, v in opts:
+        ctx.set_option(k, v)
     try:
         ev = ctx.smolgp_build_events_host(w["t_start"], w["t_end"], w["instrument"], w["n_inst"])
         out = ctx.smolgp_condition_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"], **kw)
         plan = ctx.plan_info()
         ll = ctx.smolgp_loglik_host(ev, w["kernel"], w["y"], w["sigma"], amp=w["amp"])
     finally:
-        ctx.set_option("form", 0)
+        for k in ("form", "chunk", "group", "top", "lanes"):
+            ctx.set_option(k, 0)
     return out, ll, plan
 
 
 CASES = [(1, 1000, None), (2, 3001, None), ("fig2", 400, None), ("fig3", 600, None), (3, 1500, None), (4, 1203, None), (5, 300, 6)]
 
 
+@pytest.mark.parametrize("opt", sorted(SCAN_OPTS))
 @pytest.mark.parametrize("cfg,N,batch", CASES)
-def test_sqrt_form_matches_oracle(ctx, oracle, cfg, N, batch):
+def test_sqrt_form_matches_oracle(ctx, oracle, cfg, N, batch, opt):
     w = W.make(cfg, N=N, batch=batch)
-    out, ll, plan = _run(ctx, w, 1)
-    assert "form=sqrt" in plan and "levels=0" in plan   # one chunk per series: no dense level on the path
+    out, ll, plan = _run(ctx, w, 1, SCAN_OPTS[opt])
+    assert "form=sqrt" in plan and ("levels=0" in plan) == (opt == "sequential")
     for s in ([None] if batch is None else range(batch)):
         ref = PU.reference(oracle, w, series=s)
         i = 0 if s is None else s
@@ -108,18 +121,20 @@ def test_sqrt_form_full_size_cfg5_sampled_series(ctx, oracle):
     assert np.all(np.isfinite(out["loglik"])) and np.all(out["var"] > 0)
 
 
-def test_sqrt_form_full_size_cfg3_golden(ctx, oracle):
-    """N = 1e5, n = 21, one sequential pass of 2e5 events in factor form (seconds: the chunked scan has no factor form
-    yet): the variance stays within 1e-9 of the long-double oracle with no compensated product"""
-    ll, idx, mean, var = _golden(3)
-    w = W.make(3)
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_sqrt_form_full_size_golden(ctx, oracle, cfg):
+    """N = 1e5 (n = 21) and N = 1e6 (n = 17) in the automatic plan (chunked scan, ten dense levels in factor form):
+    with no compensated product anywhere the variance stays within 1e-10 of the long-double oracle (the covariance
+    form: 1e-9 on config 3 WITH compensated products in its dense levels)"""
+    ll, idx, mean, var = _golden(cfg)
+    w = W.make(cfg)
     out, _, plan = _run(ctx, w, 1)
-    assert "form=sqrt" in plan
-    assert abs(out["loglik"][0] - ll) <= PU.LL_RTOL * abs(ll)
+    assert "form=sqrt" in plan and "levels=10" in plan
+    assert abs(out["loglik"][0] - ll) <= 1e-11 * abs(ll)
     floor = PU.prior_sd(oracle, w, idx=idx)
-    assert np.max(np.abs(out["mean"][0][idx] - mean) / (np.abs(mean) + floor)) <= PU.POST_RTOL
+    assert np.max(np.abs(out["mean"][0][idx] - mean) / (np.abs(mean) + floor)) <= 1e-10
     rel = np.abs(out["var"][0][idx] - var) / var
-    assert rel.max() <= 1e-9, (rel.max(), np.quantile(rel, [0.5, 0.9, 0.99]))
+    assert rel.max() <= 1e-10, (rel.max(), np.quantile(rel, [0.5, 0.9, 0.99]))
 
 
 def test_sqrt_form_gradient_and_unsupported_queries(ctx, oracle):
