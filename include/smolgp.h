@@ -94,7 +94,7 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * the conditioning of the covariance recursions: covariances, informations and adjoint matrices are carried
  * as factors (P = S S^T, J = Z Z^T) and re-triangularised, in the chunk recursions and in the dense combines alike; nothing
  * is subtracted from a covariance, no I + C J is formed or inverted, no product is compensated (csrc/chunk_sqrt.cuh,
- * csrc/dense_sqrt.cuh, DESIGN.md 13).  Same inputs, outputs, tolerances and scan plans ("chunk", "group", "top", "lanes"
+ * csrc/dense_sqrt.cuh, DESIGN.md 15).  Same inputs, outputs, tolerances and scan plans ("chunk", "group", "top", "lanes"
  * apply); the kernels are the generic shared-memory ones ("jit" / "reg" are ignored), about ten times slower than the
  * covariance form and one to three orders more accurate; query times (M > 0) return SMOLGP_EUNSUPPORTED.
  * A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
