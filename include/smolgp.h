@@ -96,7 +96,7 @@ const char* smolgp_last_error(const smolgp_ctx* ctx);
  * is subtracted from a covariance, no I + C J is formed or inverted, no product is compensated (csrc/chunk_sqrt.cuh,
  * csrc/dense_sqrt.cuh).  Same inputs, outputs, tolerances and scan plans ("chunk", "group", "top", "lanes"
  * apply); the kernels are the generic shared-memory ones ("jit" / "reg" are ignored), about ten times slower than the
- * covariance form and one to three orders more accurate; query times (M > 0) return SMOLGP_EUNSUPPORTED.
+ * covariance form and one to three orders more accurate; query times (M > 0) are served from the stored factors.
  * A structure is compiled once per ctx (a few seconds) and serves every hyper-parameter value; when NVRTC is missing or a
  * compilation fails the generic kernels run and smolgp_jit_log says why. */
 int smolgp_set_option(smolgp_ctx* ctx, const char* name, int64_t value);

@@ -145,7 +145,6 @@ static int run_path(smolgp_ctx* ctx, const smolgp_events* ev, const smolgp_kerne
   int rc = sg_build_model(ctx, kernel, ev->n_inst, ev->tau, ev->instant, &hm);
   if (rc) return rc;
   hm.sqrt_form = (ctx->opt_form == 1) ? 1 : 0;
-  if (hm.sqrt_form && qs.M > 0) { ctx->err = "condition: query times are not available in square-root form (option form = 1)"; return SMOLGP_EUNSUPPORTED; }
   const size_t model_b = (sizeof(ModelDev) + 255) / 256 * 256;
   const size_t disc_b = ((size_t)ev->K * hm.disc_stride * 8 + 255) / 256 * 256;
   if (ctx->pers_bytes < model_b + disc_b) {

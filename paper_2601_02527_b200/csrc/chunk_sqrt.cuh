@@ -262,6 +262,11 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
       if (i == zi) { for (int c = 0; c < n; ++c) ri[c] = 0.0; mv[zi] = 0.0; }
       g.sync();
     }
+    if (P.fstate) { // row a7: the post-event filtered state [m | S] of every event
+      double* fs = P.fstate + (series * P.K + k) * (int64_t)state_size(n);
+      for (int c = i; c <= n; c += G)
+        for (int r = 0; r < n; ++r) { if (c < n) fs[n + r * n + c] = Mx[r * LDM + c]; else fs[r] = mv[r]; }
+    }
   }
   if (g.gl == 0) P.llpart[gid] = ll;
   if (!P.want_smooth) return;
@@ -355,6 +360,11 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
       }
       g.sync();
       tria_rows<G, LDM>(g, n, n + 1, Mx);
+    }
+    if (P.binfo) { // row a7: the pre-update adjoint [lambda~ | W~] of every event
+      double* bs = P.binfo + (series * P.K + k) * (int64_t)state_size(n);
+      for (int c = i; c <= n; c += G)
+        for (int r = 0; r < n; ++r) { if (c < n) bs[n + r * n + c] = Mx[r * LDM + c]; else bs[r] = mv[r]; }
     }
     if (k == k0) break;
     const unsigned tz = kind ? zm : (zm & ~(1u << q));
@@ -480,3 +490,125 @@ template <int G, int LD>
 __global__ void __launch_bounds__(128) k_fold0_sqrt(const __grid_constant__ ScanDev P) { fold0_sqrt_body<G, LD>(P); }
 template <int G, int LD>
 __global__ void __launch_bounds__(128) k_down0_sqrt(const __grid_constant__ ScanDev P) { down0_sqrt_body<G, LD>(P); }
+
+// ---------------------------------------------------------------------------------------------------
+// Row a7 in factor form (query_body of chunk_kernels.cuh): the filtered factor after the last event at or before t*
+// is predicted over Delta_1 (one triangularisation), the pre-update adjoint factor of the next event is stepped back
+// over Delta_2 (W* = F_2^T W~: no triangularisation), and
+//   H_q m^ = h . m* - lambda* . p,   H_q P^ H_q^T = |S*^T h|^2 - |W*^T p|^2,   p = P* h = S* (S*^T h).
+// ---------------------------------------------------------------------------------------------------
+__host__ __device__ inline int querys_group_doubles(int n, int ld, int stride, int nblk, int G) {
+  return ((ld - 1) * sqrt_ldm(ld) + (ld - 1) * ld + 2 * stride + 2 + nblk * G + 5 * ld + 1) & ~1;
+}
+
+template <int G, int LD>
+__device__ __forceinline__ void query_sqrt_body(const QueryDev& P) {
+  extern __shared__ __align__(16) char smem[];
+  const Tab& T = P.T;
+  constexpr int LDM = sqrt_ldm(LD);
+  constexpr int NR = LD - 1, ld = LD;
+  const int n = TN, d = TD, nblk = TNB, nq = TD + TNB;
+  const Grp<G> g;
+  const int gpc = blockDim.x / G;
+  const int64_t gid = (int64_t)blockIdx.x * gpc + threadIdx.x / G;
+  if (gid >= P.batch * P.Mq) return;
+  double* base = (double*)smem + (size_t)(threadIdx.x / G) * querys_group_doubles(n, LD, TSTRIDE, TNB, G);
+  double* Mx = base;                 // [S | G]
+  double* Wx = Mx + NR * LDM;        // W, row stride LD
+  double* recs = Wx + NR * ld;
+  double* U = recs + 2 * TSTRIDE + 2 + g.gl;
+  double* mv = recs + 2 * TSTRIDE + 2 + TNB * G;
+  double* lam = mv + LD;
+  double* hv = lam + LD;
+  double* t1 = hv + LD;
+  double* ph = t1 + LD;
+  const int ss = state_size(n);
+  const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
+  const int64_t kp = P.kp[q];
+  const double ampv = P.amp ? P.amp[series] : 1.0;
+  if (!(ampv > 0.0) || !isfinite(ampv)) atomicOr(P.flags, NUMF_AMP);
+  const int i = g.gl;
+  double* ri = Mx + (i < n ? i : 0) * LDM;
+  RecStage rs;
+  rs.init(g, recs, TSTRIDE);
+  rs.issue(g, P.discq + q * (int64_t)TSTRIDE, 0);
+  rs.issue(g, P.discq + (P.Mq + q) * (int64_t)TSTRIDE, 1);
+  zero_fill(g, Mx, NR * LDM + NR * ld);
+  zero_fill(g, mv, 5 * LD);
+  g.sync();
+  if (i == 0)
+    for (int b = 0; b < TNB; ++b) hv[TBOFF(b)] = ((P.T.bmask[b] >> P.qinst) & 1u) ? P.T.bsig[b] : 0.0; // H of the queried (virtual) instrument
+  rs.wait(0);
+  rs.wait(1);
+  g.sync();
+  if (kp >= 0) {
+    const double* fs = P.fstate + (series * P.K + kp) * (int64_t)ss;
+    for (int c = i; c <= n; c += G)
+      for (int r = 0; r < n; ++r) { if (c < n) Mx[r * LDM + c] = fs[n + r * n + c]; else mv[r] = fs[r]; }
+    g.sync();
+    const uint32_t mp = P.meta[kp]; // idle through (t_kp, t_kp+1): zeroed after kp, except an instrument that just started
+    const unsigned idle = META_KIND(mp) ? (META_ZMASK(mp) & ~(1u << META_INST(mp))) : META_ZMASK(mp);
+    const double* rec = recs;
+    if (i < n) apply_F<G, LDM, LDM>(T, rec, idle, Mx + i, Mx + i, U);
+    else if (i == n) apply_F<G, 1, 1>(T, rec, idle, mv, mv, U);
+    for (int cg = i; cg < nq; cg += G) {
+      double* col = Mx + n + cg;
+      for (int r = 0; r < n; ++r) col[r * LDM] = 0.0;
+      for (int b = 0; b < nblk; ++b) {
+        const int db = TBDIM(b), off = TBOFF(b), l = cg - off - b;
+        if (l < 0 || l > db) continue;
+        const double* r = rec + TROFF(b);
+        if (l < db)
+          for (int r2 = l; r2 < db; ++r2) col[(off + r2) * LDM] = r[db * db + db + r2 * db + l];
+        const double lz = r[2 * db * db + db + l];
+        for (int p = 0; p < TNI; ++p)
+          if (!((idle >> p) & 1u)) col[(d + p) * LDM] = TCZ(p * nblk + b) * lz;
+      }
+    }
+    g.sync();
+    tria_rows<G, LDM>(g, n, n + nq, Mx);
+  } else { // before the first event: the stationary prior, idle z = 0 (retrodiction, reading R8)
+    chol_psd_rows<G, LDM>(g, n, P.p0, n, Mx);
+  }
+  const bool have_next = kp + 1 < P.K;
+  if (have_next) {
+    const int64_t kn = kp + 1;
+    const double* bs = P.binfo + (series * P.K + kn) * (int64_t)ss;
+    for (int c = i; c <= n; c += G)
+      for (int r = 0; r < n; ++r) { if (c < n) Wx[r * ld + c] = bs[n + r * n + c]; else lam[r] = bs[r]; }
+    g.sync();
+    const uint32_t meta = P.meta[kn];
+    const unsigned zm = META_ZMASK(meta);
+    const unsigned tz = META_KIND(meta) ? zm : (zm & ~(1u << META_INST(meta)));
+    if (i < n) apply_Ft<G, LD, LD>(T, recs + TSTRIDE, tz, Wx + i, Wx + i);
+    else if (i == n) apply_Ft<G, 1, 1>(T, recs + TSTRIDE, tz, lam, lam);
+    g.sync();
+  }
+  if (i < n) { double a = 0.0; for (int r = 0; r < n; ++r) a = fma(Mx[r * LDM + i], hv[r], a); t1[i] = a; } // S*^T h
+  g.sync();
+  double sv = 0.0, sm = 0.0;
+  if (i < n) {
+    double a = 0.0;
+    for (int c = 0; c < n; ++c) a = fma(ri[c], t1[c], a);
+    ph[i] = a;                                                                                             // P* h
+    sv = t1[i] * t1[i];
+    sm = hv[i] * mv[i];
+  }
+  g.sync();
+  if (have_next && i < n) {
+    double a = 0.0;
+    for (int r = 0; r < n; ++r) a = fma(Wx[r * ld + i], ph[r], a);                                          // (W*^T p)_i
+    sv -= a * a;
+    sm -= lam[i] * ph[i];
+  }
+  sv = group_sum(g, sv);
+  sm = group_sum(g, sm);
+  if (i == 0) {
+    if (!isfinite(sv) || !isfinite(sm)) atomicOr(P.flags, NUMF_BAD);
+    P.mean[series * P.Mtot + P.q0 + q] = ampv * sm;
+    P.var[series * P.Mtot + P.q0 + q] = ampv * ampv * sv;
+  }
+}
+
+template <int G, int LD>
+__global__ void __launch_bounds__(128) k_query_sqrt(const __grid_constant__ QueryDev P) { query_sqrt_body<G, LD>(P); }

@@ -421,6 +421,21 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
 }
 
 template <int G, int LD>
+static int launch_query_sqrt(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
+  const size_t per_group = (size_t)querys_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
+  const int gpc = groups_per_cta(per_group, G);
+  const size_t smem = per_group * gpc;
+  if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
+  const int64_t groups = Q.batch * Q.Mq;
+  SG_CUDA(ctx, cudaFuncSetAttribute(k_query_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  sg_launch_begin(ctx, KID_QUERY);
+  k_query_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
+  sg_launch_end(ctx);
+  SG_CUDA(ctx, cudaGetLastError());
+  return SMOLGP_OK;
+}
+
+template <int G, int LD>
 static int launch_query(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
   const size_t per_group = (size_t)query_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
   const int gpc = groups_per_cta(per_group, G);
@@ -459,7 +474,10 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
   Q.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); Q.discq = discq; Q.kp = kp; Q.meta = a.ev->meta; Q.fstate = a.fstate; Q.binfo = a.binfo; Q.amp = a.amp;
   Q.K = a.ev->K; Q.batch = a.batch; Q.qinst = a.qinst; Q.mean = a.mean; Q.var = a.var; Q.flags = ctx->d_flags; Q.Mtot = a.M;
   const int G = pick_lanes(ctx, n);
-  const L0Plan lp = plan_l0(ctx, Q.T, G, Q.batch * Q.K, false);
+  const bool sq = hm->sqrt_form != 0;
+  L0Plan lp;
+  if (sq) { lp.jk = nullptr; lp.cfg = make_cfg(ctx, Q.T, G); }
+  else lp = plan_l0(ctx, Q.T, G, Q.batch * Q.K, false);
   const SgJitKernels* jk = lp.jk;
   const int LD = l0_ld(lp, n);
   for (int64_t q0 = 0; q0 < a.M; q0 += slice) {
@@ -471,7 +489,11 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
     SG_CUDA(ctx, cudaGetLastError());
     rc = sg_launch_disc(ctx, a.d_model, hm, dtq, 2 * M, discq);
     if (rc) return rc;
-    if (jk) {
+    if (sq) {
+#define SG_CALL_QS(g_, ld_) rc = launch_query_sqrt<g_, ld_>(ctx, Q, hm)
+      SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_QS);
+#undef SG_CALL_QS
+    } else if (jk) {
       const size_t per_group = (size_t)query_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) * 8;
       const int gpc = groups_per_cta(per_group, G);
       const int64_t groups = Q.batch * Q.Mq;
