@@ -7,8 +7,9 @@
 //   predict   S <- tria([F S | G]),  G G^T = Q~: G is assembled from the blocks' own Cholesky factors, which k_disc
 //             writes in place of (Qxx, q12, q22) when the model asks for them (Q~ itself is singular);
 //   reset     zero row z_q of S;
-//   update    scalar observation h = hs e_z: Potter's form  S <- S - gamma (S phi) phi^T,  phi = S^T h,
-//             s = phi^T phi + r,  gamma = 1 / (s + sqrt(r s)):  no subtraction of covariances;
+//   update    scalar observation h = hs e_z: Carlson's triangular form (carlson_rows: column j of S becomes a
+//             combination of itself and of the columns after it, so S STAYS lower triangular): no subtraction of
+//             covariances, and the next [F S | G] is block lower triangular -- the triangularisation skips the zeros;
 //   adjoint   end event:  W <- tria([W - h (W^T K)^T | h / sqrt s]),   step:  W <- F^T W;
 //   smoothed  H~ P^ H~^T = hs^2 (p_z - |W^T p|^2),  p = P_f e_z (kept in kbuf by the forward pass, as in down0_body).
 // tria(M) = lower-triangular L with L L^T = M M^T: Householder reflections from the right, LANE i OWNS ROW i of M
@@ -25,10 +26,10 @@
 // row stride of the stacked matrix [S | G] (n + d + nblk <= 2.5 n columns) and [W | extra] (n + 1 columns): odd
 __host__ __device__ constexpr int sqrt_ldm(int ld) { return ((5 * ld) / 2) | 1; }
 __host__ __device__ inline int sqrt_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  return (2 * (ld - 1) * sqrt_ldm(ld) + 2 * stride + 2 + nblk * G + 6 * ld + 1) & ~1;
+  return (2 * (ld - 1) * sqrt_ldm(ld) + 2 * stride + 2 + nblk * G + 7 * ld + 1) & ~1;
 }
 __host__ __device__ inline int fold0s_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  return ((ld - 1) * sqrt_ldm(ld) + 2 * (ld - 1) * ld + 2 * stride + 2 + nblk * G + 5 * ld + 1) & ~1;
+  return ((ld - 1) * sqrt_ldm(ld) + 2 * (ld - 1) * ld + 2 * stride + 2 + nblk * G + 8 * ld + 1) & ~1;
 }
 
 // One reflection of tria, columns c0..m-1 of the reflector's row rj and of the lane's own row ri.  The loops are
@@ -50,7 +51,7 @@ __device__ __forceinline__ void hh_dots(const double* rj, const double* ri, int 
     if (act) d0 = fma(ri[c], u0, d0);
   }
   ss += s0 + s1;
-  dd = d0 + d1;
+  dd += d0 + d1;
 }
 __device__ __forceinline__ void hh_axpy(const double* rj, double* ri, int c0, int m, double ws) {
   int c = c0;
@@ -87,8 +88,12 @@ __device__ __forceinline__ void col_axpy(double* col, int st, const double* v, i
 
 // L L^T = M M^T in place: M = n rows x m columns at row stride LDM; on return the lower triangle of the first n
 // columns holds L and the rest of those columns is zero.  All lanes of the group call it.
+// e1t / g1t (optional): row j of M is known to be zero outside the columns [0, e1t[j]) and [n, g1t[j]), with both
+// bounds non-decreasing in j (the stacked matrix [F S | G] of a predict step with S lower triangular: F is block
+// diagonal over the components plus the dense integral rows, G has one group of columns per block); the reflections
+// then touch those columns only, and the nesting of the supports keeps every later row inside its own.
 template <int G, int LDM>
-__device__ __forceinline__ void tria_rows(const Grp<G>& g, int n, int m, double* Mx) {
+__device__ __forceinline__ void tria_rows(const Grp<G>& g, int n, int m, double* Mx, const short* e1t = nullptr, const short* g1t = nullptr) {
   const int i = g.gl;
   double* ri = Mx + (i < n ? i : 0) * LDM;
   for (int j = 0; j < n; ++j) {
@@ -96,7 +101,9 @@ __device__ __forceinline__ void tria_rows(const Grp<G>& g, int n, int m, double*
     const bool act = (i > j) && (i < n);
     const double u0 = rj[j];
     double ss = u0 * u0, dd = 0.0;
-    hh_dots(rj, ri, j + 1, m, act, ss, dd);
+    const int c1 = e1t ? (int)e1t[j] : m, c2 = e1t ? (int)g1t[j] : m;
+    hh_dots(rj, ri, j + 1, c1, act, ss, dd);
+    if (e1t) hh_dots(rj, ri, n, c2, act, ss, dd);
     const double sig = sqrt(ss);
     double alpha = 0.0;
     if (sig > 0.0) { // the same for every lane
@@ -107,7 +114,8 @@ __device__ __forceinline__ void tria_rows(const Grp<G>& g, int n, int m, double*
       if (act) {
         const double w = beta * fma(ri[j], v0, dd * rsig);
         ri[j] = fma(-w, v0, ri[j]);
-        hh_axpy(rj, ri, j + 1, m, w * rsig);
+        hh_axpy(rj, ri, j + 1, c1, w * rsig);
+        if (e1t) hh_axpy(rj, ri, n, c2, w * rsig);
       }
     }
     g.sync();
@@ -116,6 +124,71 @@ __device__ __forceinline__ void tria_rows(const Grp<G>& g, int n, int m, double*
   if (i < n)
     for (int c = i + 1; c < n; ++c) ri[c] = 0.0;
   g.sync();
+}
+
+// supports of the rows of [F S | G] for a lower-triangular S (see tria_rows): row j of block b is zero outside
+// [0, off_b + d_b) and [n, n + off_b + b + d_b + 1) -- its own and the earlier blocks' columns of G; integral rows are full
+template <int G>
+__device__ __forceinline__ void sq_tables(const Grp<G>& g, const Tab& T, short* e1t, short* g1t) {
+  const int n = TN, d = TD;
+  for (int j = g.gl; j < n; j += G) {
+    if (j < d) { const int b = T.blk_of[j]; e1t[j] = (short)(TBOFF(b) + TBDIM(b)); g1t[j] = (short)(n + TBOFF(b) + b + TBDIM(b) + 1); }
+    else { e1t[j] = (short)n; g1t[j] = (short)(n + d + TNB); }
+  }
+  g.sync();
+}
+// row i of G (columns n..): cleared over the row's support, then its own entries -- row-owned, no other lane writes it.
+// x row of block b: row (i - off_b) of L_xx in the block's columns; integral row p: c_pb (L_zx | L_zz) for every block.
+__device__ __forceinline__ void sq_fill_G_row(const Tab& T, const double* rec, unsigned tz, int i, double* ri, int g1) {
+  const int n = TN, d = TD, nblk = TNB;
+  for (int c = n; c < g1; ++c) ri[c] = 0.0;
+  if (i < d) {
+    const int b = T.blk_of[i], db = TBDIM(b), off = TBOFF(b), lr = i - off;
+    const double* r = rec + TROFF(b) + db * db + db + lr * db;
+    double* o = ri + n + off + b;
+    for (int l = 0; l <= lr; ++l) o[l] = r[l];
+  } else if (!((tz >> (i - d)) & 1u)) {
+    const int p = i - d;
+    for (int b = 0; b < nblk; ++b) {
+      const double c = TCZ(p * nblk + b);
+      if (c == 0.0) continue;
+      const int db = TBDIM(b);
+      const double* r = rec + TROFF(b) + 2 * db * db + db;
+      double* o = ri + n + TBOFF(b) + b;
+      for (int l = 0; l <= db; ++l) o[l] = c * r[l];
+    }
+  }
+}
+// Scalar measurement update of a LOWER-TRIANGULAR factor that keeps it lower triangular (Carlson's form, columns
+// taken from the last to the first): with f = S^T h, alpha_j = r + sum_{c > j} f_c^2,
+//   S+[:, j] = sqrt(alpha_j / alpha'_j) S[:, j] - f_j / sqrt(alpha_j alpha'_j) e_j,   alpha'_j = alpha_j + f_j^2,
+//   e_j = sum_{c > j} S[:, c] f_c;   at the end alpha' = s = h^T P h + r and e = P h.
+// Row-owned (lane i updates row i, entries 0..i); the scalars are computed one column per lane first (bt, gm: n each).
+// Returns s; a = (P h)_i.  Nothing is subtracted from a covariance.
+template <int G>
+__device__ __forceinline__ double carlson_rows(const Grp<G>& g, int n, double* ri, const double* f, double r, double* bt, double* gm, double& a) {
+  const int i = g.gl;
+  double tot = r;
+  if (i < n) {
+    double al = r;
+    for (int c = n - 1; c > i; --c) al = fma(f[c], f[c], al);
+    const double fi = f[i], al2 = fma(fi, fi, al);
+    const double q = 1.0 / al2;
+    bt[i] = sqrt(al * q);
+    gm[i] = fi * q * sqrt(al2 / al);
+  }
+  for (int c = 0; c < n; ++c) tot = fma(f[c], f[c], tot);
+  g.sync();
+  double e = 0.0;
+  if (i < n) {
+    for (int j = i; j >= 0; --j) {
+      const double x = ri[j];
+      ri[j] = fma(bt[j], x, -gm[j] * e);
+      e = fma(x, f[j], e);
+    }
+  }
+  a = e;
+  return tot;
 }
 
 // lower Cholesky factor of a positive SEMI-definite n x n matrix A (element (i, j) at A[i * lda + j]) into the first n
@@ -165,6 +238,8 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
   double* kv = pv + LD;
   double* bv = kv + LD;
   double* av = bv + LD;
+  short* e1t = (short*)(av + LD);          // supports of the rows of [F S | G] (sq_tables)
+  short* g1t = e1t + 2 * LD;
   const int ks = kbuf_stride(n);
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
@@ -179,7 +254,7 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
   rs.issue(g, P.disc + k0 * (int64_t)TSTRIDE, 0);
   zero_fill(g, Mx, NR * LDM);
   zero_fill(g, mv, 5 * LD);
-  g.sync();
+  sq_tables(g, T, e1t, g1t);
   if (P.PRE1) { // the chunk's prefix state [m | S] from the dense levels
     const double* sp = P.PRE1 + gid * (int64_t)state_size(n);
     for (int c = i; c <= n; c += G)
@@ -187,6 +262,9 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
     g.sync();
   } else chol_psd_rows<G, LDM>(g, n, P.p0, n, Mx); // S0 S0^T = blkdiag(Pinf, 0)  (Eq. 3.19, reading R6)
   double ll = 0.0;
+#ifdef SG_SQ_CLK
+  long long c_prev = clock64();
+#endif
   // ---- forward: square-root Kalman filter ----
   uint32_t meta_nx = P.meta[k0];
   int32_t ob_nx = P.obs[k0];
@@ -204,24 +282,26 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
     if (!kind) { dl_r = P.delta[k]; sg_r = P.sigma[ob]; y_r = P.y[series * P.N + ob]; }
     // [F S | G]: lane c applies F to column c of S in place (a block is read before it is written, the z rows
     // last), lane n to the mean; then the lanes write G's columns
+#ifdef SG_SQ_CLK
+    const long long c_0 = clock64();
+#endif
     if (i < n) apply_F<G, LDM, LDM>(T, rec, tz, Mx + i, Mx + i, U);
     else if (i == n) apply_F<G, 1, 1>(T, rec, tz, mv, mv, U);
-    for (int cg = i; cg < nq; cg += G) {
-      double* col = Mx + n + cg;
-      for (int r = 0; r < n; ++r) col[r * LDM] = 0.0;
-      for (int b = 0; b < nblk; ++b) {
-        const int db = TBDIM(b), off = TBOFF(b), l = cg - off - b; // block b owns columns off + b .. off + b + db
-        if (l < 0 || l > db) continue;
-        const double* r = rec + TROFF(b);
-        if (l < db)
-          for (int r2 = l; r2 < db; ++r2) col[(off + r2) * LDM] = r[db * db + db + r2 * db + l]; // L_xx
-        const double lz = r[2 * db * db + db + l];                                               // L_zx[l], or L_zz at l = db
-        for (int p = 0; p < TNI; ++p)
-          if (!((tz >> p) & 1u)) col[(d + p) * LDM] = TCZ(p * nblk + b) * lz;
-      }
-    }
+#ifdef SG_SQ_CLK
+    const long long c_1 = clock64();
+#endif
+    g.sync(); // F S complete: the rows are written next
+    if (i < n) sq_fill_G_row(T, rec, tz, i, ri, g1t[i]);
     g.sync();
-    tria_rows<G, LDM>(g, n, n + nq, Mx);
+#ifdef SG_SQ_CLK
+    const long long c_2 = clock64();
+#endif
+    tria_rows<G, LDM>(g, n, n + nq, Mx, e1t, g1t);
+#ifdef SG_SQ_CLK
+    const long long c_3 = clock64();
+    if (gid == 0 && i == 0 && (k - k0) == 20) printf("down0_sqrt fwd event: applyF %lld  Gfill %lld  tria %lld  (prev event total %lld)\n", c_1 - c_0, c_2 - c_1, c_3 - c_2, c_0 - c_prev);
+    c_prev = c_0;
+#endif
     if (!kind) {
       const int zi = d + q;
       const double hs = TTAU(q) / dl_r;
@@ -229,18 +309,15 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
       const double yy = y_r * ramp;
       if (i < n) pv[i] = hs * Mx[zi * LDM + i]; // phi = S^T h
       g.sync();
-      double ss = 0.0, a = 0.0;
-      hh_dots(pv, ri, 0, n, i < n, ss, a); // ss = |phi|^2, a = (S phi)_i = (P h)_i
-      const double S = ss + sg * sg;
       const double v = yy - hs * mv[zi];
       if (!(sg_r > 0.0) || !isfinite(sg_r)) atomicOr(P.flags, NUMF_SIGMA);
+      double a = 0.0;
+      const double S = (sg > 0.0) ? carlson_rows(g, n, ri, pv, sg * sg, av, bv, a) : 0.0; // S stays lower triangular; a = (P h)_i
       if (!(S > 0.0) || !isfinite(S) || !isfinite(v)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S;
       ll -= 0.5 * (log(6.283185307179586476925286766559 * S) + v * v * rS);
-      const double gam = 1.0 / (S + sqrt(sg * sg * S));
-      g.sync(); // every lane has read m_z
+      g.sync(); // every lane has read m_z; the rows are updated
       if (i < n) {
-        hh_axpy(pv, ri, 0, n, gam * a);
         mv[i] = fma(a * rS, v, mv[i]);
         kv[i] = a * rS;
       }
@@ -396,6 +473,10 @@ __device__ __forceinline__ void fold0_sqrt_body(const ScanDev& P) {
   double* pv = ev + LD;
   double* cv = pv + LD;
   double* av = cv + LD;                    // n + 1
+  double* bt = av + LD;                    // scalars of the triangular update (carlson_rows)
+  double* gm = bt + LD;
+  short* e1t = (short*)(gm + LD);
+  short* g1t = e1t + 2 * LD;
   const int64_t series = gid / P.c1, chunk = gid - series * P.c1;
   const int64_t k0 = chunk * P.Lc, k1 = (k0 + P.Lc < P.K) ? k0 + P.Lc : P.K;
   const double ramp = P.amp ? 1.0 / P.amp[series] : 1.0;
@@ -406,8 +487,8 @@ __device__ __forceinline__ void fold0_sqrt_body(const ScanDev& P) {
   rs.init(g, recs, TSTRIDE);
   rs.issue(g, P.disc + k0 * (int64_t)TSTRIDE, 0);
   zero_fill(g, Mx, NR * LDM + 2 * NR * ld);
-  zero_fill(g, ev, 4 * LD);
-  g.sync();
+  zero_fill(g, ev, 6 * LD);
+  sq_tables(g, T, e1t, g1t);
   for (int r = i; r < n; r += G) AB[r * ld + r] = 1.0;
   g.sync();
   uint32_t meta_nx = P.meta[k0];
@@ -427,22 +508,10 @@ __device__ __forceinline__ void fold0_sqrt_body(const ScanDev& P) {
     // [A | b] <- F [A | b];  U <- tria([F U | G])
     if (i <= n) apply_F<G, LD, LD>(T, rec, tz, AB + i, AB + i, U);
     if (i < n) apply_F<G, LDM, LDM>(T, rec, tz, Mx + i, Mx + i, U);
-    for (int cg = i; cg < nq; cg += G) {
-      double* col = Mx + n + cg;
-      for (int r = 0; r < n; ++r) col[r * LDM] = 0.0;
-      for (int b = 0; b < nblk; ++b) {
-        const int db = TBDIM(b), off = TBOFF(b), l = cg - off - b;
-        if (l < 0 || l > db) continue;
-        const double* r = rec + TROFF(b);
-        if (l < db)
-          for (int r2 = l; r2 < db; ++r2) col[(off + r2) * LDM] = r[db * db + db + r2 * db + l];
-        const double lz = r[2 * db * db + db + l];
-        for (int p = 0; p < TNI; ++p)
-          if (!((tz >> p) & 1u)) col[(d + p) * LDM] = TCZ(p * nblk + b) * lz;
-      }
-    }
+    g.sync(); // F U complete: the rows are written next
+    if (i < n) sq_fill_G_row(T, rec, tz, i, ri, g1t[i]);
     g.sync();
-    tria_rows<G, LDM>(g, n, n + nq, Mx);
+    tria_rows<G, LDM>(g, n, n + nq, Mx, e1t, g1t);
     if (!kind) {
       // fold the end event's primitive element onto the aggregate (SG21 Eq. 10, rank-one J_j: fold0_body), in factors
       const int zi = d + q;
@@ -452,15 +521,12 @@ __device__ __forceinline__ void fold0_sqrt_body(const ScanDev& P) {
       if (i < n) pv[i] = hs * Mx[zi * LDM + i];       // phi = U^T h
       if (i <= n) av[i] = hs * AB[zi * ld + i];       // a = A^T h (entry n: h . b)
       g.sync();
-      double ss = 0.0, a = 0.0;
-      hh_dots(pv, ri, 0, n, i < n, ss, a);
-      const double S = ss + sg * sg;
+      double a = 0.0;
+      const double S = (sg > 0.0) ? carlson_rows(g, n, ri, pv, sg * sg, bt, gm, a) : 0.0; // C -= c c^T / s on the factor, kept lower triangular
       if (!(S > 0.0) || !isfinite(S)) atomicOr(P.flags, NUMF_BAD);
       const double rS = 1.0 / S, resid = yy - av[n];
-      const double gam = 1.0 / (S + sqrt(sg * sg * S));
       if (i < n) {
         cv[i] = a;                                    // c = C h
-        hh_axpy(pv, ri, 0, n, gam * a);                // Potter: C -= c c^T / s
         ev[i] = fma(av[i], resid * rS, ev[i]);        // eta += a resid / s
         Bx[i * ld + n] = av[i] * sqrt(rS);            // J += a a^T / s
       }
