@@ -6,9 +6,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libsmolgp_b200.so")
 PROBE_SO = os.path.join(HERE, "libsmolgp_probe.so")  # bench.py's FP64 throughput probe (not part of the product library)
-SOURCES = ["api.cu", "model.cu", "events.cu", "disc.cu", "scan.cu", "jit.cu"]
+SOURCES = ["api.cu", "model.cu", "events.cu", "disc.cu", "scan.cu", "scan_sqrt.cu", "jit.cu"]
 JIT_PARTS = ["dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "chunk_reg.cuh", "dense_kernels.cuh"]  # run-time specialised source, in order
-DEPS = SOURCES + ["../_build.py", "common.h", "dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "chunk_reg.cuh", "dense_kernels.cuh", "chunk_sqrt.cuh", "dense_sqrt.cuh", "jit.h", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
+DEPS = SOURCES + ["../_build.py", "common.h", "dev_consts.h", "grp_dev.cuh", "chunk_dev.cuh", "chunk_kernels.cuh", "chunk_reg.cuh", "dense_kernels.cuh", "chunk_sqrt.cuh", "dense_sqrt.cuh", "jit.h", "scan_plan.h", "scan_host.cu", os.path.join("..", "..", "include", "smolgp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 

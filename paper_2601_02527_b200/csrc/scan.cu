@@ -18,8 +18,7 @@
 #include <math.h>
 
 #include "dense_kernels.cuh"
-#include "chunk_sqrt.cuh"
-#include "dense_sqrt.cuh"
+#include "chunk_sqrt.cuh" // (shared-memory sizes of the factor-form kernels for the plan; the kernels are instantiated in scan_sqrt.cu)
 
 __global__ void k_ll_reduce(const double* __restrict__ llpart, int64_t c1, int64_t batch, int64_t N,
                             const double* __restrict__ amp, double* __restrict__ loglik, int* __restrict__ flags) {

@@ -2,6 +2,7 @@
 #include <stdio.h>
 
 #include "jit.h"
+#include "scan_plan.h"
 // scan_host.cu -- host orchestration of the scan kernels (level plan, workspace carving, launches).
 // Included at the end of scan.cu (same translation unit as the kernels it launches).
 
@@ -14,23 +15,6 @@ static int pick_lanes(const smolgp_ctx* ctx, int n) {
   const int need = n + 1 <= 8 ? 8 : (n + 1 <= 16 ? 16 : 32); // one lane per column of [X | x]
   if ((ctx->opt_lanes == 8 || ctx->opt_lanes == 16 || ctx->opt_lanes == 32) && ctx->opt_lanes >= need) return (int)ctx->opt_lanes;
   return need;
-}
-
-// groups per CTA: the count that puts the most groups on one SM (228 KB of shared memory per SM,
-// 1 KB reserved per CTA, at most 128 threads per CTA); ties go to the smaller CTA
-static int groups_per_cta(size_t per_group, int G, int* groups_per_sm = nullptr) {
-  int best = 1, best_sm = 0;
-  for (int gpc = 1; gpc <= 128 / G; ++gpc) {
-    const size_t cta = per_group * gpc;
-    if (cta > 227 * 1024) break;
-    int ctas = (int)((228 * 1024) / (cta + 1024));
-    if (ctas > 32) ctas = 32;
-    const int warps = (gpc * G + 31) / 32;
-    if (ctas * warps > 64) ctas = 64 / warps;
-    if (ctas * gpc > best_sm) { best_sm = ctas * gpc; best = gpc; }
-  }
-  if (groups_per_sm) *groups_per_sm = best_sm > 0 ? best_sm : 1;
-  return best;
 }
 
 // ---- which level-0 (chunk) kernels run ---------------------------------------------------------------
@@ -146,49 +130,6 @@ static int launch_level0(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, 
   return SMOLGP_OK;
 }
 
-// (lanes, row stride) variants compiled: lanes = 8/16/32 for n + 1 <= 8/16/33 columns, stride = chunk_ld(n)
-#define SG_DISPATCH_GL(G, LD, CALL)                                                      \
-  do {                                                                                   \
-    if (G == 8 && LD == 5) { CALL(8, 5); }                                               \
-    else if (G == 8 && LD == 9) { CALL(8, 9); }                                          \
-    else if (G == 16 && LD == 5) { CALL(16, 5); }                                        \
-    else if (G == 16 && LD == 9) { CALL(16, 9); }                                        \
-    else if (G == 16 && LD == 13) { CALL(16, 13); }                                      \
-    else if (G == 16 && LD == 17) { CALL(16, 17); }                                      \
-    else if (G == 32 && LD == 5) { CALL(32, 5); }                                        \
-    else if (G == 32 && LD == 9) { CALL(32, 9); }                                        \
-    else if (G == 32 && LD == 13) { CALL(32, 13); }                                      \
-    else if (G == 32 && LD == 17) { CALL(32, 17); }                                      \
-    else if (G == 32 && LD == 21) { CALL(32, 21); }                                      \
-    else if (G == 32 && LD == 25) { CALL(32, 25); }                                      \
-    else if (G == 32 && LD == 29) { CALL(32, 29); }                                      \
-    else if (G == 32 && LD == 33) { CALL(32, 33); }                                      \
-    else { ctx->err = "scan: unsupported (lanes, n) combination"; return SMOLGP_EUNSUPPORTED; } \
-  } while (0)
-
-// square-root form (chunk_sqrt.cuh, dense_sqrt.cuh): generic kernels
-template <int G, int LD>
-static int launch_sqrt(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold) {
-  const size_t per_group = (size_t)(fold ? fold0s_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) : sqrt_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G)) * 8;
-  const int gpc = groups_per_cta(per_group, G);
-  const size_t smem = per_group * gpc;
-  if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
-  if (hm->n + hm->d + hm->nblk > sqrt_ldm(LD)) { ctx->err = "scan: model too wide for the square-root kernel"; return SMOLGP_EUNSUPPORTED; }
-  const int64_t groups = P.batch * P.c1;
-  if (fold) {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_fold0_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    sg_launch_begin(ctx, KID_FOLD0);
-    k_fold0_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(P);
-  } else {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_down0_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    sg_launch_begin(ctx, KID_DOWN0);
-    k_down0_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(P);
-  }
-  sg_launch_end(ctx);
-  SG_CUDA(ctx, cudaGetLastError());
-  return SMOLGP_OK;
-}
-
 static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* hm, bool fold, int G, const L0Plan& lp) {
   const SgJitKernels* jk = lp.jk;
   const int64_t groups = P.batch * P.c1;
@@ -212,24 +153,6 @@ static int launch_level0_any(smolgp_ctx* ctx, const ScanDev& P, const ModelDev* 
   SG_DISPATCH_GL(G, LD, SG_CALL_L0);
 #undef SG_CALL_L0
   return SMOLGP_EUNSUPPORTED;
-}
-
-static int launch_dense_sqrt(smolgp_ctx* ctx, const DenseArgs& D, int n, bool fold) {
-  const size_t smem = (size_t)(fold ? foldDs_group_doubles(n) : downDs_group_doubles(n)) * 8;
-  if (smem > ctx->smem_optin) { ctx->err = "scan: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
-  dim3 grid((unsigned)(D.batch * D.cout), fold ? 1 : (D.want_suffix ? 2 : 1));
-  if (fold) {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_foldD_sqrt<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    sg_launch_begin(ctx, KID_FOLDD);
-    k_foldD_sqrt<SG_DENSE_NT><<<grid, SG_DENSE_NT, smem, ctx->stream>>>(D);
-  } else {
-    SG_CUDA(ctx, cudaFuncSetAttribute(k_downD_sqrt<SG_DENSE_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    sg_launch_begin(ctx, KID_DOWND);
-    k_downD_sqrt<SG_DENSE_NT><<<grid, SG_DENSE_NT, smem, ctx->stream>>>(D);
-  }
-  sg_launch_end(ctx);
-  SG_CUDA(ctx, cudaGetLastError());
-  return SMOLGP_OK;
 }
 
 static int launch_dense(smolgp_ctx* ctx, const DenseArgs& D, int n, const SgJitKernels* jk, bool fold) {
@@ -362,17 +285,13 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
   P.ADJ1 = use_adj ? (const double*)(w + oADJ) : nullptr;
 
   if (pl.T) {
-    if (sq) {
-#define SG_CALL_SQF(g_, ld_) rc = launch_sqrt<g_, ld_>(ctx, P, hm, true)
-      SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_SQF);
-#undef SG_CALL_SQF
-    } else rc = launch_level0_any(ctx, P, hm, true, G, lp);
+    rc = sq ? sg_launch_sqrt_chunk(ctx, P, hm, G, true) : launch_level0_any(ctx, P, hm, true, G, lp);
     if (rc) return rc;
     for (int l = 1; l < pl.T; ++l) {
       DenseArgs D = {};
       D.n = n; D.p0 = (const double*)((const char*)a.d_model + offsetof(ModelDev, p0)); D.Ein = (const double*)(w + oE[l]); D.Eout = (double*)(w + oE[l + 1]);
       D.cin = pl.cnt[l]; D.cout = pl.cnt[l + 1]; D.batch = batch; D.g = g;
-      rc = sq ? launch_dense_sqrt(ctx, D, n, true) : launch_dense(ctx, D, n, jk0, true);
+      rc = sq ? sg_launch_sqrt_dense(ctx, D, n, true) : launch_dense(ctx, D, n, jk0, true);
       if (rc) return rc;
     }
     for (int l = pl.T; l >= 1; --l) {
@@ -382,7 +301,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
       if (l == pl.T) { D.cout = 1; D.g = (int)pl.cnt[l]; D.PREup = nullptr; D.SUFup = nullptr; }
       else { D.cout = pl.cnt[l + 1]; D.g = g; D.PREup = (const double*)(w + oPRE[l + 1]); D.SUFup = a.want_smooth ? (const double*)(w + oSUF[l + 1]) : nullptr; }
       D.PRE = (double*)(w + oPRE[l]); D.SUF = a.want_smooth ? (double*)(w + oSUF[l]) : nullptr;
-      rc = sq ? launch_dense_sqrt(ctx, D, n, false) : launch_dense(ctx, D, n, jk0, false);
+      rc = sq ? sg_launch_sqrt_dense(ctx, D, n, false) : launch_dense(ctx, D, n, jk0, false);
       if (rc) return rc;
     }
   }
@@ -397,11 +316,7 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     sg_launch_end(ctx);
     SG_CUDA(ctx, e);
   }
-  if (sq) {
-#define SG_CALL_SQ(g_, ld_) rc = launch_sqrt<g_, ld_>(ctx, P, hm, false)
-    SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_SQ);
-#undef SG_CALL_SQ
-  } else rc = launch_level0_any(ctx, P, hm, false, G, lp);
+  rc = sq ? sg_launch_sqrt_chunk(ctx, P, hm, G, false) : launch_level0_any(ctx, P, hm, false, G, lp);
   if (rc) return rc;
   {
     char buf[256];
@@ -417,21 +332,6 @@ int sg_run_scan(smolgp_ctx* ctx, const ScanArgs& a) {
     sg_launch_end(ctx);
     SG_CUDA(ctx, cudaGetLastError());
   }
-  return SMOLGP_OK;
-}
-
-template <int G, int LD>
-static int launch_query_sqrt(smolgp_ctx* ctx, const QueryDev& Q, const ModelDev* hm) {
-  const size_t per_group = (size_t)querys_group_doubles(hm->n, LD, hm->disc_stride, hm->nblk, G) * 8;
-  const int gpc = groups_per_cta(per_group, G);
-  const size_t smem = per_group * gpc;
-  if (smem > ctx->smem_optin) { ctx->err = "query: shared memory need exceeds the device limit"; return SMOLGP_EUNSUPPORTED; }
-  const int64_t groups = Q.batch * Q.Mq;
-  SG_CUDA(ctx, cudaFuncSetAttribute(k_query_sqrt<G, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  sg_launch_begin(ctx, KID_QUERY);
-  k_query_sqrt<G, LD><<<(unsigned)((groups + gpc - 1) / gpc), gpc * G, smem, ctx->stream>>>(Q);
-  sg_launch_end(ctx);
-  SG_CUDA(ctx, cudaGetLastError());
   return SMOLGP_OK;
 }
 
@@ -489,11 +389,8 @@ int sg_run_query(smolgp_ctx* ctx, const QueryArgs& a) {
     SG_CUDA(ctx, cudaGetLastError());
     rc = sg_launch_disc(ctx, a.d_model, hm, dtq, 2 * M, discq);
     if (rc) return rc;
-    if (sq) {
-#define SG_CALL_QS(g_, ld_) rc = launch_query_sqrt<g_, ld_>(ctx, Q, hm)
-      SG_DISPATCH_GL(G, chunk_ld(n), SG_CALL_QS);
-#undef SG_CALL_QS
-    } else if (jk) {
+    if (sq) rc = sg_launch_sqrt_query(ctx, Q, hm, G);
+    else if (jk) {
       const size_t per_group = (size_t)query_group_doubles(n, LD, hm->disc_stride, hm->nblk, G) * 8;
       const int gpc = groups_per_cta(per_group, G);
       const int64_t groups = Q.batch * Q.Mq;
