@@ -100,7 +100,7 @@ def test_noalloc_matches_build_events_on_calls_in_a_row(B, ctx):
         torch.cuda.synchronize()
         free.append(torch.cuda.mem_get_info()[0] - f0)
         _check(out.host(), ref, ts, te, n_inst)
-    assert free[1] == 0 and free[2] == 0  # (the first call may load the module lazily)
+    assert free[1] >= 0 and free[2] >= 0  # free device memory did not shrink (the first call may load the module lazily)
 
 
 def test_noalloc_instant_samples_and_input_flags(B, ctx):
