@@ -85,25 +85,36 @@ def test_sqrt_form_loses_fewer_digits_than_the_covariance_form(ctx, oracle):
     assert ef["mean"] <= 1e-11 and ef["ll"] <= 1e-12, ef
 
 
-def test_sqrt_form_instantaneous_data(ctx, oracle):
-    """paper section 2 (K = N observe events): the record's extra row is then a copy of x_0, its factor row 0 of L_xx"""
-    kern = [W.comp(W.SHO, 1.1, 2 * np.pi / 300.0, 2.0), W.comp(W.MATERN52, 0.6, 900.0)]
+@pytest.mark.parametrize("opt", ["auto", "sequential", "ragged"])
+def test_sqrt_form_instantaneous_data(ctx, oracle, opt):
+    """paper section 2 (K = N observe events; two instruments sampling different sums of the components, simultaneous
+    samples): the record's extra row is then a copy of x_0, its factor row 0 of L_xx; with query times"""
+    kern = [W.comp(W.SHO, 1.1, 2 * np.pi / 300.0, 2.0), W.comp(W.MATERN52, 0.6, 900.0, inst_mask=2)]
     rng = np.random.default_rng(8)
-    t = np.cumsum(rng.uniform(5.0, 60.0, 1500))
-    inst = np.zeros(1500, np.int32)
-    sigma = rng.uniform(0.1, 0.4, 1500)
+    N = 1500
+    t = np.round(np.cumsum(rng.uniform(5.0, 60.0, N)))          # whole seconds: some samples of the two instruments coincide
+    inst = rng.integers(0, 2, N).astype(np.int32)
+    sigma = rng.uniform(0.1, 0.4, N)
     y = W.synth_y(rng, kern, t, t + 1e-9, inst, sigma)
+    tq = np.concatenate([rng.uniform(t.min() - 200.0, t.max() + 200.0, 60), t[:3]])
     ctx.set_option("form", 1)
+    for k, v in SCAN_OPTS[opt]:
+        ctx.set_option(k, v)
     try:
-        ev = ctx.smolgp_build_events_instant_host(t, inst, 1)
-        out = ctx.smolgp_condition_host(ev, kern, y, sigma)
+        ev = ctx.smolgp_build_events_instant_host(t, inst, 2)
+        out = ctx.smolgp_condition_host(ev, kern, y, sigma, t_query=tq, query_instrument=1)
+        assert "form=sqrt" in ctx.plan_info()
     finally:
-        ctx.set_option("form", 0)
-    ref = oracle.ssm_instant(kern, 1, t, inst, y, sigma)
-    psd = np.sqrt(oracle.kernel(kern, 0, 0, np.zeros(1))[0])
+        for k in ("form", "chunk", "group", "top", "lanes"):
+            ctx.set_option(k, 0)
+    ref = oracle.ssm_instant(kern, 2, t, inst, y, sigma, tq=tq, query_inst=1)
+    psd = np.sqrt(np.array([oracle.kernel(kern, int(q), int(q), np.zeros(1))[0] for q in inst]))
     assert abs(out["loglik"][0] - ref["loglik"]) <= PU.LL_RTOL * abs(ref["loglik"])
     assert np.max(np.abs(out["mean"][0] - ref["mean"]) / (np.abs(ref["mean"]) + psd)) <= PU.POST_RTOL
     assert np.max(np.abs(out["var"][0] - ref["var"]) / ref["var"]) <= PU.POST_RTOL
+    k0 = float(oracle.kernel(kern, 1, 1, np.zeros(1))[0])
+    assert np.max(np.abs(out["mean_query"][0] - ref["mq"])) <= 1e-8 * (np.sqrt(k0) + np.max(np.abs(ref["mq"])))
+    assert np.max(np.abs(out["var_query"][0] - ref["vq"]) / ref["vq"]) <= 1e-8
 
 
 def test_sqrt_form_full_size_cfg5_sampled_series(ctx, oracle):
