@@ -17,7 +17,7 @@
 // reduction; reflectors are applied in the scale-free form v / |u| (information factors span hundreds of orders).
 // Generic (statically compiled) kernels, matrices in shared memory; one group of lanes per chunk.
 // Chunked scan: k_fold0_sqrt folds a chunk into ONE element (A, b, U, eta, Z) with C = U U^T, J = Z Z^T (the recursion of
-// fold0_body with C -> U by tria / Potter and J += a a^T / s as Z <- tria([Z | a / sqrt s])); the dense levels combine
+// fold0_body with C -> U by tria and the triangular update, J += a a^T / s as Z <- tria([Z | a / sqrt s])); the dense levels combine
 // such elements in factor form (dense_sqrt.cuh); k_down0_sqrt starts from the chunk's prefix state [m | S] and from the
 // chunk-end adjoint  W = Z T'^-T,  T' T'^T = I + (S^T Z)^T (S^T Z),  of the suffix information [eta | Z].
 #pragma once
