@@ -246,7 +246,7 @@ __device__ __forceinline__ void down0_sqrt_body(const ScanDev& P) {
   const double ampv = P.amp ? P.amp[series] : 1.0;
   const double ramp = 1.0 / ampv;
   if (!(ampv > 0.0) || !isfinite(ampv)) atomicOr(P.flags, NUMF_AMP);
-  const int i = g.gl;                      // the lane's row (tria, Potter update) and column (products with F)
+  const int i = g.gl;                      // the lane's row (tria, triangular update) and column (products with F)
   double* ri = Mx + (i < n ? i : 0) * LDM;
 
   RecStage rs;
