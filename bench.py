@@ -427,6 +427,8 @@ def run_predict(args, w, cfgname):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(0)
     ctx = B.Context(0)
+    if args.form == "sqrt":
+        ctx.set_option("form", 1)  # query-time prediction from stored factors
     N = w["t_start"].size
     batch = w["batch"] or 1
     n = model_dim(w)
