@@ -564,7 +564,7 @@ __global__ void __launch_bounds__(128) k_down0_sqrt(const __grid_constant__ Scan
 //   H_q m^ = h . m* - lambda* . p,   H_q P^ H_q^T = |S*^T h|^2 - |W*^T p|^2,   p = P* h = S* (S*^T h).
 // ---------------------------------------------------------------------------------------------------
 __host__ __device__ inline int querys_group_doubles(int n, int ld, int stride, int nblk, int G) {
-  return ((ld - 1) * sqrt_ldm(ld) + (ld - 1) * ld + 2 * stride + 2 + nblk * G + 5 * ld + 1) & ~1;
+  return ((ld - 1) * sqrt_ldm(ld) + (ld - 1) * ld + 2 * stride + 2 + nblk * G + 6 * ld + 1) & ~1;
 }
 
 template <int G, int LD>
@@ -588,6 +588,8 @@ __device__ __forceinline__ void query_sqrt_body(const QueryDev& P) {
   double* hv = lam + LD;
   double* t1 = hv + LD;
   double* ph = t1 + LD;
+  short* e1t = (short*)(ph + LD);
+  short* g1t = e1t + 2 * LD;
   const int ss = state_size(n);
   const int64_t series = gid / P.Mq, q = gid - series * P.Mq;
   const int64_t kp = P.kp[q];
@@ -601,7 +603,7 @@ __device__ __forceinline__ void query_sqrt_body(const QueryDev& P) {
   rs.issue(g, P.discq + (P.Mq + q) * (int64_t)TSTRIDE, 1);
   zero_fill(g, Mx, NR * LDM + NR * ld);
   zero_fill(g, mv, 5 * LD);
-  g.sync();
+  sq_tables(g, T, e1t, g1t);
   if (i == 0)
     for (int b = 0; b < TNB; ++b) hv[TBOFF(b)] = ((P.T.bmask[b] >> P.qinst) & 1u) ? P.T.bsig[b] : 0.0; // H of the queried (virtual) instrument
   rs.wait(0);
@@ -617,22 +619,10 @@ __device__ __forceinline__ void query_sqrt_body(const QueryDev& P) {
     const double* rec = recs;
     if (i < n) apply_F<G, LDM, LDM>(T, rec, idle, Mx + i, Mx + i, U);
     else if (i == n) apply_F<G, 1, 1>(T, rec, idle, mv, mv, U);
-    for (int cg = i; cg < nq; cg += G) {
-      double* col = Mx + n + cg;
-      for (int r = 0; r < n; ++r) col[r * LDM] = 0.0;
-      for (int b = 0; b < nblk; ++b) {
-        const int db = TBDIM(b), off = TBOFF(b), l = cg - off - b;
-        if (l < 0 || l > db) continue;
-        const double* r = rec + TROFF(b);
-        if (l < db)
-          for (int r2 = l; r2 < db; ++r2) col[(off + r2) * LDM] = r[db * db + db + r2 * db + l];
-        const double lz = r[2 * db * db + db + l];
-        for (int p = 0; p < TNI; ++p)
-          if (!((idle >> p) & 1u)) col[(d + p) * LDM] = TCZ(p * nblk + b) * lz;
-      }
-    }
+    g.sync(); // F S complete: the rows are written next (S from the state store is lower triangular)
+    if (i < n) sq_fill_G_row(T, rec, idle, i, ri, g1t[i]);
     g.sync();
-    tria_rows<G, LDM>(g, n, n + nq, Mx);
+    tria_rows<G, LDM>(g, n, n + nq, Mx, e1t, g1t);
   } else { // before the first event: the stationary prior, idle z = 0 (retrodiction, reading R8)
     chol_psd_rows<G, LDM>(g, n, P.p0, n, Mx);
   }
