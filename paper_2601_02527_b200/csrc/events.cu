@@ -20,7 +20,7 @@
 //   k_merge     after pass 0: when every (kind, instrument) run is already in time order -- exposures of an instrument
 //               given in time order, the usual case -- the stream is the merge of those runs, done by ranking in one
 //               launch; the eight time passes then return at once.  Otherwise they sort pass 0's output.
-// Twelve launches whatever N (round 1: 33), one small status read-back.
+// Twelve launches whatever N (round 1: 33), one small status read-back; up to 8192 events ONE launch (k_ev_small).
 #include <math.h>
 #include <stddef.h>
 #include <string.h>
@@ -402,6 +402,128 @@ __global__ void __launch_bounds__(RS_NT) k_ev_final(EvCtl* __restrict__ ctl, int
   }
 }
 
+// ---- small inputs: the whole build in ONE CTA ------------------------------------------------------------------
+// Up to EVS_MAX events (config 1: 2000) the twelve launches above cost more than the work: one CTA of 1024 threads
+// sorts the (time key, kind | instrument | exposure) pairs in shared memory (bitonic network on the composite key:
+// the same total order, so the same stream bit for bit), then gathers, scans the instrument bits and writes the
+// stream, flags and extents exactly as k_ev_init / k_ev_final do.
+#define EVS_MAX 8192
+#define EVS_NT 1024
+__global__ void __launch_bounds__(EVS_NT) k_ev_small(int64_t N, const double* __restrict__ ts, const double* __restrict__ te,
+                                                      const int32_t* __restrict__ inst, int n_inst, EvCtl* __restrict__ ctl,
+                                                      double* __restrict__ t, double* __restrict__ dt, double* __restrict__ delta,
+                                                      uint32_t* __restrict__ meta, int32_t* __restrict__ obs, int P) {
+  extern __shared__ unsigned long long sk[]; // [P] time keys, then [P] secondary keys (u32)
+  uint32_t* sv = reinterpret_cast<uint32_t*>(sk + P);
+  __shared__ uint32_t wx[32];
+  __shared__ unsigned long long smax[SG_MAXINST];
+  const int tid = threadIdx.x, NT = blockDim.x; // (1024; 256 threads with eight pairs each were measured: 68 us against 41 at K = 2000)
+  const bool instant = (te == nullptr);
+  const int K = (int)(instant ? N : 2 * N);
+  for (int e = tid; e < P; e += NT) { sk[e] = ~0ull; sv[e] = ~0u; }
+  if (tid < SG_MAXINST) smax[tid] = 0ull;
+  __syncthreads();
+  for (int i0 = 0; i0 < (int)N; i0 += NT) { // (whole warps stay in the loop: the reduction below uses shuffles)
+    const int i = i0 + tid;
+    unsigned long long dbits = 0ull; // bits of this exposure's length (0 for dead / invalid lanes)
+    int q = -1;
+    if (i < (int)N) {
+      const double s = ts[i], e = instant ? s : te[i];
+      int bad = 0;
+      q = inst[i];
+      if (!isfinite(s) || !isfinite(e) || (!instant && !(e > s))) bad |= EVF_BADTIME;
+      if (q < 0 || q >= n_inst) { bad |= EVF_BADINST; q = 0; }
+      if (bad) atomicOr(&ctl->flags, bad);
+      else if (!instant) dbits = (unsigned long long)__double_as_longlong(e - s); // positive doubles order like their bits
+      // secondary key: end (0) before start (1), then instrument, then exposure index -- the tie rule of the stream
+      sk[i] = time_key(e); sv[i] = ((uint32_t)q << 13) | (uint32_t)i;
+      if (!instant) { sk[N + i] = time_key(s); sv[N + i] = (1u << 18) | ((uint32_t)q << 13) | (uint32_t)i; }
+    }
+    for (int r = 0; r < n_inst; ++r) { // longest exposure per instrument: one shared-memory atomic per (warp, instrument)
+      unsigned long long m = (q == r) ? dbits : 0ull;
+      for (int o = 16; o; o >>= 1) { const unsigned long long y = __shfl_xor_sync(0xffffffffu, m, o); m = y > m ? y : m; }
+      if ((tid & 31) == 0 && m) atomicMax(&smax[r], m);
+    }
+  }
+  __syncthreads();
+  if (tid < n_inst) ctl->maxdelta[tid] = smax[tid];
+  // bitonic network.  A warp owns 64 consecutive positions (thread: positions 2 tid, 2 tid + 1 of each 2 NT-block), so
+  // every exchange at distance < 64 stays inside a warp: those run in registers with shuffles, and only the
+  // exchanges at distance >= 64 (15 of the 66 stages at P = 2048) go through shared memory and a barrier.
+  for (int k2 = 2; k2 <= P; k2 <<= 1) {
+    int j2 = k2 >> 1;
+    for (; j2 >= 64; j2 >>= 1) {
+      for (int e = tid; e < P; e += NT) {
+        const int x = e ^ j2;
+        if (x > e) {
+          const unsigned long long ka = sk[e], kb = sk[x];
+          const uint32_t va = sv[e], vb = sv[x];
+          const bool gt = (ka > kb) || (ka == kb && va > vb);
+          if (gt == ((e & k2) == 0)) { sk[e] = kb; sk[x] = ka; sv[e] = vb; sv[x] = va; }
+        }
+      }
+      __syncthreads();
+    }
+    for (int base = 0; base < P; base += 2 * NT) {
+      const int e0 = base + 2 * tid;
+      if (base + 2 * (tid & ~31) >= P) break; // this warp's 64 positions lie beyond the padded length (whole warps leave together)
+      unsigned long long k0r = sk[e0], k1r = sk[e0 + 1];
+      uint32_t v0r = sv[e0], v1r = sv[e0 + 1];
+      const bool up = (e0 & k2) == 0; // both positions share it: k2 >= 2
+      for (int j = j2; j >= 2; j >>= 1) { // partner position e ^ j: thread tid ^ (j / 2), same slot
+        const int lm = j >> 1;
+        const bool lower = (e0 & j) == 0;
+        const unsigned long long pk0 = __shfl_xor_sync(0xffffffffu, k0r, lm), pk1 = __shfl_xor_sync(0xffffffffu, k1r, lm);
+        const uint32_t pv0 = __shfl_xor_sync(0xffffffffu, v0r, lm), pv1 = __shfl_xor_sync(0xffffffffu, v1r, lm);
+        // the lower position keeps the smaller pair when ascending (up), the larger when descending; the upper one the other
+        const bool g0 = (k0r > pk0) || (k0r == pk0 && v0r > pv0), g1 = (k1r > pk1) || (k1r == pk1 && v1r > pv1);
+        if (g0 == (lower == up)) { k0r = pk0; v0r = pv0; }
+        if (g1 == (lower == up)) { k1r = pk1; v1r = pv1; }
+      }
+      if (j2 >= 1) { // distance 1: the thread's own two positions
+        const bool gt = (k0r > k1r) || (k0r == k1r && v0r > v1r);
+        if (gt == up) { const unsigned long long tk = k0r; k0r = k1r; k1r = tk; const uint32_t tv = v0r; v0r = v1r; v1r = tv; }
+      }
+      sk[e0] = k0r; sk[e0 + 1] = k1r; sv[e0] = v0r; sv[e0 + 1] = v1r;
+    }
+    __syncthreads();
+  }
+  // gather + inclusive XOR scan of the instrument bits (a thread holds `per` consecutive events)
+  const int per = (K + NT - 1) / NT, k0 = tid * per, k1 = (k0 + per < K) ? k0 + per : K;
+  uint32_t x = 0;
+  if (!instant)
+    for (int k = k0; k < k1; ++k) x ^= 1u << ((sv[k] >> 13) & 31u);
+  const int lane = tid & 31, w = tid >> 5;
+  uint32_t incl = x;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl ^= y; }
+  if (lane == 31) wx[w] = incl;
+  __syncthreads();
+  uint32_t pre = 0;
+  for (int ww = 0; ww < w; ++ww) pre ^= wx[ww];
+  uint32_t after = pre ^ incl ^ x; // open set before this thread's first event
+  const uint32_t all = (n_inst >= 32) ? 0xffffffffu : ((1u << n_inst) - 1u);
+  double tprev = 0.0;
+  if (k0 > 0 && k0 < K) { const uint32_t u = sv[k0 - 1]; const int ip = (int)(u & 0x1fffu); tprev = (((u >> 18) & 1u) || instant ? ts[ip] : te[ip]) + 0.0; }
+  for (int k = k0; k < k1; ++k) {
+    const uint32_t u = sv[k], kind = (u >> 18) & 1u, b = 1u << ((u >> 13) & 31u);
+    const int i = (int)(u & 0x1fffu), q = (int)((u >> 13) & 31u);
+    const double s = ts[i], e = instant ? s : te[i];
+    const double tt = (kind ? s : e) + 0.0;
+    t[k] = tt;
+    delta[k] = instant ? 1.0 : e - s;
+    obs[k] = i;
+    const uint32_t before = after;
+    after ^= instant ? 0u : b;
+    if (!instant && (kind == 1u) == ((before & b) != 0)) atomicOr(&ctl->flags, EVF_OVERLAP); // a start needs closed, an end needs open
+    meta[k] = kind | ((uint32_t)q << 1) | ((((~after) & all) | b) << 8);
+    dt[k] = (k == 0) ? 0.0 : tt - tprev;
+    tprev = tt;
+    if (k == 0) ctl->tfirst = tt;
+    if (k == K - 1) ctl->tlast = tt;
+  }
+}
+
 // look-back words of this ctx (grown on demand, zeroed when allocated; epochs start at 1)
 static int lb_reserve(smolgp_ctx* ctx, size_t words) {
   if (words <= ctx->lb_words) return SMOLGP_OK;
@@ -462,6 +584,16 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   uint32_t* vB = (uint32_t*)p;
   cudaStream_t st = ctx->stream;
   cudaMemsetAsync(ctl, 0, sizeof(EvCtl), st);
+  const bool small = K <= EVS_MAX;
+  if (small) { // one CTA does everything (k_ev_small)
+    int P2 = 64; // (a warp's 64 positions at least: k_ev_small)
+    while (P2 < K) P2 <<= 1;
+    const size_t smem = (size_t)P2 * 12;
+    cudaFuncSetAttribute(k_ev_small, cudaFuncAttributeMaxDynamicSharedMemorySize, EVS_MAX * 12);
+    sg_launch_begin(ctx, KID_EV_FINAL);
+    k_ev_small<<<1, EVS_NT, smem, st>>>(N, ts, te, inst, n_inst, ctl, ev->t, ev->dt, ev->delta, ev->meta, ev->obs, P2);
+    sg_launch_end(ctx);
+  } else {
   sg_launch_begin(ctx, KID_EV_INIT);
   k_ev_init<<<(unsigned)((N + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(N, ts, te, inst, n_inst, kA, vA, ctl);
   sg_launch_end(ctx);
@@ -483,6 +615,7 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
     k_ev_final<<<(unsigned)ntiles_ef, RS_NT, 0, st>>>(ctl, K, vA, vB, ts, te, inst, n_inst, ev->t, ev->dt, ev->delta, ev->meta, ev->obs, ctx->lb_status, epoch);
     sg_launch_end(ctx);
   }
+  } // !small
   // ONE status read-back: validation flags, longest exposures, first / last event time
   struct { int32_t pad; int32_t flags; unsigned long long md[SG_MAXINST]; double tfl[2]; } hs;
   static_assert(offsetof(EvCtl, maxdelta) == offsetof(EvCtl, flags) + 4 && offsetof(EvCtl, tfirst) == offsetof(EvCtl, maxdelta) + 8 * SG_MAXINST &&
