@@ -20,7 +20,8 @@
 //   k_merge     after pass 0: when every (kind, instrument) run is already in time order -- exposures of an instrument
 //               given in time order, the usual case -- the stream is the merge of those runs, done by ranking in one
 //               launch; the eight time passes then return at once.  Otherwise they sort pass 0's output.
-// Twelve launches whatever N (round 1: 33), one small status read-back; up to 8192 events ONE launch (k_ev_small).
+// Four launches when the merge succeeds (the host bets on it and checks the bet in the status read-back the call needs
+// anyway; twelve, after the four, when it does not; round 1: 33); up to 8192 events ONE launch (k_ev_small).
 #include <math.h>
 #include <stddef.h>
 #include <string.h>
@@ -583,8 +584,18 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
   uint32_t* vA = (uint32_t*)p; p += k4;
   uint32_t* vB = (uint32_t*)p;
   cudaStream_t st = ctx->stream;
-  cudaMemsetAsync(ctl, 0, sizeof(EvCtl), st);
   const bool small = K <= EVS_MAX;
+  // ONE status read-back per attempt: merge outcome, validation flags, longest exposures, first / last event time
+  struct { uint32_t unsorted, pad0, ungrouped; int32_t flags; unsigned long long md[SG_MAXINST]; double tfl[2]; } hs;
+  static_assert(offsetof(EvCtl, flags) == offsetof(EvCtl, unsorted) + 12 && offsetof(EvCtl, maxdelta) == offsetof(EvCtl, flags) + 4 &&
+                offsetof(EvCtl, tfirst) == offsetof(EvCtl, maxdelta) + 8 * SG_MAXINST && offsetof(EvCtl, tlast) == offsetof(EvCtl, tfirst) + 8,
+                "EvCtl: unsorted | pad | ungrouped | flags | maxdelta | tfirst | tlast must be contiguous");
+  // The first attempt bets that k_merge succeeds (every (kind, instrument) run in time order: the usual case) and does
+  // not launch the eight time passes at all -- they would all return at once; the read-back that the call needs anyway
+  // tells whether the bet held, and if not the build is redone with the passes (twice the work on unsorted input).
+  for (int attempt = 0; attempt < 2; ++attempt) {
+  const bool bet = (attempt == 0) && !small;
+  cudaMemsetAsync(ctl, 0, sizeof(EvCtl), st);
   if (small) { // one CTA does everything (k_ev_small)
     int P2 = 64; // (a warp's 64 positions at least: k_ev_small)
     while (P2 < K) P2 <<= 1;
@@ -602,6 +613,7 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
       sg_launch_begin(ctx, KID_RS_PASS);
       k_merge<<<(unsigned)((K + RS_NT - 1) / RS_NT), RS_NT, 0, st>>>(ctl, kA, vA, kB, vB, inst, n_inst, (uint32_t)K);
       sg_launch_end(ctx);
+      if (bet) break;
     }
     const uint32_t epoch = lb_next_epoch(ctx);
     sg_launch_begin(ctx, KID_RS_PASS);
@@ -616,13 +628,11 @@ static int build_events_impl(smolgp_ctx* ctx, int64_t N, const double* ts, const
     sg_launch_end(ctx);
   }
   } // !small
-  // ONE status read-back: validation flags, longest exposures, first / last event time
-  struct { int32_t pad; int32_t flags; unsigned long long md[SG_MAXINST]; double tfl[2]; } hs;
-  static_assert(offsetof(EvCtl, maxdelta) == offsetof(EvCtl, flags) + 4 && offsetof(EvCtl, tfirst) == offsetof(EvCtl, maxdelta) + 8 * SG_MAXINST &&
-                offsetof(EvCtl, tlast) == offsetof(EvCtl, tfirst) + 8, "EvCtl: flags | maxdelta | tfirst | tlast must be contiguous");
-  cudaError_t ce = cudaMemcpyAsync(&hs.flags, &ctl->flags, 4 + sizeof(hs.md) + sizeof(hs.tfl), cudaMemcpyDeviceToHost, st);
+  cudaError_t ce = cudaMemcpyAsync(&hs, &ctl->unsorted, sizeof(hs), cudaMemcpyDeviceToHost, st);
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
   if (ce != cudaSuccess) { ctx->err = std::string("build_events: ") + cudaGetErrorString(ce); cudaGetLastError(); return fail(SMOLGP_ECUDA); }
+  if (!(bet && hs.unsorted)) break; // (a lost bet: the stream written by k_ev_final means nothing; redo with the passes)
+  }
   const int flags = hs.flags;
   if (flags & EVF_BADTIME) { ctx->err = "build_events: non-finite time or t_end <= t_start"; return fail(SMOLGP_EINVAL); }
   if (flags & EVF_BADINST) { ctx->err = "build_events: instrument index out of range"; return fail(SMOLGP_EINVAL); }
